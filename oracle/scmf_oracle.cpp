@@ -1,0 +1,415 @@
+// scmf_oracle.cpp -- ORACLE (test infrastructure, not the product).
+//
+// Plain, slow, single-threaded CPU statement of the single-chain-in-mean-field (SCMF) Monte-Carlo
+// step of the SOMA particle model (section 2: "Single-Chain-in-Mean-Field (SCMF)
+// algorithm using a soft, coarse-grained polymer model", "quasi-instantaneous-field approximation
+// for non-bonded interactions"; section 2.2: kernels mc_polymer_iteration -- "trial
+// moves and energy evaluations" -- and update_density_fields -- "updates particle density
+// fields").  The paper prints no equation for the step; every concrete choice below is either
+// fixed by BASELINE.json `north_star` / `configs` (marked NS) or is the reading of SURVEY.md
+// section 8(c) listed in DESIGN.md section 3 (marked R<k>).
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+// load this file.  It shares no code, header, table or constant generator with the CUDA path
+// under paper_2606_09356_b200/; neither side includes or imports the other.
+//
+// The method is a stochastic iteration, so the oracle is the algorithm step by step, in the
+// order of DESIGN.md section 2: no blocking, no fusion, no reordering.  Arithmetic is fp32 with
+// the operation order written out (NS: "fp32" in every config; R17), compiled with
+// -ffp-contract=off so that an FMA appears only where fmaf() is written.  ln u is the correctly
+// rounded fp32 logarithm, obtained as (float)log((double)u) (R6b; the double rounding
+// is checked exhaustively over all 2^24 values of u in tests/test_oracle_rng.py).
+//
+// Pins (tests/, -m "not gpu"): Philox known-answer vectors; exact uniform maps; bin counts by
+// hand; omega against a finite difference of the grid Hamiltonian evaluated in Python; delta-E
+// against E(x') - E(x) evaluated in Python; brute-force detailed balance; ideal-chain closed
+// forms (<R_ee^2> = (N-1) b^2, Gaussian bond statistics, acceptance rate by quadrature).
+// Unpinned (no number in the paper): the ordered morphologies at chiN > 0 -- "parity unpinned"
+// for physics beyond the closed forms above; only GPU-vs-oracle agreement is claimed there.
+
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (NS: "counter-based Philox4x32-10 random numbers keyed by (seed, step,
+// half-sweep, chain, bead)"; constants and round function: DESIGN.md R13 -- the published
+// Philox4x32 parameters; pinned by three known-answer vectors in tests/golden/philox_kat.txt).
+// ---------------------------------------------------------------------------------------------
+const uint32_t PHILOX_M0 = 0xD2511F53u;   // multiplies counter word 0
+const uint32_t PHILOX_M1 = 0xCD9E8D57u;   // multiplies counter word 2
+const uint32_t PHILOX_W0 = 0x9E3779B9u;   // key word 0 increment per round
+const uint32_t PHILOX_W1 = 0xBB67AE85u;   // key word 1 increment per round
+
+void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    const uint64_t p0 = (uint64_t)PHILOX_M0 * (uint64_t)c0;
+    const uint64_t p1 = (uint64_t)PHILOX_M1 * (uint64_t)c2;
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    const uint32_t n0 = hi1 ^ c1 ^ k0;
+    const uint32_t n1 = lo1;
+    const uint32_t n2 = hi0 ^ c3 ^ k1;
+    const uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += PHILOX_W0;
+    k1 += PHILOX_W1;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// DESIGN.md R14: symmetric 23-bit uniform in (-1, 1), never 0; every step is exact in fp32.
+float tmap(uint32_t w) {
+  const uint32_t k = w >> 9;                                 // 23 bits
+  return (float)(2u * k + 1u) * 0x1p-23f - 1.0f;
+}
+// DESIGN.md R14: 24-bit uniform in (0, 1]; exact in fp32.
+float umap(uint32_t w) {
+  return (float)((w >> 8) + 1u) * 0x1p-24f;
+}
+// DESIGN.md R6b: correctly rounded fp32 natural logarithm of u.
+float lnu32(float u) {
+  return (float)std::log((double)u);
+}
+
+const uint32_t RNG_DOMAIN_MOVE = 0;   // DESIGN.md R13: counter word 3 = parity | domain<<8 | (t>>32)<<16
+
+struct Oracle {
+  // problem statement (NS: "chains, bead types, bond length b, chiN, kappaN, grid, box")
+  uint64_t n_chains;
+  uint32_t N, T, n_patterns;
+  std::vector<uint8_t> type_patterns;   // [n_patterns][N]
+  std::vector<uint8_t> chain_pattern;   // [n_chains]
+  float b, kappaN, a;
+  std::vector<float> chiN;              // [T][T]
+  uint32_t grid[3];
+  float box[3];
+  uint64_t seed;
+  // derived constants ("derived constants")
+  float kb;                             // 1.5f/(b*b): harmonic bond, H_b/kT = kb*sum |r_i - r_{i+1}|^2 (R1)
+  float inv_h[3];                       // (float)grid[d]/box[d]
+  float dens_scale;                     // (float)((double)C/(double)B) = 1/nbar (R10)
+  float invN;                           // 1.0f/(float)N (R3)
+  uint64_t B, C;
+  // state
+  std::vector<float> x, y, z;           // [B], index c*N+i, unwrapped (R7)
+  std::vector<uint32_t> counts;         // [T][C], cell = (ix*ny+iy)*nz+iz (R12)
+  std::vector<float> omega;             // [T][C]
+  uint64_t t;                           // absolute step index
+  bool loaded;
+};
+
+inline uint8_t bead_type(const Oracle& o, uint64_t c, uint32_t i) {
+  return o.type_patterns[(size_t)o.chain_pattern[c] * o.N + i];
+}
+
+// DESIGN.md section 2 step 1 (R8): floorf, then a proper non-negative modulo per axis.
+inline uint64_t cell_index(const Oracle& o, float rx, float ry, float rz) {
+  const float r[3] = {rx, ry, rz};
+  int32_t g[3];
+  for (int d = 0; d < 3; ++d) {
+    const float scaled = r[d] * o.inv_h[d];              // requires |scaled| < 2^31
+    int32_t gi = (int32_t)floorf(scaled);
+    const int32_t nd = (int32_t)o.grid[d];
+    gi %= nd;                                            // C remainder: sign of the dividend
+    if (gi < 0) gi += nd;                                // -> representative in [0, nd)
+    g[d] = gi;
+  }
+  return ((uint64_t)g[0] * o.grid[1] + (uint64_t)g[1]) * o.grid[2] + (uint64_t)g[2];
+}
+
+// DESIGN.md section 2 step 2 (NS part 2; R9 nearest-grid-point assignment): integer counts.
+void bin(Oracle& o) {
+  std::fill(o.counts.begin(), o.counts.end(), 0u);
+  for (uint64_t c = 0; c < o.n_chains; ++c)
+    for (uint32_t i = 0; i < o.N; ++i) {
+      const uint64_t j = c * o.N + i;
+      const uint64_t cell = cell_index(o, o.x[j], o.y[j], o.z[j]);
+      o.counts[(size_t)bead_type(o, c, i) * o.C + cell] += 1u;
+    }
+}
+
+// DESIGN.md section 2 step 3 (NS part 3; R2 formula):
+//   phi_s(c) = n_s(c) * C/B;  omega_t(c) = (1/N) * ( kappaN*(sum_s phi_s - 1) + sum_{s != t} chiN_ts * phi_s ).
+void compute_omega(Oracle& o) {
+  std::vector<float> phi(o.T);
+  for (uint64_t c = 0; c < o.C; ++c) {
+    float tot = 0.0f;
+    for (uint32_t s = 0; s < o.T; ++s) {
+      phi[s] = (float)o.counts[(size_t)s * o.C + c] * o.dens_scale;
+      tot = (s == 0) ? phi[0] : (tot + phi[s]);
+    }
+    const float p = o.kappaN * (tot - 1.0f);
+    for (uint32_t t = 0; t < o.T; ++t) {
+      float acc = p;
+      for (uint32_t s = 0; s < o.T; ++s)
+        if (s != t) acc = fmaf(o.chiN[(size_t)t * o.T + s], phi[s], acc);
+      o.omega[(size_t)t * o.C + c] = o.invN * acc;
+    }
+  }
+}
+
+// Squared bond length with the pinned operation order (DESIGN.md section 2 step 5.4).
+inline float bond_sq(float ax, float ay, float az, float bx, float by, float bz) {
+  const float sx = ax - bx, sy = ay - by, sz = az - bz;
+  return fmaf(sz, sz, fmaf(sy, sy, sx * sx));
+}
+
+// Delta E (in kT) of moving bead (c, i) from its current position to (nx, ny, nz):
+// DESIGN.md section 2 steps 5.4-5.5 (NS: "harmonic bond energy plus the bead type's
+// quasi-instantaneous field omega at its grid cell").
+inline float delta_energy(const Oracle& o, uint64_t c, uint32_t i, float nx, float ny, float nz) {
+  const uint64_t j = c * o.N + i;
+  const float rx = o.x[j], ry = o.y[j], rz = o.z[j];
+  float dq = 0.0f;
+  bool have = false;
+  if (i > 0) {                                          // neighbour i-1 first
+    const uint64_t k = j - 1;
+    const float q_old = bond_sq(rx, ry, rz, o.x[k], o.y[k], o.z[k]);
+    const float q_new = bond_sq(nx, ny, nz, o.x[k], o.y[k], o.z[k]);
+    dq = q_new - q_old;
+    have = true;
+  }
+  if (i + 1 < o.N) {                                    // then neighbour i+1
+    const uint64_t k = j + 1;
+    const float q_old = bond_sq(rx, ry, rz, o.x[k], o.y[k], o.z[k]);
+    const float q_new = bond_sq(nx, ny, nz, o.x[k], o.y[k], o.z[k]);
+    const float dqk = q_new - q_old;
+    dq = have ? (dq + dqk) : dqk;
+  }
+  const size_t tb = (size_t)bead_type(o, c, i) * o.C;
+  const float dw = o.omega[tb + cell_index(o, nx, ny, nz)] - o.omega[tb + cell_index(o, rx, ry, rz)];
+  return fmaf(o.kb, dq, dw);
+}
+
+// The same Delta E in double from the same fp32 inputs: used only to classify near-threshold
+// moves for the GPU-vs-oracle mismatch rule (NS: "|dE + ln u| < 1e-4 kT").
+inline double delta_energy_f64(const Oracle& o, uint64_t c, uint32_t i, float nx, float ny, float nz) {
+  const uint64_t j = c * o.N + i;
+  const double r[3] = {o.x[j], o.y[j], o.z[j]}, n[3] = {nx, ny, nz};
+  double dq = 0.0;
+  for (int side = 0; side < 2; ++side) {
+    if (side == 0 && i == 0) continue;
+    if (side == 1 && i + 1 >= o.N) continue;
+    const uint64_t k = side == 0 ? j - 1 : j + 1;
+    const double nb[3] = {o.x[k], o.y[k], o.z[k]};
+    double qo = 0.0, qn = 0.0;
+    for (int d = 0; d < 3; ++d) {
+      qo += (r[d] - nb[d]) * (r[d] - nb[d]);
+      qn += (n[d] - nb[d]) * (n[d] - nb[d]);
+    }
+    dq += qn - qo;
+  }
+  const size_t tb = (size_t)bead_type(o, c, i) * o.C;
+  const double dw = (double)o.omega[tb + cell_index(o, nx, ny, nz)] -
+                    (double)o.omega[tb + cell_index(o, (float)r[0], (float)r[1], (float)r[2])];
+  return (double)o.kb * dq + dw;
+}
+
+// One Metropolis trial move of bead (c, i) (DESIGN.md section 2 step 5).  Returns 1 if accepted.
+inline int trial_move(Oracle& o, uint64_t c, uint32_t i, uint32_t parity, double* margin64) {
+  const uint32_t ctr[4] = {i, (uint32_t)c, (uint32_t)o.t,
+                           parity | (RNG_DOMAIN_MOVE << 8) | ((uint32_t)(o.t >> 32) << 16)};
+  const uint32_t key[2] = {(uint32_t)o.seed, (uint32_t)(o.seed >> 32)};
+  uint32_t w[4];
+  philox4x32_10(ctr, key, w);
+  const float dx = o.a * tmap(w[0]);
+  const float dy = o.a * tmap(w[1]);
+  const float dz = o.a * tmap(w[2]);
+  const float u = umap(w[3]);
+  const uint64_t j = c * o.N + i;
+  const float nx = o.x[j] + dx, ny = o.y[j] + dy, nz = o.z[j] + dz;
+  const float dE = delta_energy(o, c, i, nx, ny, nz);
+  const float m = dE + lnu32(u);
+  if (margin64) *margin64 = delta_energy_f64(o, c, i, nx, ny, nz) + std::log((double)u);
+  if (m <= 0.0f) {                                      // R6: accept iff dE + ln u <= 0
+    o.x[j] = nx; o.y[j] = ny; o.z[j] = nz;
+    return 1;
+  }
+  return 0;
+}
+
+// order: 0 ascending, 1 descending, 2 = caller-supplied permutation of the same-parity bead list
+// (R5: same-parity beads of a linear chain share no bond and omega is frozen, so the
+// visiting order within a half-sweep is immaterial; tests check that bit for bit).
+uint64_t half_sweep(Oracle& o, uint32_t parity, int order, const uint64_t* perm, uint64_t n_perm,
+                    uint8_t* accept_mask, double* margins) {
+  uint64_t accepted = 0;
+  if (order == 2) {
+    for (uint64_t k = 0; k < n_perm; ++k) {
+      const uint64_t j = perm[k];
+      const uint64_t c = j / o.N;
+      const uint32_t i = (uint32_t)(j % o.N);
+      if ((i & 1u) != parity) continue;
+      const int acc = trial_move(o, c, i, parity, margins ? &margins[j] : nullptr);
+      if (accept_mask) accept_mask[j] = (uint8_t)acc;
+      accepted += (uint64_t)acc;
+    }
+    return accepted;
+  }
+  for (uint64_t cc = 0; cc < o.n_chains; ++cc) {
+    const uint64_t c = order == 0 ? cc : o.n_chains - 1 - cc;
+    const uint32_t n_par = (o.N + 1u - parity) / 2u;    // beads i = parity, parity+2, ... < N
+    for (uint32_t kk = 0; kk < n_par; ++kk) {
+      const uint32_t k = order == 0 ? kk : n_par - 1 - kk;
+      const uint32_t i = parity + 2u * k;
+      const uint64_t j = c * o.N + i;
+      const int acc = trial_move(o, c, i, parity, margins ? &margins[j] : nullptr);
+      if (accept_mask) accept_mask[j] = (uint8_t)acc;
+      accepted += (uint64_t)acc;
+    }
+  }
+  return accepted;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// C ABI of the oracle (its own; unrelated to include/soma.h).
+// ---------------------------------------------------------------------------------------------
+extern "C" {
+
+void oracle_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
+  philox4x32_10(ctr, key, out);
+}
+float oracle_tmap(uint32_t w) { return tmap(w); }
+float oracle_umap(uint32_t w) { return umap(w); }
+float oracle_lnu(float u) { return lnu32(u); }
+void oracle_lnu_array(const float* u, float* out, uint64_t n) {
+  for (uint64_t k = 0; k < n; ++k) out[k] = lnu32(u[k]);
+}
+
+void* oracle_create(uint64_t n_chains, uint32_t N, uint32_t T, uint32_t n_patterns,
+                    const uint8_t* type_patterns, const uint8_t* chain_pattern, float b,
+                    const float* chiN, float kappaN, const uint32_t* grid, const float* box,
+                    float move_halfwidth, uint64_t seed) {
+  if (!n_chains || !N || !T || !n_patterns || !type_patterns || !chiN || !grid || !box) return nullptr;
+  Oracle* o = new (std::nothrow) Oracle();
+  if (!o) return nullptr;
+  o->n_chains = n_chains; o->N = N; o->T = T; o->n_patterns = n_patterns;
+  o->type_patterns.assign(type_patterns, type_patterns + (size_t)n_patterns * N);
+  if (chain_pattern) o->chain_pattern.assign(chain_pattern, chain_pattern + n_chains);
+  else o->chain_pattern.assign(n_chains, 0);
+  o->b = b; o->kappaN = kappaN; o->a = move_halfwidth; o->seed = seed;
+  o->chiN.assign(chiN, chiN + (size_t)T * T);
+  for (int d = 0; d < 3; ++d) { o->grid[d] = grid[d]; o->box[d] = box[d]; }
+  o->B = n_chains * N;
+  o->C = (uint64_t)grid[0] * grid[1] * grid[2];
+  o->kb = 1.5f / (b * b);
+  for (int d = 0; d < 3; ++d) o->inv_h[d] = (float)grid[d] / box[d];
+  o->dens_scale = (float)((double)o->C / (double)o->B);
+  o->invN = 1.0f / (float)N;
+  o->x.assign(o->B, 0.0f); o->y.assign(o->B, 0.0f); o->z.assign(o->B, 0.0f);
+  o->counts.assign((size_t)T * o->C, 0u);
+  o->omega.assign((size_t)T * o->C, 0.0f);
+  o->t = 0; o->loaded = false;
+  return o;
+}
+
+void oracle_destroy(void* h) { delete static_cast<Oracle*>(h); }
+
+// DESIGN.md section 2 step 4: copy positions; t = step0; bin(); omega().
+int oracle_load_state(void* h, const float* x, const float* y, const float* z, uint64_t step0) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::memcpy(o.x.data(), x, o.B * sizeof(float));
+  std::memcpy(o.y.data(), y, o.B * sizeof(float));
+  std::memcpy(o.z.data(), z, o.B * sizeof(float));
+  o.t = step0;
+  bin(o);
+  compute_omega(o);
+  o.loaded = true;
+  return 0;
+}
+
+// DESIGN.md section 2 step 6 (NS): half_sweep(0); half_sweep(1); bin(); omega(); t += 1.
+uint64_t oracle_mc_steps(void* h, uint32_t n_steps) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  uint64_t accepted = 0;
+  for (uint32_t s = 0; s < n_steps; ++s) {
+    accepted += half_sweep(o, 0, 0, nullptr, 0, nullptr, nullptr);
+    accepted += half_sweep(o, 1, 0, nullptr, 0, nullptr, nullptr);
+    bin(o);
+    compute_omega(o);
+    o.t += 1;
+  }
+  return accepted;
+}
+
+// Pieces of a step, for lock-step comparison and for frozen-field tests.
+uint64_t oracle_half_sweep(void* h, uint32_t parity, int order, const uint64_t* perm, uint64_t n_perm,
+                           uint8_t* accept_mask, double* margins) {
+  return half_sweep(*static_cast<Oracle*>(h), parity, order, perm, n_perm, accept_mask, margins);
+}
+void oracle_bin(void* h) { bin(*static_cast<Oracle*>(h)); }
+void oracle_compute_omega(void* h) { compute_omega(*static_cast<Oracle*>(h)); }
+void oracle_finish_step(void* h) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  bin(o); compute_omega(o); o.t += 1;
+}
+
+void oracle_get_positions(void* h, float* x, float* y, float* z) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::memcpy(x, o.x.data(), o.B * sizeof(float));
+  std::memcpy(y, o.y.data(), o.B * sizeof(float));
+  std::memcpy(z, o.z.data(), o.B * sizeof(float));
+}
+// Overwrite the positions of selected beads (lock-step resynchronisation after a legal flip).
+void oracle_set_beads(void* h, const uint64_t* idx, uint64_t n, const float* x, const float* y, const float* z) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (uint64_t k = 0; k < n; ++k) { o.x[idx[k]] = x[k]; o.y[idx[k]] = y[k]; o.z[idx[k]] = z[k]; }
+}
+void oracle_get_density(void* h, uint32_t* counts) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::memcpy(counts, o.counts.data(), o.counts.size() * sizeof(uint32_t));
+}
+void oracle_set_density(void* h, const uint32_t* counts) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::memcpy(o.counts.data(), counts, o.counts.size() * sizeof(uint32_t));
+}
+void oracle_get_omega(void* h, float* omega) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::memcpy(omega, o.omega.data(), o.omega.size() * sizeof(float));
+}
+void oracle_set_omega(void* h, const float* omega) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::memcpy(o.omega.data(), omega, o.omega.size() * sizeof(float));
+}
+uint64_t oracle_get_step(void* h) { return static_cast<Oracle*>(h)->t; }
+void oracle_set_step(void* h, uint64_t t) { static_cast<Oracle*>(h)->t = t; }
+
+uint64_t oracle_cell_index(void* h, float x, float y, float z) {
+  return cell_index(*static_cast<Oracle*>(h), x, y, z);
+}
+float oracle_delta_energy(void* h, uint64_t bead, float nx, float ny, float nz) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  return delta_energy(o, bead / o.N, (uint32_t)(bead % o.N), nx, ny, nz);
+}
+// The trial position and u that the move stream gives bead `bead` at the current step (no move made).
+void oracle_trial(void* h, uint64_t bead, uint32_t parity, float* trial_xyz, float* u) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const uint64_t c = bead / o.N;
+  const uint32_t i = (uint32_t)(bead % o.N);
+  const uint32_t ctr[4] = {i, (uint32_t)c, (uint32_t)o.t,
+                           parity | (RNG_DOMAIN_MOVE << 8) | ((uint32_t)(o.t >> 32) << 16)};
+  const uint32_t key[2] = {(uint32_t)o.seed, (uint32_t)(o.seed >> 32)};
+  uint32_t w[4];
+  philox4x32_10(ctr, key, w);
+  trial_xyz[0] = o.x[bead] + o.a * tmap(w[0]);
+  trial_xyz[1] = o.y[bead] + o.a * tmap(w[1]);
+  trial_xyz[2] = o.z[bead] + o.a * tmap(w[2]);
+  *u = umap(w[3]);
+}
+void oracle_get_constants(void* h, float* out5) {     // kb, inv_h[3], dens_scale  (+ invN in out5[5])
+  Oracle& o = *static_cast<Oracle*>(h);
+  out5[0] = o.kb; out5[1] = o.inv_h[0]; out5[2] = o.inv_h[1]; out5[3] = o.inv_h[2];
+  out5[4] = o.dens_scale; out5[5] = o.invN;
+}
+
+}  // extern "C"

@@ -1,0 +1,170 @@
+"""Pins for the oracle's cell index, binning and omega (DESIGN.md section 2 steps 1-3; R2, R8-R10, R12).
+
+Expected values come from hand placement, conservation laws, special cases and an independent
+double-precision evaluation of the grid Hamiltonian of R2 -- never from the oracle's own formula.
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+import oracle
+import scmf_inputs as si
+
+
+def _tiny(n_chains=1, N=4, T=2, grid=(4, 4, 4), box=(2.0, 2.0, 2.0), chiN=None, kappaN=50.0, pats=None,
+          chain_pattern=None, seed=11):
+    if pats is None:
+        pats = np.array([[i * T // N for i in range(N)]], dtype=np.uint8)
+    if chiN is None:
+        chiN = np.full((T, T), 20.0, dtype=np.float32)
+        np.fill_diagonal(chiN, 0)
+    return oracle.Oracle(n_chains, N, T, pats, chain_pattern, 1.0, chiN, kappaN, grid, box, 0.5, seed)
+
+
+def test_cell_index_layout_and_boundaries():
+    # R12: cell = (ix*ny + iy)*nz + iz.  R8: floor (not truncation), face belongs to the upper
+    # cell, periodic wrap by a non-negative modulo.  Non-cubic grid so a swapped axis shows up.
+    o = _tiny(grid=(2, 3, 4), box=(1.0, 1.5, 2.0))        # h = 0.5 on every axis
+    ny, nz = 3, 4
+    idx = lambda ix, iy, iz: (ix * ny + iy) * nz + iz
+    assert o.cell_index(0.25, 0.25, 0.25) == idx(0, 0, 0)
+    assert o.cell_index(0.75, 0.25, 0.25) == idx(1, 0, 0)
+    assert o.cell_index(0.25, 1.25, 0.25) == idx(0, 2, 0)
+    assert o.cell_index(0.25, 0.25, 1.75) == idx(0, 0, 3)
+    assert o.cell_index(0.5, 0.5, 0.5) == idx(1, 1, 1)            # on a face: upper cell
+    assert o.cell_index(-0.0, 0.0, 0.0) == idx(0, 0, 0)
+    assert o.cell_index(-1e-7, 0.0, 0.0) == idx(1, 0, 0)          # just below 0 wraps to the top
+    assert o.cell_index(0.0, -1e-7, 0.0) == idx(0, 2, 0)
+    assert o.cell_index(0.0, 0.0, -0.25) == idx(0, 0, 3)
+    assert o.cell_index(1.0, 1.5, 2.0) == idx(0, 0, 0)            # r = L wraps to 0
+    assert o.cell_index(np.nextafter(np.float32(1.0), np.float32(0)), 0.0, 0.0) == idx(1, 0, 0)
+    assert o.cell_index(2.0, 3.0, 4.0) == idx(0, 0, 0)            # r = 2L
+    assert o.cell_index(-1.0 - 0.25, -1.5 - 0.25, -2.0 - 0.25) == idx(1, 2, 3)
+    assert o.cell_index(7.25, -7.25, 101.3) == idx(14 % 2, (-15) % 3, 202 % 4)
+
+
+def test_bin_hand_placed_beads():
+    # 2 chains of 3 beads, pattern A A B; beads placed by hand, some outside the box.
+    pats = np.array([[0, 0, 1]], dtype=np.uint8)
+    o = _tiny(n_chains=2, N=3, T=2, grid=(2, 2, 2), box=(1.0, 1.0, 1.0), pats=pats)
+    x = np.array([0.1, 0.6, 0.6, -0.1, 1.1, 0.25], dtype=np.float32)
+    y = np.array([0.1, 0.1, 0.6, 0.1, 0.1, 0.25], dtype=np.float32)
+    z = np.array([0.1, 0.1, 0.6, 0.1, 0.1, 2.75], dtype=np.float32)
+    o.load_state(x, y, z)
+    want = np.zeros((2, 8), dtype=np.uint32)
+    cell = lambda ix, iy, iz: (ix * 2 + iy) * 2 + iz
+    want[0, cell(0, 0, 0)] += 1      # chain 0 bead 0 (A)
+    want[0, cell(1, 0, 0)] += 1      # chain 0 bead 1 (A)
+    want[1, cell(1, 1, 1)] += 1      # chain 0 bead 2 (B)
+    want[0, cell(1, 0, 0)] += 1      # chain 1 bead 0 (A) at x=-0.1 -> wraps to ix=1
+    want[0, cell(0, 0, 0)] += 1      # chain 1 bead 1 (A) at x=1.1 -> ix=0
+    want[1, cell(0, 0, 1)] += 1      # chain 1 bead 2 (B) at z=2.75 -> iz=1
+    assert np.array_equal(o.density(), want)
+
+
+@pytest.mark.parametrize("cfg", [0])
+def test_density_sums_to_bead_counts_exactly(cfg):
+    # north_star oracle check 2: "the density grids sum to the total bead count exactly".
+    s = si.make_system(si.config(cfg))
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    types = s.bead_types()
+    for step in range(3):
+        d = o.density()
+        assert int(d.sum()) == s.workload.n_beads
+        for t in range(s.workload.n_types):
+            assert int(d[t].sum()) == int((types == t).sum())
+        o.mc_steps(1)
+
+
+def test_density_matches_numpy_histogram_of_float64_cells():
+    # Independent route: cell coordinates by float64 floor + Python modulo, counted by bincount.
+    # (positions of this workload are far from cell faces in fp32 terms except by chance; the
+    # fp32 product r*inv_h is exact here because inv_h = 2.)
+    w = si.scaled(si.config(3), 512, (8, 8, 8))
+    s = si.make_system(w)
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    o.mc_steps(2)
+    x, y, z = o.positions()
+    g = [np.floor(v.astype(np.float64) * 2.0).astype(np.int64) % 8 for v in (x, y, z)]
+    cell = (g[0] * 8 + g[1]) * 8 + g[2]
+    types = s.bead_types()
+    want = np.stack([np.bincount(cell[types == t], minlength=512) for t in range(2)])
+    assert np.array_equal(o.density().astype(np.int64), want)
+
+
+def test_omega_special_cases():
+    # R2/R10 special cases: homogeneous n_A = n_B = nbar/2 -> omega = chiN/(2N);
+    # empty cell -> omega = -kappaN/N; chiN = kappaN = 0 -> omega == 0 exactly.
+    N, n_chains, grid = 8, 16, (2, 2, 2)                          # B = 128, C = 8, nbar = 16
+    o = _tiny(n_chains=n_chains, N=N, T=2, grid=grid, box=(1.0, 1.0, 1.0), kappaN=50.0)
+    counts = np.full((2, 8), 8, dtype=np.uint32)
+    counts[:, 3] = 0                                              # one empty cell
+    o.set_density(counts)
+    o.compute_omega()
+    om = o.omega()
+    assert np.allclose(np.delete(om, 3, axis=1), 20.0 / (2 * N), rtol=0, atol=1e-6)
+    assert np.allclose(om[:, 3], -50.0 / N, rtol=0, atol=1e-6)
+    z = _tiny(n_chains=n_chains, N=N, T=2, grid=grid, box=(1.0, 1.0, 1.0), kappaN=0.0,
+              chiN=np.zeros((2, 2), dtype=np.float32))
+    z.set_density(np.arange(16, dtype=np.uint32).reshape(2, 8))
+    z.compute_omega()
+    assert np.all(z.omega() == 0.0)
+
+
+def _H_nb(counts, chiN, kappaN, N, nbar):
+    """Grid Hamiltonian of DESIGN.md R2 in double:
+    H/kT = (nbar/N) * sum_c [ kappaN/2 (sum_s phi_s - 1)^2 + sum_{s<t} chiN_st phi_s phi_t ]."""
+    phi = counts.astype(np.float64) / nbar
+    T = counts.shape[0]
+    tot = phi.sum(axis=0)
+    h = 0.5 * kappaN * (tot - 1.0) ** 2
+    for s in range(T):
+        for t in range(s + 1, T):
+            h = h + chiN[s, t] * phi[s] * phi[t]
+    return nbar / N * h.sum()
+
+
+@pytest.mark.parametrize("T", [1, 2, 3])
+def test_omega_is_the_derivative_of_the_grid_hamiltonian(T):
+    # Brute force on a 2x2x2 grid: omega_t(c) = [H(n_t(c)+1) - H(n_t(c)-1)]/2 exactly, because H
+    # is quadratic in the counts.  Asymmetric chiN-free check of the index order chiN[t][s].
+    rng = np.random.default_rng(100 + T)
+    N, n_chains = 6, 20
+    B, Cn = N * n_chains, 8
+    nbar = B / Cn
+    chi = rng.uniform(1.0, 30.0, size=(T, T))
+    chi = np.triu(chi, 1)
+    chi = (chi + chi.T).astype(np.float32)
+    kappaN = 37.0
+    pats = np.array([[i % T for i in range(N)]], dtype=np.uint8)
+    o = _tiny(n_chains=n_chains, N=N, T=T, grid=(2, 2, 2), box=(1.0, 1.0, 1.0), chiN=chi, kappaN=kappaN, pats=pats)
+    counts = rng.integers(1, 30, size=(T, Cn)).astype(np.uint32)
+    o.set_density(counts)
+    o.compute_omega()
+    om = o.omega()
+    for t, c in itertools.product(range(T), range(Cn)):
+        up, dn = counts.astype(np.int64).copy(), counts.astype(np.int64).copy()
+        up[t, c] += 1
+        dn[t, c] -= 1
+        want = 0.5 * (_H_nb(up, chi.astype(np.float64), kappaN, N, nbar) - _H_nb(dn, chi.astype(np.float64), kappaN, N, nbar))
+        assert abs(om[t, c] - want) < 2e-5 * max(1.0, abs(want)), (t, c, om[t, c], want)
+
+
+def test_load_state_bins_and_computes_omega():
+    s = si.make_system(si.config(0))
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z, step0=17)
+    assert o.step == 17
+    d = o.density()
+    assert d.sum() == s.workload.n_beads
+    # omega of the loaded state, by the route of the previous test (double, from the counts)
+    N, nbar = s.workload.N, s.workload.n_beads / s.workload.n_cells
+    phi = d.astype(np.float64) / nbar
+    want0 = (s.workload.kappaN * (phi.sum(axis=0) - 1.0) + s.workload.chiN * phi[1]) / N
+    want1 = (s.workload.kappaN * (phi.sum(axis=0) - 1.0) + s.workload.chiN * phi[0]) / N
+    om = o.omega()
+    assert np.allclose(om[0], want0, rtol=0, atol=5e-6)
+    assert np.allclose(om[1], want1, rtol=0, atol=5e-6)
