@@ -1,0 +1,151 @@
+/* soma.h -- C ABI of libsoma_b200.so: the SCMF Monte-Carlo step of the SOMA particle model on one
+ * NVIDIA B200 (sm_100a).
+ *
+ * What it computes: DESIGN.md section 2, i.e. BASELINE.json `north_star` parts (1)-(3) -- Metropolis
+ * trial moves of every bead in two half-sweeps (even beads, then odd beads) scored by harmonic bond
+ * energy plus the bead type's field omega at its grid cell; re-binning of all beads into per-type
+ * integer density grids; omega recomputed from the densities -- the two kernels the paper reports as
+ * 65 % + 25 % of SOMA's run time (section 2.2) plus the quasi-instantaneous field
+ * update (section 2).  Entry-point names are the ones `north_star` lists.
+ *
+ * Conventions
+ *   - Every function returns SOMA_OK (0) or a negative error code; nothing throws or aborts.
+ *     soma_last_error(h) gives a text for the last failure on that handle.
+ *   - One handle = one CUDA device (the current device at soma_create) + one CUDA stream.  All work
+ *     is enqueued on that stream.  Calls that hand data back to the HOST synchronise the stream
+ *     before returning; everything else is asynchronous with respect to the host.  Calls on one
+ *     handle are not thread-safe.  There is no global state.
+ *   - Ownership: the library copies everything it is given (parameters at create, positions at
+ *     load_state).  The caller owns every buffer it passes in or receives results in.  The library
+ *     owns its device memory, unless the caller lends a workspace (see soma_params.workspace).
+ *   - Layouts: positions are structure-of-arrays fp32, x[B], y[B], z[B], B = n_chains *
+ *     beads_per_chain, bead i of chain c at index c*beads_per_chain + i, UNWRAPPED (periodic images
+ *     are applied only when a bead is assigned to a cell).  Grids are [type][ix][iy][iz] with iz
+ *     fastest, cell = (ix*grid[1] + iy)*grid[2] + iz; densities are uint32 bead counts, omega fp32
+ *     in units of kT.
+ *   - "device pointer" = memory of the handle's device (e.g. a torch CUDA tensor's data_ptr);
+ *     "host pointer" = ordinary or pinned host memory.  A flag argument says which.
+ *   - There is no CPU fallback: without a usable sm_100 device every call fails with SOMA_ECUDA.
+ */
+#ifndef SOMA_B200_H
+#define SOMA_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SOMA_OK       0
+#define SOMA_EINVAL  -1   /* NULL / out-of-range / inconsistent argument                      */
+#define SOMA_ENOMEM  -2   /* device or host allocation failed, or the lent workspace is small  */
+#define SOMA_ECUDA   -3   /* CUDA runtime error (sticky: later calls on the handle fail too)   */
+#define SOMA_ESTATE  -4   /* call out of order (e.g. soma_mc_steps before soma_load_state)     */
+
+typedef struct soma_handle soma_t;   /* opaque */
+
+/* Problem statement (`north_star`: "chains, bead types, bond length b, chiN, kappaN, grid, box").
+ * All chains are linear and have the same number of beads.  Limits: n_chains < 2^32,
+ * 1 <= n_types <= 8, n_types * cells < 2^32, beads_per_chain <= 65535. */
+typedef struct soma_params {
+  uint64_t n_chains;            /* n                                                            */
+  uint32_t beads_per_chain;     /* N >= 1                                                       */
+  uint32_t n_types;             /* T                                                            */
+  uint32_t n_patterns;          /* >= 1                                                         */
+  uint32_t reserved0;           /* must be 0                                                    */
+  const uint8_t *type_patterns; /* host [n_patterns][N]: bead type at each position along a chain */
+  const uint8_t *chain_pattern; /* host [n_chains]: pattern id of each chain, or NULL = all 0     */
+  const float *chiN;            /* host [T][T]: chi*N, symmetric, zero diagonal                   */
+  float b;                      /* bond length; harmonic bonds with k = 3/(2 b^2) kT (DESIGN R1)  */
+  float kappaN;                 /* kappa*N, incompressibility                                     */
+  float move_halfwidth;         /* a: trial displacement uniform in the cube (-a, a)^3           */
+  float reserved1;              /* must be 0                                                    */
+  uint32_t grid[3];             /* cells per axis                                               */
+  uint32_t reserved2;           /* must be 0                                                    */
+  float box[3];                 /* periodic box lengths; cell size = box/grid                   */
+  float reserved3;              /* must be 0                                                    */
+  uint64_t seed;                /* Philox key                                                   */
+  void *workspace;              /* device pointer lent by the caller (>= soma_workspace_bytes,
+                                   256-byte aligned, must outlive the handle), or NULL = the
+                                   library allocates with cudaMalloc                            */
+  uint64_t workspace_bytes;     /* size of `workspace` (ignored when workspace == NULL)         */
+} soma_params;
+
+/* Device bytes a handle for `p` needs (positions x2, grids, chain tables).  0 on invalid `p`. */
+uint64_t soma_workspace_bytes(const soma_params *p);
+
+/* Create a handle on the current CUDA device.  `cuda_stream` is a cudaStream_t (e.g.
+ * torch.cuda.current_stream().cuda_stream), NULL = the default stream.  Copies all parameters.
+ * Errors: SOMA_EINVAL (bad parameter, see limits), SOMA_ENOMEM, SOMA_ECUDA.  *out is NULL on error. */
+int soma_create(const soma_params *p, void *cuda_stream, soma_t **out);
+
+/* DESIGN.md section 2 step 4: copy the positions in, set the absolute step index to `step0`, bin
+ * all beads and compute omega, so that the next step sees the field of the loaded state.
+ * x, y, z: [B] fp32, host or device according to `ptrs_are_device`.  (positions, step index) is a
+ * complete checkpoint: the random stream is a pure function of (seed, step, half-sweep, chain,
+ * bead).  Errors: SOMA_EINVAL (NULL pointer), SOMA_ECUDA. */
+int soma_load_state(soma_t *h, const float *x, const float *y, const float *z, uint64_t step0,
+                    int ptrs_are_device);
+
+/* DESIGN.md section 2 step 6, `n_steps` times: half-sweep(even), half-sweep(odd), bin, omega,
+ * step += 1.  `accepted` (host pointer, may be NULL) receives the number of accepted moves of this
+ * call; passing it synchronises the stream, passing NULL keeps the call asynchronous.
+ * n_steps == 0 is a no-op.  Errors: SOMA_ESTATE (no state loaded), SOMA_ECUDA. */
+int soma_mc_steps(soma_t *h, uint32_t n_steps, uint64_t *accepted);
+
+/* Integer bead counts of the current configuration, [T][cells] uint32. */
+int soma_get_density(soma_t *h, uint32_t *counts, int ptr_is_device);
+
+/* Current positions in the caller's (chain, bead) order, unwrapped, [B] each. */
+int soma_get_positions(soma_t *h, float *x, float *y, float *z, int ptrs_are_device);
+
+/* Current field omega, [T][cells] fp32 (helper; not in north_star's list). */
+int soma_get_omega(soma_t *h, float *omega, int ptr_is_device);
+
+/* Absolute step index (step0 + steps done). */
+int soma_get_step(soma_t *h, uint64_t *step);
+
+/* Free everything the library allocated.  soma_destroy(NULL) is a no-op returning SOMA_OK. */
+int soma_destroy(soma_t *h);
+
+/* Text of the last error on `h` ("" if none).  h == NULL: text of the last failed soma_create /
+ * debug call of this thread. */
+const char *soma_last_error(const soma_t *h);
+
+/* Tuning / test switches.  Names:
+ *   "path"            0 = automatic, 1 = generic kernels (4 launches/step, any N),
+ *                     2 = fused chain-in-registers kernel (N = 2P, P a power of two <= 32; else EINVAL)
+ *   "resort_interval" re-order chains in memory by position every k steps (0 = never); results
+ *                     are independent of it (the random stream is keyed by the logical chain id)
+ * Errors: SOMA_EINVAL (unknown name / unsupported value). */
+int soma_set_option(soma_t *h, const char *name, int64_t value);
+
+/* Counters since soma_create: [0] kernels launched by this library, [1] MC steps done,
+ * [2] chain re-orderings done.  `out` is a host pointer to 3 uint64. */
+int soma_get_counters(const soma_t *h, uint64_t *out);
+
+/* ---- test hooks (used by tests/ only; each runs on the device) --------------------------------- */
+
+/* One half-sweep only (DESIGN.md section 2 step 5); omega, densities and the step index are left
+ * untouched.  `accepted` as in soma_mc_steps. */
+int soma_debug_half_sweep(soma_t *h, uint32_t parity, uint64_t *accepted);
+/* bin + omega + step += 1 (the rest of step 6 after two soma_debug_half_sweep calls). */
+int soma_debug_finish_step(soma_t *h);
+/* Overwrite omega with caller-supplied values ([T][cells], host pointer): frozen-field tests. */
+int soma_debug_set_omega(soma_t *h, const float *omega);
+/* Device evaluation of the pieces of DESIGN.md section 2 step 5.1-5.2 on host arrays:
+ * philox: ctr [n][4], key [2] -> out [n][4];  maps: words [n] -> tmap [n], u [n], lnu [n] (lnu by the
+ * kernel's slow path, i.e. the value it uses when a move is near the threshold);
+ * accept: dE [n], words [n] -> decision [n] (0/1) by the kernel's full fast+slow accept routine. */
+int soma_debug_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
+int soma_debug_maps(const uint32_t *words, float *tmap, float *u, float *lnu, uint64_t n);
+int soma_debug_accept(const float *dE, const uint32_t *words, uint8_t *decision, uint64_t n);
+/* Cell index of host positions under the handle's grid/box. */
+int soma_debug_cell_index(soma_t *h, const float *x, const float *y, const float *z, uint32_t *cell,
+                          uint64_t n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SOMA_B200_H */

@@ -1,0 +1,344 @@
+"""paper_2606_09356_b200 -- thin Python binding of libsoma_b200.so (include/soma.h).
+
+Argument marshalling only: every step of the SCMF Monte-Carlo step runs in the library's sm_100a
+kernels.  PyTorch is used for device memory (the workspace tensor, device-side result tensors) and
+for the CUDA stream.  There is no CPU fallback: a missing library or device raises.
+
+The functions carry the C names (`soma_create`, `soma_load_state`, `soma_mc_steps`,
+`soma_get_density`, `soma_get_positions`, `soma_destroy`); `Soma` is a small convenience wrapper
+over them.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import _build
+
+SOMA_OK, SOMA_EINVAL, SOMA_ENOMEM, SOMA_ECUDA, SOMA_ESTATE = 0, -1, -2, -3, -4
+_ERR = {SOMA_EINVAL: "SOMA_EINVAL", SOMA_ENOMEM: "SOMA_ENOMEM", SOMA_ECUDA: "SOMA_ECUDA", SOMA_ESTATE: "SOMA_ESTATE"}
+
+LIB_PATH: Path = _build.LIB_PATH
+
+# every symbol include/soma.h declares (tests check the library exports exactly these)
+EXPORTS = (
+    "soma_workspace_bytes", "soma_create", "soma_load_state", "soma_mc_steps", "soma_get_density",
+    "soma_get_positions", "soma_get_omega", "soma_get_step", "soma_destroy", "soma_last_error",
+    "soma_set_option", "soma_get_counters", "soma_debug_half_sweep", "soma_debug_finish_step",
+    "soma_debug_set_omega", "soma_debug_philox", "soma_debug_maps", "soma_debug_accept",
+    "soma_debug_cell_index",
+)
+
+
+class SomaError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"{_ERR.get(code, code)}: {text}")
+        self.code = code
+
+
+class soma_params(C.Structure):
+    """Mirror of `struct soma_params` in include/soma.h."""
+    _fields_ = [
+        ("n_chains", C.c_uint64),
+        ("beads_per_chain", C.c_uint32),
+        ("n_types", C.c_uint32),
+        ("n_patterns", C.c_uint32),
+        ("reserved0", C.c_uint32),
+        ("type_patterns", C.c_void_p),
+        ("chain_pattern", C.c_void_p),
+        ("chiN", C.c_void_p),
+        ("b", C.c_float),
+        ("kappaN", C.c_float),
+        ("move_halfwidth", C.c_float),
+        ("reserved1", C.c_float),
+        ("grid", C.c_uint32 * 3),
+        ("reserved2", C.c_uint32),
+        ("box", C.c_float * 3),
+        ("reserved3", C.c_float),
+        ("seed", C.c_uint64),
+        ("workspace", C.c_void_p),
+        ("workspace_bytes", C.c_uint64),
+    ]
+
+
+_lib: Optional[C.CDLL] = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen the in-tree libsoma_b200.so; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise ImportError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'`"
+                              " (nvcc, sm_100a). There is no CPU fallback.")
+        L = C.CDLL(str(LIB_PATH))
+        vp, u64, u32, i32 = C.c_void_p, C.c_uint64, C.c_uint32, C.c_int
+        pp = C.POINTER(soma_params)
+        sig = {
+            "soma_workspace_bytes": (u64, [pp]),
+            "soma_create": (i32, [pp, vp, C.POINTER(vp)]),
+            "soma_load_state": (i32, [vp, vp, vp, vp, u64, i32]),
+            "soma_mc_steps": (i32, [vp, u32, C.POINTER(u64)]),
+            "soma_get_density": (i32, [vp, vp, i32]),
+            "soma_get_positions": (i32, [vp, vp, vp, vp, i32]),
+            "soma_get_omega": (i32, [vp, vp, i32]),
+            "soma_get_step": (i32, [vp, C.POINTER(u64)]),
+            "soma_destroy": (i32, [vp]),
+            "soma_last_error": (C.c_char_p, [vp]),
+            "soma_set_option": (i32, [vp, C.c_char_p, C.c_int64]),
+            "soma_get_counters": (i32, [vp, C.POINTER(u64)]),
+            "soma_debug_half_sweep": (i32, [vp, u32, C.POINTER(u64)]),
+            "soma_debug_finish_step": (i32, [vp]),
+            "soma_debug_set_omega": (i32, [vp, vp]),
+            "soma_debug_philox": (i32, [vp, vp, vp, u64]),
+            "soma_debug_maps": (i32, [vp, vp, vp, vp, u64]),
+            "soma_debug_accept": (i32, [vp, vp, vp, u64]),
+            "soma_debug_cell_index": (i32, [vp, vp, vp, vp, vp, u64]),
+        }
+        for name, (res, args) in sig.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, h=None):
+    if rc != SOMA_OK:
+        raise SomaError(rc, (load_library().soma_last_error(h) or b"").decode())
+
+
+def _ptr(a) -> int:
+    """Address of a numpy array (host) or torch tensor (host or device)."""
+    if isinstance(a, np.ndarray):
+        return a.ctypes.data
+    return a.data_ptr()
+
+
+def _is_device(a) -> int:
+    return 0 if isinstance(a, np.ndarray) else int(a.is_cuda)
+
+
+# ---- the C entry points, same names ------------------------------------------------------------
+
+def make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN, kappaN,
+                grid, box, move_halfwidth, seed):
+    """Build a soma_params plus the numpy arrays it points to (keep the tuple alive until create)."""
+    pats = np.ascontiguousarray(type_patterns, dtype=np.uint8)
+    n_patterns = 1 if pats.ndim < 2 else int(pats.shape[0])     # validation is the library's job
+    cp = None if chain_pattern is None else np.ascontiguousarray(chain_pattern, dtype=np.uint8)
+    chi = np.ascontiguousarray(chiN, dtype=np.float32)
+    p = soma_params()
+    p.n_chains, p.beads_per_chain, p.n_types, p.n_patterns = int(n_chains), int(beads_per_chain), int(n_types), n_patterns
+    p.type_patterns = pats.ctypes.data
+    p.chain_pattern = None if cp is None else cp.ctypes.data
+    p.chiN = chi.ctypes.data
+    p.b, p.kappaN, p.move_halfwidth = float(b), float(kappaN), float(move_halfwidth)
+    p.grid = (C.c_uint32 * 3)(*[int(g) for g in grid])
+    p.box = (C.c_float * 3)(*[float(v) for v in box])
+    p.seed = int(seed)
+    p.workspace, p.workspace_bytes = None, 0
+    return p, (pats, cp, chi)
+
+
+def soma_workspace_bytes(p: soma_params) -> int:
+    return int(load_library().soma_workspace_bytes(C.byref(p)))
+
+
+def soma_create(p: soma_params, cuda_stream: int = 0) -> int:
+    h = C.c_void_p()
+    _check(load_library().soma_create(C.byref(p), C.c_void_p(cuda_stream), C.byref(h)))
+    return h.value
+
+
+def soma_load_state(h, x, y, z, step0: int = 0):
+    dev = _is_device(x)
+    assert _is_device(y) == dev and _is_device(z) == dev
+    _check(load_library().soma_load_state(h, _ptr(x), _ptr(y), _ptr(z), int(step0), dev), h)
+
+
+def soma_mc_steps(h, n_steps: int, want_accepted: bool = False) -> Optional[int]:
+    acc = C.c_uint64(0)
+    _check(load_library().soma_mc_steps(h, int(n_steps), C.byref(acc) if want_accepted else None), h)
+    return int(acc.value) if want_accepted else None
+
+
+def soma_get_density(h, out):
+    _check(load_library().soma_get_density(h, _ptr(out), _is_device(out)), h)
+    return out
+
+
+def soma_get_positions(h, x, y, z):
+    dev = _is_device(x)
+    _check(load_library().soma_get_positions(h, _ptr(x), _ptr(y), _ptr(z), dev), h)
+    return x, y, z
+
+
+def soma_get_omega(h, out):
+    _check(load_library().soma_get_omega(h, _ptr(out), _is_device(out)), h)
+    return out
+
+
+def soma_get_step(h) -> int:
+    s = C.c_uint64(0)
+    _check(load_library().soma_get_step(h, C.byref(s)), h)
+    return int(s.value)
+
+
+def soma_destroy(h):
+    _check(load_library().soma_destroy(h))
+
+
+def soma_set_option(h, name: str, value: int):
+    _check(load_library().soma_set_option(h, name.encode(), int(value)), h)
+
+
+def soma_get_counters(h) -> dict:
+    out = (C.c_uint64 * 3)()
+    _check(load_library().soma_get_counters(h, out), h)
+    return {"launches": int(out[0]), "steps": int(out[1]), "resorts": int(out[2])}
+
+
+def soma_debug_half_sweep(h, parity: int, want_accepted: bool = True):
+    acc = C.c_uint64(0)
+    _check(load_library().soma_debug_half_sweep(h, int(parity), C.byref(acc) if want_accepted else None), h)
+    return int(acc.value)
+
+
+def soma_debug_finish_step(h):
+    _check(load_library().soma_debug_finish_step(h), h)
+
+
+def soma_debug_set_omega(h, omega: np.ndarray):
+    omega = np.ascontiguousarray(omega, dtype=np.float32)
+    _check(load_library().soma_debug_set_omega(h, omega.ctypes.data), h)
+
+
+def soma_debug_philox(ctr: np.ndarray, key: Sequence[int]) -> np.ndarray:
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.empty_like(ctr)
+    _check(load_library().soma_debug_philox(ctr.ctypes.data, k.ctypes.data, out.ctypes.data, ctr.shape[0]))
+    return out
+
+
+def soma_debug_maps(words: np.ndarray):
+    words = np.ascontiguousarray(words, dtype=np.uint32).reshape(-1)
+    t, u, l = (np.empty(words.size, dtype=np.float32) for _ in range(3))
+    _check(load_library().soma_debug_maps(words.ctypes.data, t.ctypes.data, u.ctypes.data, l.ctypes.data, words.size))
+    return t, u, l
+
+
+def soma_debug_accept(dE: np.ndarray, words: np.ndarray) -> np.ndarray:
+    dE = np.ascontiguousarray(dE, dtype=np.float32).reshape(-1)
+    words = np.ascontiguousarray(words, dtype=np.uint32).reshape(-1)
+    assert dE.size == words.size
+    out = np.empty(dE.size, dtype=np.uint8)
+    _check(load_library().soma_debug_accept(dE.ctypes.data, words.ctypes.data, out.ctypes.data, dE.size))
+    return out
+
+
+def soma_debug_cell_index(h, x, y, z) -> np.ndarray:
+    x, y, z = (np.ascontiguousarray(v, dtype=np.float32).reshape(-1) for v in (x, y, z))
+    out = np.empty(x.size, dtype=np.uint32)
+    _check(load_library().soma_debug_cell_index(h, x.ctypes.data, y.ctypes.data, z.ctypes.data, out.ctypes.data, x.size), h)
+    return out
+
+
+# ---- convenience wrapper -----------------------------------------------------------------------
+
+class Soma:
+    """One SCMF system on the current CUDA device.  Device memory and stream come from PyTorch."""
+
+    def __init__(self, n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN,
+                 kappaN, grid, box, move_halfwidth, seed, stream=None, lend_workspace: bool = True):
+        import torch
+        if not torch.cuda.is_available():
+            raise SomaError(SOMA_ECUDA, "no CUDA device: this package has no CPU fallback")
+        self.n_chains, self.N, self.T = int(n_chains), int(beads_per_chain), int(n_types)
+        self.B = self.n_chains * self.N
+        self.grid = tuple(int(g) for g in grid)
+        self.cells = self.grid[0] * self.grid[1] * self.grid[2]
+        p, keep = make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN,
+                              kappaN, grid, box, move_halfwidth, seed)
+        self._workspace = None
+        if lend_workspace:
+            nbytes = soma_workspace_bytes(p)
+            if nbytes == 0:
+                raise SomaError(SOMA_EINVAL, (load_library().soma_last_error(None) or b"").decode())
+            self._workspace = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+            p.workspace, p.workspace_bytes = self._workspace.data_ptr(), nbytes
+        self._stream = stream if stream is not None else torch.cuda.current_stream()
+        self._h = soma_create(p, self._stream.cuda_stream)
+        del keep
+
+    @classmethod
+    def from_system(cls, s, **kw) -> "Soma":
+        """`s` is a scmf_inputs.System (duck-typed)."""
+        w = s.workload
+        return cls(w.n_chains, w.N, w.n_types, s.type_patterns, s.chain_pattern, w.b, s.chiN,
+                   w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed, **kw)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            soma_destroy(self._h)
+            self._h = None
+            self._workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def load_state(self, x, y, z, step0: int = 0):
+        soma_load_state(self._h, x, y, z, step0)
+
+    def mc_steps(self, n: int, want_accepted: bool = False):
+        return soma_mc_steps(self._h, n, want_accepted)
+
+    def positions(self):
+        x, y, z = (np.empty(self.B, dtype=np.float32) for _ in range(3))
+        return soma_get_positions(self._h, x, y, z)
+
+    def positions_device(self):
+        import torch
+        x, y, z = (torch.empty(self.B, dtype=torch.float32, device="cuda") for _ in range(3))
+        return soma_get_positions(self._h, x, y, z)
+
+    def density(self) -> np.ndarray:
+        return soma_get_density(self._h, np.empty((self.T, self.cells), dtype=np.uint32))
+
+    def omega(self) -> np.ndarray:
+        return soma_get_omega(self._h, np.empty((self.T, self.cells), dtype=np.float32))
+
+    @property
+    def step(self) -> int:
+        return soma_get_step(self._h)
+
+    def set_option(self, name: str, value: int):
+        soma_set_option(self._h, name, value)
+
+    def counters(self) -> dict:
+        return soma_get_counters(self._h)
+
+    # test hooks
+    def debug_half_sweep(self, parity: int) -> int:
+        return soma_debug_half_sweep(self._h, parity)
+
+    def debug_finish_step(self):
+        soma_debug_finish_step(self._h)
+
+    def debug_set_omega(self, omega):
+        soma_debug_set_omega(self._h, omega)
+
+    def debug_cell_index(self, x, y, z):
+        return soma_debug_cell_index(self._h, x, y, z)

@@ -1,0 +1,49 @@
+"""Build libsoma_b200.so (the C-ABI library of include/soma.h) in-tree with nvcc for sm_100a."""
+from __future__ import annotations
+
+import os
+import subprocess
+from pathlib import Path
+
+_PKG = Path(__file__).resolve().parent
+_CSRC = _PKG / "csrc"
+LIB_PATH = _PKG / "libsoma_b200.so"
+
+# --fmad=false: an FMA appears only where the source writes __fmaf_rn (R17); the kernels
+# spell every floating-point operation of the move with __f*_rn intrinsics as well.
+NVCC_FLAGS = [
+    "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+    "--fmad=false", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v",
+]
+
+
+def sources():
+    return sorted(_CSRC.glob("*.cu"))
+
+
+def _stale() -> bool:
+    if not LIB_PATH.exists():
+        return True
+    t = LIB_PATH.stat().st_mtime
+    deps = list(_CSRC.glob("*.cu")) + list(_CSRC.glob("*.cuh")) + [_PKG.parent / "include" / "soma.h"]
+    return any(d.stat().st_mtime > t for d in deps)
+
+
+def build(force: bool = False, verbose: bool = False) -> Path:
+    """Compile every CUDA source into libsoma_b200.so.  nvcc cross-compiles without a GPU."""
+    if force or _stale():
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        tmp = LIB_PATH.with_suffix(f".tmp{os.getpid()}.so")
+        cmd = [nvcc, *NVCC_FLAGS, *map(str, sources()), "-o", str(tmp)]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if verbose or r.returncode != 0:
+            print(r.stdout + r.stderr)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed:\n" + r.stderr[-4000:])
+        os.replace(tmp, LIB_PATH)
+        (_PKG / "ptxas_info.txt").write_text(r.stderr)
+    return LIB_PATH
+
+
+if __name__ == "__main__":
+    print(build(force=True, verbose=True))

@@ -1,0 +1,609 @@
+// soma_api.cu -- host side of libsoma_b200.so: the C ABI of include/soma.h.
+// Argument checking, device memory layout, launch sequencing.  All arithmetic of the Monte-Carlo
+// step runs in the kernels of soma_kernels.cuh.
+#include "../../include/soma.h"
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "soma_kernels.cuh"
+
+using namespace soma;
+
+namespace {
+
+thread_local char g_last_error[256] = "";
+
+constexpr uint64_t kAlign = 256;
+inline uint64_t align_up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {            // byte offsets into the workspace
+  uint64_t pos[2][3];      // two position sets (x,y,z): the live one and a staging / re-order target
+  uint64_t counts[2];      // [T][C] uint32, double-buffered
+  uint64_t omega;          // [T][C] fp32
+  uint64_t slot_chain;     // [n] uint32
+  uint64_t slot_pattern;   // [n] uint8
+  uint64_t patterns;       // [n_patterns][N] uint8
+  uint64_t accepted;       // uint64
+  uint64_t total;
+};
+
+Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes) {
+  Layout L{};
+  uint64_t off = 0;
+  for (int s = 0; s < 2; ++s)
+    for (int d = 0; d < 3; ++d) { L.pos[s][d] = off; off += align_up(B * 4); }
+  for (int s = 0; s < 2; ++s) { L.counts[s] = off; off += align_up(TC * 4); }
+  L.omega = off; off += align_up(TC * 4);
+  L.slot_chain = off; off += align_up(n * 4);
+  L.slot_pattern = off; off += align_up(n);
+  L.patterns = off; off += align_up(pat_bytes);
+  L.accepted = off; off += align_up(8);
+  L.total = off;
+  return L;
+}
+
+bool is_pow2(uint32_t v) { return v && !(v & (v - 1)); }
+
+const char* validate(const soma_params* p) {
+  if (!p) return "params is NULL";
+  if (p->n_chains == 0 || p->n_chains >= (1ull << 32)) return "n_chains must be in [1, 2^32)";
+  if (p->beads_per_chain == 0 || p->beads_per_chain > 65535) return "beads_per_chain must be in [1, 65535]";
+  if (p->n_types == 0 || p->n_types > (uint32_t)kMaxTypes) return "n_types must be in [1, 8]";
+  if (p->n_patterns == 0 || p->n_patterns > 256) return "n_patterns must be in [1, 256]";
+  if (p->reserved0 || p->reserved1 != 0.0f || p->reserved2 || p->reserved3 != 0.0f) return "reserved fields must be 0";
+  if (!p->type_patterns) return "type_patterns is NULL";
+  if (!p->chiN) return "chiN is NULL";
+  if (!(p->b > 0.0f)) return "b must be > 0";
+  if (!(p->move_halfwidth >= 0.0f)) return "move_halfwidth must be >= 0";
+  if (!(p->kappaN == p->kappaN)) return "kappaN is NaN";
+  uint64_t cells = 1;
+  for (int d = 0; d < 3; ++d) {
+    if (p->grid[d] == 0 || p->grid[d] > (1u << 20)) return "grid[d] must be in [1, 2^20]";
+    if (!(p->box[d] > 0.0f)) return "box[d] must be > 0";
+    cells *= p->grid[d];
+    if (cells >= (1ull << 32)) return "too many cells";
+  }
+  if (cells * p->n_types >= (1ull << 32)) return "n_types * cells must be < 2^32";
+  const uint64_t npat = (uint64_t)p->n_patterns * p->beads_per_chain;
+  for (uint64_t k = 0; k < npat; ++k)
+    if (p->type_patterns[k] >= p->n_types) return "type_patterns holds a type >= n_types";
+  if (p->chain_pattern)
+    for (uint64_t c = 0; c < p->n_chains; ++c)
+      if (p->chain_pattern[c] >= p->n_patterns) return "chain_pattern holds an id >= n_patterns";
+  if (p->n_patterns > 1 && !p->chain_pattern) return "chain_pattern is NULL but n_patterns > 1";
+  const uint32_t T = p->n_types;
+  for (uint32_t s = 0; s < T; ++s)
+    for (uint32_t t = 0; t < T; ++t) {
+      const float v = p->chiN[s * T + t];
+      if (!(v == v)) return "chiN holds a NaN";
+      if (s == t && v != 0.0f) return "chiN diagonal must be 0";
+      if (v != p->chiN[t * T + s]) return "chiN must be symmetric";
+    }
+  return nullptr;
+}
+
+int fused_lanes(uint32_t N) {   // P = N/2 if the fused kernel supports N, else 0
+  if (N < 2 || (N & 1u)) return 0;
+  const uint32_t P = N / 2;
+  return (P <= 32 && is_pow2(P)) ? (int)P : 0;
+}
+
+}  // namespace
+
+struct soma_handle {
+  // problem
+  uint64_t n_chains, B;
+  uint32_t N, T, n_patterns, cells;
+  Grid grid;
+  bool pow2;
+  float a, kb, dens_scale, invN, kappaN;
+  float chiN[kMaxTypes * kMaxTypes];
+  uint64_t seed;
+  // device
+  int device;
+  cudaStream_t stream;
+  char* ws;
+  bool owns_ws;
+  Layout L;
+  int live;              // which position set is current
+  int cur;               // which count buffer holds the current densities
+  // state
+  bool loaded;
+  bool identity_order;   // slot_chain is the identity
+  uint64_t step;
+  int sm_count;
+  // options
+  int path;              // 0 auto, 1 generic, 2 fused
+  int64_t resort_interval;
+  // counters
+  uint64_t launches, steps_done, resorts;
+  bool sticky;
+  char err[256];
+
+  float* pos(int set, int d) const { return reinterpret_cast<float*>(ws + L.pos[set][d]); }
+  uint32_t* counts(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts[s]); }
+  float* omega() const { return reinterpret_cast<float*>(ws + L.omega); }
+  uint32_t* slot_chain() const { return reinterpret_cast<uint32_t*>(ws + L.slot_chain); }
+  uint8_t* slot_pattern() const { return reinterpret_cast<uint8_t*>(ws + L.slot_pattern); }
+  uint8_t* patterns() const { return reinterpret_cast<uint8_t*>(ws + L.patterns); }
+  unsigned long long* accepted() const { return reinterpret_cast<unsigned long long*>(ws + L.accepted); }
+};
+
+namespace {
+
+int fail(soma_handle* h, int code, const char* msg) {
+  snprintf(h ? h->err : g_last_error, 256, "%s", msg);
+  return code;
+}
+int cuda_fail(soma_handle* h, cudaError_t e, const char* where) {
+  char buf[256];
+  snprintf(buf, sizeof buf, "%s: %s", where, cudaGetErrorString(e));
+  if (h) h->sticky = true;
+  return fail(h, SOMA_ECUDA, buf);
+}
+#define CU(h, call)                                            \
+  do {                                                         \
+    cudaError_t e_ = (call);                                   \
+    if (e_ != cudaSuccess) return cuda_fail((h), e_, #call);   \
+  } while (0)
+
+inline unsigned blocks_for(uint64_t n, unsigned bs) { return (unsigned)((n + bs - 1) / bs); }
+
+StepArgs step_args(const soma_handle* h) {
+  StepArgs A{};
+  A.grid = h->grid;
+  A.cells = h->cells;
+  A.n_chains = (uint32_t)h->n_chains;
+  A.N = h->N;
+  A.a = h->a;
+  A.kb = h->kb;
+  A.key0 = (uint32_t)h->seed;
+  A.key1 = (uint32_t)(h->seed >> 32);
+  A.ctr2 = (uint32_t)h->step;
+  A.ctr3_base = (0u << 8) | ((uint32_t)(h->step >> 32) << 16);   // domain 0 = MC move
+  A.x = h->pos(h->live, 0);
+  A.y = h->pos(h->live, 1);
+  A.z = h->pos(h->live, 2);
+  A.omega = h->omega();
+  A.counts_next = h->counts(h->cur ^ 1);
+  A.slot_chain = h->slot_chain();
+  A.slot_pattern = h->slot_pattern();
+  A.patterns = h->patterns();
+  A.accepted = h->accepted();
+  return A;
+}
+
+int launch_half_sweep(soma_handle* h, uint32_t parity) {
+  const uint32_t n_par = (h->N + 1u - parity) / 2u;
+  if (n_par == 0) return SOMA_OK;                               // N == 1 has no odd beads
+  const uint64_t total = h->n_chains * n_par;
+  const StepArgs A = step_args(h);
+  if (h->pow2) half_sweep_kernel<true><<<blocks_for(total, 256), 256, 0, h->stream>>>(A, parity, n_par);
+  else half_sweep_kernel<false><<<blocks_for(total, 256), 256, 0, h->stream>>>(A, parity, n_par);
+  h->launches++;
+  CU(h, cudaGetLastError());
+  return SOMA_OK;
+}
+
+int launch_bin(soma_handle* h, uint32_t* counts) {
+  if (h->pow2)
+    bin_kernel<true><<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
+        h->grid, h->cells, h->N, h->B, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2),
+        h->slot_pattern(), h->patterns(), counts);
+  else
+    bin_kernel<false><<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
+        h->grid, h->cells, h->N, h->B, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2),
+        h->slot_pattern(), h->patterns(), counts);
+  h->launches++;
+  CU(h, cudaGetLastError());
+  return SOMA_OK;
+}
+
+// omega from counts(cur); zero counts(cur^1) for the next step's binning.
+int launch_omega(soma_handle* h) {
+  OmegaArgs A{};
+  A.cells = h->cells; A.T = h->T;
+  A.dens_scale = h->dens_scale; A.kappaN = h->kappaN; A.invN = h->invN;
+  std::memcpy(A.chiN, h->chiN, sizeof A.chiN);
+  A.counts = h->counts(h->cur);
+  A.counts_to_zero = h->counts(h->cur ^ 1);
+  A.omega = h->omega();
+  const unsigned g = blocks_for(h->cells, 256);
+  switch (h->T) {
+    case 1: omega_kernel<1><<<g, 256, 0, h->stream>>>(A); break;
+    case 2: omega_kernel<2><<<g, 256, 0, h->stream>>>(A); break;
+    case 3: omega_kernel<3><<<g, 256, 0, h->stream>>>(A); break;
+    default: omega_kernel<0><<<g, 256, 0, h->stream>>>(A); break;
+  }
+  h->launches++;
+  CU(h, cudaGetLastError());
+  return SOMA_OK;
+}
+
+template <int P>
+int launch_fused_p(soma_handle* h) {
+  const StepArgs A = step_args(h);
+  constexpr int G = 32 / P;
+  const uint64_t n_groups = (h->n_chains + G - 1) / G;           // warps of work
+  const unsigned bs = 256, wpb = bs / 32;
+  uint64_t blocks = (n_groups + wpb - 1) / wpb;
+  const uint64_t cap = (uint64_t)h->sm_count * 64;               // grid-stride beyond this
+  if (blocks > cap) blocks = cap;
+  if (h->pow2) fused_step_kernel<P, true><<<(unsigned)blocks, bs, 0, h->stream>>>(A);
+  else fused_step_kernel<P, false><<<(unsigned)blocks, bs, 0, h->stream>>>(A);
+  h->launches++;
+  CU(h, cudaGetLastError());
+  return SOMA_OK;
+}
+
+int launch_fused(soma_handle* h) {
+  switch (fused_lanes(h->N)) {
+    case 1: return launch_fused_p<1>(h);
+    case 2: return launch_fused_p<2>(h);
+    case 4: return launch_fused_p<4>(h);
+    case 8: return launch_fused_p<8>(h);
+    case 16: return launch_fused_p<16>(h);
+    case 32: return launch_fused_p<32>(h);
+  }
+  return fail(h, SOMA_EINVAL, "fused path does not support this beads_per_chain");
+}
+
+bool use_fused(const soma_handle* h) {
+  if (h->path == 1) return false;
+  return fused_lanes(h->N) != 0;
+}
+
+int one_step(soma_handle* h) {
+  int rc;
+  if (use_fused(h)) {
+    if ((rc = launch_fused(h)) != SOMA_OK) return rc;            // a1 + a2 + a3 (+a5)
+  } else {
+    if ((rc = launch_half_sweep(h, 0)) != SOMA_OK) return rc;    // a1
+    if ((rc = launch_half_sweep(h, 1)) != SOMA_OK) return rc;    // a2
+    if ((rc = launch_bin(h, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;   // a3
+  }
+  h->cur ^= 1;
+  if ((rc = launch_omega(h)) != SOMA_OK) return rc;              // a4
+  h->step += 1;
+  h->steps_done += 1;
+  return SOMA_OK;
+}
+
+int check(soma_handle* h) {
+  if (!h) return fail(nullptr, SOMA_EINVAL, "handle is NULL");
+  if (h->sticky) return SOMA_ECUDA;
+  CU(h, cudaSetDevice(h->device));
+  return SOMA_OK;
+}
+
+// copy [count] elements to the caller, host or device
+template <typename Tp>
+int copy_out(soma_handle* h, Tp* dst, const Tp* src, uint64_t count, int dst_is_device) {
+  CU(h, cudaMemcpyAsync(dst, src, count * sizeof(Tp),
+                        dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+  if (!dst_is_device) CU(h, cudaStreamSynchronize(h->stream));
+  return SOMA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+uint64_t soma_workspace_bytes(const soma_params* p) {
+  const char* bad = validate(p);
+  if (bad) { fail(nullptr, SOMA_EINVAL, bad); return 0; }
+  const uint64_t B = p->n_chains * p->beads_per_chain;
+  const uint64_t TC = (uint64_t)p->grid[0] * p->grid[1] * p->grid[2] * p->n_types;
+  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain).total;
+}
+
+int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
+  if (!out) return fail(nullptr, SOMA_EINVAL, "out is NULL");
+  *out = nullptr;
+  const char* bad = validate(p);
+  if (bad) return fail(nullptr, SOMA_EINVAL, bad);
+  soma_handle* h = new (std::nothrow) soma_handle();
+  if (!h) return fail(nullptr, SOMA_ENOMEM, "host allocation failed");
+  std::memset(static_cast<void*>(h), 0, sizeof *h);
+  cudaError_t e = cudaGetDevice(&h->device);
+  cudaDeviceProp prop{};
+  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, h->device);
+  if (e != cudaSuccess) {
+    snprintf(g_last_error, 256, "no usable CUDA device: %s", cudaGetErrorString(e));
+    delete h;
+    return SOMA_ECUDA;
+  }
+  if (prop.major != 10) {
+    snprintf(g_last_error, 256, "device is sm_%d%d; this library holds sm_100a code only", prop.major, prop.minor);
+    delete h;
+    return SOMA_ECUDA;
+  }
+  h->sm_count = prop.multiProcessorCount;
+  h->stream = static_cast<cudaStream_t>(cuda_stream);
+  h->n_chains = p->n_chains; h->N = p->beads_per_chain; h->T = p->n_types; h->n_patterns = p->n_patterns;
+  h->B = h->n_chains * h->N;
+  h->cells = p->grid[0] * p->grid[1] * p->grid[2];
+  h->grid.nx = p->grid[0]; h->grid.ny = p->grid[1]; h->grid.nz = p->grid[2];
+  h->grid.inv_hx = (float)p->grid[0] / p->box[0];
+  h->grid.inv_hy = (float)p->grid[1] / p->box[1];
+  h->grid.inv_hz = (float)p->grid[2] / p->box[2];
+  h->pow2 = is_pow2(p->grid[0]) && is_pow2(p->grid[1]) && is_pow2(p->grid[2]);
+  h->a = p->move_halfwidth;
+  h->kb = 1.5f / (p->b * p->b);
+  h->dens_scale = (float)((double)h->cells / (double)h->B);
+  h->invN = 1.0f / (float)h->N;
+  h->kappaN = p->kappaN;
+  for (uint32_t k = 0; k < h->T * h->T; ++k) h->chiN[k] = p->chiN[k];
+  h->seed = p->seed;
+  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N);
+  if (p->workspace) {
+    if (p->workspace_bytes < h->L.total || (reinterpret_cast<uintptr_t>(p->workspace) % kAlign)) {
+      delete h;
+      return fail(nullptr, SOMA_ENOMEM, "lent workspace is too small or not 256-byte aligned");
+    }
+    h->ws = static_cast<char*>(p->workspace);
+    h->owns_ws = false;
+  } else {
+    void* ptr = nullptr;
+    e = cudaMalloc(&ptr, h->L.total);
+    if (e != cudaSuccess) {
+      snprintf(g_last_error, 256, "cudaMalloc(%llu bytes): %s", (unsigned long long)h->L.total, cudaGetErrorString(e));
+      cudaGetLastError();
+      delete h;
+      return SOMA_ENOMEM;
+    }
+    h->ws = static_cast<char*>(ptr);
+    h->owns_ws = true;
+  }
+  // chain tables: identity slot order; pattern id per slot; pattern table
+  auto bail = [&](cudaError_t err, const char* where) {
+    snprintf(g_last_error, 256, "%s: %s", where, cudaGetErrorString(err));
+    if (h->owns_ws) cudaFree(h->ws);
+    delete h;
+    return SOMA_ECUDA;
+  };
+  iota_kernel<<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>((uint32_t)h->n_chains, h->slot_chain());
+  h->launches++;
+  if ((e = cudaGetLastError()) != cudaSuccess) return bail(e, "iota_kernel");
+  if (p->chain_pattern) e = cudaMemcpyAsync(h->slot_pattern(), p->chain_pattern, h->n_chains, cudaMemcpyHostToDevice, h->stream);
+  else e = cudaMemsetAsync(h->slot_pattern(), 0, h->n_chains, h->stream);
+  if (e != cudaSuccess) return bail(e, "chain_pattern upload");
+  e = cudaMemcpyAsync(h->patterns(), p->type_patterns, (size_t)h->n_patterns * h->N, cudaMemcpyHostToDevice, h->stream);
+  if (e != cudaSuccess) return bail(e, "type_patterns upload");
+  if ((e = cudaStreamSynchronize(h->stream)) != cudaSuccess) return bail(e, "create sync");   // host buffers may go away
+  h->identity_order = true;
+  h->path = 0;
+  h->resort_interval = 0;
+  *out = h;
+  return SOMA_OK;
+}
+
+int soma_load_state(soma_t* h, const float* x, const float* y, const float* z, uint64_t step0, int dev) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!x || !y || !z) return fail(h, SOMA_EINVAL, "position pointer is NULL");
+  if (step0 >= (1ull << 48)) return fail(h, SOMA_EINVAL, "step0 must be < 2^48");
+  const cudaMemcpyKind kind = dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  h->live = 0;
+  const float* src[3] = {x, y, z};
+  for (int d = 0; d < 3; ++d) CU(h, cudaMemcpyAsync(h->pos(0, d), src[d], h->B * 4, kind, h->stream));
+  h->step = step0;
+  h->cur = 0;
+  CU(h, cudaMemsetAsync(h->counts(0), 0, (size_t)h->cells * h->T * 4, h->stream));
+  if ((rc = launch_bin(h, h->counts(0))) != SOMA_OK) return rc;
+  if ((rc = launch_omega(h)) != SOMA_OK) return rc;     // also zeroes counts(1)
+  if (!dev) CU(h, cudaStreamSynchronize(h->stream));    // the caller may reuse its host buffers
+  h->loaded = true;
+  return SOMA_OK;
+}
+
+int soma_mc_steps(soma_t* h, uint32_t n_steps, uint64_t* accepted) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!h->loaded) return fail(h, SOMA_ESTATE, "soma_mc_steps before soma_load_state");
+  if (h->step + n_steps >= (1ull << 48)) return fail(h, SOMA_EINVAL, "step index would reach 2^48");
+  CU(h, cudaMemsetAsync(h->accepted(), 0, 8, h->stream));
+  for (uint32_t s = 0; s < n_steps; ++s)
+    if ((rc = one_step(h)) != SOMA_OK) return rc;
+  if (accepted) {
+    unsigned long long v = 0;
+    CU(h, cudaMemcpyAsync(&v, h->accepted(), 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    *accepted = v;
+  }
+  return SOMA_OK;
+}
+
+int soma_get_density(soma_t* h, uint32_t* counts, int dev) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!counts) return fail(h, SOMA_EINVAL, "counts is NULL");
+  if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
+  return copy_out(h, counts, h->counts(h->cur), (uint64_t)h->cells * h->T, dev);
+}
+
+int soma_get_omega(soma_t* h, float* omega, int dev) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!omega) return fail(h, SOMA_EINVAL, "omega is NULL");
+  if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
+  return copy_out(h, omega, h->omega(), (uint64_t)h->cells * h->T, dev);
+}
+
+int soma_get_positions(soma_t* h, float* x, float* y, float* z, int dev) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!x || !y || !z) return fail(h, SOMA_EINVAL, "position pointer is NULL");
+  if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
+  float* dst[3] = {x, y, z};
+  int set = h->live;
+  if (!h->identity_order) {      // back to the caller's chain order through the staging set
+    set = h->live ^ 1;
+    unpermute_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
+        h->B, h->N, h->slot_chain(), h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2),
+        h->pos(set, 0), h->pos(set, 1), h->pos(set, 2));
+    h->launches++;
+    CU(h, cudaGetLastError());
+  }
+  for (int d = 0; d < 3; ++d)
+    CU(h, cudaMemcpyAsync(dst[d], h->pos(set, d), h->B * 4,
+                          dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+  if (!dev) CU(h, cudaStreamSynchronize(h->stream));
+  return SOMA_OK;
+}
+
+int soma_get_step(soma_t* h, uint64_t* step) {
+  if (!h || !step) return fail(h, SOMA_EINVAL, "NULL argument");
+  *step = h->step;
+  return SOMA_OK;
+}
+
+int soma_destroy(soma_t* h) {
+  if (!h) return SOMA_OK;
+  cudaSetDevice(h->device);
+  cudaStreamSynchronize(h->stream);
+  if (h->owns_ws) cudaFree(h->ws);
+  delete h;
+  return SOMA_OK;
+}
+
+const char* soma_last_error(const soma_t* h) { return h ? h->err : g_last_error; }
+
+int soma_set_option(soma_t* h, const char* name, int64_t value) {
+  if (!h || !name) return fail(h, SOMA_EINVAL, "NULL argument");
+  if (!std::strcmp(name, "path")) {
+    if (value < 0 || value > 2) return fail(h, SOMA_EINVAL, "path must be 0, 1 or 2");
+    if (value == 2 && !fused_lanes(h->N))
+      return fail(h, SOMA_EINVAL, "fused path needs beads_per_chain = 2P, P a power of two <= 32");
+    h->path = (int)value;
+    return SOMA_OK;
+  }
+  if (!std::strcmp(name, "resort_interval")) {
+    if (value != 0) return fail(h, SOMA_EINVAL, "chain re-ordering is not available in this build");
+    h->resort_interval = value;
+    return SOMA_OK;
+  }
+  return fail(h, SOMA_EINVAL, "unknown option name");
+}
+
+int soma_get_counters(const soma_t* h, uint64_t* out) {
+  if (!h || !out) return SOMA_EINVAL;
+  out[0] = h->launches; out[1] = h->steps_done; out[2] = h->resorts;
+  return SOMA_OK;
+}
+
+// ---- test hooks ----------------------------------------------------------------------------------
+
+int soma_debug_half_sweep(soma_t* h, uint32_t parity, uint64_t* accepted) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
+  if (parity > 1) return fail(h, SOMA_EINVAL, "parity must be 0 or 1");
+  CU(h, cudaMemsetAsync(h->accepted(), 0, 8, h->stream));
+  if ((rc = launch_half_sweep(h, parity)) != SOMA_OK) return rc;
+  if (accepted) {
+    unsigned long long v = 0;
+    CU(h, cudaMemcpyAsync(&v, h->accepted(), 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    *accepted = v;
+  }
+  return SOMA_OK;
+}
+
+int soma_debug_finish_step(soma_t* h) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
+  if ((rc = launch_bin(h, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;
+  h->cur ^= 1;
+  if ((rc = launch_omega(h)) != SOMA_OK) return rc;
+  h->step += 1;
+  return SOMA_OK;
+}
+
+int soma_debug_set_omega(soma_t* h, const float* omega) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!omega) return fail(h, SOMA_EINVAL, "omega is NULL");
+  CU(h, cudaMemcpyAsync(h->omega(), omega, (size_t)h->cells * h->T * 4, cudaMemcpyHostToDevice, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  return SOMA_OK;
+}
+
+namespace {
+struct DevBuf {                       // tiny RAII device buffer for the debug entry points
+  void* p = nullptr;
+  cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 1); }
+  ~DevBuf() { if (p) cudaFree(p); }
+};
+#define CUG(call)                                                                   \
+  do {                                                                              \
+    cudaError_t e_ = (call);                                                        \
+    if (e_ != cudaSuccess) {                                                        \
+      snprintf(g_last_error, 256, "%s: %s", #call, cudaGetErrorString(e_));         \
+      return SOMA_ECUDA;                                                            \
+    }                                                                               \
+  } while (0)
+}  // namespace
+
+int soma_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, uint64_t n) {
+  if (!ctr || !key || !out) return fail(nullptr, SOMA_EINVAL, "NULL argument");
+  if (n == 0) return SOMA_OK;
+  DevBuf c, o;
+  CUG(c.alloc(n * 16)); CUG(o.alloc(n * 16));
+  CUG(cudaMemcpy(c.p, ctr, n * 16, cudaMemcpyHostToDevice));
+  debug_philox_kernel<<<blocks_for(n, 256), 256>>>(n, (const uint32_t*)c.p, key[0], key[1], (uint32_t*)o.p);
+  CUG(cudaGetLastError());
+  CUG(cudaMemcpy(out, o.p, n * 16, cudaMemcpyDeviceToHost));
+  return SOMA_OK;
+}
+
+int soma_debug_maps(const uint32_t* words, float* t, float* u, float* lnu, uint64_t n) {
+  if (!words || !t || !u || !lnu) return fail(nullptr, SOMA_EINVAL, "NULL argument");
+  if (n == 0) return SOMA_OK;
+  DevBuf w, a, b, c;
+  CUG(w.alloc(n * 4)); CUG(a.alloc(n * 4)); CUG(b.alloc(n * 4)); CUG(c.alloc(n * 4));
+  CUG(cudaMemcpy(w.p, words, n * 4, cudaMemcpyHostToDevice));
+  debug_maps_kernel<<<blocks_for(n, 256), 256>>>(n, (const uint32_t*)w.p, (float*)a.p, (float*)b.p, (float*)c.p);
+  CUG(cudaGetLastError());
+  CUG(cudaMemcpy(t, a.p, n * 4, cudaMemcpyDeviceToHost));
+  CUG(cudaMemcpy(u, b.p, n * 4, cudaMemcpyDeviceToHost));
+  CUG(cudaMemcpy(lnu, c.p, n * 4, cudaMemcpyDeviceToHost));
+  return SOMA_OK;
+}
+
+int soma_debug_accept(const float* dE, const uint32_t* words, uint8_t* decision, uint64_t n) {
+  if (!dE || !words || !decision) return fail(nullptr, SOMA_EINVAL, "NULL argument");
+  if (n == 0) return SOMA_OK;
+  DevBuf e, w, d;
+  CUG(e.alloc(n * 4)); CUG(w.alloc(n * 4)); CUG(d.alloc(n));
+  CUG(cudaMemcpy(e.p, dE, n * 4, cudaMemcpyHostToDevice));
+  CUG(cudaMemcpy(w.p, words, n * 4, cudaMemcpyHostToDevice));
+  debug_accept_kernel<<<blocks_for(n, 256), 256>>>(n, (const float*)e.p, (const uint32_t*)w.p, (uint8_t*)d.p);
+  CUG(cudaGetLastError());
+  CUG(cudaMemcpy(decision, d.p, n, cudaMemcpyDeviceToHost));
+  return SOMA_OK;
+}
+
+int soma_debug_cell_index(soma_t* h, const float* x, const float* y, const float* z, uint32_t* cell, uint64_t n) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!x || !y || !z || !cell) return fail(h, SOMA_EINVAL, "NULL argument");
+  if (n == 0) return SOMA_OK;
+  DevBuf a, b, c, o;
+  CUG(a.alloc(n * 4)); CUG(b.alloc(n * 4)); CUG(c.alloc(n * 4)); CUG(o.alloc(n * 4));
+  CUG(cudaMemcpy(a.p, x, n * 4, cudaMemcpyHostToDevice));
+  CUG(cudaMemcpy(b.p, y, n * 4, cudaMemcpyHostToDevice));
+  CUG(cudaMemcpy(c.p, z, n * 4, cudaMemcpyHostToDevice));
+  if (h->pow2) debug_cell_kernel<true><<<blocks_for(n, 256), 256>>>(h->grid, n, (float*)a.p, (float*)b.p, (float*)c.p, (uint32_t*)o.p);
+  else debug_cell_kernel<false><<<blocks_for(n, 256), 256>>>(h->grid, n, (float*)a.p, (float*)b.p, (float*)c.p, (uint32_t*)o.p);
+  CUG(cudaGetLastError());
+  CUG(cudaMemcpy(cell, o.p, n * 4, cudaMemcpyDeviceToHost));
+  return SOMA_OK;
+}
+
+}  // extern "C"

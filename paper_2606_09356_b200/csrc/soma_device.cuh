@@ -1,0 +1,110 @@
+// soma_device.cuh -- per-move device arithmetic of the SCMF Monte-Carlo step.
+//
+// Everything here is fp32 with the operation order of DESIGN.md section 2 spelled out through
+// __f*_rn intrinsics (never contracted by the compiler), so that the result of every move is
+// bit-identical to the definition regardless of optimisation level.  No code is shared with oracle/.
+#pragma once
+
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace soma {
+
+// ---- Philox4x32-10 (R13; `north_star`: keyed by (seed, step, half-sweep, chain, bead)) ----
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u;
+constexpr uint32_t kPhiloxM1 = 0xCD9E8D57u;
+constexpr uint32_t kPhiloxW0 = 0x9E3779B9u;
+constexpr uint32_t kPhiloxW1 = 0xBB67AE85u;
+
+struct Words4 { uint32_t w0, w1, w2, w3; };
+
+__device__ __forceinline__ Words4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(kPhiloxM0, c0), lo0 = kPhiloxM0 * c0;
+    const uint32_t hi1 = __umulhi(kPhiloxM1, c2), lo1 = kPhiloxM1 * c2;
+    c0 = hi1 ^ c1 ^ k0;
+    c1 = lo1;
+    c2 = hi0 ^ c3 ^ k1;
+    c3 = lo0;
+    k0 += kPhiloxW0;
+    k1 += kPhiloxW1;
+  }
+  return Words4{c0, c1, c2, c3};
+}
+
+// ---- uniform maps (R14) ----
+// tmap(w) = (2k+1) 2^-23 - 1 with k = w >> 9.  Built from the bit pattern instead of an int->float
+// conversion: as_float(0x3f800000 | k) - 1 = k 2^-23 exactly, then fma(2, ., 2^-23 - 1) is exact
+// because the result (an odd multiple of 2^-23 below 1 in magnitude) is representable.
+__device__ __forceinline__ float tmap(uint32_t w) {
+  const float h = __fadd_rn(__uint_as_float(0x3f800000u | (w >> 9)), -1.0f);
+  return __fmaf_rn(2.0f, h, -0.99999988079071044921875f);   // 2^-23 - 1
+}
+// u = ((w >> 8) + 1) 2^-24 in (0, 1]; the integer (w >> 8) + 1 <= 2^24 converts exactly.
+__device__ __forceinline__ float umap_int(uint32_t w) { return (float)((w >> 8) + 1u); }   // = u * 2^24
+__device__ __forceinline__ float umap(uint32_t w) { return __fmul_rn(umap_int(w), 0x1p-24f); }
+
+// lnu = ln(u) correctly rounded to fp32 (R6b), slow path: double log, one rounding.
+__device__ __noinline__ float lnu_exact(float u) { return (float)log((double)u); }
+
+// ---- Metropolis decision (DESIGN.md section 2 step 5.6): accept iff fl32(dE + lnu) <= 0 ----
+// Result-equivalent shortcuts:
+//  * dE <= 0: lnu <= 0, so the fp32 sum is <= 0 -> accept without looking at u.
+//  * otherwise m~ = dE + ln2*(log2(k) - 24) with the hardware log2 (absolute error of ln u below
+//    6e-6 over k in [1, 2^24]); if |m~| > 1e-4 the sign of the exact margin
+//    is the sign of m~.  Only the ~6e-5 of moves inside that band take the double-precision path.
+__device__ __forceinline__ bool metropolis_accept(float dE, uint32_t w3) {
+  if (dE <= 0.0f) return true;
+  const float kf = umap_int(w3);
+  const float l2 = __fadd_rn(__log2f(kf), -24.0f);
+  const float m_fast = __fmaf_rn(l2, 0.693147182464599609375f, dE);
+  if (fabsf(m_fast) > 1.0e-4f) return m_fast < 0.0f;
+  const float m = __fadd_rn(dE, lnu_exact(__fmul_rn(kf, 0x1p-24f)));
+  return m <= 0.0f;
+}
+
+// ---- geometry ----
+struct Grid {
+  uint32_t nx, ny, nz;          // cells per axis
+  float inv_hx, inv_hy, inv_hz; // (float)grid[d]/box[d]
+};
+
+template <bool POW2>
+__device__ __forceinline__ uint32_t wrap(int g, uint32_t n) {
+  if (POW2) return (uint32_t)g & (n - 1u);          // two's complement: the non-negative residue
+  if ((uint32_t)g >= n) {                           // rare: bead outside the primary box
+    g %= (int)n;
+    if (g < 0) g += (int)n;
+  }
+  return (uint32_t)g;
+}
+
+// DESIGN.md section 2 step 1 (R8, R12).  cvt.rmi.s32.f32 = floor then convert.
+template <bool POW2>
+__device__ __forceinline__ uint32_t cell_of(const Grid& g, float x, float y, float z) {
+  const uint32_t ix = wrap<POW2>(__float2int_rd(__fmul_rn(x, g.inv_hx)), g.nx);
+  const uint32_t iy = wrap<POW2>(__float2int_rd(__fmul_rn(y, g.inv_hy)), g.ny);
+  const uint32_t iz = wrap<POW2>(__float2int_rd(__fmul_rn(z, g.inv_hz)), g.nz);
+  return (ix * g.ny + iy) * g.nz + iz;
+}
+
+// squared bond length, DESIGN.md section 2 step 5.4: fma(sz,sz, fma(sy,sy, sx*sx))
+__device__ __forceinline__ float bond_sq(float ax, float ay, float az, float bx, float by, float bz) {
+  const float sx = __fsub_rn(ax, bx), sy = __fsub_rn(ay, by), sz = __fsub_rn(az, bz);
+  return __fmaf_rn(sz, sz, __fmaf_rn(sy, sy, __fmul_rn(sx, sx)));
+}
+
+struct Trial { float x, y, z; };
+
+// DESIGN.md section 2 steps 5.1-5.3: the trial position of bead (chain c, index i).
+__device__ __forceinline__ Trial trial_position(float rx, float ry, float rz, float a, const Words4& w) {
+  Trial t;
+  t.x = __fadd_rn(rx, __fmul_rn(a, tmap(w.w0)));
+  t.y = __fadd_rn(ry, __fmul_rn(a, tmap(w.w1)));
+  t.z = __fadd_rn(rz, __fmul_rn(a, tmap(w.w2)));
+  return t;
+}
+
+}  // namespace soma

@@ -1,0 +1,260 @@
+// soma_kernels.cuh -- sm_100a kernels of the SCMF Monte-Carlo step (DESIGN.md sections 6-7).
+//
+//   fused_step_kernel<P>   rows a1+a2+a3+a5: a chain lives in the registers of P = N/2 lanes (two
+//                          consecutive beads per lane), both half-sweeps run there with warp
+//                          shuffles for the cross-lane neighbours, positions are read once and
+//                          written once, and every bead is binned into the next density grid with
+//                          one red.global.add.u32.
+//   half_sweep_kernel      rows a1/a2 for any N (one thread per same-parity bead, neighbours from
+//                          global memory); bin_kernel = row a3.  The generic path.
+//   omega_kernel<T>        row a4: omega from the fresh counts; also zeroes the other count buffer.
+#pragma once
+
+#include "soma_device.cuh"
+
+namespace soma {
+
+constexpr int kMaxTypes = 8;
+
+// Everything a move needs, passed by value as a kernel parameter.
+struct StepArgs {
+  Grid grid;
+  uint32_t cells;             // C
+  uint32_t n_chains;          // n
+  uint32_t N;                 // beads per chain
+  float a;                    // trial half-width
+  float kb;                   // 1.5f/(b*b)
+  uint32_t key0, key1;        // Philox key = (seed lo, seed hi)
+  uint32_t ctr2;              // (uint32) step
+  uint32_t ctr3_base;         // domain << 8 | (uint32)(step >> 32) << 16; parity is or-ed in
+  float* __restrict__ x;      // positions in slot order: bead i of slot s at s*N + i
+  float* __restrict__ y;
+  float* __restrict__ z;
+  const float* __restrict__ omega;          // [T][C], field of the previous step
+  uint32_t* __restrict__ counts_next;       // [T][C], zeroed, receives this step's binning
+  const uint32_t* __restrict__ slot_chain;  // [n] logical chain id held by each slot
+  const uint8_t* __restrict__ slot_pattern; // [n] pattern id of that chain
+  const uint8_t* __restrict__ patterns;     // [n_patterns][N]
+  unsigned long long* __restrict__ accepted;
+};
+
+// One Metropolis trial move given the bead's position and its (up to two) bonded neighbours.
+// Returns the accept decision; on accept (rx,ry,rz) and `cell` are replaced by the trial values.
+template <bool POW2>
+__device__ __forceinline__ bool move_bead(const StepArgs& A, uint32_t chain, uint32_t i, uint32_t parity,
+                                          const float* __restrict__ omega_t,   // omega + type*C
+                                          float& rx, float& ry, float& rz, uint32_t& cell,
+                                          bool has_l, float lx, float ly, float lz,
+                                          bool has_r, float qx, float qy, float qz) {
+  const Words4 w = philox4x32_10(i, chain, A.ctr2, A.ctr3_base | parity, A.key0, A.key1);
+  const Trial t = trial_position(rx, ry, rz, A.a, w);
+  float dq = 0.0f;
+  if (has_l) dq = __fsub_rn(bond_sq(t.x, t.y, t.z, lx, ly, lz), bond_sq(rx, ry, rz, lx, ly, lz));
+  if (has_r) {
+    const float dqr = __fsub_rn(bond_sq(t.x, t.y, t.z, qx, qy, qz), bond_sq(rx, ry, rz, qx, qy, qz));
+    dq = has_l ? __fadd_rn(dq, dqr) : dqr;
+  }
+  const uint32_t cell_new = cell_of<POW2>(A.grid, t.x, t.y, t.z);
+  const float dw = __fsub_rn(__ldg(omega_t + cell_new), __ldg(omega_t + cell));
+  const float dE = __fmaf_rn(A.kb, dq, dw);
+  const bool acc = metropolis_accept(dE, w.w3);
+  if (acc) { rx = t.x; ry = t.y; rz = t.z; cell = cell_new; }
+  return acc;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Generic path: one thread per bead of the given parity.
+// ---------------------------------------------------------------------------------------------
+template <bool POW2>
+__global__ void __launch_bounds__(256)
+half_sweep_kernel(StepArgs A, uint32_t parity, uint32_t n_par /* beads of this parity per chain */) {
+  const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const uint64_t total = (uint64_t)A.n_chains * n_par;
+  bool acc = false;
+  if (k < total) {
+    const uint32_t slot = (uint32_t)(k / n_par);
+    const uint32_t i = parity + 2u * (uint32_t)(k % n_par);
+    const uint64_t j = (uint64_t)slot * A.N + i;
+    const uint32_t chain = A.slot_chain[slot];
+    const uint32_t type = A.patterns[(uint32_t)A.slot_pattern[slot] * A.N + i];
+    float rx = A.x[j], ry = A.y[j], rz = A.z[j];
+    const bool has_l = i > 0, has_r = i + 1 < A.N;
+    float lx = 0, ly = 0, lz = 0, qx = 0, qy = 0, qz = 0;
+    if (has_l) { lx = A.x[j - 1]; ly = A.y[j - 1]; lz = A.z[j - 1]; }
+    if (has_r) { qx = A.x[j + 1]; qy = A.y[j + 1]; qz = A.z[j + 1]; }
+    uint32_t cell = cell_of<POW2>(A.grid, rx, ry, rz);
+    acc = move_bead<POW2>(A, chain, i, parity, A.omega + (size_t)type * A.cells, rx, ry, rz, cell,
+                          has_l, lx, ly, lz, has_r, qx, qy, qz);
+    if (acc) { A.x[j] = rx; A.y[j] = ry; A.z[j] = rz; }
+  }
+  const unsigned n_acc = __popc(__ballot_sync(0xffffffffu, acc));
+  if ((threadIdx.x & 31u) == 0 && n_acc) atomicAdd(A.accepted, (unsigned long long)n_acc);
+}
+
+template <bool POW2>
+__global__ void __launch_bounds__(256)
+bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint64_t B, const float* __restrict__ x,
+           const float* __restrict__ y, const float* __restrict__ z,
+           const uint8_t* __restrict__ slot_pattern, const uint8_t* __restrict__ patterns,
+           uint32_t* __restrict__ counts) {
+  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= B) return;
+  const uint32_t slot = (uint32_t)(j / N), i = (uint32_t)(j % N);
+  const uint32_t type = patterns[(uint32_t)slot_pattern[slot] * N + i];
+  atomicAdd(counts + (size_t)type * cells + cell_of<POW2>(grid, x[j], y[j], z[j]), 1u);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused path: N = 2P, P in {1,2,4,8,16,32}.  Lane l of a P-lane group holds beads 2l and 2l+1.
+// A warp carries 32/P chains; warps walk the slot list with a grid stride.
+// ---------------------------------------------------------------------------------------------
+template <int P, bool POW2>
+__global__ void __launch_bounds__(256)
+fused_step_kernel(StepArgs A) {
+  constexpr int G = 32 / P;                                   // chains per warp
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t l = lane % P;                                // position of the lane in its chain
+  const uint32_t warps_per_block = blockDim.x >> 5;
+  const uint64_t warp0 = (uint64_t)blockIdx.x * warps_per_block + (threadIdx.x >> 5);
+  const uint64_t n_warps = (uint64_t)gridDim.x * warps_per_block;
+  const uint64_t n_groups = ((uint64_t)A.n_chains + G - 1) / G;
+  unsigned n_acc = 0;
+
+  for (uint64_t wg = warp0; wg < n_groups; wg += n_warps) {
+    const uint64_t slot64 = wg * G + lane / P;
+    const bool live = slot64 < A.n_chains;
+    const uint32_t slot = live ? (uint32_t)slot64 : 0u;       // dead lanes shadow slot 0, never store
+    const uint64_t j = (uint64_t)slot * A.N + 2u * l;
+    const float2 X = *reinterpret_cast<const float2*>(A.x + j);
+    const float2 Y = *reinterpret_cast<const float2*>(A.y + j);
+    const float2 Z = *reinterpret_cast<const float2*>(A.z + j);
+    const uint32_t chain = A.slot_chain[slot];
+    const uint8_t* pat = A.patterns + (uint32_t)A.slot_pattern[slot] * A.N + 2u * l;
+    const uint32_t type0 = pat[0], type1 = pat[1];
+    const float* om0 = A.omega + (size_t)type0 * A.cells;
+    const float* om1 = A.omega + (size_t)type1 * A.cells;
+
+    float ex = X.x, ey = Y.x, ez = Z.x;                       // even bead 2l
+    float ox = X.y, oy = Y.y, oz = Z.y;                       // odd bead 2l+1
+    uint32_t cell_e = cell_of<POW2>(A.grid, ex, ey, ez);
+    uint32_t cell_o = cell_of<POW2>(A.grid, ox, oy, oz);
+
+    // half-sweep 0: even bead; left neighbour = odd bead of lane l-1, right neighbour = own odd bead
+    {
+      const float lx = __shfl_up_sync(0xffffffffu, ox, 1, P);
+      const float ly = __shfl_up_sync(0xffffffffu, oy, 1, P);
+      const float lz = __shfl_up_sync(0xffffffffu, oz, 1, P);
+      const bool acc = move_bead<POW2>(A, chain, 2u * l, 0u, om0, ex, ey, ez, cell_e,
+                                       l > 0, lx, ly, lz, true, ox, oy, oz);
+      n_acc += (acc && live) ? 1u : 0u;
+    }
+    // half-sweep 1: odd bead; left = own even bead (new), right = even bead of lane l+1 (new)
+    {
+      const float qx = __shfl_down_sync(0xffffffffu, ex, 1, P);
+      const float qy = __shfl_down_sync(0xffffffffu, ey, 1, P);
+      const float qz = __shfl_down_sync(0xffffffffu, ez, 1, P);
+      const bool acc = move_bead<POW2>(A, chain, 2u * l + 1u, 1u, om1, ox, oy, oz, cell_o,
+                                       true, ex, ey, ez, l + 1 < P, qx, qy, qz);
+      n_acc += (acc && live) ? 1u : 0u;
+    }
+    if (live) {
+      *reinterpret_cast<float2*>(A.x + j) = make_float2(ex, ox);
+      *reinterpret_cast<float2*>(A.y + j) = make_float2(ey, oy);
+      *reinterpret_cast<float2*>(A.z + j) = make_float2(ez, oz);
+      atomicAdd(A.counts_next + (size_t)type0 * A.cells + cell_e, 1u);
+      atomicAdd(A.counts_next + (size_t)type1 * A.cells + cell_o, 1u);
+    }
+  }
+  // accepted-move count: warp reduce, one atomic per warp
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) n_acc += __shfl_xor_sync(0xffffffffu, n_acc, o);
+  if (lane == 0 && n_acc) atomicAdd(A.accepted, (unsigned long long)n_acc);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Row a4: omega from the counts (DESIGN.md section 2 step 3).  One thread per cell; the same pass
+// zeroes the count buffer the next step will bin into.
+// ---------------------------------------------------------------------------------------------
+struct OmegaArgs {
+  uint32_t cells, T;
+  float dens_scale, kappaN, invN;
+  float chiN[kMaxTypes * kMaxTypes];         // [T][T]
+  const uint32_t* __restrict__ counts;       // [T][C] fresh counts
+  uint32_t* __restrict__ counts_to_zero;     // [T][C] buffer for the next step (may be null)
+  float* __restrict__ omega;                 // [T][C]
+};
+
+template <int T_>
+__global__ void __launch_bounds__(256)
+omega_kernel(OmegaArgs A) {
+  const uint32_t T = T_ > 0 ? (uint32_t)T_ : A.T;
+  const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= A.cells) return;
+  float phi[kMaxTypes];
+  float tot = 0.0f;
+#pragma unroll
+  for (uint32_t s = 0; s < (T_ > 0 ? T_ : kMaxTypes); ++s) {
+    if (s < T) {
+      phi[s] = __fmul_rn((float)A.counts[(size_t)s * A.cells + c], A.dens_scale);
+      tot = s == 0 ? phi[0] : __fadd_rn(tot, phi[s]);
+      if (A.counts_to_zero) A.counts_to_zero[(size_t)s * A.cells + c] = 0u;
+    }
+  }
+  const float p = __fmul_rn(A.kappaN, __fsub_rn(tot, 1.0f));
+#pragma unroll
+  for (uint32_t t = 0; t < (T_ > 0 ? T_ : kMaxTypes); ++t) {
+    if (t < T) {
+      float acc = p;
+#pragma unroll
+      for (uint32_t s = 0; s < (T_ > 0 ? T_ : kMaxTypes); ++s)
+        if (s < T && s != t) acc = __fmaf_rn(A.chiN[t * T + s], phi[s], acc);
+      A.omega[(size_t)t * A.cells + c] = __fmul_rn(A.invN, acc);
+    }
+  }
+}
+
+// ---- data movement helpers ----
+// dst[slot_chain[s]*N + i] = src[s*N + i]  (slot order -> caller's chain order), one thread per bead
+__global__ void __launch_bounds__(256)
+unpermute_kernel(uint64_t B, uint32_t N, const uint32_t* __restrict__ slot_chain,
+                 const float* __restrict__ sx, const float* __restrict__ sy, const float* __restrict__ sz,
+                 float* __restrict__ dx, float* __restrict__ dy, float* __restrict__ dz) {
+  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= B) return;
+  const uint32_t slot = (uint32_t)(j / N), i = (uint32_t)(j % N);
+  const uint64_t d = (uint64_t)slot_chain[slot] * N + i;
+  dx[d] = sx[j]; dy[d] = sy[j]; dz[d] = sz[j];
+}
+
+__global__ void __launch_bounds__(256)
+iota_kernel(uint32_t n, uint32_t* __restrict__ out) {
+  const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < n) out[k] = k;
+}
+
+// ---- test hooks ----
+__global__ void debug_philox_kernel(uint64_t n, const uint32_t* ctr, uint32_t k0, uint32_t k1, uint32_t* out) {
+  const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const Words4 w = philox4x32_10(ctr[4 * k], ctr[4 * k + 1], ctr[4 * k + 2], ctr[4 * k + 3], k0, k1);
+  out[4 * k] = w.w0; out[4 * k + 1] = w.w1; out[4 * k + 2] = w.w2; out[4 * k + 3] = w.w3;
+}
+__global__ void debug_maps_kernel(uint64_t n, const uint32_t* words, float* t, float* u, float* lnu) {
+  const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  t[k] = tmap(words[k]);
+  u[k] = umap(words[k]);
+  lnu[k] = lnu_exact(umap(words[k]));
+}
+__global__ void debug_accept_kernel(uint64_t n, const float* dE, const uint32_t* words, uint8_t* out) {
+  const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  out[k] = metropolis_accept(dE[k], words[k]) ? 1 : 0;
+}
+template <bool POW2>
+__global__ void debug_cell_kernel(Grid g, uint64_t n, const float* x, const float* y, const float* z, uint32_t* out) {
+  const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < n) out[k] = cell_of<POW2>(g, x[k], y[k], z[k]);
+}
+
+}  // namespace soma
