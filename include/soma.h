@@ -116,6 +116,8 @@ const char *soma_last_error(const soma_t *h);
 /* Tuning / test switches.  Names:
  *   "path"            0 = automatic, 1 = generic kernels (4 launches/step, any N),
  *                     2 = fused chain-in-registers kernel (N = 2P, P a power of two <= 32; else EINVAL)
+ *   "kernel_timing"   1 = record CUDA events on the handle's stream around the kernels of every step
+ *                     (read them with soma_get_kernel_times), 0 = off (default)
  *   "resort_interval" re-order chains in memory by position every k steps (0 = never); results
  *                     are independent of it (the random stream is keyed by the logical chain id)
  * Errors: SOMA_EINVAL (unknown name / unsupported value). */
@@ -124,6 +126,12 @@ int soma_set_option(soma_t *h, const char *name, int64_t value);
 /* Counters since soma_create: [0] kernels launched by this library, [1] MC steps done,
  * [2] chain re-orderings done.  `out` is a host pointer to 3 uint64. */
 int soma_get_counters(const soma_t *h, uint64_t *out);
+
+/* Device time spent since the last call (or since "kernel_timing" was switched on), summed over the
+ * recorded steps (at most 16384 between two reads): ms[0] = rows a1+a2+a3 (the move and binning
+ * kernels), ms[1] = row a4 (the omega kernel); *steps = number of steps recorded.  Synchronises the
+ * stream.  `ms` is a host pointer to 2 doubles. */
+int soma_get_kernel_times(soma_t *h, double *ms, uint64_t *steps);
 
 /* ---- test hooks (used by tests/ only; each runs on the device) --------------------------------- */
 

@@ -27,7 +27,7 @@ LIB_PATH: Path = _build.LIB_PATH
 EXPORTS = (
     "soma_workspace_bytes", "soma_create", "soma_load_state", "soma_mc_steps", "soma_get_density",
     "soma_get_positions", "soma_get_omega", "soma_get_step", "soma_destroy", "soma_last_error",
-    "soma_set_option", "soma_get_counters", "soma_debug_half_sweep", "soma_debug_finish_step",
+    "soma_set_option", "soma_get_counters", "soma_get_kernel_times", "soma_debug_half_sweep", "soma_debug_finish_step",
     "soma_debug_set_omega", "soma_debug_philox", "soma_debug_maps", "soma_debug_accept",
     "soma_debug_cell_index",
 )
@@ -90,6 +90,7 @@ def load_library() -> C.CDLL:
             "soma_last_error": (C.c_char_p, [vp]),
             "soma_set_option": (i32, [vp, C.c_char_p, C.c_int64]),
             "soma_get_counters": (i32, [vp, C.POINTER(u64)]),
+            "soma_get_kernel_times": (i32, [vp, C.POINTER(C.c_double), C.POINTER(u64)]),
             "soma_debug_half_sweep": (i32, [vp, u32, C.POINTER(u64)]),
             "soma_debug_finish_step": (i32, [vp]),
             "soma_debug_set_omega": (i32, [vp, vp]),
@@ -199,6 +200,13 @@ def soma_get_counters(h) -> dict:
     out = (C.c_uint64 * 3)()
     _check(load_library().soma_get_counters(h, out), h)
     return {"launches": int(out[0]), "steps": int(out[1]), "resorts": int(out[2])}
+
+
+def soma_get_kernel_times(h) -> dict:
+    ms = (C.c_double * 2)()
+    n = C.c_uint64(0)
+    _check(load_library().soma_get_kernel_times(h, ms, C.byref(n)), h)
+    return {"move_bin_ms": float(ms[0]), "omega_ms": float(ms[1]), "steps": int(n.value)}
 
 
 def soma_debug_half_sweep(h, parity: int, want_accepted: bool = True):
@@ -329,6 +337,9 @@ class Soma:
 
     def counters(self) -> dict:
         return soma_get_counters(self._h)
+
+    def kernel_times(self) -> dict:
+        return soma_get_kernel_times(self._h)
 
     # test hooks
     def debug_half_sweep(self, parity: int) -> int:

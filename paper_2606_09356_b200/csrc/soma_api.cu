@@ -121,6 +121,10 @@ struct soma_handle {
   int64_t resort_interval;
   // counters
   uint64_t launches, steps_done, resorts;
+  // per-kernel timing ("kernel_timing" option): event triples (before moves, after moves+bin, after omega)
+  bool timing;
+  std::vector<cudaEvent_t>* ev;      // 3 per recorded step
+  size_t ev_used;                    // events recorded since the last soma_get_kernel_times
   bool sticky;
   char err[256];
 
@@ -134,6 +138,14 @@ struct soma_handle {
 };
 
 namespace {
+
+void free_handle(soma_handle* h) {
+  if (h->ev) {
+    for (cudaEvent_t e : *h->ev) cudaEventDestroy(e);
+    delete h->ev;
+  }
+  delete h;
+}
 
 int fail(soma_handle* h, int code, const char* msg) {
   snprintf(h ? h->err : g_last_error, 256, "%s", msg);
@@ -257,8 +269,25 @@ bool use_fused(const soma_handle* h) {
   return fused_lanes(h->N) != 0;
 }
 
+constexpr size_t kMaxTimedSteps = 16384;
+
+// next event of the timing pool, recorded on the handle's stream (nullptr: pool exhausted / error)
+cudaEvent_t timing_mark(soma_handle* h) {
+  if (h->ev_used >= 3 * kMaxTimedSteps) return nullptr;
+  if (h->ev_used == h->ev->size()) {
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+    h->ev->push_back(e);
+  }
+  cudaEvent_t e = (*h->ev)[h->ev_used++];
+  cudaEventRecord(e, h->stream);
+  return e;
+}
+
 int one_step(soma_handle* h) {
   int rc;
+  const bool timed = h->timing && h->ev_used + 3 <= 3 * kMaxTimedSteps;
+  if (timed) timing_mark(h);
   if (use_fused(h)) {
     if ((rc = launch_fused(h)) != SOMA_OK) return rc;            // a1 + a2 + a3 (+a5)
   } else {
@@ -267,7 +296,9 @@ int one_step(soma_handle* h) {
     if ((rc = launch_bin(h, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;   // a3
   }
   h->cur ^= 1;
+  if (timed) timing_mark(h);
   if ((rc = launch_omega(h)) != SOMA_OK) return rc;              // a4
+  if (timed) timing_mark(h);
   h->step += 1;
   h->steps_done += 1;
   return SOMA_OK;
@@ -309,17 +340,19 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   soma_handle* h = new (std::nothrow) soma_handle();
   if (!h) return fail(nullptr, SOMA_ENOMEM, "host allocation failed");
   std::memset(static_cast<void*>(h), 0, sizeof *h);
+  h->ev = new (std::nothrow) std::vector<cudaEvent_t>();
+  if (!h->ev) { free_handle(h); return fail(nullptr, SOMA_ENOMEM, "host allocation failed"); }
   cudaError_t e = cudaGetDevice(&h->device);
   cudaDeviceProp prop{};
   if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, h->device);
   if (e != cudaSuccess) {
     snprintf(g_last_error, 256, "no usable CUDA device: %s", cudaGetErrorString(e));
-    delete h;
+    free_handle(h);
     return SOMA_ECUDA;
   }
   if (prop.major != 10) {
     snprintf(g_last_error, 256, "device is sm_%d%d; this library holds sm_100a code only", prop.major, prop.minor);
-    delete h;
+    free_handle(h);
     return SOMA_ECUDA;
   }
   h->sm_count = prop.multiProcessorCount;
@@ -342,7 +375,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N);
   if (p->workspace) {
     if (p->workspace_bytes < h->L.total || (reinterpret_cast<uintptr_t>(p->workspace) % kAlign)) {
-      delete h;
+      free_handle(h);
       return fail(nullptr, SOMA_ENOMEM, "lent workspace is too small or not 256-byte aligned");
     }
     h->ws = static_cast<char*>(p->workspace);
@@ -353,7 +386,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
     if (e != cudaSuccess) {
       snprintf(g_last_error, 256, "cudaMalloc(%llu bytes): %s", (unsigned long long)h->L.total, cudaGetErrorString(e));
       cudaGetLastError();
-      delete h;
+      free_handle(h);
       return SOMA_ENOMEM;
     }
     h->ws = static_cast<char*>(ptr);
@@ -363,7 +396,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   auto bail = [&](cudaError_t err, const char* where) {
     snprintf(g_last_error, 256, "%s: %s", where, cudaGetErrorString(err));
     if (h->owns_ws) cudaFree(h->ws);
-    delete h;
+    free_handle(h);
     return SOMA_ECUDA;
   };
   iota_kernel<<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>((uint32_t)h->n_chains, h->slot_chain());
@@ -467,7 +500,7 @@ int soma_destroy(soma_t* h) {
   cudaSetDevice(h->device);
   cudaStreamSynchronize(h->stream);
   if (h->owns_ws) cudaFree(h->ws);
-  delete h;
+  free_handle(h);
   return SOMA_OK;
 }
 
@@ -482,6 +515,12 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     h->path = (int)value;
     return SOMA_OK;
   }
+  if (!std::strcmp(name, "kernel_timing")) {
+    if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "kernel_timing must be 0 or 1");
+    h->timing = value != 0;
+    h->ev_used = 0;
+    return SOMA_OK;
+  }
   if (!std::strcmp(name, "resort_interval")) {
     if (value != 0) return fail(h, SOMA_EINVAL, "chain re-ordering is not available in this build");
     h->resort_interval = value;
@@ -493,6 +532,24 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
 int soma_get_counters(const soma_t* h, uint64_t* out) {
   if (!h || !out) return SOMA_EINVAL;
   out[0] = h->launches; out[1] = h->steps_done; out[2] = h->resorts;
+  return SOMA_OK;
+}
+
+int soma_get_kernel_times(soma_t* h, double* ms, uint64_t* steps) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!ms || !steps) return fail(h, SOMA_EINVAL, "NULL argument");
+  CU(h, cudaStreamSynchronize(h->stream));
+  ms[0] = ms[1] = 0.0;
+  const size_t n = h->ev_used / 3;
+  for (size_t k = 0; k < n; ++k) {
+    float a = 0.f, b = 0.f;
+    CU(h, cudaEventElapsedTime(&a, (*h->ev)[3 * k], (*h->ev)[3 * k + 1]));
+    CU(h, cudaEventElapsedTime(&b, (*h->ev)[3 * k + 1], (*h->ev)[3 * k + 2]));
+    ms[0] += a; ms[1] += b;
+  }
+  *steps = n;
+  h->ev_used = 0;
   return SOMA_OK;
 }
 

@@ -1,0 +1,156 @@
+"""GPU-vs-oracle parity of the whole SCMF Monte-Carlo step through the C ABI (BASELINE.json
+`north_star` comparison rules).
+
+Bar: density grids bit-exact, omega bit-exact, positions bit-identical (north_star's 1e-6 b is below
+one fp32 ulp for |r| >= 16 b), accepted-move counts equal -- after 1 and after 10 MC steps from the
+same seeded state, for both kernel paths.  With DESIGN.md reading R6b the accept decisions are
+implementation-independent, so no flip is expected; the lock-step test keeps north_star's
+allowance (|dE + ln u| < 1e-4, <= 1e-6 of the moves) as the outer bound and reports what it saw.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import scmf_inputs as si
+from helpers import assert_same_state, gpu_system, lockstep
+
+pytestmark = pytest.mark.gpu
+
+FUSED, GENERIC = 2, 1
+
+
+def _run_both(s, steps_list, path, **kw):
+    """Advance GPU and oracle through cumulative step counts, comparing the full state at each."""
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s, path=path, **kw) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert_same_state(g, o, f"{s.workload.name} after load_state")
+        done = 0
+        for upto in steps_list:
+            acc_g = g.mc_steps(upto - done, want_accepted=True)
+            acc_o = o.mc_steps(upto - done)
+            done = upto
+            assert acc_g == acc_o, f"{s.workload.name} path {path}: accepted {acc_g} vs oracle {acc_o} after {upto} steps"
+            assert_same_state(g, o, f"{s.workload.name} path {path} after {upto} steps")
+            assert g.step == o.step == upto
+            d = g.density()
+            assert int(d.sum()) == s.workload.n_beads
+        launches = g.counters()["launches"]
+    assert launches > 0
+    return launches
+
+
+# ---- the five BASELINE.json configs, the small one at full size, the others scaled down so that the
+# ---- oracle finishes in seconds but several tiles/warps and a ragged tail are covered ------------
+
+def _scaled(i, n_chains, grid):
+    return si.make_system(si.scaled(si.config(i), n_chains, grid))
+
+
+CASES = {
+    "cfg0_full": lambda: si.make_system(si.config(0)),
+    "cfg1_scaled": lambda: _scaled(1, 4099, (16, 16, 16)),          # N=64, T=1, omega == 0; 4099 = ragged
+    "cfg2_scaled": lambda: _scaled(2, 8193, (16, 16, 16)),          # N=32 diblock, 64 beads/cell
+    "cfg3_scaled": lambda: _scaled(3, 4098, (32, 16, 16)),          # N=64 blend, 2 patterns, non-cubic
+    "cfg4_scaled": lambda: _scaled(4, 16385, (32, 32, 16)),         # N=32 diblock, chiN=30
+}
+
+
+@pytest.mark.parametrize("path", [FUSED, GENERIC])
+@pytest.mark.parametrize("case", sorted(CASES))
+def test_parity_after_1_and_10_steps(case, path):
+    _run_both(CASES[case](), [1, 10], path)
+
+
+def test_cfg0_lockstep_protocol_no_flips():
+    n_moves, n_flips, worst = lockstep(si.make_system(si.config(0)), 10)
+    assert n_moves == 81920
+    assert n_flips <= 1e-6 * n_moves          # = 0 for cfg 0
+    print(f"lockstep cfg0: {n_moves} moves, {n_flips} flips, worst |margin| {worst:g}")
+
+
+def test_scaled_cfg4_lockstep_protocol():
+    n_moves, n_flips, worst = lockstep(_scaled(4, 16385, (32, 32, 16)), 5)
+    assert n_flips <= max(0, int(1e-6 * n_moves))
+    print(f"lockstep cfg4 scaled: {n_moves} moves, {n_flips} flips, worst |margin| {worst:g}")
+
+
+# ---- degenerate and edge cases ---------------------------------------------------------------------
+
+def _custom(n, N, T, pats, cp, chi, kappaN, grid, box, seed, **kw):
+    return si.custom_system(n, N, T, pats, cp, chi, kappaN, grid, box, seed, **kw)
+
+
+EDGE = {
+    # N=1: no bonds, no odd beads;  N=2: one bond;  N=3, 5, 33: odd lengths -> generic path only
+    "N1": lambda: _custom(777, 1, 2, [[0], [1]], np.arange(777) % 2, [[0, 9], [9, 0]], 30.0, (8, 8, 8), (4, 4, 4), 21),
+    "N2": lambda: _custom(1001, 2, 2, [[0, 1]], None, [[0, 15], [15, 0]], 40.0, (8, 8, 8), (4, 4, 4), 22),
+    "N3": lambda: _custom(513, 3, 2, [[0, 1, 0]], None, [[0, 15], [15, 0]], 40.0, (8, 8, 8), (4, 4, 4), 23),
+    "N33": lambda: _custom(130, 33, 2, [[0] * 16 + [1] * 17], None, [[0, 15], [15, 0]], 40.0, (8, 8, 8), (4, 4, 4), 24),
+    "N4": lambda: _custom(999, 4, 2, [[0, 0, 1, 1]], None, [[0, 15], [15, 0]], 40.0, (8, 8, 8), (4, 4, 4), 25),
+    "N8": lambda: _custom(517, 8, 2, [[0, 0, 0, 1, 1, 1, 1, 0]], None, [[0, 15], [15, 0]], 40.0, (8, 8, 8), (4, 4, 4), 26),
+    "N16": lambda: _custom(259, 16, 2, [[0] * 8 + [1] * 8], None, [[0, 15], [15, 0]], 40.0, (8, 8, 8), (4, 4, 4), 27),
+    # three types with an asymmetric-valued chi matrix, three patterns, non-power-of-two non-cubic grid
+    "T3_npot": lambda: _custom(600, 32, 3, [[0] * 10 + [1] * 12 + [2] * 10, [2] * 32, [1] * 16 + [0] * 16],
+                               np.arange(600) % 3, [[0, 12, 5], [12, 0, 21], [5, 21, 0]], 35.0, (12, 10, 7), (6.0, 5.0, 3.5), 28),
+    # T = 8 (the maximum), generic omega kernel
+    "T8": lambda: _custom(300, 16, 8, [[0, 1, 2, 3, 4, 5, 6, 7] * 2], None,
+                          (np.arange(64).reshape(8, 8) + np.arange(64).reshape(8, 8).T) * (1 - np.eye(8)) * 0.3, 25.0,
+                          (6, 6, 6), (3, 3, 3), 29),
+    # one chain, one cell, big moves, b != 1, a != 0.5, box far from cubic
+    "one_chain": lambda: _custom(1, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (1, 1, 1), (3, 3, 3), 30),
+    "b_and_a": lambda: _custom(700, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (20, 4, 9), (14.0, 2.8, 6.3), 31,
+                               b=0.7, move_halfwidth=0.9),
+    # zero move width: every trial equals the current position, dE = 0, all accepted, nothing changes
+    "a0": lambda: _custom(100, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (8, 8, 8), (4, 4, 4), 32, move_halfwidth=0.0),
+}
+
+
+@pytest.mark.parametrize("case", sorted(EDGE))
+def test_edge_cases_generic_path(case):
+    _run_both(EDGE[case](), [1, 4], GENERIC)
+
+
+@pytest.mark.parametrize("case", ["N2", "N4", "N8", "N16", "T3_npot", "T8", "one_chain", "b_and_a", "a0"])
+def test_edge_cases_fused_path(case):
+    _run_both(EDGE[case](), [1, 4], FUSED)
+
+
+def test_fused_path_refuses_unsupported_chain_lengths():
+    import paper_2606_09356_b200 as soma
+    with gpu_system(EDGE["N33"]()) as g:
+        with pytest.raises(soma.SomaError) as e:
+            g.set_option("path", FUSED)
+        assert e.value.code == soma.SOMA_EINVAL
+
+
+def test_a0_accepts_everything_and_moves_nothing():
+    s = EDGE["a0"]()
+    with gpu_system(s) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert g.mc_steps(3, want_accepted=True) == 3 * s.workload.n_beads
+        x, y, z = g.positions()
+        assert np.array_equal(x, s.x) and np.array_equal(y, s.y) and np.array_equal(z, s.z)
+
+
+def test_large_seed_step_and_chain_ids_reach_the_counter():
+    """64-bit seed (both key words), step0 beyond 2^32 (counter word 3 bits 16..31)."""
+    w = si.scaled(si.config(0), 300, (8, 8, 8))
+    from dataclasses import replace
+    s = si.make_system(replace(w, seed=0xFEDCBA9876543210))
+    step0 = (5 << 32) + 0xFFFFFFFE           # crosses a 2^32 boundary during the run
+    for path in (FUSED, GENERIC):
+        o = oracle.Oracle.from_system(s)
+        o.load_state(s.x, s.y, s.z, step0)
+        with gpu_system(s, path=path) as g:
+            g.load_state(s.x, s.y, s.z, step0)
+            assert g.mc_steps(4, want_accepted=True) == o.mc_steps(4)
+            assert_same_state(g, o, "large seed/step")
+            assert g.step == step0 + 4
+    # and the seed really matters
+    s2 = si.make_system(replace(w, seed=0xFEDCBA9876543211))
+    with gpu_system(s2) as g2:
+        g2.load_state(s.x, s.y, s.z, step0)
+        g2.mc_steps(1)
+        assert not np.array_equal(g2.positions()[0], o.positions()[0])
