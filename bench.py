@@ -144,3 +144,203 @@ def barrier():
     import torch.distributed as dist
     if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
         dist.barrier()
+
+
+# --------------------------------------------------------------------------------------------------
+# the CPU oracle as a timed baseline (test infrastructure; never on the product path)
+# --------------------------------------------------------------------------------------------------
+
+def sample_workload(w, factor: int):
+    """The same melt (beads per cell, cell size, fields, architecture) at 1/factor of the chains and
+    cells; factor a power of two, grid axes halved in turn (x, y, z, x, ...)."""
+    import scmf_inputs as si
+    grid, d, f = list(w.grid), 0, factor
+    while f > 1:
+        if grid[d % 3] % 2 == 0 and grid[d % 3] > 1:
+            grid[d % 3] //= 2
+            f //= 2
+        d += 1
+    return si.scaled(w, w.n_chains // factor, tuple(grid))
+
+
+def time_oracle(system, steps: int, warmup: int = 0, budget_s: float | None = None):
+    """Oracle MC steps on `system`, single-threaded, as it stands.  Returns (seconds, steps timed)."""
+    import oracle
+    o = oracle.Oracle.from_system(system)
+    o.load_state(system.x, system.y, system.z)
+    if warmup:
+        o.mc_steps(warmup)
+    done, t0 = 0, time.perf_counter()
+    while done < steps:
+        o.mc_steps(1)
+        done += 1
+        if budget_s is not None and time.perf_counter() - t0 >= budget_s:
+            break
+    dt = time.perf_counter() - t0
+    o.close()
+    return dt, done
+
+
+def run_reference(args):
+    """`--impl reference`: the oracle on the host cores, on a bounded sample of the same workload."""
+    import scmf_inputs as si
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    w = si.config(args.config)
+    # size the sample so that (K + W) oracle steps take about 90 s at ~120 ns per attempted move
+    target_beads = 90.0 / (120e-9 * max(1, args.steps + args.warmup))
+    factor = 1
+    while w.n_beads // factor > target_beads and w.n_chains // (factor * 2) >= 1024:
+        factor *= 2
+    ws = sample_workload(w, factor) if factor > 1 else w
+    s = si.make_system(ws)
+    dt, done = time_oracle(s, args.steps, warmup=args.warmup)
+    value = ws.n_beads * done / dt
+    sample = (f"{ws.n_chains} chains x {ws.N} beads on a {ws.grid[0]}x{ws.grid[1]}x{ws.grid[2]} grid = 1/{factor} of "
+              f"{w.name} at the same beads per cell; every step is one oracle MC step over that sample")
+    cores = 1
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": done,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / done, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "sample": sample, "mc_steps_per_s": done / dt},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# --------------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------------
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_09356_b200 as soma
+    import scmf_inputs as si
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    soma.load_library()                                 # raises if the CUDA library is missing
+
+    w = si.config(args.config)
+    s = si.make_system(w)                               # every rank: an independent replica of the config
+    B = w.n_beads
+    pinned = [torch.from_numpy(v).pin_memory() for v in (s.x, s.y, s.z)]
+    out_pos = [torch.empty(B, dtype=torch.float32).pin_memory() for _ in range(3)]
+    out_den = torch.empty((w.n_types, w.n_cells), dtype=torch.int32).pin_memory()
+    stream = torch.cuda.current_stream()
+    g = soma.Soma.from_system(s)
+    if args.path:
+        g.set_option("path", args.path)
+    clocks = ClockSampler(local_rank)
+
+    # ---- device-resident timing: K steps after W warm-up steps --------------------------------
+    g.load_state(pinned[0], pinned[1], pinned[2])
+    g.mc_steps(max(args.warmup, 0))
+    g.set_option("kernel_timing", 1)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    barrier()
+    c0 = g.counters()
+    clocks.start()
+    ev0.record(stream)
+    g.mc_steps(args.steps)                              # asynchronous: no host sync inside
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    clk = clocks.stop()
+    barrier()
+    local_ms = ev0.elapsed_time(ev1)
+    kt = g.kernel_times()
+    g.set_option("kernel_timing", 0)
+    launches = g.counters()["launches"] - c0["launches"]
+    ms, moves = aggregate_over_ranks(local_ms, float(B) * args.steps, dev)
+    value = moves / (ms * 1e-3)
+
+    # ---- end to end: the config's own run through the C ABI, host buffers in and out -----------
+    S = w.steps
+    torch.cuda.synchronize()
+    barrier()
+    t0 = time.perf_counter()
+    g.load_state(pinned[0], pinned[1], pinned[2])       # H2D 12 B/bead
+    g.mc_steps(S)
+    soma.soma_get_density(g._h, out_den)                # D2H 4 T C
+    soma.soma_get_positions(g._h, *out_pos)             # D2H 12 B/bead
+    torch.cuda.synchronize()
+    e2e_local = (time.perf_counter() - t0) * 1e3
+    barrier()
+    e2e_ms, e2e_moves = aggregate_over_ranks(e2e_local, float(B) * S, dev)
+    assert int(out_den.sum()) == B, "density grids do not sum to the bead count"
+    g.close()
+
+    # ---- roofline of the dominant kernel (fused move + bin), from the live event times ---------
+    peak, peak_src = measured_peaks()
+    ab = algorithmic_bytes(w)
+    n_t = max(1, kt["steps"])
+    move_ms, omega_ms = kt["move_bin_ms"] / n_t, kt["omega_ms"] / n_t
+    achieved = ab["move_bin_kernel"] / (move_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "fused_step_kernel (rows a1+a2+a3+a5)" if launches == 2 * args.steps else "move+bin kernels",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": args.traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": ab["move_bin_kernel"],
+                "kernel_ms": move_ms, "omega_kernel_ms": omega_ms,
+                "omega_kernel_frac": ab["omega_kernel"] / (omega_ms * 1e-3) / 1e9 / peak if omega_ms > 0 else None,
+                "step_frac": ab["step"] / (local_ms / args.steps * 1e-3) / 1e9 / peak,
+                "step_frac_of_8TBps": ab["step"] / (local_ms / args.steps * 1e-3) / 8e12,
+                "bytes_per_move": ab["step"] / B}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "n_chains": w.n_chains, "beads_per_chain": w.N, "beads": B, "grid": list(w.grid),
+                   "chiN": w.chiN, "kappaN": w.kappaN, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": f"inputs larger than L2: positions {12 * B / 1e6:.0f} MB + grids {12 * w.n_types * w.n_cells / 1e6:.0f} MB per step",
+                   "mc_steps_per_s": world * args.steps / (ms * 1e-3)},
+        "clocks": clk, "gpu_launches": int(launches),
+        "e2e": {"value": e2e_moves / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 12 * B / S,
+                "d2h_bytes_per_step": (12 * B + 4 * w.n_types * w.n_cells) / S, "mc_steps": S, "ms": e2e_ms,
+                "what": f"soma_load_state(pinned host) + soma_mc_steps({S}) + soma_get_density(host) + soma_get_positions(pinned host); "
+                        f"the copies happen once per {S}-step run, bytes are per MC step"},
+        "roofline": roofline,
+    }
+
+    # ---- the oracle on the host cores, rank 0 at N = 1 only ------------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        dt, done = time_oracle(s, steps=4, budget_s=12.0)
+        line["cpu_baseline"] = {"value": B * done / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"{done} full MC step(s) of {w.name} ({B} beads) from the same initial state, {dt:.1f} s"}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: 134 M beads)")
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--path", type=int, default=0, help="library kernel path: 0 auto, 1 generic, 2 fused")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                   # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
