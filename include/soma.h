@@ -18,6 +18,9 @@
  *   - Ownership: the library copies everything it is given (parameters at create, positions at
  *     load_state).  The caller owns every buffer it passes in or receives results in.  The library
  *     owns its device memory, unless the caller lends a workspace (see soma_params.workspace).
+ *   - Positions must stay within 2^21 cells of the origin (|r_d| * grid[d] / box[d] < 2^21);
+ *     soma_load_state rejects others with SOMA_EINVAL and soma_mc_steps re-verifies before drift
+ *     could exceed it.
  *   - Layouts: positions are structure-of-arrays fp32, x[B], y[B], z[B], B = n_chains *
  *     beads_per_chain, bead i of chain c at index c*beads_per_chain + i, UNWRAPPED (periodic images
  *     are applied only when a bead is assigned to a cell).  Grids are [type][ix][iy][iz] with iz
@@ -84,7 +87,8 @@ int soma_create(const soma_params *p, void *cuda_stream, soma_t **out);
  * all beads and compute omega, so that the next step sees the field of the loaded state.
  * x, y, z: [B] fp32, host or device according to `ptrs_are_device`.  (positions, step index) is a
  * complete checkpoint: the random stream is a pure function of (seed, step, half-sweep, chain,
- * bead).  Errors: SOMA_EINVAL (NULL pointer), SOMA_ECUDA. */
+ * bead).  Synchronises the stream before returning (also for device pointers).
+ * Errors: SOMA_EINVAL (NULL pointer, NaN or out-of-range position), SOMA_ECUDA. */
 int soma_load_state(soma_t *h, const float *x, const float *y, const float *z, uint64_t step0,
                     int ptrs_are_device);
 
@@ -118,8 +122,11 @@ const char *soma_last_error(const soma_t *h);
  *                     2 = fused chain-in-registers kernel (N = 2P, P a power of two <= 32; else EINVAL)
  *   "kernel_timing"   1 = record CUDA events on the handle's stream around the kernels of every step
  *                     (read them with soma_get_kernel_times), 0 = off (default)
- *   "resort_interval" re-order chains in memory by position every k steps (0 = never); results
- *                     are independent of it (the random stream is keyed by the logical chain id)
+ *   "resort_interval" re-order the chains in memory by position at soma_load_state and then every k
+ *                     steps (0 = never; default 64 for >= 4096 chains, else 0); results are
+ *                     independent of it (the random stream is keyed by the logical chain id)
+ *   "resort_now"      re-order once, now (value ignored)
+ *   "fused_blocks_per_sm", "fused_waves"   launch shape of the fused kernel (tuning)
  * Errors: SOMA_EINVAL (unknown name / unsupported value). */
 int soma_set_option(soma_t *h, const char *name, int64_t value);
 
@@ -144,10 +151,11 @@ int soma_debug_finish_step(soma_t *h);
 int soma_debug_set_omega(soma_t *h, const float *omega);
 /* Device evaluation of the pieces of DESIGN.md section 2 step 5.1-5.2 on host arrays:
  * philox: ctr [n][4], key [2] -> out [n][4];  maps: words [n] -> tmap [n], u [n], lnu [n] (lnu by the
- * kernel's slow path, i.e. the value it uses when a move is near the threshold);
+ * kernel's slow path, i.e. the value it uses when a move is near the threshold), lnu_fast [n] (may
+ * be NULL; the hardware-logarithm value that decides every move outside the +-1e-4 band);
  * accept: dE [n], words [n] -> decision [n] (0/1) by the kernel's full fast+slow accept routine. */
 int soma_debug_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
-int soma_debug_maps(const uint32_t *words, float *tmap, float *u, float *lnu, uint64_t n);
+int soma_debug_maps(const uint32_t *words, float *tmap, float *u, float *lnu, float *lnu_fast, uint64_t n);
 int soma_debug_accept(const float *dE, const uint32_t *words, uint8_t *decision, uint64_t n);
 /* Cell index of host positions under the handle's grid/box. */
 int soma_debug_cell_index(soma_t *h, const float *x, const float *y, const float *z, uint32_t *cell,

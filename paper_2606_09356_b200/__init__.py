@@ -95,7 +95,7 @@ def load_library() -> C.CDLL:
             "soma_debug_finish_step": (i32, [vp]),
             "soma_debug_set_omega": (i32, [vp, vp]),
             "soma_debug_philox": (i32, [vp, vp, vp, u64]),
-            "soma_debug_maps": (i32, [vp, vp, vp, vp, u64]),
+            "soma_debug_maps": (i32, [vp, vp, vp, vp, vp, u64]),
             "soma_debug_accept": (i32, [vp, vp, vp, u64]),
             "soma_debug_cell_index": (i32, [vp, vp, vp, vp, vp, u64]),
         }
@@ -234,9 +234,9 @@ def soma_debug_philox(ctr: np.ndarray, key: Sequence[int]) -> np.ndarray:
 
 def soma_debug_maps(words: np.ndarray):
     words = np.ascontiguousarray(words, dtype=np.uint32).reshape(-1)
-    t, u, l = (np.empty(words.size, dtype=np.float32) for _ in range(3))
-    _check(load_library().soma_debug_maps(words.ctypes.data, t.ctypes.data, u.ctypes.data, l.ctypes.data, words.size))
-    return t, u, l
+    t, u, l, lf = (np.empty(words.size, dtype=np.float32) for _ in range(4))
+    _check(load_library().soma_debug_maps(words.ctypes.data, t.ctypes.data, u.ctypes.data, l.ctypes.data, lf.ctypes.data, words.size))
+    return t, u, l, lf
 
 
 def soma_debug_accept(dE: np.ndarray, words: np.ndarray) -> np.ndarray:

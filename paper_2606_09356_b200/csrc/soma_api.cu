@@ -24,24 +24,42 @@ struct Layout {            // byte offsets into the workspace
   uint64_t pos[2][3];      // two position sets (x,y,z): the live one and a staging / re-order target
   uint64_t counts[2];      // [T][C] uint32, double-buffered
   uint64_t omega;          // [T][C] fp32
-  uint64_t slot_chain;     // [n] uint32
-  uint64_t slot_pattern;   // [n] uint8
+  uint64_t slot_chain[2];  // [n] uint32: logical chain id of every slot (second copy: re-order target)
+  uint64_t slot_pattern[2];// [n] uint8
   uint64_t patterns;       // [n_patterns][N] uint8
+  uint64_t pattern0;       // [n] uint8: pattern id of every chain in the caller's order
   uint64_t accepted;       // uint64
+  uint64_t range_flag;     // uint32
+  uint64_t sort_key;       // [n] uint32
+  uint64_t sort_rank;      // [n] uint32
+  uint64_t sort_bins;      // [n_bins] uint32
   uint64_t total;
 };
 
-Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes) {
+// coarse bins of the chain re-ordering: cubes of kSortBinEdge cells
+constexpr uint32_t kSortBinEdge = 4;
+uint64_t sort_bin_count(const uint32_t grid[3]) {
+  uint64_t n = 1;
+  for (int d = 0; d < 3; ++d) n *= (grid[d] + kSortBinEdge - 1) / kSortBinEdge;
+  return n;
+}
+
+Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins) {
   Layout L{};
   uint64_t off = 0;
   for (int s = 0; s < 2; ++s)
     for (int d = 0; d < 3; ++d) { L.pos[s][d] = off; off += align_up(B * 4); }
   for (int s = 0; s < 2; ++s) { L.counts[s] = off; off += align_up(TC * 4); }
   L.omega = off; off += align_up(TC * 4);
-  L.slot_chain = off; off += align_up(n * 4);
-  L.slot_pattern = off; off += align_up(n);
+  for (int s = 0; s < 2; ++s) { L.slot_chain[s] = off; off += align_up(n * 4); }
+  for (int s = 0; s < 2; ++s) { L.slot_pattern[s] = off; off += align_up(n); }
   L.patterns = off; off += align_up(pat_bytes);
+  L.pattern0 = off; off += align_up(n);
   L.accepted = off; off += align_up(8);
+  L.range_flag = off; off += align_up(4);
+  L.sort_key = off; off += align_up(n * 4);
+  L.sort_rank = off; off += align_up(n * 4);
+  L.sort_bins = off; off += align_up(n_bins * 4);
   L.total = off;
   return L;
 }
@@ -109,8 +127,13 @@ struct soma_handle {
   char* ws;
   bool owns_ws;
   Layout L;
-  int live;              // which position set is current
+  int live;              // which position set (and slot table) is current
   int cur;               // which count buffer holds the current densities
+  uint32_t n_bins;       // coarse bins of the chain re-ordering
+  PhiloxKeys keys;
+  uint64_t steps_since_check;   // MC steps since the cell-coordinate range was last verified
+  uint64_t steps_since_sort;
+  uint64_t range_check_interval;
   // state
   bool loaded;
   bool identity_order;   // slot_chain is the identity
@@ -118,7 +141,8 @@ struct soma_handle {
   int sm_count;
   // options
   int path;              // 0 auto, 1 generic, 2 fused
-  int64_t resort_interval;
+  int64_t resort_interval;      // re-order the chains every k steps (0 = never)
+  int fused_blocks_per_sm, fused_waves;
   // counters
   uint64_t launches, steps_done, resorts;
   // per-kernel timing ("kernel_timing" option): event triples (before moves, after moves+bin, after omega)
@@ -131,9 +155,16 @@ struct soma_handle {
   float* pos(int set, int d) const { return reinterpret_cast<float*>(ws + L.pos[set][d]); }
   uint32_t* counts(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts[s]); }
   float* omega() const { return reinterpret_cast<float*>(ws + L.omega); }
-  uint32_t* slot_chain() const { return reinterpret_cast<uint32_t*>(ws + L.slot_chain); }
-  uint8_t* slot_pattern() const { return reinterpret_cast<uint8_t*>(ws + L.slot_pattern); }
+  uint32_t* slot_chain(int s) const { return reinterpret_cast<uint32_t*>(ws + L.slot_chain[s]); }
+  uint8_t* slot_pattern(int s) const { return reinterpret_cast<uint8_t*>(ws + L.slot_pattern[s]); }
+  uint32_t* slot_chain() const { return slot_chain(live); }
+  uint8_t* slot_pattern() const { return slot_pattern(live); }
+  uint32_t* range_flag() const { return reinterpret_cast<uint32_t*>(ws + L.range_flag); }
+  uint32_t* sort_key() const { return reinterpret_cast<uint32_t*>(ws + L.sort_key); }
+  uint32_t* sort_rank() const { return reinterpret_cast<uint32_t*>(ws + L.sort_rank); }
+  uint32_t* sort_bins() const { return reinterpret_cast<uint32_t*>(ws + L.sort_bins); }
   uint8_t* patterns() const { return reinterpret_cast<uint8_t*>(ws + L.patterns); }
+  uint8_t* pattern0() const { return reinterpret_cast<uint8_t*>(ws + L.pattern0); }
   unsigned long long* accepted() const { return reinterpret_cast<unsigned long long*>(ws + L.accepted); }
 };
 
@@ -173,8 +204,7 @@ StepArgs step_args(const soma_handle* h) {
   A.N = h->N;
   A.a = h->a;
   A.kb = h->kb;
-  A.key0 = (uint32_t)h->seed;
-  A.key1 = (uint32_t)(h->seed >> 32);
+  A.keys = h->keys;
   A.ctr2 = (uint32_t)h->step;
   A.ctr3_base = (0u << 8) | ((uint32_t)(h->step >> 32) << 16);   // domain 0 = MC move
   A.x = h->pos(h->live, 0);
@@ -201,15 +231,16 @@ int launch_half_sweep(soma_handle* h, uint32_t parity) {
   return SOMA_OK;
 }
 
-int launch_bin(soma_handle* h, uint32_t* counts) {
+int launch_bin(soma_handle* h, uint32_t* counts, bool check_range = false) {
+  uint32_t* flag = check_range ? h->range_flag() : nullptr;
   if (h->pow2)
     bin_kernel<true><<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
         h->grid, h->cells, h->N, h->B, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2),
-        h->slot_pattern(), h->patterns(), counts);
+        h->slot_pattern(), h->patterns(), counts, flag);
   else
     bin_kernel<false><<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
         h->grid, h->cells, h->N, h->B, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2),
-        h->slot_pattern(), h->patterns(), counts);
+        h->slot_pattern(), h->patterns(), counts, flag);
   h->launches++;
   CU(h, cudaGetLastError());
   return SOMA_OK;
@@ -242,11 +273,20 @@ int launch_fused_p(soma_handle* h) {
   constexpr int G = 32 / P;
   const uint64_t n_groups = (h->n_chains + G - 1) / G;           // warps of work
   const unsigned bs = 256, wpb = bs / 32;
-  uint64_t blocks = (n_groups + wpb - 1) / wpb;
-  const uint64_t cap = (uint64_t)h->sm_count * 64;               // grid-stride beyond this
-  if (blocks > cap) blocks = cap;
-  if (h->pow2) fused_step_kernel<P, true><<<(unsigned)blocks, bs, 0, h->stream>>>(A);
-  else fused_step_kernel<P, false><<<(unsigned)blocks, bs, 0, h->stream>>>(A);
+  // every block owns a contiguous run of warp groups: a multiple of the warps per block, sized so
+  // that the grid is about `waves` full waves of resident blocks
+  const uint64_t resident = (uint64_t)h->sm_count * h->fused_blocks_per_sm;
+  uint64_t blocks = resident * (uint64_t)h->fused_waves;
+  uint64_t gpb = (n_groups + blocks - 1) / blocks;
+  gpb = (gpb + wpb - 1) / wpb * wpb;
+  if (gpb == 0) gpb = wpb;
+  blocks = (n_groups + gpb - 1) / gpb;
+  const bool multi = h->n_patterns > 1;
+#define SOMA_LAUNCH_FUSED(POW2, MULTI) \
+  fused_step_kernel<P, POW2, MULTI><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb)
+  if (h->pow2) { if (multi) SOMA_LAUNCH_FUSED(true, true); else SOMA_LAUNCH_FUSED(true, false); }
+  else         { if (multi) SOMA_LAUNCH_FUSED(false, true); else SOMA_LAUNCH_FUSED(false, false); }
+#undef SOMA_LAUNCH_FUSED
   h->launches++;
   CU(h, cudaGetLastError());
   return SOMA_OK;
@@ -269,6 +309,50 @@ bool use_fused(const soma_handle* h) {
   return fused_lanes(h->N) != 0;
 }
 
+// Re-order the chains in memory by the coarse bin of their middle bead (counting sort on the device).
+int resort(soma_handle* h) {
+  SortArgs S{};
+  S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N; S.cb = kSortBinEdge;
+  S.ncy = (h->grid.ny + kSortBinEdge - 1) / kSortBinEdge;
+  S.ncz = (h->grid.nz + kSortBinEdge - 1) / kSortBinEdge;
+  S.n_bins = h->n_bins;
+  const int src = h->live, dst = h->live ^ 1;
+  CU(h, cudaMemsetAsync(h->sort_bins(), 0, (size_t)h->n_bins * 4, h->stream));
+  if (h->pow2)
+    chain_key_kernel<true><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
+        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
+  else
+    chain_key_kernel<false><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
+        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
+  bin_scan_kernel<<<1, 1024, 0, h->stream>>>(h->n_bins, h->sort_bins());
+  chain_permute_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
+      h->B, h->N, h->sort_bins(), h->sort_key(), h->sort_rank(),
+      h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->pos(dst, 0), h->pos(dst, 1), h->pos(dst, 2),
+      h->slot_chain(src), h->slot_pattern(src), h->slot_chain(dst), h->slot_pattern(dst));
+  h->launches += 3;
+  CU(h, cudaGetLastError());
+  h->live = dst;
+  h->identity_order = false;
+  h->resorts++;
+  h->steps_since_sort = 0;
+  return SOMA_OK;
+}
+
+// The conversion-free floor needs |r * inv_h| < 2^22; positions are verified to be below 2^21 and a
+// bead drifts by at most a * inv_h cells per step and axis, so the check is repeated before 2^21
+// cells of drift could have accumulated.
+int verify_range(soma_handle* h) {
+  uint32_t flag = 0;
+  CU(h, cudaMemcpyAsync(&flag, h->range_flag(), 4, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  if (flag) {
+    h->loaded = false;
+    return fail(h, SOMA_EINVAL, "a position is NaN or beyond 2^21 cells from the origin");
+  }
+  h->steps_since_check = 0;
+  return SOMA_OK;
+}
+
 constexpr size_t kMaxTimedSteps = 16384;
 
 // next event of the timing pool, recorded on the handle's stream (nullptr: pool exhausted / error)
@@ -286,6 +370,8 @@ cudaEvent_t timing_mark(soma_handle* h) {
 
 int one_step(soma_handle* h) {
   int rc;
+  if (h->resort_interval > 0 && h->steps_since_sort >= (uint64_t)h->resort_interval)
+    if ((rc = resort(h)) != SOMA_OK) return rc;
   const bool timed = h->timing && h->ev_used + 3 <= 3 * kMaxTimedSteps;
   if (timed) timing_mark(h);
   if (use_fused(h)) {
@@ -301,6 +387,8 @@ int one_step(soma_handle* h) {
   if (timed) timing_mark(h);
   h->step += 1;
   h->steps_done += 1;
+  h->steps_since_sort += 1;
+  h->steps_since_check += 1;
   return SOMA_OK;
 }
 
@@ -329,7 +417,7 @@ uint64_t soma_workspace_bytes(const soma_params* p) {
   if (bad) { fail(nullptr, SOMA_EINVAL, bad); return 0; }
   const uint64_t B = p->n_chains * p->beads_per_chain;
   const uint64_t TC = (uint64_t)p->grid[0] * p->grid[1] * p->grid[2] * p->n_types;
-  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain).total;
+  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bin_count(p->grid)).total;
 }
 
 int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
@@ -372,7 +460,8 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->kappaN = p->kappaN;
   for (uint32_t k = 0; k < h->T * h->T; ++k) h->chiN[k] = p->chiN[k];
   h->seed = p->seed;
-  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N);
+  h->n_bins = (uint32_t)sort_bin_count(p->grid);
+  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, h->n_bins);
   if (p->workspace) {
     if (p->workspace_bytes < h->L.total || (reinterpret_cast<uintptr_t>(p->workspace) % kAlign)) {
       free_handle(h);
@@ -399,18 +488,25 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
     free_handle(h);
     return SOMA_ECUDA;
   };
-  iota_kernel<<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>((uint32_t)h->n_chains, h->slot_chain());
-  h->launches++;
-  if ((e = cudaGetLastError()) != cudaSuccess) return bail(e, "iota_kernel");
-  if (p->chain_pattern) e = cudaMemcpyAsync(h->slot_pattern(), p->chain_pattern, h->n_chains, cudaMemcpyHostToDevice, h->stream);
-  else e = cudaMemsetAsync(h->slot_pattern(), 0, h->n_chains, h->stream);
+  if (p->chain_pattern) e = cudaMemcpyAsync(h->pattern0(), p->chain_pattern, h->n_chains, cudaMemcpyHostToDevice, h->stream);
+  else e = cudaMemsetAsync(h->pattern0(), 0, h->n_chains, h->stream);
   if (e != cudaSuccess) return bail(e, "chain_pattern upload");
   e = cudaMemcpyAsync(h->patterns(), p->type_patterns, (size_t)h->n_patterns * h->N, cudaMemcpyHostToDevice, h->stream);
   if (e != cudaSuccess) return bail(e, "type_patterns upload");
   if ((e = cudaStreamSynchronize(h->stream)) != cudaSuccess) return bail(e, "create sync");   // host buffers may go away
+  for (int r = 0; r < 10; ++r) {
+    h->keys.k0[r] = (uint32_t)p->seed + (uint32_t)r * kPhiloxW0;
+    h->keys.k1[r] = (uint32_t)(p->seed >> 32) + (uint32_t)r * kPhiloxW1;
+  }
   h->identity_order = true;
   h->path = 0;
-  h->resort_interval = 0;
+  // chains are kept sorted by position when the system is large enough for it to matter
+  h->resort_interval = h->n_chains >= 4096 ? 64 : 0;
+  h->fused_blocks_per_sm = 3;
+  h->fused_waves = 1;
+  const double cells_per_step = (double)h->a * (double)fmaxf(h->grid.inv_hx, fmaxf(h->grid.inv_hy, h->grid.inv_hz));
+  const double k = cells_per_step > 0.0 ? 2097152.0 / cells_per_step : 1e18;
+  h->range_check_interval = k >= 1e18 ? (1ull << 60) : (k < 1.0 ? 1ull : (uint64_t)k);
   *out = h;
   return SOMA_OK;
 }
@@ -422,14 +518,24 @@ int soma_load_state(soma_t* h, const float* x, const float* y, const float* z, u
   if (step0 >= (1ull << 48)) return fail(h, SOMA_EINVAL, "step0 must be < 2^48");
   const cudaMemcpyKind kind = dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   h->live = 0;
+  h->loaded = false;
   const float* src[3] = {x, y, z};
   for (int d = 0; d < 3; ++d) CU(h, cudaMemcpyAsync(h->pos(0, d), src[d], h->B * 4, kind, h->stream));
+  // slot s holds chain s again
+  iota_kernel<<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>((uint32_t)h->n_chains, h->slot_chain(0));
+  h->launches++;
+  CU(h, cudaGetLastError());
+  CU(h, cudaMemcpyAsync(h->slot_pattern(0), h->pattern0(), h->n_chains, cudaMemcpyDeviceToDevice, h->stream));
+  h->identity_order = true;
   h->step = step0;
   h->cur = 0;
   CU(h, cudaMemsetAsync(h->counts(0), 0, (size_t)h->cells * h->T * 4, h->stream));
-  if ((rc = launch_bin(h, h->counts(0))) != SOMA_OK) return rc;
+  CU(h, cudaMemsetAsync(h->range_flag(), 0, 4, h->stream));
+  if ((rc = launch_bin(h, h->counts(0), true)) != SOMA_OK) return rc;
   if ((rc = launch_omega(h)) != SOMA_OK) return rc;     // also zeroes counts(1)
-  if (!dev) CU(h, cudaStreamSynchronize(h->stream));    // the caller may reuse its host buffers
+  if ((rc = verify_range(h)) != SOMA_OK) return rc;     // synchronises: the caller may reuse its buffers
+  h->steps_since_sort = 0;
+  if (h->resort_interval > 0 && (rc = resort(h)) != SOMA_OK) return rc;
   h->loaded = true;
   return SOMA_OK;
 }
@@ -440,8 +546,16 @@ int soma_mc_steps(soma_t* h, uint32_t n_steps, uint64_t* accepted) {
   if (!h->loaded) return fail(h, SOMA_ESTATE, "soma_mc_steps before soma_load_state");
   if (h->step + n_steps >= (1ull << 48)) return fail(h, SOMA_EINVAL, "step index would reach 2^48");
   CU(h, cudaMemsetAsync(h->accepted(), 0, 8, h->stream));
-  for (uint32_t s = 0; s < n_steps; ++s)
+  for (uint32_t s = 0; s < n_steps; ++s) {
+    if (h->steps_since_check >= h->range_check_interval) {
+      range_check_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
+          h->grid, h->B, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2), h->range_flag());
+      h->launches++;
+      CU(h, cudaGetLastError());
+      if ((rc = verify_range(h)) != SOMA_OK) return rc;
+    }
     if ((rc = one_step(h)) != SOMA_OK) return rc;
+  }
   if (accepted) {
     unsigned long long v = 0;
     CU(h, cudaMemcpyAsync(&v, h->accepted(), 8, cudaMemcpyDeviceToHost, h->stream));
@@ -522,8 +636,24 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     return SOMA_OK;
   }
   if (!std::strcmp(name, "resort_interval")) {
-    if (value != 0) return fail(h, SOMA_EINVAL, "chain re-ordering is not available in this build");
+    if (value < 0) return fail(h, SOMA_EINVAL, "resort_interval must be >= 0");
     h->resort_interval = value;
+    return SOMA_OK;
+  }
+  if (!std::strcmp(name, "resort_now")) {
+    int rc = check(h);
+    if (rc != SOMA_OK) return rc;
+    if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
+    return resort(h);
+  }
+  if (!std::strcmp(name, "fused_blocks_per_sm")) {
+    if (value < 1 || value > 32) return fail(h, SOMA_EINVAL, "fused_blocks_per_sm must be in [1, 32]");
+    h->fused_blocks_per_sm = (int)value;
+    return SOMA_OK;
+  }
+  if (!std::strcmp(name, "fused_waves")) {
+    if (value < 1 || value > 1024) return fail(h, SOMA_EINVAL, "fused_waves must be in [1, 1024]");
+    h->fused_waves = (int)value;
     return SOMA_OK;
   }
   return fail(h, SOMA_EINVAL, "unknown option name");
@@ -613,20 +743,23 @@ int soma_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, u
   DevBuf c, o;
   CUG(c.alloc(n * 16)); CUG(o.alloc(n * 16));
   CUG(cudaMemcpy(c.p, ctr, n * 16, cudaMemcpyHostToDevice));
-  debug_philox_kernel<<<blocks_for(n, 256), 256>>>(n, (const uint32_t*)c.p, key[0], key[1], (uint32_t*)o.p);
+  PhiloxKeys K;
+  for (int r = 0; r < 10; ++r) { K.k0[r] = key[0] + (uint32_t)r * kPhiloxW0; K.k1[r] = key[1] + (uint32_t)r * kPhiloxW1; }
+  debug_philox_kernel<<<blocks_for(n, 256), 256>>>(n, (const uint32_t*)c.p, K, (uint32_t*)o.p);
   CUG(cudaGetLastError());
   CUG(cudaMemcpy(out, o.p, n * 16, cudaMemcpyDeviceToHost));
   return SOMA_OK;
 }
 
-int soma_debug_maps(const uint32_t* words, float* t, float* u, float* lnu, uint64_t n) {
+int soma_debug_maps(const uint32_t* words, float* t, float* u, float* lnu, float* lnu_fast, uint64_t n) {
   if (!words || !t || !u || !lnu) return fail(nullptr, SOMA_EINVAL, "NULL argument");
   if (n == 0) return SOMA_OK;
-  DevBuf w, a, b, c;
-  CUG(w.alloc(n * 4)); CUG(a.alloc(n * 4)); CUG(b.alloc(n * 4)); CUG(c.alloc(n * 4));
+  DevBuf w, a, b, c, d;
+  CUG(w.alloc(n * 4)); CUG(a.alloc(n * 4)); CUG(b.alloc(n * 4)); CUG(c.alloc(n * 4)); CUG(d.alloc(n * 4));
   CUG(cudaMemcpy(w.p, words, n * 4, cudaMemcpyHostToDevice));
-  debug_maps_kernel<<<blocks_for(n, 256), 256>>>(n, (const uint32_t*)w.p, (float*)a.p, (float*)b.p, (float*)c.p);
+  debug_maps_kernel<<<blocks_for(n, 256), 256>>>(n, (const uint32_t*)w.p, (float*)a.p, (float*)b.p, (float*)c.p, (float*)d.p);
   CUG(cudaGetLastError());
+  if (lnu_fast) CUG(cudaMemcpy(lnu_fast, d.p, n * 4, cudaMemcpyDeviceToHost));
   CUG(cudaMemcpy(t, a.p, n * 4, cudaMemcpyDeviceToHost));
   CUG(cudaMemcpy(u, b.p, n * 4, cudaMemcpyDeviceToHost));
   CUG(cudaMemcpy(lnu, c.p, n * 4, cudaMemcpyDeviceToHost));

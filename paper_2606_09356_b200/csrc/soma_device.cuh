@@ -34,6 +34,24 @@ __device__ __forceinline__ Words4 philox4x32_10(uint32_t c0, uint32_t c1, uint32
   return Words4{c0, c1, c2, c3};
 }
 
+// The same generator with the ten round keys (k + r*W) precomputed on the host and read from the
+// kernel's constant bank: every round is 2 IMAD.WIDE.U32 + 2 LOP3, no key arithmetic.
+struct PhiloxKeys { uint32_t k0[10], k1[10]; };
+
+__device__ __forceinline__ Words4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                const PhiloxKeys& K) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;
+    const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ K.k0[r];
+    c1 = (uint32_t)p1;
+    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ K.k1[r];
+    c3 = (uint32_t)p0;
+  }
+  return Words4{c0, c1, c2, c3};
+}
+
 // ---- uniform maps (R14) ----
 // tmap(w) = (2k+1) 2^-23 - 1 with k = w >> 9.  Built from the bit pattern instead of an int->float
 // conversion: as_float(0x3f800000 | k) - 1 = k 2^-23 exactly, then fma(2, ., 2^-23 - 1) is exact
@@ -42,27 +60,41 @@ __device__ __forceinline__ float tmap(uint32_t w) {
   const float h = __fadd_rn(__uint_as_float(0x3f800000u | (w >> 9)), -1.0f);
   return __fmaf_rn(2.0f, h, -0.99999988079071044921875f);   // 2^-23 - 1
 }
-// u = ((w >> 8) + 1) 2^-24 in (0, 1]; the integer (w >> 8) + 1 <= 2^24 converts exactly.
-__device__ __forceinline__ float umap_int(uint32_t w) { return (float)((w >> 8) + 1u); }   // = u * 2^24
+// u * 2^24 = (w >> 8) + 1 in [1, 2^24]: the integer converts exactly (I2FP.F32.U32, one instruction).
+__device__ __forceinline__ float umap_int(uint32_t w) { return (float)((w >> 8) + 1u); }
 __device__ __forceinline__ float umap(uint32_t w) { return __fmul_rn(umap_int(w), 0x1p-24f); }
 
 // lnu = ln(u) correctly rounded to fp32 (R6b), slow path: double log, one rounding.
 __device__ __noinline__ float lnu_exact(float u) { return (float)log((double)u); }
 
+// hardware base-2 logarithm, one MUFU.LG2 (the argument is a normal number in [1, 2^24])
+__device__ __forceinline__ float lg2_approx(float v) {
+  float r;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
+  return r;
+}
+
+// ln(u) by the fast route, |error| < kLnBand/16 over all 2^24 values of u (checked exhaustively by
+// tests/test_gpu_units.py through soma_debug_maps).
+__device__ __forceinline__ float lnu_fast(uint32_t w3) {
+  return __fmul_rn(__fadd_rn(lg2_approx(umap_int(w3)), -24.0f), 0.693147182464599609375f);
+}
+constexpr float kLnBand = 1.0e-4f;
+
 // ---- Metropolis decision (DESIGN.md section 2 step 5.6): accept iff fl32(dE + lnu) <= 0 ----
 // Result-equivalent shortcuts:
 //  * dE <= 0: lnu <= 0, so the fp32 sum is <= 0 -> accept without looking at u.
-//  * otherwise m~ = dE + ln2*(log2(k) - 24) with the hardware log2 (absolute error of ln u below
-//    6e-6 over k in [1, 2^24]); if |m~| > 1e-4 the sign of the exact margin
-//    is the sign of m~.  Only the ~6e-5 of moves inside that band take the double-precision path.
+//  * otherwise m~ = dE + lnu_fast; if |m~| > kLnBand the sign of the exact margin is the sign of m~
+//    (the fp32 rounding of dE + lnu moves it by < 1e-6).  Only the ~6e-5 of moves inside that band
+//    take the double-precision path.
 __device__ __forceinline__ bool metropolis_accept(float dE, uint32_t w3) {
-  if (dE <= 0.0f) return true;
-  const float kf = umap_int(w3);
-  const float l2 = __fadd_rn(__log2f(kf), -24.0f);
-  const float m_fast = __fmaf_rn(l2, 0.693147182464599609375f, dE);
-  if (fabsf(m_fast) > 1.0e-4f) return m_fast < 0.0f;
-  const float m = __fadd_rn(dE, lnu_exact(__fmul_rn(kf, 0x1p-24f)));
-  return m <= 0.0f;
+  const float m_fast = __fadd_rn(dE, lnu_fast(w3));
+  bool acc = (dE <= 0.0f) | (m_fast < -kLnBand);
+  if (dE > 0.0f && fabsf(m_fast) <= kLnBand) {
+    const float m = __fadd_rn(dE, lnu_exact(umap(w3)));
+    acc = m <= 0.0f;
+  }
+  return acc;
 }
 
 // ---- geometry ----
@@ -81,12 +113,26 @@ __device__ __forceinline__ uint32_t wrap(int g, uint32_t n) {
   return (uint32_t)g;
 }
 
-// DESIGN.md section 2 step 1 (R8, R12).  cvt.rmi.s32.f32 = floor then convert.
+// floor(s) mod n for n a power of two without a conversion: s + 1.5*2^23 rounded DOWN has ulp 1, so
+// its bit pattern is 0x4b400000 + floor(s) for |s| < 2^22, and the low bits under the mask n-1 are
+// the non-negative residue (two's complement borrow for negative floors).  The library checks
+// |s| < 2^21 when positions are loaded and re-checks before a bead could have drifted out of range.
+constexpr float kFloorMagic = 12582912.0f;       // 1.5 * 2^23
+constexpr float kCellCoordLimit = 2097152.0f;    // 2^21
+__device__ __forceinline__ uint32_t floor_bits(float s) { return __float_as_uint(__fadd_rd(s, kFloorMagic)); }
+
+// DESIGN.md section 2 step 1 (R8, R12).  Generic grids: cvt.rmi.s32.f32 = floor then convert.
 template <bool POW2>
 __device__ __forceinline__ uint32_t cell_of(const Grid& g, float x, float y, float z) {
-  const uint32_t ix = wrap<POW2>(__float2int_rd(__fmul_rn(x, g.inv_hx)), g.nx);
-  const uint32_t iy = wrap<POW2>(__float2int_rd(__fmul_rn(y, g.inv_hy)), g.ny);
-  const uint32_t iz = wrap<POW2>(__float2int_rd(__fmul_rn(z, g.inv_hz)), g.nz);
+  if (POW2) {
+    const uint32_t ix = floor_bits(__fmul_rn(x, g.inv_hx)) & (g.nx - 1u);
+    const uint32_t iy = floor_bits(__fmul_rn(y, g.inv_hy)) & (g.ny - 1u);
+    const uint32_t iz = floor_bits(__fmul_rn(z, g.inv_hz)) & (g.nz - 1u);
+    return (ix * g.ny + iy) * g.nz + iz;
+  }
+  const uint32_t ix = wrap<false>(__float2int_rd(__fmul_rn(x, g.inv_hx)), g.nx);
+  const uint32_t iy = wrap<false>(__float2int_rd(__fmul_rn(y, g.inv_hy)), g.ny);
+  const uint32_t iz = wrap<false>(__float2int_rd(__fmul_rn(z, g.inv_hz)), g.nz);
   return (ix * g.ny + iy) * g.nz + iz;
 }
 

@@ -8,6 +8,9 @@
 //   half_sweep_kernel      rows a1/a2 for any N (one thread per same-parity bead, neighbours from
 //                          global memory); bin_kernel = row a3.  The generic path.
 //   omega_kernel<T>        row a4: omega from the fresh counts; also zeroes the other count buffer.
+//   chain_key / bin_scan / chain_permute   internal re-ordering of the chains in memory by the
+//                          coarse cell of their middle bead (results do not depend on it: the
+//                          random stream is keyed by the logical chain id).
 #pragma once
 
 #include "soma_device.cuh"
@@ -24,7 +27,7 @@ struct StepArgs {
   uint32_t N;                 // beads per chain
   float a;                    // trial half-width
   float kb;                   // 1.5f/(b*b)
-  uint32_t key0, key1;        // Philox key = (seed lo, seed hi)
+  PhiloxKeys keys;            // round keys of (seed lo, seed hi)
   uint32_t ctr2;              // (uint32) step
   uint32_t ctr3_base;         // domain << 8 | (uint32)(step >> 32) << 16; parity is or-ed in
   float* __restrict__ x;      // positions in slot order: bead i of slot s at s*N + i
@@ -46,7 +49,7 @@ __device__ __forceinline__ bool move_bead(const StepArgs& A, uint32_t chain, uin
                                           float& rx, float& ry, float& rz, uint32_t& cell,
                                           bool has_l, float lx, float ly, float lz,
                                           bool has_r, float qx, float qy, float qz) {
-  const Words4 w = philox4x32_10(i, chain, A.ctr2, A.ctr3_base | parity, A.key0, A.key1);
+  const Words4 w = philox4x32_10(i, chain, A.ctr2, A.ctr3_base | parity, A.keys);
   const Trial t = trial_position(rx, ry, rz, A.a, w);
   float dq = 0.0f;
   if (has_l) dq = __fsub_rn(bond_sq(t.x, t.y, t.z, lx, ly, lz), bond_sq(rx, ry, rz, lx, ly, lz));
@@ -91,37 +94,56 @@ half_sweep_kernel(StepArgs A, uint32_t parity, uint32_t n_par /* beads of this p
   if ((threadIdx.x & 31u) == 0 && n_acc) atomicAdd(A.accepted, (unsigned long long)n_acc);
 }
 
+// Row a3 on its own.  `range_flag` (may be null) is set to 1 if any bead's cell coordinate leaves
+// the range in which the conversion-free floor of soma_device.cuh is exact.
 template <bool POW2>
 __global__ void __launch_bounds__(256)
 bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint64_t B, const float* __restrict__ x,
            const float* __restrict__ y, const float* __restrict__ z,
            const uint8_t* __restrict__ slot_pattern, const uint8_t* __restrict__ patterns,
-           uint32_t* __restrict__ counts) {
+           uint32_t* __restrict__ counts, uint32_t* __restrict__ range_flag) {
   const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= B) return;
   const uint32_t slot = (uint32_t)(j / N), i = (uint32_t)(j % N);
   const uint32_t type = patterns[(uint32_t)slot_pattern[slot] * N + i];
-  atomicAdd(counts + (size_t)type * cells + cell_of<POW2>(grid, x[j], y[j], z[j]), 1u);
+  const float px = x[j], py = y[j], pz = z[j];
+  if (range_flag) {
+    const float m = fmaxf(fabsf(__fmul_rn(px, grid.inv_hx)), fmaxf(fabsf(__fmul_rn(py, grid.inv_hy)), fabsf(__fmul_rn(pz, grid.inv_hz))));
+    if (!(m < kCellCoordLimit)) *range_flag = 1u;            // also catches NaN
+  }
+  atomicAdd(counts + (size_t)type * cells + cell_of<POW2>(grid, px, py, pz), 1u);
 }
 
 // ---------------------------------------------------------------------------------------------
 // Fused path: N = 2P, P in {1,2,4,8,16,32}.  Lane l of a P-lane group holds beads 2l and 2l+1.
-// A warp carries 32/P chains; warps walk the slot list with a grid stride.
+// A warp carries G = 32/P chains.  Every block owns a CONTIGUOUS run of `groups_per_block` warp
+// groups of the slot list and its warps walk that run side by side, so that -- the chains being
+// kept sorted by position -- the omega gathers of a block stay inside a small neighbourhood that
+// the L1 keeps, and the atomics of concurrently running blocks fall into a bounded part of L2.
 // ---------------------------------------------------------------------------------------------
-template <int P, bool POW2>
+template <int P, bool POW2, bool MULTI_PAT>
 __global__ void __launch_bounds__(256)
-fused_step_kernel(StepArgs A) {
+fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
   constexpr int G = 32 / P;                                   // chains per warp
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t l = lane % P;                                // position of the lane in its chain
-  const uint32_t warps_per_block = blockDim.x >> 5;
-  const uint64_t warp0 = (uint64_t)blockIdx.x * warps_per_block + (threadIdx.x >> 5);
-  const uint64_t n_warps = (uint64_t)gridDim.x * warps_per_block;
+  const uint32_t sub = lane / P;                              // which of the warp's chains
+  const uint32_t wpb = blockDim.x >> 5;
   const uint64_t n_groups = ((uint64_t)A.n_chains + G - 1) / G;
+  const uint64_t g_begin = (uint64_t)blockIdx.x * groups_per_block;
+  uint64_t g_end = g_begin + groups_per_block;
+  if (g_end > n_groups) g_end = n_groups;
   unsigned n_acc = 0;
 
-  for (uint64_t wg = warp0; wg < n_groups; wg += n_warps) {
-    const uint64_t slot64 = wg * G + lane / P;
+  // bead types of this lane (loop-invariant when every chain has the same pattern)
+  uint32_t type0 = 0, type1 = 0;
+  if (!MULTI_PAT) {
+    const uint16_t tt = *reinterpret_cast<const uint16_t*>(A.patterns + 2u * l);
+    type0 = tt & 0xffu; type1 = tt >> 8;
+  }
+
+  for (uint64_t wg = g_begin + (threadIdx.x >> 5); wg < g_end; wg += wpb) {
+    const uint64_t slot64 = wg * G + sub;
     const bool live = slot64 < A.n_chains;
     const uint32_t slot = live ? (uint32_t)slot64 : 0u;       // dead lanes shadow slot 0, never store
     const uint64_t j = (uint64_t)slot * A.N + 2u * l;
@@ -129,8 +151,10 @@ fused_step_kernel(StepArgs A) {
     const float2 Y = *reinterpret_cast<const float2*>(A.y + j);
     const float2 Z = *reinterpret_cast<const float2*>(A.z + j);
     const uint32_t chain = A.slot_chain[slot];
-    const uint8_t* pat = A.patterns + (uint32_t)A.slot_pattern[slot] * A.N + 2u * l;
-    const uint32_t type0 = pat[0], type1 = pat[1];
+    if (MULTI_PAT) {
+      const uint16_t tt = *reinterpret_cast<const uint16_t*>(A.patterns + (uint32_t)A.slot_pattern[slot] * A.N + 2u * l);
+      type0 = tt & 0xffu; type1 = tt >> 8;
+    }
     const float* om0 = A.omega + (size_t)type0 * A.cells;
     const float* om1 = A.omega + (size_t)type1 * A.cells;
 
@@ -213,6 +237,100 @@ omega_kernel(OmegaArgs A) {
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Chain re-ordering: a counting sort of the slots by the coarse bin (cb^3 cells, row-major) that
+// holds the chain's middle bead.  key -> per-bin count and rank (one atomic with return per chain),
+// exclusive scan of the bin counts, then every chain is copied to slot bin_start[bin] + rank.
+// The rank order inside a bin depends on atomic arrival order; nothing observable depends on the
+// slot a chain sits in.
+// ---------------------------------------------------------------------------------------------
+struct SortArgs {
+  Grid grid;
+  uint32_t n_chains, N;
+  uint32_t cb;                     // coarse bin edge in cells
+  uint32_t ncy, ncz;               // coarse bins along y and z (x is implied)
+  uint32_t n_bins;
+};
+
+template <bool POW2>
+__global__ void __launch_bounds__(256)
+chain_key_kernel(SortArgs S, const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ z,
+                 uint32_t* __restrict__ bin_count, uint32_t* __restrict__ key, uint32_t* __restrict__ rank) {
+  const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= S.n_chains) return;
+  const uint64_t j = (uint64_t)s * S.N + S.N / 2u;
+  const uint32_t cell = cell_of<POW2>(S.grid, x[j], y[j], z[j]);
+  const uint32_t iz = cell % S.grid.nz, iy = (cell / S.grid.nz) % S.grid.ny, ix = cell / (S.grid.nz * S.grid.ny);
+  const uint32_t bin = ((ix / S.cb) * S.ncy + iy / S.cb) * S.ncz + iz / S.cb;
+  key[s] = bin;
+  rank[s] = atomicAdd(bin_count + bin, 1u);
+}
+
+// exclusive scan of `n` counts in place, one block; n is at most a few million
+__global__ void __launch_bounds__(1024)
+bin_scan_kernel(uint32_t n, uint32_t* __restrict__ v) {
+  __shared__ uint32_t warp_sum[32];
+  __shared__ uint32_t carry_s;
+  const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (uint32_t base = 0; base < n; base += 1024u) {
+    const uint32_t k = base + threadIdx.x;
+    const uint32_t val = k < n ? v[k] : 0u;
+    uint32_t inc = val;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= (uint32_t)o) inc += t;
+    }
+    if (lane == 31) warp_sum[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+      uint32_t ws = warp_sum[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, ws, o);
+        if (lane >= (uint32_t)o) ws += t;
+      }
+      warp_sum[lane] = ws;                                   // inclusive over warps
+    }
+    __syncthreads();
+    const uint32_t carry = carry_s;
+    const uint32_t before = carry + (w ? warp_sum[w - 1] : 0u) + inc - val;
+    if (k < n) v[k] = before;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry_s = carry + warp_sum[31];
+    __syncthreads();
+  }
+}
+
+// one thread per bead: slot s -> slot bin_start[key[s]] + rank[s]
+__global__ void __launch_bounds__(256)
+chain_permute_kernel(uint64_t B, uint32_t N, const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ key,
+                     const uint32_t* __restrict__ rank,
+                     const float* __restrict__ sx, const float* __restrict__ sy, const float* __restrict__ sz,
+                     float* __restrict__ dx, float* __restrict__ dy, float* __restrict__ dz,
+                     const uint32_t* __restrict__ s_chain, const uint8_t* __restrict__ s_pat,
+                     uint32_t* __restrict__ d_chain, uint8_t* __restrict__ d_pat) {
+  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= B) return;
+  const uint32_t s = (uint32_t)(j / N), i = (uint32_t)(j % N);
+  const uint32_t d = bin_start[key[s]] + rank[s];
+  const uint64_t k = (uint64_t)d * N + i;
+  dx[k] = sx[j]; dy[k] = sy[j]; dz[k] = sz[j];
+  if (i == 0) { d_chain[d] = s_chain[s]; d_pat[d] = s_pat[s]; }
+}
+
+// sets *range_flag if a bead's cell coordinate is NaN or beyond kCellCoordLimit (see floor_bits)
+__global__ void __launch_bounds__(256)
+range_check_kernel(Grid grid, uint64_t B, const float* __restrict__ x, const float* __restrict__ y,
+                   const float* __restrict__ z, uint32_t* __restrict__ range_flag) {
+  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= B) return;
+  const float m = fmaxf(fabsf(__fmul_rn(x[j], grid.inv_hx)), fmaxf(fabsf(__fmul_rn(y[j], grid.inv_hy)), fabsf(__fmul_rn(z[j], grid.inv_hz))));
+  if (!(m < kCellCoordLimit)) *range_flag = 1u;
+}
+
 // ---- data movement helpers ----
 // dst[slot_chain[s]*N + i] = src[s*N + i]  (slot order -> caller's chain order), one thread per bead
 __global__ void __launch_bounds__(256)
@@ -233,18 +351,19 @@ iota_kernel(uint32_t n, uint32_t* __restrict__ out) {
 }
 
 // ---- test hooks ----
-__global__ void debug_philox_kernel(uint64_t n, const uint32_t* ctr, uint32_t k0, uint32_t k1, uint32_t* out) {
+__global__ void debug_philox_kernel(uint64_t n, const uint32_t* ctr, PhiloxKeys K, uint32_t* out) {
   const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= n) return;
-  const Words4 w = philox4x32_10(ctr[4 * k], ctr[4 * k + 1], ctr[4 * k + 2], ctr[4 * k + 3], k0, k1);
+  const Words4 w = philox4x32_10(ctr[4 * k], ctr[4 * k + 1], ctr[4 * k + 2], ctr[4 * k + 3], K);
   out[4 * k] = w.w0; out[4 * k + 1] = w.w1; out[4 * k + 2] = w.w2; out[4 * k + 3] = w.w3;
 }
-__global__ void debug_maps_kernel(uint64_t n, const uint32_t* words, float* t, float* u, float* lnu) {
+__global__ void debug_maps_kernel(uint64_t n, const uint32_t* words, float* t, float* u, float* lnu, float* lnu_f) {
   const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= n) return;
   t[k] = tmap(words[k]);
   u[k] = umap(words[k]);
   lnu[k] = lnu_exact(umap(words[k]));
+  if (lnu_f) lnu_f[k] = lnu_fast(words[k]);
 }
 __global__ void debug_accept_kernel(uint64_t n, const float* dE, const uint32_t* words, uint8_t* out) {
   const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;

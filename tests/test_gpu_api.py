@@ -163,7 +163,7 @@ def test_launch_counter_counts_kernels(small):
         g.mc_steps(5)
         after = g.counters()
         assert after["steps"] - before["steps"] == 5
-        assert after["launches"] - before["launches"] == 5 * 2          # fused move+bin, omega
+        assert after["launches"] - before["launches"] == 5 * 2 + 3 * (after["resorts"] - before["resorts"])   # fused move+bin, omega
     with gpu_system(s, path=1) as g:
         g.load_state(s.x, s.y, s.z)
         before = g.counters()

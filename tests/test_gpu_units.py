@@ -57,16 +57,19 @@ def test_uniform_maps_and_lnu_all_2_24_values(soma):
     rounded one (R6b), i.e. the oracle's bits."""
     k = np.arange(1 << 24, dtype=np.uint32)
     words = (k << np.uint32(8)) | np.uint32(0xA5)
-    t, u, l = soma.soma_debug_maps(words)
+    t, u, l, lf = soma.soma_debug_maps(words)
     u_want = ((k.astype(np.float64) + 1.0) * 2.0 ** -24).astype(np.float32)
     assert np.array_equal(u, u_want)
     k23 = (words >> np.uint32(9)).astype(np.float64)
     t_want = ((2.0 * k23 + 1.0) * 2.0 ** -23 - 1.0).astype(np.float32)      # exact in double
     assert np.array_equal(t, t_want)
     assert np.array_equal(l.view(np.uint32), oracle.lnu(u_want).view(np.uint32))
+    # the hardware logarithm that decides every move outside the +-1e-4 band is far inside that band
+    err = np.abs(lf.astype(np.float64) - np.log(u_want.astype(np.float64)))
+    assert err.max() < 1e-4 / 16, err.max()
     # spot check against the oracle's own scalar maps
     for w in (0, 1, 0x1FF, 0x200, 0x7FFFFFFF, 0x80000000, 0xFFFFFFFF, 0xFFFFFE00, 0xDEADBEEF):
-        tt, uu, _ = soma.soma_debug_maps(np.array([w], dtype=np.uint32))
+        tt, uu, _, _ = soma.soma_debug_maps(np.array([w], dtype=np.uint32))
         assert float(tt[0]) == oracle.tmap(w) and float(uu[0]) == oracle.umap(w)
 
 
