@@ -119,7 +119,12 @@ const char *soma_last_error(const soma_t *h);
 
 /* Tuning / test switches.  Names:
  *   "path"            0 = automatic, 1 = generic kernels (4 launches/step, any N),
- *                     2 = fused chain-in-registers kernel (N = 2P, P a power of two <= 32; else EINVAL)
+ *                     2 = fused chain-in-registers kernel (N = 2P, P a power of two <= 32; else EINVAL),
+ *                     3 = tiled kernel: omega and density tiles in shared memory, moved by TMA (as 2,
+ *                         plus: power-of-two grid axes >= 16 and >= the tile; else EINVAL)
+ *   "tile_cx|cy|cz", "tile_hx|hy|hz"   tile core and halo in cells (defaults 12,12,8 and 6,6,6);
+ *   "tile_threads"    512, 768 or 1024 threads per CTA of the tiled kernel.  A combination the
+ *                     tiled kernel cannot use switches it off (see soma_get_counters [3])
  *   "kernel_timing"   1 = record CUDA events on the handle's stream around the kernels of every step
  *                     (read them with soma_get_kernel_times), 0 = off (default)
  *   "resort_interval" re-order the chains in memory by position at soma_load_state and then every k
@@ -131,7 +136,8 @@ const char *soma_last_error(const soma_t *h);
 int soma_set_option(soma_t *h, const char *name, int64_t value);
 
 /* Counters since soma_create: [0] kernels launched by this library, [1] MC steps done,
- * [2] chain re-orderings done.  `out` is a host pointer to 3 uint64. */
+ * [2] chain re-orderings done; [3] the kernel path the next step will take (1, 2 or 3).
+ * `out` is a host pointer to 4 uint64. */
 int soma_get_counters(const soma_t *h, uint64_t *out);
 
 /* Device time spent since the last call (or since "kernel_timing" was switched on), summed over the

@@ -197,9 +197,9 @@ def soma_set_option(h, name: str, value: int):
 
 
 def soma_get_counters(h) -> dict:
-    out = (C.c_uint64 * 3)()
+    out = (C.c_uint64 * 4)()
     _check(load_library().soma_get_counters(h, out), h)
-    return {"launches": int(out[0]), "steps": int(out[1]), "resorts": int(out[2])}
+    return {"launches": int(out[0]), "steps": int(out[1]), "resorts": int(out[2]), "path": int(out[3])}
 
 
 def soma_get_kernel_times(h) -> dict:

@@ -9,7 +9,7 @@
 #include <string>
 #include <vector>
 
-#include "soma_kernels.cuh"
+#include "soma_tile.cuh"
 
 using namespace soma;
 
@@ -32,7 +32,9 @@ struct Layout {            // byte offsets into the workspace
   uint64_t range_flag;     // uint32
   uint64_t sort_key;       // [n] uint32
   uint64_t sort_rank;      // [n] uint32
-  uint64_t sort_bins;      // [n_bins] uint32
+  uint64_t sort_bins;      // [n_bins_max + 1] uint32: bin counts, then bin starts (= tile_start)
+  uint64_t omega_pad;      // [T][pad cells] fp32: ghost-padded omega for the tile loads (0 bytes if unused)
+  uint64_t counts_pad[2];  // [T][pad cells] uint32: ghost-padded density grids the tiles flush into
   uint64_t total;
 };
 
@@ -44,7 +46,20 @@ uint64_t sort_bin_count(const uint32_t grid[3]) {
   return n;
 }
 
-Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins) {
+// the ghost-padded omega copy is sized for the largest tile the options allow
+constexpr uint32_t kMaxTileCore = 32, kMaxTileHalo = 16;
+uint64_t omega_pad_cells_max(const uint32_t grid[3]) {
+  uint64_t n = 1;
+  for (int d = 0; d < 3; ++d) n *= (uint64_t)grid[d] + kMaxTileCore + 2 * kMaxTileHalo + 3;
+  return n;
+}
+bool tile_capable_grid(const uint32_t grid[3]) {      // power-of-two axes, at least 16 cells each
+  for (int d = 0; d < 3; ++d)
+    if (grid[d] < 16 || (grid[d] & (grid[d] - 1))) return false;
+  return true;
+}
+
+Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins, uint64_t pad_words) {
   Layout L{};
   uint64_t off = 0;
   for (int s = 0; s < 2; ++s)
@@ -59,7 +74,9 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   L.range_flag = off; off += align_up(4);
   L.sort_key = off; off += align_up(n * 4);
   L.sort_rank = off; off += align_up(n * 4);
-  L.sort_bins = off; off += align_up(n_bins * 4);
+  L.sort_bins = off; off += align_up((n_bins + 1) * 4);
+  L.omega_pad = off; off += align_up(pad_words * 4);
+  for (int s = 0; s < 2; ++s) { L.counts_pad[s] = off; off += align_up(pad_words * 4); }
   L.total = off;
   return L;
 }
@@ -143,6 +160,22 @@ struct soma_handle {
   int path;              // 0 auto, 1 generic, 2 fused
   int64_t resort_interval;      // re-order the chains every k steps (0 = never)
   int fused_blocks_per_sm, fused_waves;
+  // tiled kernel (soma_tile.cuh)
+  bool tile_grid_ok;            // the grid allows tiles at all
+  bool tile_ready;              // geometry + tensor maps are set up for the current options
+  uint32_t tc[3], th[3];        // tile core and halo in cells
+  int tile_threads;             // 512, 768 or 1024
+  uint32_t te[3], tm[3], n_tiles, pad[3];
+  size_t tile_smem;
+  uint32_t tile_counts_offset;
+  CUtensorMap tm_omega, tm_counts[2];
+  int sorted_kind;              // bins the slots are currently sorted by: 0 none, 1 cubes of 4 cells, 2 tiles
+  bool tile_auto;               // path 0 picks the tiled kernel
+  bool pad_valid;               // the ghost-padded omega copy matches the linear field
+  int pad_cur;                  // padded density grid the next tiled step bins into (zeroed)
+  bool counts_in_pad;           // the last move kernel binned into counts_pad(pad_cur), not into the linear grid
+  bool omega_custom;            // omega was overwritten by soma_debug_set_omega (tiles off until the next load)
+  char tile_why[96];            // why tiles are unavailable ("" if they are)
   // counters
   uint64_t launches, steps_done, resorts;
   // per-kernel timing ("kernel_timing" option): event triples (before moves, after moves+bin, after omega)
@@ -163,6 +196,8 @@ struct soma_handle {
   uint32_t* sort_key() const { return reinterpret_cast<uint32_t*>(ws + L.sort_key); }
   uint32_t* sort_rank() const { return reinterpret_cast<uint32_t*>(ws + L.sort_rank); }
   uint32_t* sort_bins() const { return reinterpret_cast<uint32_t*>(ws + L.sort_bins); }
+  float* omega_pad() const { return reinterpret_cast<float*>(ws + L.omega_pad); }
+  uint32_t* counts_pad(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts_pad[s]); }
   uint8_t* patterns() const { return reinterpret_cast<uint8_t*>(ws + L.patterns); }
   uint8_t* pattern0() const { return reinterpret_cast<uint8_t*>(ws + L.pattern0); }
   unsigned long long* accepted() const { return reinterpret_cast<unsigned long long*>(ws + L.accepted); }
@@ -247,6 +282,8 @@ int launch_bin(soma_handle* h, uint32_t* counts, bool check_range = false) {
 }
 
 // omega from counts(cur); zero counts(cur^1) for the next step's binning.
+bool use_tile(const soma_handle* h);
+
 int launch_omega(soma_handle* h) {
   OmegaArgs A{};
   A.cells = h->cells; A.T = h->T;
@@ -255,12 +292,30 @@ int launch_omega(soma_handle* h) {
   A.counts = h->counts(h->cur);
   A.counts_to_zero = h->counts(h->cur ^ 1);
   A.omega = h->omega();
-  const unsigned g = blocks_for(h->cells, 256);
-  switch (h->T) {
-    case 1: omega_kernel<1><<<g, 256, 0, h->stream>>>(A); break;
-    case 2: omega_kernel<2><<<g, 256, 0, h->stream>>>(A); break;
-    case 3: omega_kernel<3><<<g, 256, 0, h->stream>>>(A); break;
-    default: omega_kernel<0><<<g, 256, 0, h->stream>>>(A); break;
+  if (use_tile(h)) {            // also fills the ghost-padded copy the tiles are loaded from
+    PadGeom pg{h->pad[0], h->pad[1], h->pad[2], h->th[0], h->th[1], h->th[2]};
+    const unsigned g = blocks_for((uint64_t)h->pad[0] * h->pad[1] * h->pad[2], 256);
+    const uint32_t* in = h->counts_in_pad ? h->counts_pad(h->pad_cur) : nullptr;   // fold the tiles' ghost layers
+    uint32_t* out = h->counts(h->cur);
+    uint32_t* zero = h->counts_pad(h->pad_cur ^ 1);
+    switch (h->T) {
+      case 1: omega_pad_kernel<1><<<g, 256, 0, h->stream>>>(A, h->grid, pg, h->omega_pad(), in, out, zero); break;
+      case 2: omega_pad_kernel<2><<<g, 256, 0, h->stream>>>(A, h->grid, pg, h->omega_pad(), in, out, zero); break;
+      case 3: omega_pad_kernel<3><<<g, 256, 0, h->stream>>>(A, h->grid, pg, h->omega_pad(), in, out, zero); break;
+      default: omega_pad_kernel<0><<<g, 256, 0, h->stream>>>(A, h->grid, pg, h->omega_pad(), in, out, zero); break;
+    }
+    if (h->counts_in_pad) h->pad_cur ^= 1;       // the grid just folded is zeroed by the NEXT omega pass
+    h->counts_in_pad = false;
+    h->pad_valid = true;
+  } else {
+    h->pad_valid = false;
+    const unsigned g = blocks_for(h->cells, 256);
+    switch (h->T) {
+      case 1: omega_kernel<1><<<g, 256, 0, h->stream>>>(A); break;
+      case 2: omega_kernel<2><<<g, 256, 0, h->stream>>>(A); break;
+      case 3: omega_kernel<3><<<g, 256, 0, h->stream>>>(A); break;
+      default: omega_kernel<0><<<g, 256, 0, h->stream>>>(A); break;
+    }
   }
   h->launches++;
   CU(h, cudaGetLastError());
@@ -308,23 +363,159 @@ bool use_fused(const soma_handle* h) {
   if (h->path == 1) return false;
   return fused_lanes(h->N) != 0;
 }
+bool use_tile(const soma_handle* h) {
+  if (!h->tile_ready || h->omega_custom) return false;
+  return h->path == 3 || (h->path == 0 && h->tile_auto);
+}
 
-// Re-order the chains in memory by the coarse bin of their middle bead (counting sort on the device).
-int resort(soma_handle* h) {
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 4-D tensor map over a [T][X][Y][Z] array (Z fastest) with a [T][ex][ey][ez] box
+bool encode_map(EncodeTiledFn enc, CUtensorMap* tm, CUtensorMapDataType dt, void* base, uint32_t T, const uint32_t dims[3],
+                const uint32_t box[3]) {
+  const cuuint64_t gdim[4] = {dims[2], dims[1], dims[0], T};
+  const cuuint64_t gstr[3] = {(cuuint64_t)dims[2] * 4, (cuuint64_t)dims[2] * dims[1] * 4, (cuuint64_t)dims[2] * dims[1] * dims[0] * 4};
+  const cuuint32_t bdim[4] = {box[2], box[1], box[0], T};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  return enc(tm, dt, 4, base, gdim, gstr, bdim, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int P, int NT>
+cudaError_t tile_attr(size_t smem) {
+  cudaError_t e = cudaFuncSetAttribute(tile_step_kernel<P, false, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, true, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  return e;
+}
+template <int NT>
+cudaError_t tile_attr_p(int P, size_t smem) {
+  switch (P) {
+    case 1: return tile_attr<1, NT>(smem);   case 2: return tile_attr<2, NT>(smem);
+    case 4: return tile_attr<4, NT>(smem);   case 8: return tile_attr<8, NT>(smem);
+    case 16: return tile_attr<16, NT>(smem); case 32: return tile_attr<32, NT>(smem);
+  }
+  return cudaErrorInvalidValue;
+}
+
+// Derive the tile geometry from the options and build the tensor maps.  Leaves tile_ready false
+// (with the reason in h->tile_why) when tiles cannot be used; that is not an error.
+void tile_setup(soma_handle* h) {
+  h->tile_ready = false;
+  h->tile_auto = false;
+  h->pad_valid = false;
+  auto no = [&](const char* why) { snprintf(h->tile_why, sizeof h->tile_why, "%s", why); };
+  if (!h->tile_grid_ok) return no("grid axes must be powers of two >= 16");
+  const int P = fused_lanes(h->N);
+  if (!P) return no("beads_per_chain must be 2P, P a power of two <= 32");
+  const uint32_t n[3] = {h->grid.nx, h->grid.ny, h->grid.nz};
+  uint64_t E = 1, nt = 1;
+  for (int d = 0; d < 3; ++d) {
+    if (h->tc[d] < 4 || h->tc[d] > kMaxTileCore || h->th[d] > kMaxTileHalo) return no("tile core must be in [4, 32], halo <= 16");
+    h->te[d] = h->tc[d] + 2 * h->th[d];
+    if (h->te[d] > n[d]) return no("tile (core + 2 halo) is larger than the grid");
+    h->tm[d] = (n[d] + h->tc[d] - 1) / h->tc[d];
+    h->pad[d] = h->tm[d] * h->tc[d] + 2 * h->th[d];
+    E *= h->te[d];
+    nt *= h->tm[d];
+  }
+  if (h->tc[2] % 4 || h->te[2] % 4) return no("tile core and extent along z must be multiples of 4 cells");
+  for (int d = 0; d < 3; ++d)
+    if (h->pad[d] > 2 * n[d]) return no("padded grid would hold a cell three times");
+  h->pad[2] = (h->pad[2] + 3u) / 4u * 4u;
+  if (nt > h->n_bins) return no("too many tiles");
+  h->n_tiles = (uint32_t)nt;
+  const uint64_t tile_bytes = E * h->T * 4;
+  h->tile_counts_offset = (uint32_t)((tile_bytes + 127) / 128 * 128);
+  h->tile_smem = (size_t)h->tile_counts_offset + tile_bytes;
+  if (h->tile_smem > 227 * 1024 - 1024) return no("tile does not fit in shared memory");
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) {
+    cudaGetLastError();
+    return no("cuTensorMapEncodeTiled is not available");
+  }
+  EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(fn);
+  if (!encode_map(enc, &h->tm_omega, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, h->omega_pad(), h->T, h->pad, h->te)) return no("tensor map (omega) rejected");
+  for (int s = 0; s < 2; ++s)
+    if (!encode_map(enc, &h->tm_counts[s], CU_TENSOR_MAP_DATA_TYPE_UINT32, h->counts_pad(s), h->T, h->pad, h->te)) return no("tensor map (counts) rejected");
+  // both padded density grids start zeroed; from here on the omega pass keeps them so
+  const size_t pad_bytes = (size_t)h->pad[0] * h->pad[1] * h->pad[2] * h->T * 4;
+  if (cudaMemsetAsync(h->counts_pad(0), 0, pad_bytes, h->stream) != cudaSuccess ||
+      cudaMemsetAsync(h->counts_pad(1), 0, pad_bytes, h->stream) != cudaSuccess) { cudaGetLastError(); return no("cudaMemsetAsync failed"); }
+  h->pad_cur = 0;
+  h->counts_in_pad = false;
+  cudaError_t e = h->tile_threads == 1024 ? tile_attr_p<1024>(P, h->tile_smem)
+                : h->tile_threads == 768 ? tile_attr_p<768>(P, h->tile_smem) : tile_attr_p<512>(P, h->tile_smem);
+  if (e != cudaSuccess) { cudaGetLastError(); return no("cudaFuncSetAttribute(max dynamic shared memory) failed"); }
+  h->tile_ready = true;
+  // automatic choice: tiles pay off when there are several rounds of them over the SMs
+  h->tile_auto = h->n_tiles >= 4u * (uint32_t)h->sm_count;
+  h->tile_why[0] = 0;
+}
+
+template <int P, int NT>
+int launch_tile_pn(soma_handle* h) {
+  TileArgs A{};
+  A.S = step_args(h);
+  A.T = h->T;
+  A.ex = h->te[0]; A.ey = h->te[1]; A.ez = h->te[2]; A.E = h->te[0] * h->te[1] * h->te[2];
+  A.cx = h->tc[0]; A.cy = h->tc[1]; A.cz = h->tc[2];
+  A.hx = h->th[0]; A.hy = h->th[1]; A.hz = h->th[2];
+  A.mty = h->tm[1]; A.mtz = h->tm[2]; A.n_tiles = h->n_tiles;
+  A.counts_offset = h->tile_counts_offset;
+  A.tile_start = h->sort_bins();
+  A.counts_pad = h->counts_pad(h->pad_cur);
+  A.px = h->pad[0]; A.py = h->pad[1]; A.pz = h->pad[2];
+  const unsigned grid = (unsigned)(h->n_tiles < (uint32_t)h->sm_count ? h->n_tiles : (uint32_t)h->sm_count);
+  const CUtensorMap& tmc = h->tm_counts[h->pad_cur];
+  h->counts_in_pad = true;
+  if (h->n_patterns > 1) tile_step_kernel<P, true, NT><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc);
+  else tile_step_kernel<P, false, NT><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc);
+  h->launches++;
+  CU(h, cudaGetLastError());
+  return SOMA_OK;
+}
+template <int NT>
+int launch_tile_n(soma_handle* h) {
+  switch (fused_lanes(h->N)) {
+    case 1: return launch_tile_pn<1, NT>(h);   case 2: return launch_tile_pn<2, NT>(h);
+    case 4: return launch_tile_pn<4, NT>(h);   case 8: return launch_tile_pn<8, NT>(h);
+    case 16: return launch_tile_pn<16, NT>(h); case 32: return launch_tile_pn<32, NT>(h);
+  }
+  return fail(h, SOMA_EINVAL, "tiled path does not support this beads_per_chain");
+}
+int launch_tile(soma_handle* h) {
+  return h->tile_threads == 1024 ? launch_tile_n<1024>(h) : h->tile_threads == 768 ? launch_tile_n<768>(h) : launch_tile_n<512>(h);
+}
+
+// Re-order the chains in memory by the coarse bin of their centre of mass (counting sort on the
+// device).  kind 1: cubes of kSortBinEdge cells; kind 2: the tiles of the tiled kernel, whose
+// tile_start table is the scanned bin array.
+int resort(soma_handle* h, int kind) {
   SortArgs S{};
-  S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N; S.cb = kSortBinEdge;
-  S.ncy = (h->grid.ny + kSortBinEdge - 1) / kSortBinEdge;
-  S.ncz = (h->grid.nz + kSortBinEdge - 1) / kSortBinEdge;
-  S.n_bins = h->n_bins;
+  S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
+  uint32_t n_bins;
+  if (kind == 2) {
+    S.cbx = h->tc[0]; S.cby = h->tc[1]; S.cbz = h->tc[2];
+    S.ncy = h->tm[1]; S.ncz = h->tm[2];
+    n_bins = h->n_tiles;
+  } else {
+    S.cbx = S.cby = S.cbz = kSortBinEdge;
+    S.ncy = (h->grid.ny + kSortBinEdge - 1) / kSortBinEdge;
+    S.ncz = (h->grid.nz + kSortBinEdge - 1) / kSortBinEdge;
+    n_bins = h->n_bins;
+  }
   const int src = h->live, dst = h->live ^ 1;
-  CU(h, cudaMemsetAsync(h->sort_bins(), 0, (size_t)h->n_bins * 4, h->stream));
+  CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
   if (h->pow2)
     chain_key_kernel<true><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
         S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
   else
     chain_key_kernel<false><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
         S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
-  bin_scan_kernel<<<1, 1024, 0, h->stream>>>(h->n_bins, h->sort_bins());
+  bin_scan_kernel<<<1, 1024, 0, h->stream>>>(n_bins + 1, h->sort_bins());      // entry n_bins becomes the total
   chain_permute_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
       h->B, h->N, h->sort_bins(), h->sort_key(), h->sort_rank(),
       h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->pos(dst, 0), h->pos(dst, 1), h->pos(dst, 2),
@@ -335,6 +526,7 @@ int resort(soma_handle* h) {
   h->identity_order = false;
   h->resorts++;
   h->steps_since_sort = 0;
+  h->sorted_kind = kind;
   return SOMA_OK;
 }
 
@@ -370,11 +562,19 @@ cudaEvent_t timing_mark(soma_handle* h) {
 
 int one_step(soma_handle* h) {
   int rc;
-  if (h->resort_interval > 0 && h->steps_since_sort >= (uint64_t)h->resort_interval)
-    if ((rc = resort(h)) != SOMA_OK) return rc;
+  const bool tiled = use_tile(h);
+  const int kind = tiled ? 2 : 1;
+  // the tiled kernel needs the slots sorted by tile; otherwise sorting is an optimisation
+  if (tiled && !h->pad_valid)                                    // path switched after the last omega pass
+    if ((rc = launch_omega(h)) != SOMA_OK) return rc;
+  if ((tiled && h->sorted_kind != 2) ||
+      (h->resort_interval > 0 && (h->steps_since_sort >= (uint64_t)h->resort_interval || h->sorted_kind != kind)))
+    if ((rc = resort(h, kind)) != SOMA_OK) return rc;
   const bool timed = h->timing && h->ev_used + 3 <= 3 * kMaxTimedSteps;
   if (timed) timing_mark(h);
-  if (use_fused(h)) {
+  if (tiled) {
+    if ((rc = launch_tile(h)) != SOMA_OK) return rc;             // a1 + a2 + a3 (+a5), tiled
+  } else if (use_fused(h)) {
     if ((rc = launch_fused(h)) != SOMA_OK) return rc;            // a1 + a2 + a3 (+a5)
   } else {
     if ((rc = launch_half_sweep(h, 0)) != SOMA_OK) return rc;    // a1
@@ -417,7 +617,8 @@ uint64_t soma_workspace_bytes(const soma_params* p) {
   if (bad) { fail(nullptr, SOMA_EINVAL, bad); return 0; }
   const uint64_t B = p->n_chains * p->beads_per_chain;
   const uint64_t TC = (uint64_t)p->grid[0] * p->grid[1] * p->grid[2] * p->n_types;
-  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bin_count(p->grid)).total;
+  const uint64_t pad_words = tile_capable_grid(p->grid) ? omega_pad_cells_max(p->grid) * p->n_types : 0;
+  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bin_count(p->grid), pad_words).total;
 }
 
 int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
@@ -461,7 +662,9 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   for (uint32_t k = 0; k < h->T * h->T; ++k) h->chiN[k] = p->chiN[k];
   h->seed = p->seed;
   h->n_bins = (uint32_t)sort_bin_count(p->grid);
-  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, h->n_bins);
+  h->tile_grid_ok = tile_capable_grid(p->grid);
+  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, h->n_bins,
+                     h->tile_grid_ok ? omega_pad_cells_max(p->grid) * h->T : 0);
   if (p->workspace) {
     if (p->workspace_bytes < h->L.total || (reinterpret_cast<uintptr_t>(p->workspace) % kAlign)) {
       free_handle(h);
@@ -504,6 +707,10 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->resort_interval = h->n_chains >= 4096 ? 64 : 0;
   h->fused_blocks_per_sm = 3;
   h->fused_waves = 1;
+  h->tc[0] = 12; h->tc[1] = 12; h->tc[2] = 8;
+  h->th[0] = h->th[1] = h->th[2] = 6;
+  h->tile_threads = 1024;
+  tile_setup(h);
   const double cells_per_step = (double)h->a * (double)fmaxf(h->grid.inv_hx, fmaxf(h->grid.inv_hy, h->grid.inv_hz));
   const double k = cells_per_step > 0.0 ? 2097152.0 / cells_per_step : 1e18;
   h->range_check_interval = k >= 1e18 ? (1ull << 60) : (k < 1.0 ? 1ull : (uint64_t)k);
@@ -535,7 +742,10 @@ int soma_load_state(soma_t* h, const float* x, const float* y, const float* z, u
   if ((rc = launch_omega(h)) != SOMA_OK) return rc;     // also zeroes counts(1)
   if ((rc = verify_range(h)) != SOMA_OK) return rc;     // synchronises: the caller may reuse its buffers
   h->steps_since_sort = 0;
-  if (h->resort_interval > 0 && (rc = resort(h)) != SOMA_OK) return rc;
+  h->sorted_kind = 0;
+  h->omega_custom = false;
+  if (use_tile(h) || h->resort_interval > 0)
+    if ((rc = resort(h, use_tile(h) ? 2 : 1)) != SOMA_OK) return rc;
   h->loaded = true;
   return SOMA_OK;
 }
@@ -623,7 +833,12 @@ const char* soma_last_error(const soma_t* h) { return h ? h->err : g_last_error;
 int soma_set_option(soma_t* h, const char* name, int64_t value) {
   if (!h || !name) return fail(h, SOMA_EINVAL, "NULL argument");
   if (!std::strcmp(name, "path")) {
-    if (value < 0 || value > 2) return fail(h, SOMA_EINVAL, "path must be 0, 1 or 2");
+    if (value < 0 || value > 3) return fail(h, SOMA_EINVAL, "path must be 0, 1, 2 or 3");
+    if (value == 3 && !h->tile_ready) {
+      char buf[160];
+      snprintf(buf, sizeof buf, "tiled path unavailable: %s", h->tile_why);
+      return fail(h, SOMA_EINVAL, buf);
+    }
     if (value == 2 && !fused_lanes(h->N))
       return fail(h, SOMA_EINVAL, "fused path needs beads_per_chain = 2P, P a power of two <= 32");
     h->path = (int)value;
@@ -644,12 +859,28 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     int rc = check(h);
     if (rc != SOMA_OK) return rc;
     if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
-    return resort(h);
+    return resort(h, use_tile(h) ? 2 : 1);
   }
   if (!std::strcmp(name, "fused_blocks_per_sm")) {
     if (value < 1 || value > 32) return fail(h, SOMA_EINVAL, "fused_blocks_per_sm must be in [1, 32]");
     h->fused_blocks_per_sm = (int)value;
     return SOMA_OK;
+  }
+  {
+    static const char* const tn[7] = {"tile_cx", "tile_cy", "tile_cz", "tile_hx", "tile_hy", "tile_hz", "tile_threads"};
+    for (int k = 0; k < 7; ++k)
+      if (!std::strcmp(name, tn[k])) {
+        if (k == 6) {
+          if (value != 512 && value != 768 && value != 1024) return fail(h, SOMA_EINVAL, "tile_threads must be 512, 768 or 1024");
+          h->tile_threads = (int)value;
+        } else {
+          if (value < 0 || value > 64) return fail(h, SOMA_EINVAL, "tile size out of range");
+          (k < 3 ? h->tc[k] : h->th[k - 3]) = (uint32_t)value;
+        }
+        tile_setup(h);
+        if (!h->tile_ready && h->path == 3) h->path = 0;
+        return SOMA_OK;                      // soma_get_counters()[3] tells whether tiles are usable now
+      }
   }
   if (!std::strcmp(name, "fused_waves")) {
     if (value < 1 || value > 1024) return fail(h, SOMA_EINVAL, "fused_waves must be in [1, 1024]");
@@ -662,6 +893,7 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
 int soma_get_counters(const soma_t* h, uint64_t* out) {
   if (!h || !out) return SOMA_EINVAL;
   out[0] = h->launches; out[1] = h->steps_done; out[2] = h->resorts;
+  out[3] = use_tile(h) ? 3 : (use_fused(h) ? 2 : 1);
   return SOMA_OK;
 }
 
@@ -718,6 +950,8 @@ int soma_debug_set_omega(soma_t* h, const float* omega) {
   if (!omega) return fail(h, SOMA_EINVAL, "omega is NULL");
   CU(h, cudaMemcpyAsync(h->omega(), omega, (size_t)h->cells * h->T * 4, cudaMemcpyHostToDevice, h->stream));
   CU(h, cudaStreamSynchronize(h->stream));
+  h->omega_custom = true;
+  h->pad_valid = false;
   return SOMA_OK;
 }
 

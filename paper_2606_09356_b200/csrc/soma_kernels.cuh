@@ -247,21 +247,33 @@ omega_kernel(OmegaArgs A) {
 struct SortArgs {
   Grid grid;
   uint32_t n_chains, N;
-  uint32_t cb;                     // coarse bin edge in cells
+  uint32_t cbx, cby, cbz;          // coarse bin edges in cells
   uint32_t ncy, ncz;               // coarse bins along y and z (x is implied)
-  uint32_t n_bins;
 };
 
+// bin of a chain = coarse bin of the cell that holds its centre of mass (fp32 mean of the beads)
 template <bool POW2>
 __global__ void __launch_bounds__(256)
 chain_key_kernel(SortArgs S, const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ z,
                  uint32_t* __restrict__ bin_count, uint32_t* __restrict__ key, uint32_t* __restrict__ rank) {
   const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= S.n_chains) return;
-  const uint64_t j = (uint64_t)s * S.N + S.N / 2u;
-  const uint32_t cell = cell_of<POW2>(S.grid, x[j], y[j], z[j]);
+  const uint64_t j0 = (uint64_t)s * S.N;
+  float sx = 0.f, sy = 0.f, sz = 0.f;
+  if ((S.N & 3u) == 0) {
+    for (uint32_t i = 0; i < S.N; i += 4) {
+      const float4 a = *reinterpret_cast<const float4*>(x + j0 + i);
+      const float4 b = *reinterpret_cast<const float4*>(y + j0 + i);
+      const float4 c = *reinterpret_cast<const float4*>(z + j0 + i);
+      sx += (a.x + a.y) + (a.z + a.w); sy += (b.x + b.y) + (b.z + b.w); sz += (c.x + c.y) + (c.z + c.w);
+    }
+  } else {
+    for (uint32_t i = 0; i < S.N; ++i) { sx += x[j0 + i]; sy += y[j0 + i]; sz += z[j0 + i]; }
+  }
+  const float inv = 1.0f / (float)S.N;
+  const uint32_t cell = cell_of<POW2>(S.grid, sx * inv, sy * inv, sz * inv);
   const uint32_t iz = cell % S.grid.nz, iy = (cell / S.grid.nz) % S.grid.ny, ix = cell / (S.grid.nz * S.grid.ny);
-  const uint32_t bin = ((ix / S.cb) * S.ncy + iy / S.cb) * S.ncz + iz / S.cb;
+  const uint32_t bin = ((ix / S.cbx) * S.ncy + iy / S.cby) * S.ncz + iz / S.cbz;
   key[s] = bin;
   rank[s] = atomicAdd(bin_count + bin, 1u);
 }

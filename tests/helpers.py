@@ -8,9 +8,11 @@ import oracle
 import scmf_inputs as si
 
 
-def gpu_system(s, path: int = 0, **kw):
+def gpu_system(s, path: int = 0, options=None, **kw):
     import paper_2606_09356_b200 as soma
     g = soma.Soma.from_system(s, **kw)
+    for name, value in (options or {}).items():
+        g.set_option(name, value)
     if path:
         g.set_option("path", path)
     return g

@@ -16,7 +16,7 @@ from helpers import assert_same_state, gpu_system, lockstep
 
 pytestmark = pytest.mark.gpu
 
-FUSED, GENERIC = 2, 1
+FUSED, GENERIC, TILED = 2, 1, 3
 
 
 def _run_both(s, steps_list, path, **kw):
@@ -154,3 +154,94 @@ def test_large_seed_step_and_chain_ids_reach_the_counter():
         g2.load_state(s.x, s.y, s.z, step0)
         g2.mc_steps(1)
         assert not np.array_equal(g2.positions()[0], o.positions()[0])
+
+
+# ---- the tiled kernel (omega and density tiles in shared memory, TMA in and out) --------------------
+# Small tiles on small grids so that the oracle stays fast while the run still covers many tiles,
+# tiles that wrap around every periodic face, partial last tiles (core not dividing the grid), beads
+# outside their tile's halo (global-memory fallback) and drift between re-sorts.
+
+SMALL_TILES = dict(tile_cx=4, tile_cy=4, tile_cz=4, tile_hx=2, tile_hy=2, tile_hz=2)          # 8^3 tiles, most chains stick out
+ODD_TILES = dict(tile_cx=12, tile_cy=5, tile_cz=8, tile_hx=3, tile_hy=4, tile_hz=6)           # cores not dividing the grid
+WIDE_HALO = dict(tile_cx=4, tile_cy=4, tile_cz=4, tile_hx=6, tile_hy=6, tile_hz=6)            # 16^3 tiles: nearly all beads inside
+
+TILE_CASES = {
+    "cfg0_full_small_tiles": (lambda: si.make_system(si.config(0)), SMALL_TILES),
+    "cfg0_full_wide_halo": (lambda: si.make_system(si.config(0)), WIDE_HALO),
+    "cfg1_scaled_T1_N64": (lambda: _scaled(1, 4099, (16, 16, 16)), SMALL_TILES),
+    "cfg2_scaled_odd_tiles": (lambda: _scaled(2, 8193, (32, 16, 32)), ODD_TILES),
+    "cfg3_scaled_blend_N64": (lambda: _scaled(3, 4098, (32, 16, 16)), WIDE_HALO),
+    "cfg4_scaled_default_tiles": (lambda: _scaled(4, 16385, (32, 32, 32)), {}),                 # 12x12x8 + 6: the bench shape
+    "cfg4_scaled_threads_512": (lambda: _scaled(4, 16385, (32, 32, 16)), dict(WIDE_HALO, tile_threads=512)),
+    "cfg4_scaled_threads_768": (lambda: _scaled(4, 16385, (32, 32, 16)), dict(SMALL_TILES, tile_threads=768)),
+    "T3_three_patterns": (lambda: _custom(900, 32, 3, [[0] * 10 + [1] * 12 + [2] * 10, [2] * 32, [1] * 16 + [0] * 16],
+                                          np.arange(900) % 3, [[0, 12, 5], [12, 0, 21], [5, 21, 0]], 35.0, (16, 32, 16), (8.0, 16.0, 8.0), 41),
+                          SMALL_TILES),
+    "N2": (lambda: _custom(3001, 2, 2, [[0, 1]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 42), SMALL_TILES),
+    "N8": (lambda: _custom(1517, 8, 2, [[0, 0, 0, 1, 1, 1, 1, 0]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 43), SMALL_TILES),
+    "one_chain": (lambda: _custom(1, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (16, 16, 16), (8, 8, 8), 44), SMALL_TILES),
+    "big_moves_unit_cells": (lambda: _custom(700, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (16, 16, 32), (11.2, 14.0, 25.6), 45,
+                                             b=0.7, move_halfwidth=0.9), WIDE_HALO),
+}
+
+
+@pytest.mark.parametrize("case", sorted(TILE_CASES))
+def test_tiled_path_parity_after_1_and_10_steps(case):
+    make, opts = TILE_CASES[case]
+    s = make()
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s, path=TILED, options=opts) as g:
+        assert g.counters()["path"] == TILED
+        g.load_state(s.x, s.y, s.z)
+        done = 0
+        for upto in (1, 10):
+            assert g.mc_steps(upto - done, want_accepted=True) == o.mc_steps(upto - done)
+            done = upto
+            assert_same_state(g, o, f"{case} tiled after {upto} steps")
+        assert g.counters()["path"] == TILED
+
+
+@pytest.mark.parametrize("interval", [0, 1, 3])
+def test_tiled_path_with_drift_and_resorts(interval):
+    """40 steps: without re-sorting the chains drift out of their tiles (fallback path); with
+    frequent re-sorting the slot order keeps changing.  The trajectory may not depend on either."""
+    s = _scaled(4, 6000, (16, 16, 16))
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    acc_o = o.mc_steps(40)
+    with gpu_system(s, path=TILED, options=dict(SMALL_TILES, resort_interval=interval)) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert g.mc_steps(40, want_accepted=True) == acc_o
+        assert_same_state(g, o, f"tiled, resort_interval={interval}")
+        assert g.counters()["resorts"] == (1 if interval == 0 else 1 + (40 - 1) // interval)
+
+
+def test_switching_paths_mid_run_keeps_the_trajectory():
+    s = _scaled(2, 5000, (16, 16, 16))
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    o.mc_steps(8)
+    with gpu_system(s, path=FUSED, options=SMALL_TILES) as g:
+        g.load_state(s.x, s.y, s.z)
+        for path in (FUSED, TILED, GENERIC, TILED, FUSED, TILED, TILED, GENERIC):
+            g.set_option("path", path)
+            g.mc_steps(1)
+        assert_same_state(g, o, "path switched every step")
+
+
+def test_tiled_path_is_refused_where_it_cannot_run():
+    import paper_2606_09356_b200 as soma
+    for make in (EDGE["T3_npot"], EDGE["N33"], EDGE["one_chain"]):          # non-power-of-two grid, odd N, 1-cell grid
+        with gpu_system(make()) as g:
+            with pytest.raises(soma.SomaError) as e:
+                g.set_option("path", TILED)
+            assert e.value.code == soma.SOMA_EINVAL and "tiled path unavailable" in str(e.value)
+    with gpu_system(si.make_system(si.config(0))) as g:                      # default 24x24x20 tile > 16^3 grid
+        with pytest.raises(soma.SomaError):
+            g.set_option("path", TILED)
+        g.set_option("tile_cx", 4); g.set_option("tile_cy", 4); g.set_option("tile_cz", 4)
+        g.set_option("tile_hx", 2); g.set_option("tile_hy", 2); g.set_option("tile_hz", 2)
+        g.set_option("path", TILED)
+        g.set_option("tile_hz", 3)                                           # extent 10 along z: not a multiple of 4 -> tiles off
+        assert g.counters()["path"] != TILED
