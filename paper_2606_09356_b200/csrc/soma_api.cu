@@ -3,6 +3,7 @@
 // step runs in the kernels of soma_kernels.cuh.
 #include "../../include/soma.h"
 
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -32,7 +33,9 @@ struct Layout {            // byte offsets into the workspace
   uint64_t range_flag;     // uint32
   uint64_t sort_key;       // [n] uint32
   uint64_t sort_rank;      // [n] uint32
-  uint64_t sort_bins;      // [n_bins_max + 1] uint32: bin counts, then bin starts (= tile_start)
+  uint64_t sort_bins;      // [2 n_bins_max + 2] uint32: bin counts, then bin starts (= tile_start)
+  uint64_t slot_meta;      // [n] float4: per slot floor offsets + chain id, written by the tile sort
+  uint64_t meta_src;       // [n] float4: the same in the order before the sort (scratch)
   uint64_t omega_pad;      // [T][pad cells] fp32: ghost-padded omega for the tile loads (0 bytes if unused)
   uint64_t counts_pad[2];  // [T][pad cells] uint32: ghost-padded density grids the tiles flush into
   uint64_t total;
@@ -74,7 +77,9 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   L.range_flag = off; off += align_up(4);
   L.sort_key = off; off += align_up(n * 4);
   L.sort_rank = off; off += align_up(n * 4);
-  L.sort_bins = off; off += align_up((n_bins + 1) * 4);
+  L.sort_bins = off; off += align_up((2 * n_bins + 2) * 4);
+  L.slot_meta = off; off += align_up(n * 16);
+  L.meta_src = off; off += align_up(n * 16);
   L.omega_pad = off; off += align_up(pad_words * 4);
   for (int s = 0; s < 2; ++s) { L.counts_pad[s] = off; off += align_up(pad_words * 4); }
   L.total = off;
@@ -165,6 +170,8 @@ struct soma_handle {
   bool tile_ready;              // geometry + tensor maps are set up for the current options
   uint32_t tc[3], th[3];        // tile core and halo in cells
   int tile_threads;             // 512, 768 or 1024
+  bool tile_fast;               // inv_h a power of two >= 1 on every axis and a a power of two
+  uint32_t tile_margin;         // chains with a bead this close to a tile face sort behind the others
   uint32_t te[3], tm[3], n_tiles, pad[3];
   size_t tile_smem;
   uint32_t tile_counts_offset;
@@ -197,6 +204,8 @@ struct soma_handle {
   uint32_t* sort_rank() const { return reinterpret_cast<uint32_t*>(ws + L.sort_rank); }
   uint32_t* sort_bins() const { return reinterpret_cast<uint32_t*>(ws + L.sort_bins); }
   float* omega_pad() const { return reinterpret_cast<float*>(ws + L.omega_pad); }
+  float4* slot_meta() const { return reinterpret_cast<float4*>(ws + L.slot_meta); }
+  float4* meta_src() const { return reinterpret_cast<float4*>(ws + L.meta_src); }
   uint32_t* counts_pad(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts_pad[s]); }
   uint8_t* patterns() const { return reinterpret_cast<uint8_t*>(ws + L.patterns); }
   uint8_t* pattern0() const { return reinterpret_cast<uint8_t*>(ws + L.pattern0); }
@@ -385,8 +394,10 @@ bool encode_map(EncodeTiledFn enc, CUtensorMap* tm, CUtensorMapDataType dt, void
 
 template <int P, int NT>
 cudaError_t tile_attr(size_t smem) {
-  cudaError_t e = cudaFuncSetAttribute(tile_step_kernel<P, false, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, true, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(tile_step_kernel<P, false, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, true, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, false, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, true, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   return e;
 }
 template <int NT>
@@ -405,6 +416,7 @@ void tile_setup(soma_handle* h) {
   h->tile_ready = false;
   h->tile_auto = false;
   h->pad_valid = false;
+  if (h->sorted_kind == 2) h->sorted_kind = 0;       // the per-slot floor offsets belong to the old geometry
   auto no = [&](const char* why) { snprintf(h->tile_why, sizeof h->tile_why, "%s", why); };
   if (!h->tile_grid_ok) return no("grid axes must be powers of two >= 16");
   const int P = fused_lanes(h->N);
@@ -459,6 +471,7 @@ template <int P, int NT>
 int launch_tile_pn(soma_handle* h) {
   TileArgs A{};
   A.S = step_args(h);
+  A.slot_meta = h->slot_meta();
   A.T = h->T;
   A.ex = h->te[0]; A.ey = h->te[1]; A.ez = h->te[2]; A.E = h->te[0] * h->te[1] * h->te[2];
   A.cx = h->tc[0]; A.cy = h->tc[1]; A.cz = h->tc[2];
@@ -468,11 +481,20 @@ int launch_tile_pn(soma_handle* h) {
   A.tile_start = h->sort_bins();
   A.counts_pad = h->counts_pad(h->pad_cur);
   A.px = h->pad[0]; A.py = h->pad[1]; A.pz = h->pad[2];
+  const uint64_t m1 = (uint64_t)kPhiloxM1 * A.S.ctr2;
+  A.philox_u0 = (uint32_t)(m1 >> 32) ^ h->keys.k0[0];
+  A.philox_u1 = (uint32_t)m1;
+  A.a2 = 2.0f * h->a;
+  A.ac = h->a * -0.99999988079071044921875f;      // a (2^-23 - 1), exact when a is a power of two
   const unsigned grid = (unsigned)(h->n_tiles < (uint32_t)h->sm_count ? h->n_tiles : (uint32_t)h->sm_count);
   const CUtensorMap& tmc = h->tm_counts[h->pad_cur];
   h->counts_in_pad = true;
-  if (h->n_patterns > 1) tile_step_kernel<P, true, NT><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc);
-  else tile_step_kernel<P, false, NT><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc);
+  const bool multi = h->n_patterns > 1;
+#define SOMA_LAUNCH_TILE(MULTI, FAST) \
+  tile_step_kernel<P, MULTI, NT, FAST><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc)
+  if (h->tile_fast) { if (multi) SOMA_LAUNCH_TILE(true, true); else SOMA_LAUNCH_TILE(false, true); }
+  else              { if (multi) SOMA_LAUNCH_TILE(true, false); else SOMA_LAUNCH_TILE(false, false); }
+#undef SOMA_LAUNCH_TILE
   h->launches++;
   CU(h, cudaGetLastError());
   return SOMA_OK;
@@ -494,32 +516,42 @@ int launch_tile(soma_handle* h) {
 // device).  kind 1: cubes of kSortBinEdge cells; kind 2: the tiles of the tiled kernel, whose
 // tile_start table is the scanned bin array.
 int resort(soma_handle* h, int kind) {
-  SortArgs S{};
-  S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
+  const int src = h->live, dst = h->live ^ 1;
   uint32_t n_bins;
   if (kind == 2) {
-    S.cbx = h->tc[0]; S.cby = h->tc[1]; S.cbz = h->tc[2];
-    S.ncy = h->tm[1]; S.ncz = h->tm[2];
-    n_bins = h->n_tiles;
+    TileSortArgs S{};
+    S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
+    S.cx = h->tc[0]; S.cy = h->tc[1]; S.cz = h->tc[2];
+    S.hx = h->th[0]; S.hy = h->th[1]; S.hz = h->th[2];
+    S.ex = h->te[0]; S.ey = h->te[1]; S.ez = h->te[2];
+    S.mty = h->tm[1]; S.mtz = h->tm[2];
+    S.margin = h->tile_margin;
+    n_bins = 2u * h->n_tiles;
+    CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
+    tile_key_kernel<<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
+        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->slot_chain(src), h->sort_bins(), h->sort_key(),
+        h->sort_rank(), h->meta_src());
   } else {
+    SortArgs S{};
+    S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
     S.cbx = S.cby = S.cbz = kSortBinEdge;
     S.ncy = (h->grid.ny + kSortBinEdge - 1) / kSortBinEdge;
     S.ncz = (h->grid.nz + kSortBinEdge - 1) / kSortBinEdge;
     n_bins = h->n_bins;
+    CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
+    if (h->pow2)
+      chain_key_kernel<true><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
+          S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
+    else
+      chain_key_kernel<false><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
+          S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
   }
-  const int src = h->live, dst = h->live ^ 1;
-  CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
-  if (h->pow2)
-    chain_key_kernel<true><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
-        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
-  else
-    chain_key_kernel<false><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
-        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
   bin_scan_kernel<<<1, 1024, 0, h->stream>>>(n_bins + 1, h->sort_bins());      // entry n_bins becomes the total
   chain_permute_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
       h->B, h->N, h->sort_bins(), h->sort_key(), h->sort_rank(),
       h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->pos(dst, 0), h->pos(dst, 1), h->pos(dst, 2),
-      h->slot_chain(src), h->slot_pattern(src), h->slot_chain(dst), h->slot_pattern(dst));
+      h->slot_chain(src), h->slot_pattern(src), h->slot_chain(dst), h->slot_pattern(dst),
+      kind == 2 ? h->meta_src() : nullptr, kind == 2 ? h->slot_meta() : nullptr);
   h->launches += 3;
   CU(h, cudaGetLastError());
   h->live = dst;
@@ -709,7 +741,13 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->fused_waves = 1;
   h->tc[0] = 12; h->tc[1] = 12; h->tc[2] = 8;
   h->th[0] = h->th[1] = h->th[2] = 6;
-  h->tile_threads = 1024;
+  h->tile_threads = 768;
+  h->tile_margin = 1;
+  {
+    auto pow2f = [](float v) { int e; return v > 0.0f && std::frexp(v, &e) == 0.5f && e > -100 && e < 100; };
+    h->tile_fast = pow2f(h->a) && pow2f(h->grid.inv_hx) && pow2f(h->grid.inv_hy) && pow2f(h->grid.inv_hz) &&
+                   h->grid.inv_hx >= 1.0f && h->grid.inv_hy >= 1.0f && h->grid.inv_hz >= 1.0f;
+  }
   tile_setup(h);
   const double cells_per_step = (double)h->a * (double)fmaxf(h->grid.inv_hx, fmaxf(h->grid.inv_hy, h->grid.inv_hz));
   const double k = cells_per_step > 0.0 ? 2097152.0 / cells_per_step : 1e18;
@@ -881,6 +919,17 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
         if (!h->tile_ready && h->path == 3) h->path = 0;
         return SOMA_OK;                      // soma_get_counters()[3] tells whether tiles are usable now
       }
+  }
+  if (!std::strcmp(name, "tile_margin")) {
+    if (value < 0 || value > 16) return fail(h, SOMA_EINVAL, "tile_margin must be in [0, 16]");
+    h->tile_margin = (uint32_t)value;
+    if (h->sorted_kind == 2) h->sorted_kind = 0;
+    return SOMA_OK;
+  }
+  if (!std::strcmp(name, "tile_fast")) {               // 0: use the general arithmetic even where the shortcuts apply
+    if (value != 0) return fail(h, SOMA_EINVAL, "tile_fast can only be switched off");
+    h->tile_fast = false;
+    return SOMA_OK;
   }
   if (!std::strcmp(name, "fused_waves")) {
     if (value < 1 || value > 1024) return fail(h, SOMA_EINVAL, "fused_waves must be in [1, 1024]");

@@ -323,14 +323,18 @@ chain_permute_kernel(uint64_t B, uint32_t N, const uint32_t* __restrict__ bin_st
                      const float* __restrict__ sx, const float* __restrict__ sy, const float* __restrict__ sz,
                      float* __restrict__ dx, float* __restrict__ dy, float* __restrict__ dz,
                      const uint32_t* __restrict__ s_chain, const uint8_t* __restrict__ s_pat,
-                     uint32_t* __restrict__ d_chain, uint8_t* __restrict__ d_pat) {
+                     uint32_t* __restrict__ d_chain, uint8_t* __restrict__ d_pat,
+                     const float4* __restrict__ s_meta, float4* __restrict__ d_meta /* both may be null */) {
   const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= B) return;
   const uint32_t s = (uint32_t)(j / N), i = (uint32_t)(j % N);
   const uint32_t d = bin_start[key[s]] + rank[s];
   const uint64_t k = (uint64_t)d * N + i;
   dx[k] = sx[j]; dy[k] = sy[j]; dz[k] = sz[j];
-  if (i == 0) { d_chain[d] = s_chain[s]; d_pat[d] = s_pat[s]; }
+  if (i == 0) {
+    d_chain[d] = s_chain[s]; d_pat[d] = s_pat[s];
+    if (d_meta) d_meta[d] = s_meta[s];
+  }
 }
 
 // sets *range_flag if a bead's cell coordinate is NaN or beyond kCellCoordLimit (see floor_bits)

@@ -27,21 +27,6 @@
 
 namespace soma {
 
-constexpr uint32_t kOutside = 0xffffffffu;
-
-struct TileArgs {
-  StepArgs S;                 // omega = linear field (fallback); counts_next is not used by this kernel
-  uint32_t* __restrict__ counts_pad;   // [T][px][py][pz] ghost-padded density grid this step bins into
-  uint32_t px, py, pz;        // padded dims: padded coordinate q holds cell (q - halo) mod n
-  uint32_t T;
-  uint32_t ex, ey, ez, E;     // tile extent in cells (core + 2*halo), E = ex*ey*ez
-  uint32_t cx, cy, cz;        // core
-  uint32_t hx, hy, hz;        // halo
-  uint32_t mty, mtz, n_tiles; // tiles along y and z, total
-  uint32_t counts_offset;     // byte offset of the density tile in dynamic shared memory
-  const uint32_t* __restrict__ tile_start;   // [n_tiles + 1] first slot of every tile
-};
-
 // ---- PTX wrappers -----------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -77,56 +62,128 @@ __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.comm
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-// Per-tile geometry held in registers: floor magic minus the tile origin, so that the masked bit
-// pattern of fadd_rd(r*inv_h, m) is directly the coordinate RELATIVE to the tile origin (mod grid).
-struct TileGeom {
-  float mx, my, mz;
-};
-
-__device__ __forceinline__ uint32_t local_cell(const TileArgs& A, const TileGeom& g, float x, float y, float z) {
-  const Grid& G = A.S.grid;
-  const uint32_t bx = __float_as_uint(__fadd_rd(__fmul_rn(x, G.inv_hx), g.mx)) & (G.nx - 1u);
-  const uint32_t by = __float_as_uint(__fadd_rd(__fmul_rn(y, G.inv_hy), g.my)) & (G.ny - 1u);
-  const uint32_t bz = __float_as_uint(__fadd_rd(__fmul_rn(z, G.inv_hz), g.mz)) & (G.nz - 1u);
-  const bool inside = (bx < A.ex) & (by < A.ey) & (bz < A.ez);
-  return inside ? (bx * A.ey + by) * A.ez + bz : kOutside;
+// ---- shared-memory access by 32-bit shared address ---------------------------------------------
+__device__ __forceinline__ float lds_f32(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void reds_inc(uint32_t addr) {
+  asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(addr) : "memory");
 }
 
-__device__ __forceinline__ float omega_lookup(const TileArgs& A, const float* __restrict__ omega_s_t, uint32_t type_cells,
-                                              uint32_t idx, float x, float y, float z) {
-  if (idx != kOutside) return omega_s_t[idx];
-  return __ldg(A.S.omega + type_cells + cell_of<true>(A.S.grid, x, y, z));
+// ---- Philox4x32-10 with the loop-invariant part of the first three rounds folded ---------------
+// Counter of a move = (bead i, chain c, step, parity | domain<<8 | step_hi<<16).  Only c differs
+// between the moves a lane makes, and it enters through round 1 as c0' = u0 ^ c, so for every lane
+// and parity the values below are fixed for the whole kernel (derivation in DESIGN.md section 7):
+//   LC = lo(M0 i) ^ k1[1]                       (xor-ed onto hi(M0 c0') in round 2)
+//   LD = lo(M1 c2') ^ k0[2],  c2' = hi(M0 i) ^ ctr3 ^ k1[0]
+//   LE = hi(M0 c0'') ^ k1[2], c0'' = hi(M1 c2') ^ u1 ^ k0[1]
+//   LF = lo(M0 c0'')
+// which leaves 16 wide multiplies and 18 xors per move instead of 20 + 20.
+struct PhiloxLane { uint32_t LC, LD, LE, LF; };
+
+__device__ __forceinline__ PhiloxLane philox_lane(const PhiloxKeys& K, uint32_t u1, uint32_t i, uint32_t ctr3) {
+  const uint64_t p0 = (uint64_t)kPhiloxM0 * i;
+  const uint32_t c2_1 = (uint32_t)(p0 >> 32) ^ ctr3 ^ K.k1[0];
+  const uint64_t p1 = (uint64_t)kPhiloxM1 * c2_1;
+  const uint32_t c0_2 = (uint32_t)(p1 >> 32) ^ u1 ^ K.k0[1];
+  const uint64_t q0 = (uint64_t)kPhiloxM0 * c0_2;
+  PhiloxLane L;
+  L.LC = (uint32_t)p0 ^ K.k1[1];
+  L.LD = (uint32_t)p1 ^ K.k0[2];
+  L.LE = (uint32_t)(q0 >> 32) ^ K.k1[2];
+  L.LF = (uint32_t)q0;
+  return L;
 }
 
-// One Metropolis trial move inside a tile.  Same arithmetic as move_bead; only where omega is read
-// from differs.  `idx` is the bead's tile-local cell (or kOutside) and follows the bead.
-__device__ __forceinline__ bool move_bead_tile(const TileArgs& A, const TileGeom& g, uint32_t chain, uint32_t i, uint32_t parity,
-                                               const float* __restrict__ omega_s_t, uint32_t type_cells,
-                                               float& rx, float& ry, float& rz, uint32_t& idx,
-                                               bool has_l, float lx, float ly, float lz,
-                                               bool has_r, float qx, float qy, float qz) {
-  const StepArgs& S = A.S;
-  const Words4 w = philox4x32_10(i, chain, S.ctr2, S.ctr3_base | parity, S.keys);
-  const Trial t = trial_position(rx, ry, rz, S.a, w);
-  float dq = 0.0f;
-  if (has_l) dq = __fsub_rn(bond_sq(t.x, t.y, t.z, lx, ly, lz), bond_sq(rx, ry, rz, lx, ly, lz));
-  if (has_r) {
-    const float dqr = __fsub_rn(bond_sq(t.x, t.y, t.z, qx, qy, qz), bond_sq(rx, ry, rz, qx, qy, qz));
-    dq = has_l ? __fadd_rn(dq, dqr) : dqr;
+// c0_1 = u0 ^ chain, u0 = hi(M1 step) ^ k0[0]
+__device__ __forceinline__ Words4 philox_tail(const PhiloxKeys& K, const PhiloxLane& L, uint32_t c0_1) {
+  const uint64_t r2 = (uint64_t)kPhiloxM0 * c0_1;                       // round 2
+  const uint32_t c2_2 = (uint32_t)(r2 >> 32) ^ L.LC;
+  const uint64_t r3 = (uint64_t)kPhiloxM1 * c2_2;                       // round 3
+  uint32_t c0 = (uint32_t)(r3 >> 32) ^ L.LD;
+  uint32_t c1 = (uint32_t)r3;
+  uint32_t c2 = L.LE ^ (uint32_t)r2;
+  uint32_t c3 = L.LF;
+#pragma unroll
+  for (int r = 3; r < 10; ++r) {
+    const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;
+    const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ K.k0[r];
+    c1 = (uint32_t)p1;
+    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ K.k1[r];
+    c3 = (uint32_t)p0;
   }
-  const uint32_t idx_new = local_cell(A, g, t.x, t.y, t.z);
-  const float w_new = omega_lookup(A, omega_s_t, type_cells, idx_new, t.x, t.y, t.z);
-  const float w_old = omega_lookup(A, omega_s_t, type_cells, idx, rx, ry, rz);
-  const float dE = __fmaf_rn(S.kb, dq, __fsub_rn(w_new, w_old));
-  const bool acc = metropolis_accept(dE, w.w3);
-  if (acc) { rx = t.x; ry = t.y; rz = t.z; idx = idx_new; }
+  return Words4{c0, c1, c2, c3};
+}
+
+// ---- Metropolis decision, one fused multiply-add from the hardware logarithm --------------------
+// m = lg2(u 2^24) ln2 + dE = dE + ln u + 24 ln2 up to ~1e-5.  accept iff fl(dE + lnu) <= 0
+// (DESIGN.md section 2 step 5.6); m outside [T - band, T + band] decides that exactly (this
+// includes dE <= 0: then the exact rule accepts, and either m < T - band or the slow path runs).
+constexpr float kLn2 = 0.693147182464599609375f;
+constexpr float kLnT = 16.6355323791503906250f;            // 24 ln 2
+__device__ __forceinline__ bool metropolis_accept_fma(float dE, uint32_t w3) {
+  const float m = __fmaf_rn(lg2_approx(umap_int(w3)), kLn2, dE);
+  bool acc = m < kLnT - kLnBand;
+  if (!acc && m <= kLnT + kLnBand) acc = __fadd_rn(dE, lnu_exact(umap(w3))) <= 0.0f;
   return acc;
 }
 
-__device__ __forceinline__ void count_bead(const TileArgs& A, uint32_t* __restrict__ counts_s, uint32_t type,
-                                           uint32_t idx, float x, float y, float z) {
-  if (idx != kOutside) { atomicAdd(counts_s + type * A.E + idx, 1u); return; }
-  // outside the tile: straight into the padded grid, at the image that lies `halo` inside it
+// ---- tile-local cell -----------------------------------------------------------------------------
+// `off` = kFloorMagic - tile origin + the chain's periodic image shift (whole cells, set when the
+// chains are sorted), so the bit pattern of RD(r inv_h + off) is kFloorMagicBits + the bead's cell
+// coordinate RELATIVE to the tile origin, with no periodic wrap left to do.  FASTH: inv_h is a
+// power of two >= 1, so r inv_h is exact and one FFMA.RD gives the same bits as FMUL + FADD.RD.
+constexpr uint32_t kFloorMagicBits = 0x4b400000u;
+
+struct TileGeo {
+  float inv_hx, inv_hy, inv_hz;
+  uint32_t ex, ey, ez;          // tile extent in cells
+  uint32_t sx, sy;              // byte strides of x and y in the shared-memory tile (z: 4)
+};
+
+template <bool FASTH>
+__device__ __forceinline__ bool tile_addr(const TileGeo& g, float x, float y, float z, float offx, float offy, float offz,
+                                          uint32_t base_t, uint32_t& addr) {
+  float fx, fy, fz;
+  if (FASTH) {
+    fx = __fmaf_rd(x, g.inv_hx, offx); fy = __fmaf_rd(y, g.inv_hy, offy); fz = __fmaf_rd(z, g.inv_hz, offz);
+  } else {
+    fx = __fadd_rd(__fmul_rn(x, g.inv_hx), offx); fy = __fadd_rd(__fmul_rn(y, g.inv_hy), offy); fz = __fadd_rd(__fmul_rn(z, g.inv_hz), offz);
+  }
+  const uint32_t ux = __float_as_uint(fx) - kFloorMagicBits;
+  const uint32_t uy = __float_as_uint(fy) - kFloorMagicBits;
+  const uint32_t uz = __float_as_uint(fz) - kFloorMagicBits;
+  addr = ux * g.sx + (uy * g.sy + (uz * 4u + base_t));
+  return (ux < g.ex) & (uy < g.ey) & (uz < g.ez);
+}
+
+struct TileArgs {
+  StepArgs S;                 // omega = linear field (slow path); counts_next is not used by this kernel
+  const float4* __restrict__ slot_meta;     // [n] per slot: floor offsets x, y, z and the chain id (bits)
+  uint32_t* __restrict__ counts_pad;        // [T][px][py][pz] ghost-padded density grid this step bins into
+  const uint32_t* __restrict__ tile_start;  // [2 n_tiles + 1]: compact chains of tile k, then its extended ones
+  uint32_t px, py, pz;        // padded dims: padded coordinate q holds cell (q - halo) mod n
+  uint32_t T;
+  uint32_t ex, ey, ez, E;     // tile extent in cells (core + 2*halo), E = ex*ey*ez
+  uint32_t cx, cy, cz;        // core
+  uint32_t hx, hy, hz;        // halo
+  uint32_t mty, mtz, n_tiles; // tiles along y and z, total
+  uint32_t counts_offset;     // byte offset of the density tile in dynamic shared memory
+  uint32_t philox_u0, philox_u1;   // hi(M1 step) ^ k0[0], lo(M1 step)
+  float a2, ac;               // APOW2: 2a and a (2^-23 - 1)
+};
+
+// omega at a bead's cell on the slow path (some lane of the warp has a bead outside the tile)
+__device__ __noinline__ float omega_outside(const float* __restrict__ omega_t, Grid grid, float x, float y, float z) {
+  return __ldg(omega_t + cell_of<true>(grid, x, y, z));
+}
+
+// density increment of a bead outside the tile: straight into the padded grid, at the image that
+// lies `halo` inside it
+__device__ __noinline__ void count_outside(const TileArgs& A, uint32_t type, float x, float y, float z) {
   const Grid& G = A.S.grid;
   const uint32_t gx = floor_bits(__fmul_rn(x, G.inv_hx)) & (G.nx - 1u);
   const uint32_t gy = floor_bits(__fmul_rn(y, G.inv_hy)) & (G.ny - 1u);
@@ -134,15 +191,74 @@ __device__ __forceinline__ void count_bead(const TileArgs& A, uint32_t* __restri
   atomicAdd(A.counts_pad + ((size_t)(type * A.px + gx + A.hx) * A.py + gy + A.hy) * A.pz + gz + A.hz, 1u);
 }
 
-template <int P, bool MULTI_PAT, int NT>
+// Kernel-constant scalars a move needs.
+struct LaneCtx {
+  TileGeo g;
+  float a, a2, ac, kb;
+};
+
+// trial displacement along one axis (DESIGN.md section 2 steps 5.2-5.3): r' = r + a tmap(w)
+template <bool FAST, class Ctx>
+__device__ __forceinline__ float trial_axis(const Ctx& C, float r, uint32_t w) {
+  if (FAST) {   // a is a power of two: a tmap(w) = 2a h + a(2^-23 - 1) is exact, one FFMA
+    const float h = __fadd_rn(__uint_as_float(0x3f800000u | (w >> 9)), -1.0f);
+    return __fadd_rn(r, __fmaf_rn(C.a2, h, C.ac));
+  }
+  return __fadd_rn(r, __fmul_rn(C.a, tmap(w)));
+}
+
+// One Metropolis trial move inside a tile.  (rx,ry,rz), addr (shared address of omega at the bead's
+// cell), in (bead inside the tile) follow the bead.  q_l / q_r: current squared lengths of the bonds
+// to the left / right neighbour; on return they hold the lengths after the move.
+template <bool FAST, bool EVEN, class Ctx>
+__device__ __forceinline__ bool tile_move(const TileArgs& A, const Ctx& C, const PhiloxLane& L, uint32_t c0_1,
+                                          float offx, float offy, float offz, uint32_t base_t, const float* __restrict__ omega_t,
+                                          float& rx, float& ry, float& rz, uint32_t& addr, bool& in,
+                                          float lx, float ly, float lz, float& q_l,
+                                          float qx, float qy, float qz, float& q_r, float h) {
+  const Words4 w = philox_tail(A.S.keys, L, c0_1);
+  const float tx = trial_axis<FAST>(C, rx, w.w0);
+  const float ty = trial_axis<FAST>(C, ry, w.w1);
+  const float tz = trial_axis<FAST>(C, rz, w.w2);
+  const float ql_new = bond_sq(tx, ty, tz, lx, ly, lz);
+  const float qr_new = bond_sq(tx, ty, tz, qx, qy, qz);
+  // dq = dq_left + dq_right (one fp32 add).  An even bead always has its right neighbour and an odd
+  // bead its left one; the other may be missing, and then contributes h * (finite) = 0.
+  const float dql = __fsub_rn(ql_new, q_l), dqr = __fsub_rn(qr_new, q_r);
+  const float dq = EVEN ? __fmaf_rn(h, dql, dqr) : __fmaf_rn(h, dqr, dql);
+  uint32_t addr_new;
+  const bool in_new = tile_addr<FAST>(C.g, tx, ty, tz, offx, offy, offz, base_t, addr_new);
+  float w_new, w_old;
+  if (__any_sync(0xffffffffu, !(in_new && in))) {                  // rare, warp-uniform
+    w_new = in_new ? lds_f32(addr_new) : omega_outside(omega_t, A.S.grid, tx, ty, tz);
+    w_old = in ? lds_f32(addr) : omega_outside(omega_t, A.S.grid, rx, ry, rz);
+  } else {
+    w_new = lds_f32(addr_new);
+    w_old = lds_f32(addr);
+  }
+  const float dE = __fmaf_rn(C.kb, dq, __fsub_rn(w_new, w_old));
+  const bool acc = metropolis_accept_fma(dE, w.w3);
+  if (acc) { rx = tx; ry = ty; rz = tz; addr = addr_new; in = in_new; q_l = ql_new; q_r = qr_new; }
+  return acc;
+}
+
+// ---------------------------------------------------------------------------------------------
+// The kernel: one CTA per SM walks over tiles; per tile: TMA-load the omega sub-box, zero the
+// density tile, run both half-sweeps for the tile's chains (chain in registers: two beads per
+// lane, P = N/2 lanes per chain, next chain group prefetched), TMA reduce-add the density tile.
+// FAST: inv_h is a power of two >= 1 on every axis and a is a power of two (see tile_addr,
+// trial_axis); the results are identical either way.
+// ---------------------------------------------------------------------------------------------
+template <int P, bool MULTI_PAT, int NT, bool FAST>
 __global__ void __launch_bounds__(NT, 1)
 tile_step_kernel(const __grid_constant__ TileArgs A, const __grid_constant__ CUtensorMap tm_omega,
                  const __grid_constant__ CUtensorMap tm_counts) {
   constexpr int G = 32 / P;
   constexpr uint32_t NW = NT / 32;
+  constexpr uint32_t N = 2u * P;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t mbar;
-  float* omega_s = reinterpret_cast<float*>(smem_raw);                        // [T][E]
+  float* omega_s = reinterpret_cast<float*>(smem_raw);                            // [T][E]
   uint32_t* counts_s = reinterpret_cast<uint32_t*>(smem_raw + A.counts_offset);   // [T][E]
   const StepArgs& S = A.S;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -154,6 +270,17 @@ tile_step_kernel(const __grid_constant__ TileArgs A, const __grid_constant__ CUt
   if (tid == 0) mbar_init(&mbar, 1);
   __syncthreads();
 
+  LaneCtx C;
+  C.g.inv_hx = S.grid.inv_hx; C.g.inv_hy = S.grid.inv_hy; C.g.inv_hz = S.grid.inv_hz;
+  C.g.ex = A.ex; C.g.ey = A.ey; C.g.ez = A.ez;
+  C.g.sy = A.ez * 4u; C.g.sx = A.ey * A.ez * 4u;
+  C.a = S.a; C.a2 = A.a2; C.ac = A.ac; C.kb = S.kb;
+  const float hl = l > 0 ? 1.0f : 0.0f, hr = l + 1 < P ? 1.0f : 0.0f;
+  const PhiloxLane L0 = philox_lane(S.keys, A.philox_u1, 2u * l, S.ctr3_base);
+  const PhiloxLane L1 = philox_lane(S.keys, A.philox_u1, 2u * l + 1u, S.ctr3_base | 1u);
+
+  const uint32_t omega_base = smem_u32(omega_s);
+  const uint32_t type_stride = A.E * 4u;
   uint32_t type0 = 0, type1 = 0;
   if (!MULTI_PAT) {
     const uint16_t tt = *reinterpret_cast<const uint16_t*>(S.patterns + 2u * l);
@@ -161,18 +288,16 @@ tile_step_kernel(const __grid_constant__ TileArgs A, const __grid_constant__ CUt
   }
 
   for (uint32_t tile = blockIdx.x; tile < A.n_tiles; tile += gridDim.x) {
-    const uint32_t start = A.tile_start[tile], end = A.tile_start[tile + 1];
+    const uint32_t start = A.tile_start[2u * tile], end = A.tile_start[2u * tile + 2u];
     if (start == end) continue;                                               // uniform over the CTA
     const uint32_t tz = tile % A.mtz, ty = (tile / A.mtz) % A.mty, tx = tile / (A.mtz * A.mty);
-    const int ox = (int)(tx * A.cx) - (int)A.hx, oy = (int)(ty * A.cy) - (int)A.hy, oz = (int)(tz * A.cz) - (int)A.hz;
-    TileGeom g;
-    g.mx = kFloorMagic - (float)ox; g.my = kFloorMagic - (float)oy; g.mz = kFloorMagic - (float)oz;
+    const int qx = (int)(tx * A.cx), qy = (int)(ty * A.cy), qz = (int)(tz * A.cz);   // padded coordinates of the tile box
 
-    // omega tile in (the padded copy is indexed from -halo, so the coordinates are never negative);
-    // the previous tile's density flush must have finished READING shared memory before it is zeroed
+    // omega tile in; the previous tile's density flush must have finished READING shared memory
+    // before the density tile is zeroed
     if (tid == 0) {
       mbar_expect_tx(&mbar, tile_words * 4u);
-      tma_load_4d(omega_s, &tm_omega, &mbar, oz + (int)A.hz, oy + (int)A.hy, ox + (int)A.hx, 0);
+      tma_load_4d(omega_s, &tm_omega, &mbar, qz, qy, qx, 0);
       bulk_wait_read0();
     }
     __syncthreads();
@@ -183,52 +308,75 @@ tile_step_kernel(const __grid_constant__ TileArgs A, const __grid_constant__ CUt
 
     const uint32_t n_slots = end - start;
     const uint32_t n_groups = (n_slots + G - 1) / G;
-    for (uint32_t wg = warp; wg < n_groups; wg += NW) {
+    // software pipeline: the loads of group wg + NW are in flight while group wg is computed
+    float2 Xn, Yn, Zn;
+    float4 Mn;
+    uint32_t slot_n = 0;
+    bool live_n = false;
+    auto fetch = [&](uint32_t wg) {
       const uint32_t rel = wg * G + sub;
-      const bool live = rel < n_slots;
-      const uint32_t slot = start + (live ? rel : 0u);                        // dead lanes shadow the first slot
-      const uint64_t j = (uint64_t)slot * S.N + 2u * l;
-      const float2 X = *reinterpret_cast<const float2*>(S.x + j);
-      const float2 Y = *reinterpret_cast<const float2*>(S.y + j);
-      const float2 Z = *reinterpret_cast<const float2*>(S.z + j);
-      const uint32_t chain = S.slot_chain[slot];
+      live_n = rel < n_slots;
+      slot_n = start + (live_n ? rel : 0u);                                   // dead lanes shadow the first slot
+      const uint64_t j = (uint64_t)slot_n * N + 2u * l;
+      Xn = *reinterpret_cast<const float2*>(S.x + j);
+      Yn = *reinterpret_cast<const float2*>(S.y + j);
+      Zn = *reinterpret_cast<const float2*>(S.z + j);
+      Mn = __ldg(A.slot_meta + slot_n);
+    };
+    if (warp < n_groups) fetch(warp);
+    for (uint32_t wg = warp; wg < n_groups; wg += NW) {
+      const float2 X = Xn, Y = Yn, Z = Zn;
+      const float4 M = Mn;
+      const uint32_t slot = slot_n;
+      const bool live = live_n;
+      if (wg + NW < n_groups) fetch(wg + NW);
+      const uint32_t c0_1 = A.philox_u0 ^ __float_as_uint(M.w);
       if (MULTI_PAT) {
-        const uint16_t tt = *reinterpret_cast<const uint16_t*>(S.patterns + (uint32_t)S.slot_pattern[slot] * S.N + 2u * l);
+        const uint16_t tt = *reinterpret_cast<const uint16_t*>(S.patterns + (uint32_t)S.slot_pattern[slot] * N + 2u * l);
         type0 = tt & 0xffu; type1 = tt >> 8;
       }
+      const uint32_t base0 = omega_base + type0 * type_stride, base1 = omega_base + type1 * type_stride;
       float ex = X.x, ey = Y.x, ez = Z.x;                                     // even bead 2l
-      float ox_ = X.y, oy_ = Y.y, oz_ = Z.y;                                  // odd bead 2l+1
-      uint32_t idx_e = local_cell(A, g, ex, ey, ez);
-      uint32_t idx_o = local_cell(A, g, ox_, oy_, oz_);
+      float ox = X.y, oy = Y.y, oz = Z.y;                                     // odd bead 2l+1
+      uint32_t addr_e, addr_o;
+      bool in_e = tile_addr<FAST>(C.g, ex, ey, ez, M.x, M.y, M.z, base0, addr_e);
+      bool in_o = tile_addr<FAST>(C.g, ox, oy, oz, M.x, M.y, M.z, base1, addr_o);
+      // squared lengths of this lane's two bonds: A = (even, odd), B = (odd of lane l-1, even)
+      const float lx = __shfl_up_sync(0xffffffffu, ox, 1, P);
+      const float ly = __shfl_up_sync(0xffffffffu, oy, 1, P);
+      const float lz = __shfl_up_sync(0xffffffffu, oz, 1, P);
+      float qA = bond_sq(ex, ey, ez, ox, oy, oz);
+      float qB = bond_sq(ex, ey, ez, lx, ly, lz);
+      // half-sweep 0: even bead; left neighbour = odd bead of lane l-1, right neighbour = own odd bead
       {
-        const float lx = __shfl_up_sync(0xffffffffu, ox_, 1, P);
-        const float ly = __shfl_up_sync(0xffffffffu, oy_, 1, P);
-        const float lz = __shfl_up_sync(0xffffffffu, oz_, 1, P);
-        const bool acc = move_bead_tile(A, g, chain, 2u * l, 0u, omega_s + type0 * A.E, type0 * S.cells, ex, ey, ez, idx_e,
-                                        l > 0, lx, ly, lz, true, ox_, oy_, oz_);
+        const bool acc = tile_move<FAST, true>(A, C, L0, c0_1, M.x, M.y, M.z, base0, S.omega + (size_t)type0 * S.cells,
+                                               ex, ey, ez, addr_e, in_e, lx, ly, lz, qB, ox, oy, oz, qA, hl);
         n_acc += (acc && live) ? 1u : 0u;
       }
+      // half-sweep 1: odd bead; left = own even bead (new), right = even bead of lane l+1 (new)
       {
-        const float qx = __shfl_down_sync(0xffffffffu, ex, 1, P);
-        const float qy = __shfl_down_sync(0xffffffffu, ey, 1, P);
-        const float qz = __shfl_down_sync(0xffffffffu, ez, 1, P);
-        const bool acc = move_bead_tile(A, g, chain, 2u * l + 1u, 1u, omega_s + type1 * A.E, type1 * S.cells, ox_, oy_, oz_, idx_o,
-                                        true, ex, ey, ez, l + 1 < P, qx, qy, qz);
+        const float rx = __shfl_down_sync(0xffffffffu, ex, 1, P);
+        const float ry = __shfl_down_sync(0xffffffffu, ey, 1, P);
+        const float rz = __shfl_down_sync(0xffffffffu, ez, 1, P);
+        float qR = __shfl_down_sync(0xffffffffu, qB, 1, P);
+        const bool acc = tile_move<FAST, false>(A, C, L1, c0_1, M.x, M.y, M.z, base1, S.omega + (size_t)type1 * S.cells,
+                                                ox, oy, oz, addr_o, in_o, ex, ey, ez, qA, rx, ry, rz, qR, hr);
         n_acc += (acc && live) ? 1u : 0u;
       }
       if (live) {
-        *reinterpret_cast<float2*>(S.x + j) = make_float2(ex, ox_);
-        *reinterpret_cast<float2*>(S.y + j) = make_float2(ey, oy_);
-        *reinterpret_cast<float2*>(S.z + j) = make_float2(ez, oz_);
-        count_bead(A, counts_s, type0, idx_e, ex, ey, ez);
-        count_bead(A, counts_s, type1, idx_o, ox_, oy_, oz_);
+        const uint64_t j = (uint64_t)slot * N + 2u * l;
+        *reinterpret_cast<float2*>(S.x + j) = make_float2(ex, ox);
+        *reinterpret_cast<float2*>(S.y + j) = make_float2(ey, oy);
+        *reinterpret_cast<float2*>(S.z + j) = make_float2(ez, oz);
+        if (in_e) reds_inc(addr_e + A.counts_offset); else count_outside(A, type0, ex, ey, ez);
+        if (in_o) reds_inc(addr_o + A.counts_offset); else count_outside(A, type1, ox, oy, oz);
       }
     }
     // density tile out
     fence_proxy_async();
     __syncthreads();
-    if (tid == 0) {                                                           // padded coordinates: origin + halo = tile * core
-      tma_reduce_add_4d(&tm_counts, counts_s, oz + (int)A.hz, oy + (int)A.hy, ox + (int)A.hx, 0);
+    if (tid == 0) {
+      tma_reduce_add_4d(&tm_counts, counts_s, qz, qy, qx, 0);
       bulk_commit();
     }
   }
@@ -236,6 +384,56 @@ tile_step_kernel(const __grid_constant__ TileArgs A, const __grid_constant__ CUt
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) n_acc += __shfl_xor_sync(0xffffffffu, n_acc, o);
   if (lane == 0 && n_acc) atomicAdd(S.accepted, (unsigned long long)n_acc);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Sorting the chains for the tiled kernel.  Key of a chain = 2 * (tile whose core holds the cell of
+// its centre of mass) + (1 if a bead lies within `margin` cells of the tile's faces or beyond, else
+// 0): a tile's compact chains come first, so that the warps working on them never take the slow
+// path, and the extended ones share warps among themselves.  The same pass writes the chain's
+// floor offsets (see tile_addr): off = kFloorMagic + (g - G) - origin per axis, G the unwrapped and
+// g the wrapped cell coordinate of the centre of mass.
+// ---------------------------------------------------------------------------------------------
+struct TileSortArgs {
+  Grid grid;
+  uint32_t n_chains, N;
+  uint32_t cx, cy, cz, hx, hy, hz, ex, ey, ez, mty, mtz;
+  uint32_t margin;
+};
+
+__global__ void __launch_bounds__(256)
+tile_key_kernel(TileSortArgs S, const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ z,
+                const uint32_t* __restrict__ slot_chain, uint32_t* __restrict__ bin_count, uint32_t* __restrict__ key,
+                uint32_t* __restrict__ rank, float4* __restrict__ meta) {
+  const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= S.n_chains) return;
+  const uint64_t j0 = (uint64_t)s * S.N;
+  float sx = 0.f, sy = 0.f, sz = 0.f;
+  for (uint32_t i = 0; i < S.N; ++i) { sx += x[j0 + i]; sy += y[j0 + i]; sz += z[j0 + i]; }
+  const float inv = 1.0f / (float)S.N;
+  const int Gx = __float2int_rd(__fmul_rn(sx * inv, S.grid.inv_hx));
+  const int Gy = __float2int_rd(__fmul_rn(sy * inv, S.grid.inv_hy));
+  const int Gz = __float2int_rd(__fmul_rn(sz * inv, S.grid.inv_hz));
+  const int gx = Gx & (int)(S.grid.nx - 1u), gy = Gy & (int)(S.grid.ny - 1u), gz = Gz & (int)(S.grid.nz - 1u);
+  const uint32_t tx = (uint32_t)gx / S.cx, ty = (uint32_t)gy / S.cy, tz = (uint32_t)gz / S.cz;
+  // relative cell of a bead = floor(r inv_h) + d, d = (g - G) - origin
+  const int dx = gx - Gx - ((int)(tx * S.cx) - (int)S.hx);
+  const int dy = gy - Gy - ((int)(ty * S.cy) - (int)S.hy);
+  const int dz = gz - Gz - ((int)(tz * S.cz) - (int)S.hz);
+  bool ext = false;
+  const int m = (int)S.margin;
+  for (uint32_t i = 0; i < S.N; ++i) {
+    const int rx = __float2int_rd(__fmul_rn(x[j0 + i], S.grid.inv_hx)) + dx;
+    const int ry = __float2int_rd(__fmul_rn(y[j0 + i], S.grid.inv_hy)) + dy;
+    const int rz = __float2int_rd(__fmul_rn(z[j0 + i], S.grid.inv_hz)) + dz;
+    ext |= rx < m || rx >= (int)S.ex - m || ry < m || ry >= (int)S.ey - m || rz < m || rz >= (int)S.ez - m;
+  }
+  const uint32_t tile = (tx * S.mty + ty) * S.mtz + tz;
+  const uint32_t k = 2u * tile + (ext ? 1u : 0u);
+  key[s] = k;
+  rank[s] = atomicAdd(bin_count + k, 1u);
+  meta[s] = make_float4(kFloorMagic + (float)dx, kFloorMagic + (float)dy, kFloorMagic + (float)dz,
+                        __uint_as_float(slot_chain[s]));
 }
 
 // ---------------------------------------------------------------------------------------------
