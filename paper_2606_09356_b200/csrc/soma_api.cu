@@ -49,6 +49,12 @@ uint64_t sort_bin_count(const uint32_t grid[3]) {
   return n;
 }
 
+// entries of the bin array: the cube bins of the plain re-ordering, or 2 bins per (unit, slice) of the sweep
+uint64_t sort_bins_capacity(const uint32_t grid[3]) {
+  const uint64_t a = sort_bin_count(grid) + 2, b = (uint64_t)grid[0] * grid[1] * grid[2] / 8 + 2;
+  return a > b ? a : b;
+}
+
 // the ghost-padded omega copy is sized for the largest tile the options allow
 constexpr uint32_t kMaxTileCore = 32, kMaxTileHalo = 16;
 uint64_t omega_pad_cells_max(const uint32_t grid[3]) {
@@ -62,6 +68,7 @@ bool tile_capable_grid(const uint32_t grid[3]) {      // power-of-two axes, at l
   return true;
 }
 
+// n_bins: entries of the sort_bins array (see sort_bins_capacity)
 Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins, uint64_t pad_words) {
   Layout L{};
   uint64_t off = 0;
@@ -77,7 +84,7 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   L.range_flag = off; off += align_up(4);
   L.sort_key = off; off += align_up(n * 4);
   L.sort_rank = off; off += align_up(n * 4);
-  L.sort_bins = off; off += align_up((2 * n_bins + 2) * 4);
+  L.sort_bins = off; off += align_up(n_bins * 4);
   L.slot_meta = off; off += align_up(n * 16);
   L.meta_src = off; off += align_up(n * 16);
   L.omega_pad = off; off += align_up(pad_words * 4);
@@ -171,7 +178,10 @@ struct soma_handle {
   uint32_t tc[3], th[3];        // tile core and halo in cells
   int tile_threads;             // 512, 768 or 1024
   bool tile_fast;               // inv_h a power of two >= 1 on every axis and a a power of two
-  uint32_t tile_margin;         // chains with a bead this close to a tile face sort behind the others
+  uint32_t tile_margin;         // chains with a bead this close to a window face sort behind the others
+  uint32_t tile_slice, tile_ring_opt;   // slice width in cells; ring slots (0 = as many as fit)
+  uint32_t tile_lseg, tile_K, tile_R, tile_slab_bytes, tile_slab_stride, tile_aux_offset;
+  uint64_t sort_bins_cap;       // entries of the sort_bins array
   uint32_t te[3], tm[3], n_tiles, pad[3];
   size_t tile_smem;
   uint32_t tile_counts_offset;
@@ -422,26 +432,46 @@ void tile_setup(soma_handle* h) {
   const int P = fused_lanes(h->N);
   if (!P) return no("beads_per_chain must be 2P, P a power of two <= 32");
   const uint32_t n[3] = {h->grid.nx, h->grid.ny, h->grid.nz};
-  uint64_t E = 1, nt = 1;
+  // x: segments of tc[0] cells swept in slices; y, z: column cores tc[1] x tc[2]
+  if (h->tile_slice < 1 || h->tile_slice > 16) return no("tile_slice must be in [1, 16]");
+  uint32_t Lseg = h->tc[0] < n[0] ? h->tc[0] : n[0];
+  if (Lseg < h->tile_slice || (Lseg & (Lseg - 1)) || Lseg % h->tile_slice) return no("segment length must be a power of two and a multiple of the slice");
+  if (Lseg / h->tile_slice > kMaxSlices) return no("too many slices per segment");
+  for (int d = 1; d < 3; ++d)
+    if (h->tc[d] < 4 || h->tc[d] > kMaxTileCore) return no("column core must be in [4, 32] cells");
+  for (int d = 0; d < 3; ++d)
+    if (h->th[d] > kMaxTileHalo) return no("halo must be <= 16 cells");
+  h->te[0] = h->tile_slice + 2 * h->th[0];
+  h->te[1] = h->tc[1] + 2 * h->th[1];
+  h->te[2] = h->tc[2] + 2 * h->th[2];
+  uint64_t nt = 1;
   for (int d = 0; d < 3; ++d) {
-    if (h->tc[d] < 4 || h->tc[d] > kMaxTileCore || h->th[d] > kMaxTileHalo) return no("tile core must be in [4, 32], halo <= 16");
-    h->te[d] = h->tc[d] + 2 * h->th[d];
-    if (h->te[d] > n[d]) return no("tile (core + 2 halo) is larger than the grid");
-    h->tm[d] = (n[d] + h->tc[d] - 1) / h->tc[d];
-    h->pad[d] = h->tm[d] * h->tc[d] + 2 * h->th[d];
-    E *= h->te[d];
+    const uint32_t core = d == 0 ? Lseg : h->tc[d];
+    if (h->te[d] > n[d]) return no("window (core + 2 halo) is larger than the grid");
+    h->tm[d] = (n[d] + core - 1) / core;
+    h->pad[d] = h->tm[d] * core + 2 * h->th[d];
+    if (h->pad[d] > 2 * n[d]) return no("padded grid would hold a cell three times");
     nt *= h->tm[d];
   }
-  if (h->tc[2] % 4 || h->te[2] % 4) return no("tile core and extent along z must be multiples of 4 cells");
-  for (int d = 0; d < 3; ++d)
-    if (h->pad[d] > 2 * n[d]) return no("padded grid would hold a cell three times");
+  if (h->tc[2] % 4 || h->te[2] % 4) return no("column core and extent along z must be multiples of 4 cells");
   h->pad[2] = (h->pad[2] + 3u) / 4u * 4u;
-  if (nt > h->n_bins) return no("too many tiles");
+  h->tile_lseg = Lseg;
+  h->tile_K = Lseg / h->tile_slice;
+  if (2 * nt * h->tile_K + 1 > h->sort_bins_cap) return no("too many units");
   h->n_tiles = (uint32_t)nt;
-  const uint64_t tile_bytes = E * h->T * 4;
-  h->tile_counts_offset = (uint32_t)((tile_bytes + 127) / 128 * 128);
-  h->tile_smem = (size_t)h->tile_counts_offset + tile_bytes;
-  if (h->tile_smem > 227 * 1024 - 1024) return no("tile does not fit in shared memory");
+  h->tile_slab_bytes = h->T * h->te[1] * h->te[2] * 4;
+  h->tile_slab_stride = (h->tile_slab_bytes + 127u) / 128u * 128u;
+  const uint32_t smem_max = 227u * 1024u;
+  uint32_t R = (smem_max - kSweepAuxBytes) / (2u * h->tile_slab_stride);
+  if (R > kMaxRing) R = kMaxRing;
+  if (R > Lseg + 2 * h->th[0]) R = Lseg + 2 * h->th[0];
+  if (h->tile_ring_opt) { if (h->tile_ring_opt > R) return no("tile_ring does not fit in shared memory"); R = h->tile_ring_opt; }
+  if (R < h->te[0]) return no("the ring cannot hold one window (slice + 2 hx slabs)");
+  if ((uint64_t)R * h->tile_slab_stride >= (1u << 22)) return no("ring too large");
+  h->tile_R = R;
+  h->tile_counts_offset = R * h->tile_slab_stride;
+  h->tile_aux_offset = 2u * R * h->tile_slab_stride;
+  h->tile_smem = (size_t)h->tile_aux_offset + kSweepAuxBytes;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult q;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) {
@@ -449,9 +479,10 @@ void tile_setup(soma_handle* h) {
     return no("cuTensorMapEncodeTiled is not available");
   }
   EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(fn);
-  if (!encode_map(enc, &h->tm_omega, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, h->omega_pad(), h->T, h->pad, h->te)) return no("tensor map (omega) rejected");
+  const uint32_t box[3] = {1, h->te[1], h->te[2]};                    // one slab: [T][1][ey][ez]
+  if (!encode_map(enc, &h->tm_omega, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, h->omega_pad(), h->T, h->pad, box)) return no("tensor map (omega) rejected");
   for (int s = 0; s < 2; ++s)
-    if (!encode_map(enc, &h->tm_counts[s], CU_TENSOR_MAP_DATA_TYPE_UINT32, h->counts_pad(s), h->T, h->pad, h->te)) return no("tensor map (counts) rejected");
+    if (!encode_map(enc, &h->tm_counts[s], CU_TENSOR_MAP_DATA_TYPE_UINT32, h->counts_pad(s), h->T, h->pad, box)) return no("tensor map (counts) rejected");
   // both padded density grids start zeroed; from here on the omega pass keeps them so
   const size_t pad_bytes = (size_t)h->pad[0] * h->pad[1] * h->pad[2] * h->T * 4;
   if (cudaMemsetAsync(h->counts_pad(0), 0, pad_bytes, h->stream) != cudaSuccess ||
@@ -473,12 +504,14 @@ int launch_tile_pn(soma_handle* h) {
   A.S = step_args(h);
   A.slot_meta = h->slot_meta();
   A.T = h->T;
-  A.ex = h->te[0]; A.ey = h->te[1]; A.ez = h->te[2]; A.E = h->te[0] * h->te[1] * h->te[2];
-  A.cx = h->tc[0]; A.cy = h->tc[1]; A.cz = h->tc[2];
+  A.wx = h->te[0]; A.ey = h->te[1]; A.ez = h->te[2];
+  A.cy = h->tc[1]; A.cz = h->tc[2];
   A.hx = h->th[0]; A.hy = h->th[1]; A.hz = h->th[2];
-  A.mty = h->tm[1]; A.mtz = h->tm[2]; A.n_tiles = h->n_tiles;
-  A.counts_offset = h->tile_counts_offset;
-  A.tile_start = h->sort_bins();
+  A.slice = h->tile_slice; A.R = h->tile_R; A.K = h->tile_K; A.Lseg = h->tile_lseg;
+  A.mtz = h->tm[2]; A.nseg = h->tm[0]; A.n_units = h->n_tiles;
+  A.slab_bytes = h->tile_slab_bytes; A.slab_stride = h->tile_slab_stride;
+  A.counts_offset = h->tile_counts_offset; A.aux_offset = h->tile_aux_offset;
+  A.bin_start = h->sort_bins();
   A.counts_pad = h->counts_pad(h->pad_cur);
   A.px = h->pad[0]; A.py = h->pad[1]; A.pz = h->pad[2];
   const uint64_t m1 = (uint64_t)kPhiloxM1 * A.S.ctr2;
@@ -521,12 +554,12 @@ int resort(soma_handle* h, int kind) {
   if (kind == 2) {
     TileSortArgs S{};
     S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
-    S.cx = h->tc[0]; S.cy = h->tc[1]; S.cz = h->tc[2];
+    S.cy = h->tc[1]; S.cz = h->tc[2];
     S.hx = h->th[0]; S.hy = h->th[1]; S.hz = h->th[2];
-    S.ex = h->te[0]; S.ey = h->te[1]; S.ez = h->te[2];
-    S.mty = h->tm[1]; S.mtz = h->tm[2];
+    S.wx = h->te[0]; S.ey = h->te[1]; S.ez = h->te[2];
+    S.slice = h->tile_slice; S.K = h->tile_K; S.Lseg = h->tile_lseg; S.mtz = h->tm[2]; S.nseg = h->tm[0];
     S.margin = h->tile_margin;
-    n_bins = 2u * h->n_tiles;
+    n_bins = 2u * h->n_tiles * h->tile_K;
     CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
     tile_key_kernel<<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
         S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->slot_chain(src), h->sort_bins(), h->sort_key(),
@@ -650,7 +683,7 @@ uint64_t soma_workspace_bytes(const soma_params* p) {
   const uint64_t B = p->n_chains * p->beads_per_chain;
   const uint64_t TC = (uint64_t)p->grid[0] * p->grid[1] * p->grid[2] * p->n_types;
   const uint64_t pad_words = tile_capable_grid(p->grid) ? omega_pad_cells_max(p->grid) * p->n_types : 0;
-  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bin_count(p->grid), pad_words).total;
+  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bins_capacity(p->grid), pad_words).total;
 }
 
 int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
@@ -695,7 +728,8 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->seed = p->seed;
   h->n_bins = (uint32_t)sort_bin_count(p->grid);
   h->tile_grid_ok = tile_capable_grid(p->grid);
-  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, h->n_bins,
+  h->sort_bins_cap = sort_bins_capacity(p->grid);
+  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, h->sort_bins_cap,
                      h->tile_grid_ok ? omega_pad_cells_max(p->grid) * h->T : 0);
   if (p->workspace) {
     if (p->workspace_bytes < h->L.total || (reinterpret_cast<uintptr_t>(p->workspace) % kAlign)) {
@@ -739,8 +773,10 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->resort_interval = h->n_chains >= 4096 ? 64 : 0;
   h->fused_blocks_per_sm = 3;
   h->fused_waves = 1;
-  h->tc[0] = 12; h->tc[1] = 12; h->tc[2] = 8;
-  h->th[0] = h->th[1] = h->th[2] = 6;
+  h->tc[0] = 64; h->tc[1] = 8; h->tc[2] = 8;
+  h->th[0] = h->th[1] = h->th[2] = 8;
+  h->tile_slice = 2;
+  h->tile_ring_opt = 0;
   h->tile_threads = 768;
   h->tile_margin = 1;
   {
@@ -905,14 +941,21 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     return SOMA_OK;
   }
   {
-    static const char* const tn[7] = {"tile_cx", "tile_cy", "tile_cz", "tile_hx", "tile_hy", "tile_hz", "tile_threads"};
-    for (int k = 0; k < 7; ++k)
+    static const char* const tn[9] = {"tile_cx", "tile_cy", "tile_cz", "tile_hx", "tile_hy", "tile_hz", "tile_threads",
+                                      "tile_slice", "tile_ring"};
+    for (int k = 0; k < 9; ++k)
       if (!std::strcmp(name, tn[k])) {
         if (k == 6) {
           if (value != 512 && value != 768 && value != 1024) return fail(h, SOMA_EINVAL, "tile_threads must be 512, 768 or 1024");
           h->tile_threads = (int)value;
+        } else if (k == 7) {
+          if (value < 1 || value > 16) return fail(h, SOMA_EINVAL, "tile_slice must be in [1, 16]");
+          h->tile_slice = (uint32_t)value;
+        } else if (k == 8) {
+          if (value < 0 || value > (int64_t)kMaxRing) return fail(h, SOMA_EINVAL, "tile_ring must be in [0, 32]");
+          h->tile_ring_opt = (uint32_t)value;
         } else {
-          if (value < 0 || value > 64) return fail(h, SOMA_EINVAL, "tile size out of range");
+          if (value < 0 || value > 4096) return fail(h, SOMA_EINVAL, "tile size out of range");
           (k < 3 ? h->tc[k] : h->th[k - 3]) = (uint32_t)value;
         }
         tile_setup(h);

@@ -131,57 +131,82 @@ __device__ __forceinline__ bool metropolis_accept_fma(float dE, uint32_t w3) {
   return acc;
 }
 
-// ---- tile-local cell -----------------------------------------------------------------------------
-// `off` = kFloorMagic - tile origin + the chain's periodic image shift (whole cells, set when the
-// chains are sorted), so the bit pattern of RD(r inv_h + off) is kFloorMagicBits + the bead's cell
-// coordinate RELATIVE to the tile origin, with no periodic wrap left to do.  FASTH: inv_h is a
-// power of two >= 1, so r inv_h is exact and one FFMA.RD gives the same bits as FMUL + FADD.RD.
-constexpr uint32_t kFloorMagicBits = 0x4b400000u;
-
-struct TileGeo {
+// ---- window-local cell ---------------------------------------------------------------------------
+// A chain group works inside a WINDOW of the grid: wx x ey x ez cells whose omega values and
+// density counters sit in shared memory, slab by slab along x (a slab = one x layer, [T][ey][ez]),
+// the slabs forming a ring of R slots (slab a of the sweep lives in slot a mod R).
+// `off` = kFloorMagic - window origin + the chain's periodic image shift (whole cells, set when the
+// chains are sorted), so RD(r inv_h + off) - kFloorMagic is the bead's cell coordinate RELATIVE to
+// the window origin as an exact small float, with no periodic wrap left to do.  FAST: inv_h is a
+// power of two >= 1, so r inv_h is exact and one FFMA.RD gives the same value as FMUL + FADD.RD.
+//
+// Everything stays on the FMA pipe: the range test compares float bit patterns (a negative float
+// has the sign bit set, so one unsigned compare per axis covers both ends); the ring slot of a bead
+// at window-relative x is u - R [u >= R] with u = x + p, p = (slab of the window origin) mod R --
+// the window is at most R slabs wide, so it crosses the ring seam at most once, and the indicator
+// is a saturating add, sat(x + p - R + 1); and the shared address is assembled by FFMAs on
+// DENORMALS: a float with bit pattern n is n 2^-149, so fma(idx, as_float(stride), as_float(base))
+// has the bit pattern base + idx*stride as long as that stays below 2^23.
+struct WinGeo {
   float inv_hx, inv_hy, inv_hz;
-  uint32_t ex, ey, ez;          // tile extent in cells
-  uint32_t sx, sy;              // byte strides of x and y in the shared-memory tile (z: 4)
+  float wx_f, ey_f, ez_f;       // window extent in cells (as floats: compared as bit patterns)
+  float neg_R;                  // -R
+  float slab_stride_d, sy_d, four_d;   // denormals whose bit patterns are the byte strides (slot, y, z)
 };
 
+__device__ __forceinline__ float fadd_sat(float a, float b) {
+  float r;
+  asm("add.sat.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+  return r;
+}
+
 template <bool FASTH>
-__device__ __forceinline__ bool tile_addr(const TileGeo& g, float x, float y, float z, float offx, float offy, float offz,
-                                          uint32_t base_t, uint32_t& addr) {
+__device__ __forceinline__ bool win_addr(const WinGeo& g, float x, float y, float z, float offx, float offy, float offz,
+                                         float p_f /* slab of the window origin mod R */, float seam_f /* p - R + 1 */,
+                                         float base_t_d, uint32_t& addr) {
   float fx, fy, fz;
   if (FASTH) {
     fx = __fmaf_rd(x, g.inv_hx, offx); fy = __fmaf_rd(y, g.inv_hy, offy); fz = __fmaf_rd(z, g.inv_hz, offz);
   } else {
     fx = __fadd_rd(__fmul_rn(x, g.inv_hx), offx); fy = __fadd_rd(__fmul_rn(y, g.inv_hy), offy); fz = __fadd_rd(__fmul_rn(z, g.inv_hz), offz);
   }
-  const uint32_t ux = __float_as_uint(fx) - kFloorMagicBits;
-  const uint32_t uy = __float_as_uint(fy) - kFloorMagicBits;
-  const uint32_t uz = __float_as_uint(fz) - kFloorMagicBits;
-  addr = ux * g.sx + (uy * g.sy + (uz * 4u + base_t));
-  return (ux < g.ex) & (uy < g.ey) & (uz < g.ez);
+  const float rx = __fadd_rn(fx, -kFloorMagic), ry = __fadd_rn(fy, -kFloorMagic), rz = __fadd_rn(fz, -kFloorMagic);
+  const float slot = __fmaf_rn(fadd_sat(rx, seam_f), g.neg_R, __fadd_rn(rx, p_f));
+  addr = __float_as_uint(__fmaf_rn(slot, g.slab_stride_d, __fmaf_rn(ry, g.sy_d, __fmaf_rn(rz, g.four_d, base_t_d))));
+  return (__float_as_uint(rx) < __float_as_uint(g.wx_f)) & (__float_as_uint(ry) < __float_as_uint(g.ey_f)) &
+         (__float_as_uint(rz) < __float_as_uint(g.ez_f));
 }
+
+constexpr uint32_t kMaxRing = 32;      // ring slots
+constexpr uint32_t kMaxSlices = 128;   // slices per unit
+constexpr uint32_t kSweepAuxBytes = 4096;
 
 struct TileArgs {
   StepArgs S;                 // omega = linear field (slow path); counts_next is not used by this kernel
   const float4* __restrict__ slot_meta;     // [n] per slot: floor offsets x, y, z and the chain id (bits)
   uint32_t* __restrict__ counts_pad;        // [T][px][py][pz] ghost-padded density grid this step bins into
-  const uint32_t* __restrict__ tile_start;  // [2 n_tiles + 1]: compact chains of tile k, then its extended ones
+  const uint32_t* __restrict__ bin_start;   // [2 K n_units + 1]: per unit and slice, compact chains then extended ones
   uint32_t px, py, pz;        // padded dims: padded coordinate q holds cell (q - halo) mod n
   uint32_t T;
-  uint32_t ex, ey, ez, E;     // tile extent in cells (core + 2*halo), E = ex*ey*ez
-  uint32_t cx, cy, cz;        // core
+  uint32_t ey, ez, wx;        // window extent in cells: wx = slice + 2 hx
+  uint32_t cy, cz;            // column core
   uint32_t hx, hy, hz;        // halo
-  uint32_t mty, mtz, n_tiles; // tiles along y and z, total
-  uint32_t counts_offset;     // byte offset of the density tile in dynamic shared memory
+  uint32_t slice, R, K, Lseg; // slice width (cells), ring slots, slices per unit, segment length = K * slice
+  uint32_t mtz, nseg, n_units;// columns along z, segments along x, units = columns * segments
+  uint32_t slab_bytes;        // T*ey*ez*4: bytes one TMA slab box writes
+  uint32_t slab_stride;       // slab_bytes rounded up to 128
+  uint32_t counts_offset;     // byte offset of the density ring in dynamic shared memory
+  uint32_t aux_offset;        // byte offset of the barriers and slice tables
   uint32_t philox_u0, philox_u1;   // hi(M1 step) ^ k0[0], lo(M1 step)
-  float a2, ac;               // APOW2: 2a and a (2^-23 - 1)
+  float a2, ac;               // FAST: 2a and a (2^-23 - 1)
 };
 
-// omega at a bead's cell on the slow path (some lane of the warp has a bead outside the tile)
+// omega at a bead's cell on the slow path (some lane of the warp has a bead outside the window)
 __device__ __noinline__ float omega_outside(const float* __restrict__ omega_t, Grid grid, float x, float y, float z) {
   return __ldg(omega_t + cell_of<true>(grid, x, y, z));
 }
 
-// density increment of a bead outside the tile: straight into the padded grid, at the image that
+// density increment of a bead outside the window: straight into the padded grid, at the image that
 // lies `halo` inside it
 __device__ __noinline__ void count_outside(const TileArgs& A, uint32_t type, float x, float y, float z) {
   const Grid& G = A.S.grid;
@@ -193,13 +218,13 @@ __device__ __noinline__ void count_outside(const TileArgs& A, uint32_t type, flo
 
 // Kernel-constant scalars a move needs.
 struct LaneCtx {
-  TileGeo g;
+  WinGeo g;
   float a, a2, ac, kb;
 };
 
 // trial displacement along one axis (DESIGN.md section 2 steps 5.2-5.3): r' = r + a tmap(w)
-template <bool FAST, class Ctx>
-__device__ __forceinline__ float trial_axis(const Ctx& C, float r, uint32_t w) {
+template <bool FAST>
+__device__ __forceinline__ float trial_axis(const LaneCtx& C, float r, uint32_t w) {
   if (FAST) {   // a is a power of two: a tmap(w) = 2a h + a(2^-23 - 1) is exact, one FFMA
     const float h = __fadd_rn(__uint_as_float(0x3f800000u | (w >> 9)), -1.0f);
     return __fadd_rn(r, __fmaf_rn(C.a2, h, C.ac));
@@ -207,12 +232,13 @@ __device__ __forceinline__ float trial_axis(const Ctx& C, float r, uint32_t w) {
   return __fadd_rn(r, __fmul_rn(C.a, tmap(w)));
 }
 
-// One Metropolis trial move inside a tile.  (rx,ry,rz), addr (shared address of omega at the bead's
-// cell), in (bead inside the tile) follow the bead.  q_l / q_r: current squared lengths of the bonds
-// to the left / right neighbour; on return they hold the lengths after the move.
-template <bool FAST, bool EVEN, class Ctx>
-__device__ __forceinline__ bool tile_move(const TileArgs& A, const Ctx& C, const PhiloxLane& L, uint32_t c0_1,
-                                          float offx, float offy, float offz, uint32_t base_t, const float* __restrict__ omega_t,
+// One Metropolis trial move inside a window.  (rx,ry,rz), addr (shared address of omega at the
+// bead's cell), in (bead inside the window) follow the bead.  q_l / q_r: current squared lengths of
+// the bonds to the left / right neighbour; on return they hold the lengths after the move.
+template <bool FAST, bool EVEN>
+__device__ __forceinline__ bool tile_move(const TileArgs& A, const LaneCtx& C, const PhiloxLane& L, uint32_t c0_1,
+                                          float offx, float offy, float offz, float p_f, float seam_f, float base_t_d,
+                                          const float* __restrict__ omega_t,
                                           float& rx, float& ry, float& rz, uint32_t& addr, bool& in,
                                           float lx, float ly, float lz, float& q_l,
                                           float qx, float qy, float qz, float& q_r, float h) {
@@ -227,7 +253,7 @@ __device__ __forceinline__ bool tile_move(const TileArgs& A, const Ctx& C, const
   const float dql = __fsub_rn(ql_new, q_l), dqr = __fsub_rn(qr_new, q_r);
   const float dq = EVEN ? __fmaf_rn(h, dql, dqr) : __fmaf_rn(h, dqr, dql);
   uint32_t addr_new;
-  const bool in_new = tile_addr<FAST>(C.g, tx, ty, tz, offx, offy, offz, base_t, addr_new);
+  const bool in_new = win_addr<FAST>(C.g, tx, ty, tz, offx, offy, offz, p_f, seam_f, base_t_d, addr_new);
   float w_new, w_old;
   if (__any_sync(0xffffffffu, !(in_new && in))) {                  // rare, warp-uniform
     w_new = in_new ? lds_f32(addr_new) : omega_outside(omega_t, A.S.grid, tx, ty, tz);
@@ -242,11 +268,26 @@ __device__ __forceinline__ bool tile_move(const TileArgs& A, const Ctx& C, const
   return acc;
 }
 
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_inval(uint64_t* bar) {
+  asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
 // ---------------------------------------------------------------------------------------------
-// The kernel: one CTA per SM walks over tiles; per tile: TMA-load the omega sub-box, zero the
-// density tile, run both half-sweeps for the tile's chains (chain in registers: two beads per
-// lane, P = N/2 lanes per chain, next chain group prefetched), TMA reduce-add the density tile.
-// FAST: inv_h is a power of two >= 1 on every axis and a is a power of two (see tile_addr,
+// The kernel.  Work unit = (column, segment): a column is a cy x cz patch of the (y, z) plane with
+// its halo, a segment is Lseg cells of x.  One CTA per SM takes units round-robin and SWEEPS each
+// along x: the unit's chains are sorted by the x slice (`slice` cells) that holds their centre of
+// mass; a chain of slice k works in the window of slabs [k slice, k slice + wx) of the unit
+// (slab a = x layer a - hx of the segment).  Warp 0 is the producer: it TMA-loads omega slabs into
+// the ring ahead of the sweep and, once every consumer warp has left slice j, TMA-reduce-adds the
+// slabs that slice finished into the ghost-padded global density grid, zeroes them and loads the
+// omega of the slabs R further on into their slots.  The other warps are consumers: chain in
+// registers (two beads per lane, P = N/2 lanes per chain, next chain group prefetched), both
+// half-sweeps, LDS for omega, RED.shared for the densities.  mbarriers: full[slot] (TMA bytes
+// landed, counters zeroed), done[slice] (all consumer warps are past it).
+// FAST: inv_h is a power of two >= 1 on every axis and a is a power of two (see win_addr,
 // trial_axis); the results are identical either way.
 // ---------------------------------------------------------------------------------------------
 template <int P, bool MULTI_PAT, int NT, bool FAST>
@@ -254,130 +295,200 @@ __global__ void __launch_bounds__(NT, 1)
 tile_step_kernel(const __grid_constant__ TileArgs A, const __grid_constant__ CUtensorMap tm_omega,
                  const __grid_constant__ CUtensorMap tm_counts) {
   constexpr int G = 32 / P;
-  constexpr uint32_t NW = NT / 32;
+  constexpr uint32_t NWC = NT / 32 - 1;                                       // consumer warps
   constexpr uint32_t N = 2u * P;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  __shared__ __align__(8) uint64_t mbar;
-  float* omega_s = reinterpret_cast<float*>(smem_raw);                            // [T][E]
-  uint32_t* counts_s = reinterpret_cast<uint32_t*>(smem_raw + A.counts_offset);   // [T][E]
+  unsigned char* omega_ring = smem_raw;
+  unsigned char* counts_ring = smem_raw + A.counts_offset;
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + A.aux_offset);     // [kMaxRing]
+  uint64_t* done = full + kMaxRing;                                           // [kMaxSlices]
+  uint32_t* cum = reinterpret_cast<uint32_t*>(done + kMaxSlices);             // [K + 1] chain groups before slice k
+  uint32_t* sstart = cum + kMaxSlices + 1;                                    // [K + 1] first slot of slice k
   const StepArgs& S = A.S;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const uint32_t l = lane % P, sub = lane / P;
-  const uint32_t tile_words = A.T * A.E;
+  const uint32_t R = A.R, K = A.K, stride = A.slab_stride;
+  const uint32_t A_tot = A.Lseg + 2u * A.hx;                                  // slabs of a unit
   unsigned n_acc = 0;
-  uint32_t phase = 0;
-
-  if (tid == 0) mbar_init(&mbar, 1);
-  __syncthreads();
 
   LaneCtx C;
   C.g.inv_hx = S.grid.inv_hx; C.g.inv_hy = S.grid.inv_hy; C.g.inv_hz = S.grid.inv_hz;
-  C.g.ex = A.ex; C.g.ey = A.ey; C.g.ez = A.ez;
-  C.g.sy = A.ez * 4u; C.g.sx = A.ey * A.ez * 4u;
+  C.g.wx_f = (float)A.wx; C.g.ey_f = (float)A.ey; C.g.ez_f = (float)A.ez;
+  C.g.neg_R = -(float)R;
+  C.g.slab_stride_d = __uint_as_float(stride); C.g.sy_d = __uint_as_float(A.ez * 4u); C.g.four_d = __uint_as_float(4u);
   C.a = S.a; C.a2 = A.a2; C.ac = A.ac; C.kb = S.kb;
   const float hl = l > 0 ? 1.0f : 0.0f, hr = l + 1 < P ? 1.0f : 0.0f;
   const PhiloxLane L0 = philox_lane(S.keys, A.philox_u1, 2u * l, S.ctr3_base);
   const PhiloxLane L1 = philox_lane(S.keys, A.philox_u1, 2u * l + 1u, S.ctr3_base | 1u);
-
-  const uint32_t omega_base = smem_u32(omega_s);
-  const uint32_t type_stride = A.E * 4u;
+  const uint32_t omega_base = smem_u32(omega_ring);
+  const uint32_t type_stride = A.ey * A.ez * 4u;
   uint32_t type0 = 0, type1 = 0;
   if (!MULTI_PAT) {
     const uint16_t tt = *reinterpret_cast<const uint16_t*>(S.patterns + 2u * l);
     type0 = tt & 0xffu; type1 = tt >> 8;
   }
 
-  for (uint32_t tile = blockIdx.x; tile < A.n_tiles; tile += gridDim.x) {
-    const uint32_t start = A.tile_start[2u * tile], end = A.tile_start[2u * tile + 2u];
-    if (start == end) continue;                                               // uniform over the CTA
-    const uint32_t tz = tile % A.mtz, ty = (tile / A.mtz) % A.mty, tx = tile / (A.mtz * A.mty);
-    const int qx = (int)(tx * A.cx), qy = (int)(ty * A.cy), qz = (int)(tz * A.cz);   // padded coordinates of the tile box
-
-    // omega tile in; the previous tile's density flush must have finished READING shared memory
-    // before the density tile is zeroed
+  for (uint32_t unit = blockIdx.x; unit < A.n_units; unit += gridDim.x) {
+    const uint32_t sg = unit % A.nseg, col = unit / A.nseg;
+    const int x0 = (int)(sg * A.Lseg), y0 = (int)((col / A.mtz) * A.cy), z0 = (int)((col % A.mtz) * A.cz);   // padded coordinates of slab 0
+    __syncthreads();                                    // the previous unit is finished, its flushes have read the ring
+    for (uint32_t k = tid; k <= K; k += NT) sstart[k] = A.bin_start[2u * (unit * K + k)];
+    for (uint32_t k = tid; k < R * stride / 16u; k += NT) reinterpret_cast<uint4*>(counts_ring)[k] = make_uint4(0u, 0u, 0u, 0u);
     if (tid == 0) {
-      mbar_expect_tx(&mbar, tile_words * 4u);
-      tma_load_4d(omega_s, &tm_omega, &mbar, qz, qy, qx, 0);
-      bulk_wait_read0();
+      for (uint32_t r = 0; r < R; ++r) { mbar_inval(&full[r]); mbar_init(&full[r], 1); }
+      for (uint32_t k = 0; k < K; ++k) { mbar_inval(&done[k]); mbar_init(&done[k], NWC); }
     }
     __syncthreads();
-    for (uint32_t k = tid; k < tile_words / 4u; k += NT) reinterpret_cast<uint4*>(counts_s)[k] = make_uint4(0u, 0u, 0u, 0u);
-    __syncthreads();
-    mbar_wait(&mbar, phase);
-    phase ^= 1u;
-
-    const uint32_t n_slots = end - start;
-    const uint32_t n_groups = (n_slots + G - 1) / G;
-    // software pipeline: the loads of group wg + NW are in flight while group wg is computed
-    float2 Xn, Yn, Zn;
-    float4 Mn;
-    uint32_t slot_n = 0;
-    bool live_n = false;
-    auto fetch = [&](uint32_t wg) {
-      const uint32_t rel = wg * G + sub;
-      live_n = rel < n_slots;
-      slot_n = start + (live_n ? rel : 0u);                                   // dead lanes shadow the first slot
-      const uint64_t j = (uint64_t)slot_n * N + 2u * l;
-      Xn = *reinterpret_cast<const float2*>(S.x + j);
-      Yn = *reinterpret_cast<const float2*>(S.y + j);
-      Zn = *reinterpret_cast<const float2*>(S.z + j);
-      Mn = __ldg(A.slot_meta + slot_n);
-    };
-    if (warp < n_groups) fetch(warp);
-    for (uint32_t wg = warp; wg < n_groups; wg += NW) {
-      const float2 X = Xn, Y = Yn, Z = Zn;
-      const float4 M = Mn;
-      const uint32_t slot = slot_n;
-      const bool live = live_n;
-      if (wg + NW < n_groups) fetch(wg + NW);
-      const uint32_t c0_1 = A.philox_u0 ^ __float_as_uint(M.w);
-      if (MULTI_PAT) {
-        const uint16_t tt = *reinterpret_cast<const uint16_t*>(S.patterns + (uint32_t)S.slot_pattern[slot] * N + 2u * l);
-        type0 = tt & 0xffu; type1 = tt >> 8;
+    if (warp == 0) {                                    // chain groups per slice, exclusive scan (K <= 128: four slices per lane)
+      uint32_t g[4], sum = 0;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const uint32_t k = 4u * lane + q;
+        g[q] = k < K ? (sstart[k + 1] - sstart[k] + G - 1) / G : 0u;
+        sum += g[q];
       }
-      const uint32_t base0 = omega_base + type0 * type_stride, base1 = omega_base + type1 * type_stride;
-      float ex = X.x, ey = Y.x, ez = Z.x;                                     // even bead 2l
-      float ox = X.y, oy = Y.y, oz = Z.y;                                     // odd bead 2l+1
-      uint32_t addr_e, addr_o;
-      bool in_e = tile_addr<FAST>(C.g, ex, ey, ez, M.x, M.y, M.z, base0, addr_e);
-      bool in_o = tile_addr<FAST>(C.g, ox, oy, oz, M.x, M.y, M.z, base1, addr_o);
-      // squared lengths of this lane's two bonds: A = (even, odd), B = (odd of lane l-1, even)
-      const float lx = __shfl_up_sync(0xffffffffu, ox, 1, P);
-      const float ly = __shfl_up_sync(0xffffffffu, oy, 1, P);
-      const float lz = __shfl_up_sync(0xffffffffu, oz, 1, P);
-      float qA = bond_sq(ex, ey, ez, ox, oy, oz);
-      float qB = bond_sq(ex, ey, ez, lx, ly, lz);
-      // half-sweep 0: even bead; left neighbour = odd bead of lane l-1, right neighbour = own odd bead
-      {
-        const bool acc = tile_move<FAST, true>(A, C, L0, c0_1, M.x, M.y, M.z, base0, S.omega + (size_t)type0 * S.cells,
-                                               ex, ey, ez, addr_e, in_e, lx, ly, lz, qB, ox, oy, oz, qA, hl);
-        n_acc += (acc && live) ? 1u : 0u;
+      uint32_t inc = sum;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= (uint32_t)o) inc += t;
       }
-      // half-sweep 1: odd bead; left = own even bead (new), right = even bead of lane l+1 (new)
-      {
-        const float rx = __shfl_down_sync(0xffffffffu, ex, 1, P);
-        const float ry = __shfl_down_sync(0xffffffffu, ey, 1, P);
-        const float rz = __shfl_down_sync(0xffffffffu, ez, 1, P);
-        float qR = __shfl_down_sync(0xffffffffu, qB, 1, P);
-        const bool acc = tile_move<FAST, false>(A, C, L1, c0_1, M.x, M.y, M.z, base1, S.omega + (size_t)type1 * S.cells,
-                                                ox, oy, oz, addr_o, in_o, ex, ey, ez, qA, rx, ry, rz, qR, hr);
-        n_acc += (acc && live) ? 1u : 0u;
-      }
-      if (live) {
-        const uint64_t j = (uint64_t)slot * N + 2u * l;
-        *reinterpret_cast<float2*>(S.x + j) = make_float2(ex, ox);
-        *reinterpret_cast<float2*>(S.y + j) = make_float2(ey, oy);
-        *reinterpret_cast<float2*>(S.z + j) = make_float2(ez, oz);
-        if (in_e) reds_inc(addr_e + A.counts_offset); else count_outside(A, type0, ex, ey, ez);
-        if (in_o) reds_inc(addr_o + A.counts_offset); else count_outside(A, type1, ox, oy, oz);
+      uint32_t run = inc - sum;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const uint32_t k = 4u * lane + q;
+        if (k <= K) cum[k] = run;
+        run += g[q];
       }
     }
-    // density tile out
-    fence_proxy_async();
     __syncthreads();
-    if (tid == 0) {
-      tma_reduce_add_4d(&tm_counts, counts_s, qz, qy, qx, 0);
-      bulk_commit();
+    const uint32_t F = cum[K];                          // chain groups of the unit
+    if (F == 0) continue;                               // uniform over the CTA; nothing was binned
+
+    if (warp == 0) {
+      // ---------------- producer ----------------
+      if (lane == 0) {
+        const uint32_t first = R < A_tot ? R : A_tot;
+        for (uint32_t a = 0; a < first; ++a) {
+          mbar_expect_tx(&full[a], A.slab_bytes);
+          tma_load_4d(omega_ring + a * stride, &tm_omega, &full[a], z0, y0, x0 + (int)a, 0);
+        }
+      }
+      for (uint32_t j = 0; j < K; ++j) {
+        if (lane == 0) mbar_wait(&done[j], 0);
+        __syncwarp();
+        const uint32_t lo = j * A.slice, hi = (j + 1 == K) ? A_tot : lo + A.slice;   // slabs no later slice touches
+        if (lane == 0) {
+          fence_proxy_async();
+          for (uint32_t a = lo; a < hi; ++a)
+            tma_reduce_add_4d(&tm_counts, counts_ring + (a % R) * stride, z0, y0, x0 + (int)a, 0);
+          bulk_commit();
+        }
+        if (j + 1 == K) break;
+        if (lo + R < A_tot) {                           // their slots take the slabs R further on
+          if (lane == 0) bulk_wait_read0();
+          __syncwarp();
+          for (uint32_t a = lo; a < hi && a + R < A_tot; ++a) {
+            uint4* c = reinterpret_cast<uint4*>(counts_ring + (a % R) * stride);
+            for (uint32_t k = lane; k < A.slab_bytes / 16u; k += 32u) c[k] = make_uint4(0u, 0u, 0u, 0u);
+          }
+          __syncwarp();
+          if (lane == 0)
+            for (uint32_t a = lo; a < hi && a + R < A_tot; ++a) {
+              mbar_expect_tx(&full[a % R], A.slab_bytes);      // release: the zeroes are visible to whoever sees the phase complete
+              tma_load_4d(omega_ring + (a % R) * stride, &tm_omega, &full[a % R], z0, y0, x0 + (int)(a + R), 0);
+            }
+        }
+      }
+      if (lane == 0) bulk_wait_read0();
+    } else {
+      // ---------------- consumers ----------------
+      const uint32_t wc = warp - 1u;
+      uint32_t kf = 0;                                  // slice cursor of the prefetch
+      float2 Xn, Yn, Zn;
+      float4 Mn;
+      uint32_t slot_n = 0, k_n = 0;
+      bool live_n = false;
+      auto fetch = [&](uint32_t f) {
+        while (f >= cum[kf + 1]) ++kf;
+        const uint32_t s0 = sstart[kf], n = sstart[kf + 1] - s0;
+        const uint32_t rel = (f - cum[kf]) * G + sub;
+        live_n = rel < n;
+        slot_n = s0 + (live_n ? rel : 0u);                                    // dead lanes shadow the slice's first slot
+        k_n = kf;
+        const uint64_t j = (uint64_t)slot_n * N + 2u * l;
+        Xn = *reinterpret_cast<const float2*>(S.x + j);
+        Yn = *reinterpret_cast<const float2*>(S.y + j);
+        Zn = *reinterpret_cast<const float2*>(S.z + j);
+        Mn = __ldg(A.slot_meta + slot_n);
+      };
+      int kc = -1;                                      // slice being computed
+      float p_f = 0.0f, seam_f = 0.0f;
+      if (wc < F) fetch(wc);
+      for (uint32_t f = wc; f < F; f += NWC) {
+        const float2 X = Xn, Y = Yn, Z = Zn;
+        const float4 M = Mn;
+        const uint32_t slot = slot_n, k_this = k_n;
+        const bool live = live_n;
+        if (f + NWC < F) fetch(f + NWC);
+        if ((int)k_this != kc) {                        // entering a new slice (uniform over the warp)
+          __syncwarp();
+          if (lane == 0)
+            for (uint32_t j = kc < 0 ? 0u : (uint32_t)kc; j < k_this; ++j) mbar_arrive(&done[j]);
+          uint32_t a_lo = kc < 0 ? 0u : (uint32_t)kc * A.slice + A.wx;
+          uint32_t a_hi = k_this * A.slice + A.wx;
+          if (a_hi > A_tot) a_hi = A_tot;
+          for (uint32_t a = a_lo; a < a_hi; ++a) mbar_wait(&full[a % R], (a / R) & 1u);
+          kc = (int)k_this;
+          const uint32_t p = (k_this * A.slice) % R;
+          p_f = (float)p;
+          seam_f = (float)((int)p - (int)R + 1);
+        }
+        const uint32_t c0_1 = A.philox_u0 ^ __float_as_uint(M.w);
+        if (MULTI_PAT) {
+          const uint16_t tt = *reinterpret_cast<const uint16_t*>(S.patterns + (uint32_t)S.slot_pattern[slot] * N + 2u * l);
+          type0 = tt & 0xffu; type1 = tt >> 8;
+        }
+        const float base0 = __uint_as_float(omega_base + type0 * type_stride), base1 = __uint_as_float(omega_base + type1 * type_stride);
+        float ex = X.x, ey = Y.x, ez = Z.x;                                   // even bead 2l
+        float ox = X.y, oy = Y.y, oz = Z.y;                                   // odd bead 2l+1
+        uint32_t addr_e, addr_o;
+        bool in_e = win_addr<FAST>(C.g, ex, ey, ez, M.x, M.y, M.z, p_f, seam_f, base0, addr_e);
+        bool in_o = win_addr<FAST>(C.g, ox, oy, oz, M.x, M.y, M.z, p_f, seam_f, base1, addr_o);
+        // squared lengths of this lane's two bonds: A = (even, odd), B = (odd of lane l-1, even)
+        const float lx = __shfl_up_sync(0xffffffffu, ox, 1, P);
+        const float ly = __shfl_up_sync(0xffffffffu, oy, 1, P);
+        const float lz = __shfl_up_sync(0xffffffffu, oz, 1, P);
+        float qA = bond_sq(ex, ey, ez, ox, oy, oz);
+        float qB = bond_sq(ex, ey, ez, lx, ly, lz);
+        // half-sweep 0: even bead; left neighbour = odd bead of lane l-1, right neighbour = own odd bead
+        {
+          const bool acc = tile_move<FAST, true>(A, C, L0, c0_1, M.x, M.y, M.z, p_f, seam_f, base0, S.omega + (size_t)type0 * S.cells,
+                                                 ex, ey, ez, addr_e, in_e, lx, ly, lz, qB, ox, oy, oz, qA, hl);
+          n_acc += (acc && live) ? 1u : 0u;
+        }
+        // half-sweep 1: odd bead; left = own even bead (new), right = even bead of lane l+1 (new)
+        {
+          const float rx = __shfl_down_sync(0xffffffffu, ex, 1, P);
+          const float ry = __shfl_down_sync(0xffffffffu, ey, 1, P);
+          const float rz = __shfl_down_sync(0xffffffffu, ez, 1, P);
+          float qR = __shfl_down_sync(0xffffffffu, qB, 1, P);
+          const bool acc = tile_move<FAST, false>(A, C, L1, c0_1, M.x, M.y, M.z, p_f, seam_f, base1, S.omega + (size_t)type1 * S.cells,
+                                                  ox, oy, oz, addr_o, in_o, ex, ey, ez, qA, rx, ry, rz, qR, hr);
+          n_acc += (acc && live) ? 1u : 0u;
+        }
+        if (live) {
+          const uint64_t j = (uint64_t)slot * N + 2u * l;
+          *reinterpret_cast<float2*>(S.x + j) = make_float2(ex, ox);
+          *reinterpret_cast<float2*>(S.y + j) = make_float2(ey, oy);
+          *reinterpret_cast<float2*>(S.z + j) = make_float2(ez, oz);
+          if (in_e) reds_inc(addr_e + A.counts_offset); else count_outside(A, type0, ex, ey, ez);
+          if (in_o) reds_inc(addr_o + A.counts_offset); else count_outside(A, type1, ox, oy, oz);
+        }
+      }
+      __syncwarp();
+      if (lane == 0)
+        for (uint32_t j = kc < 0 ? 0u : (uint32_t)kc; j < K; ++j) mbar_arrive(&done[j]);
     }
   }
   if (tid == 0) bulk_wait0();
@@ -387,17 +498,18 @@ tile_step_kernel(const __grid_constant__ TileArgs A, const __grid_constant__ CUt
 }
 
 // ---------------------------------------------------------------------------------------------
-// Sorting the chains for the tiled kernel.  Key of a chain = 2 * (tile whose core holds the cell of
-// its centre of mass) + (1 if a bead lies within `margin` cells of the tile's faces or beyond, else
-// 0): a tile's compact chains come first, so that the warps working on them never take the slow
-// path, and the extended ones share warps among themselves.  The same pass writes the chain's
-// floor offsets (see tile_addr): off = kFloorMagic + (g - G) - origin per axis, G the unwrapped and
-// g the wrapped cell coordinate of the centre of mass.
+// Sorting the chains for the kernel above.  Key of a chain = 2 (unit K + slice) + e: the unit and
+// slice whose core holds the cell of its centre of mass, and e = 1 if a bead lies within `margin`
+// cells of the window's faces or beyond (extended chains come last in their slice, so they share
+// warps among themselves and the other warps never take the slow path).  The same pass writes the
+// chain's floor offsets (see win_addr): off = kFloorMagic + (g - G) - window origin per axis, G the
+// unwrapped and g the wrapped cell coordinate of the centre of mass.
 // ---------------------------------------------------------------------------------------------
 struct TileSortArgs {
   Grid grid;
   uint32_t n_chains, N;
-  uint32_t cx, cy, cz, hx, hy, hz, ex, ey, ez, mty, mtz;
+  uint32_t cy, cz, hx, hy, hz, wx, ey, ez;
+  uint32_t slice, K, Lseg, mtz, nseg;
   uint32_t margin;
 };
 
@@ -415,9 +527,10 @@ tile_key_kernel(TileSortArgs S, const float* __restrict__ x, const float* __rest
   const int Gy = __float2int_rd(__fmul_rn(sy * inv, S.grid.inv_hy));
   const int Gz = __float2int_rd(__fmul_rn(sz * inv, S.grid.inv_hz));
   const int gx = Gx & (int)(S.grid.nx - 1u), gy = Gy & (int)(S.grid.ny - 1u), gz = Gz & (int)(S.grid.nz - 1u);
-  const uint32_t tx = (uint32_t)gx / S.cx, ty = (uint32_t)gy / S.cy, tz = (uint32_t)gz / S.cz;
-  // relative cell of a bead = floor(r inv_h) + d, d = (g - G) - origin
-  const int dx = gx - Gx - ((int)(tx * S.cx) - (int)S.hx);
+  const uint32_t sg = (uint32_t)gx / S.Lseg, k = ((uint32_t)gx % S.Lseg) / S.slice;
+  const uint32_t ty = (uint32_t)gy / S.cy, tz = (uint32_t)gz / S.cz;
+  // window-relative cell of a bead = floor(r inv_h) + d, d = (g - G) - window origin
+  const int dx = gx - Gx - ((int)(sg * S.Lseg + k * S.slice) - (int)S.hx);
   const int dy = gy - Gy - ((int)(ty * S.cy) - (int)S.hy);
   const int dz = gz - Gz - ((int)(tz * S.cz) - (int)S.hz);
   bool ext = false;
@@ -426,12 +539,12 @@ tile_key_kernel(TileSortArgs S, const float* __restrict__ x, const float* __rest
     const int rx = __float2int_rd(__fmul_rn(x[j0 + i], S.grid.inv_hx)) + dx;
     const int ry = __float2int_rd(__fmul_rn(y[j0 + i], S.grid.inv_hy)) + dy;
     const int rz = __float2int_rd(__fmul_rn(z[j0 + i], S.grid.inv_hz)) + dz;
-    ext |= rx < m || rx >= (int)S.ex - m || ry < m || ry >= (int)S.ey - m || rz < m || rz >= (int)S.ez - m;
+    ext |= rx < m || rx >= (int)S.wx - m || ry < m || ry >= (int)S.ey - m || rz < m || rz >= (int)S.ez - m;
   }
-  const uint32_t tile = (tx * S.mty + ty) * S.mtz + tz;
-  const uint32_t k = 2u * tile + (ext ? 1u : 0u);
-  key[s] = k;
-  rank[s] = atomicAdd(bin_count + k, 1u);
+  const uint32_t unit = (ty * S.mtz + tz) * S.nseg + sg;
+  const uint32_t kk = 2u * (unit * S.K + k) + (ext ? 1u : 0u);
+  key[s] = kk;
+  rank[s] = atomicAdd(bin_count + kk, 1u);
   meta[s] = make_float4(kFloorMagic + (float)dx, kFloorMagic + (float)dy, kFloorMagic + (float)dz,
                         __uint_as_float(slot_chain[s]));
 }

@@ -156,14 +156,17 @@ def test_large_seed_step_and_chain_ids_reach_the_counter():
         assert not np.array_equal(g2.positions()[0], o.positions()[0])
 
 
-# ---- the tiled kernel (omega and density tiles in shared memory, TMA in and out) --------------------
-# Small tiles on small grids so that the oracle stays fast while the run still covers many tiles,
-# tiles that wrap around every periodic face, partial last tiles (core not dividing the grid), beads
-# outside their tile's halo (global-memory fallback) and drift between re-sorts.
+# ---- the tiled kernel (x-sweep over columns: omega and density slabs in a shared-memory ring, TMA in and out)
+# Small windows on small grids so that the oracle stays fast while the run still covers many units,
+# windows that wrap around every periodic face, partial last columns (core not dividing the grid),
+# ring slots reused several times per sweep, beads outside their window (global-memory slow path)
+# and drift between re-sorts.  tile_cx = segment length along x, tile_cy/cz = column core,
+# tile_h* = halo, tile_slice = cells per slice, tile_ring = ring slots (0: as many as fit).
 
-SMALL_TILES = dict(tile_cx=4, tile_cy=4, tile_cz=4, tile_hx=2, tile_hy=2, tile_hz=2)          # 8^3 tiles, most chains stick out
-ODD_TILES = dict(tile_cx=12, tile_cy=5, tile_cz=8, tile_hx=3, tile_hy=4, tile_hz=6)           # cores not dividing the grid
-WIDE_HALO = dict(tile_cx=4, tile_cy=4, tile_cz=4, tile_hx=6, tile_hy=6, tile_hz=6)            # 16^3 tiles: nearly all beads inside
+SMALL_TILES = dict(tile_cx=4, tile_cy=4, tile_cz=4, tile_hx=2, tile_hy=2, tile_hz=2)          # 6x8x8 windows, most chains stick out
+ODD_TILES = dict(tile_cx=16, tile_cy=5, tile_cz=8, tile_hx=3, tile_hy=4, tile_hz=6, tile_slice=4, tile_ring=11)   # cores not dividing the grid, ring = one window + 1
+WIDE_HALO = dict(tile_cx=8, tile_cy=4, tile_cz=4, tile_hx=5, tile_hy=6, tile_hz=6, tile_slice=1)   # 11x16x16 windows: nearly all beads inside
+TIGHT_RING = dict(tile_cx=32, tile_cy=4, tile_cz=4, tile_hx=3, tile_hy=4, tile_hz=2, tile_slice=2, tile_ring=8)   # ring = exactly one window: no load-ahead
 
 TILE_CASES = {
     "cfg0_full_small_tiles": (lambda: si.make_system(si.config(0)), SMALL_TILES),
@@ -171,7 +174,9 @@ TILE_CASES = {
     "cfg1_scaled_T1_N64": (lambda: _scaled(1, 4099, (16, 16, 16)), SMALL_TILES),
     "cfg2_scaled_odd_tiles": (lambda: _scaled(2, 8193, (32, 16, 32)), ODD_TILES),
     "cfg3_scaled_blend_N64": (lambda: _scaled(3, 4098, (32, 16, 16)), WIDE_HALO),
-    "cfg4_scaled_default_tiles": (lambda: _scaled(4, 16385, (32, 32, 32)), {}),                 # 12x12x8 + 6: the bench shape
+    "cfg4_scaled_default_tiles": (lambda: _scaled(4, 16385, (32, 32, 32)), {}),                 # 8x8 columns + 8, slices of 2: the bench shape
+    "cfg4_scaled_tight_ring": (lambda: _scaled(4, 16385, (32, 32, 16)), TIGHT_RING),
+    "cfg2_scaled_general_arithmetic": (lambda: _scaled(2, 8193, (32, 16, 32)), dict(SMALL_TILES, tile_fast=0, tile_margin=0)),
     "cfg4_scaled_threads_512": (lambda: _scaled(4, 16385, (32, 32, 16)), dict(WIDE_HALO, tile_threads=512)),
     "cfg4_scaled_threads_768": (lambda: _scaled(4, 16385, (32, 32, 16)), dict(SMALL_TILES, tile_threads=768)),
     "T3_three_patterns": (lambda: _custom(900, 32, 3, [[0] * 10 + [1] * 12 + [2] * 10, [2] * 32, [1] * 16 + [0] * 16],
@@ -237,11 +242,11 @@ def test_tiled_path_is_refused_where_it_cannot_run():
             with pytest.raises(soma.SomaError) as e:
                 g.set_option("path", TILED)
             assert e.value.code == soma.SOMA_EINVAL and "tiled path unavailable" in str(e.value)
-    with gpu_system(si.make_system(si.config(0))) as g:                      # default 24x24x20 tile > 16^3 grid
+    with gpu_system(si.make_system(si.config(0))) as g:                      # default 18x24x24 window > 16^3 grid
         with pytest.raises(soma.SomaError):
             g.set_option("path", TILED)
         g.set_option("tile_cx", 4); g.set_option("tile_cy", 4); g.set_option("tile_cz", 4)
         g.set_option("tile_hx", 2); g.set_option("tile_hy", 2); g.set_option("tile_hz", 2)
         g.set_option("path", TILED)
-        g.set_option("tile_hz", 3)                                           # extent 10 along z: not a multiple of 4 -> tiles off
+        g.set_option("tile_hz", 3)                                           # window 10 cells along z: not a multiple of 4 -> tiles off
         assert g.counters()["path"] != TILED
