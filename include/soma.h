@@ -118,25 +118,34 @@ int soma_destroy(soma_t *h);
 const char *soma_last_error(const soma_t *h);
 
 /* Tuning / test switches.  Names:
- *   "path"            0 = automatic, 1 = generic kernels (4 launches/step, any N),
+ *   "path"            0 = automatic (the fused kernel where N allows it, else the generic ones),
+ *                     1 = generic kernels (4 launches/step, any N),
  *                     2 = fused chain-in-registers kernel (N = 2P, P a power of two <= 32; else EINVAL),
- *                     3 = tiled kernel: omega and density tiles in shared memory, moved by TMA (as 2,
- *                         plus: power-of-two grid axes >= 16 and >= the tile; else EINVAL)
- *   "tile_cx|cy|cz", "tile_hx|hy|hz"   tile core and halo in cells (defaults 12,12,8 and 6,6,6);
- *   "tile_threads"    512, 768 or 1024 threads per CTA of the tiled kernel.  A combination the
- *                     tiled kernel cannot use switches it off (see soma_get_counters [3])
+ *                     3 = first windowed kernel (soma_tile.cuh): omega and density slabs of a column in a
+ *                         shared-memory ring, moved by TMA (as 2, plus: power-of-two grid axes >= 16
+ *                         and >= the window; else EINVAL),
+ *                     4 = swept-window kernel (soma_sweep.cuh): the same data flow with a branch-free
+ *                         body for chains inside their window (same conditions as 3)
+ *   "tile_cx"         segment length along x in cells (default 64); "tile_cy|cz" column core (8, 8);
+ *   "tile_hx|hy|hz"   halo in cells (8, 8, 8); "tile_slice" cells per x slice (2); "tile_ring" ring
+ *                     slots (0 = as many as fit); "tile_margin" (1) chains with a bead this close to a
+ *                     window face sort behind the others; "tile_fast" 0 = general arithmetic only;
+ *   "tile_threads"    512, 768 or 1024 threads per CTA of the windowed kernels.  A combination they
+ *                     cannot use switches them off (see soma_get_counters [3])
  *   "kernel_timing"   1 = record CUDA events on the handle's stream around the kernels of every step
  *                     (read them with soma_get_kernel_times), 0 = off (default)
  *   "resort_interval" re-order the chains in memory by position at soma_load_state and then every k
  *                     steps (0 = never; default 64 for >= 4096 chains, else 0); results are
  *                     independent of it (the random stream is keyed by the logical chain id)
  *   "resort_now"      re-order once, now (value ignored)
- *   "fused_blocks_per_sm", "fused_waves"   launch shape of the fused kernel (tuning)
+ *   "fused_chunk"     warp groups (32 beads-pairs each) per block of the fused kernel (default 224);
+ *   "fused_persistent" 1 = one resident wave of "fused_blocks_per_sm" blocks per SM takes the chunks
+ *                     cyclically, 0 (default) = one block per chunk in launch order (tuning)
  * Errors: SOMA_EINVAL (unknown name / unsupported value). */
 int soma_set_option(soma_t *h, const char *name, int64_t value);
 
 /* Counters since soma_create: [0] kernels launched by this library, [1] MC steps done,
- * [2] chain re-orderings done; [3] the kernel path the next step will take (1, 2 or 3).
+ * [2] chain re-orderings done; [3] the kernel path the next step will take (1, 2, 3 or 4).
  * `out` is a host pointer to 4 uint64. */
 int soma_get_counters(const soma_t *h, uint64_t *out);
 

@@ -10,7 +10,7 @@
 #include <string>
 #include <vector>
 
-#include "soma_tile.cuh"
+#include "soma_sweep.cuh"
 
 using namespace soma;
 
@@ -36,6 +36,7 @@ struct Layout {            // byte offsets into the workspace
   uint64_t sort_bins;      // [2 n_bins_max + 2] uint32: bin counts, then bin starts (= tile_start)
   uint64_t slot_meta;      // [n] float4: per slot floor offsets + chain id, written by the tile sort
   uint64_t meta_src;       // [n] float4: the same in the order before the sort (scratch)
+  uint64_t slot_k;         // [n] uint16: slice index of every slot's chain (swept-window kernel)
   uint64_t omega_pad;      // [T][pad cells] fp32: ghost-padded omega for the tile loads (0 bytes if unused)
   uint64_t counts_pad[2];  // [T][pad cells] uint32: ghost-padded density grids the tiles flush into
   uint64_t total;
@@ -87,6 +88,7 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   L.sort_bins = off; off += align_up(n_bins * 4);
   L.slot_meta = off; off += align_up(n * 16);
   L.meta_src = off; off += align_up(n * 16);
+  L.slot_k = off; off += align_up(n * 2);
   L.omega_pad = off; off += align_up(pad_words * 4);
   for (int s = 0; s < 2; ++s) { L.counts_pad[s] = off; off += align_up(pad_words * 4); }
   L.total = off;
@@ -171,7 +173,7 @@ struct soma_handle {
   // options
   int path;              // 0 auto, 1 generic, 2 fused
   int64_t resort_interval;      // re-order the chains every k steps (0 = never)
-  int fused_blocks_per_sm, fused_waves;
+  int fused_blocks_per_sm, fused_chunk, fused_persistent;
   // tiled kernel (soma_tile.cuh)
   bool tile_grid_ok;            // the grid allows tiles at all
   bool tile_ready;              // geometry + tensor maps are set up for the current options
@@ -216,6 +218,7 @@ struct soma_handle {
   float* omega_pad() const { return reinterpret_cast<float*>(ws + L.omega_pad); }
   float4* slot_meta() const { return reinterpret_cast<float4*>(ws + L.slot_meta); }
   float4* meta_src() const { return reinterpret_cast<float4*>(ws + L.meta_src); }
+  uint16_t* slot_k() const { return reinterpret_cast<uint16_t*>(ws + L.slot_k); }
   uint32_t* counts_pad(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts_pad[s]); }
   uint8_t* patterns() const { return reinterpret_cast<uint8_t*>(ws + L.patterns); }
   uint8_t* pattern0() const { return reinterpret_cast<uint8_t*>(ws + L.pattern0); }
@@ -347,14 +350,15 @@ int launch_fused_p(soma_handle* h) {
   constexpr int G = 32 / P;
   const uint64_t n_groups = (h->n_chains + G - 1) / G;           // warps of work
   const unsigned bs = 256, wpb = bs / 32;
-  // every block owns a contiguous run of warp groups: a multiple of the warps per block, sized so
-  // that the grid is about `waves` full waves of resident blocks
+  // chunks of fused_chunk warp groups (a multiple of the warps per block), dealt out cyclically to
+  // at most one resident wave of blocks
   const uint64_t resident = (uint64_t)h->sm_count * h->fused_blocks_per_sm;
-  uint64_t blocks = resident * (uint64_t)h->fused_waves;
-  uint64_t gpb = (n_groups + blocks - 1) / blocks;
-  gpb = (gpb + wpb - 1) / wpb * wpb;
-  if (gpb == 0) gpb = wpb;
-  blocks = (n_groups + gpb - 1) / gpb;
+  uint64_t gpb = ((uint64_t)h->fused_chunk + wpb - 1) / wpb * wpb;
+  const uint64_t n_chunks = (n_groups + gpb - 1) / gpb;
+  // fused_persistent = 1: one resident wave of blocks takes the chunks cyclically; 0 (default): one
+  // block per chunk, handed out in order by the hardware block scheduler as blocks retire -- the
+  // dynamic order keeps the blocks closer together in the chain list (measured: 1.12 vs 1.23 ms on cfg4)
+  const uint64_t blocks = (h->fused_persistent && n_chunks > resident) ? resident : n_chunks;
   const bool multi = h->n_patterns > 1;
 #define SOMA_LAUNCH_FUSED(POW2, MULTI) \
   fused_step_kernel<P, POW2, MULTI><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb)
@@ -384,7 +388,7 @@ bool use_fused(const soma_handle* h) {
 }
 bool use_tile(const soma_handle* h) {
   if (!h->tile_ready || h->omega_custom) return false;
-  return h->path == 3 || (h->path == 0 && h->tile_auto);
+  return h->path == 3 || h->path == 4 || (h->path == 0 && h->tile_auto);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -408,14 +412,21 @@ cudaError_t tile_attr(size_t smem) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, true, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, false, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, true, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_step_kernel<P, false, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_step_kernel<P, true, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_step_kernel<P, false, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_step_kernel<P, true, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   return e;
 }
 template <int NT>
 cudaError_t tile_attr_p(int P, size_t smem) {
   switch (P) {
+#ifndef SOMA_MIN_BUILD      /* development builds instantiate N = 32 only */
     case 1: return tile_attr<1, NT>(smem);   case 2: return tile_attr<2, NT>(smem);
     case 4: return tile_attr<4, NT>(smem);   case 8: return tile_attr<8, NT>(smem);
-    case 16: return tile_attr<16, NT>(smem); case 32: return tile_attr<32, NT>(smem);
+    case 32: return tile_attr<32, NT>(smem);
+#endif
+    case 16: return tile_attr<16, NT>(smem);
   }
   return cudaErrorInvalidValue;
 }
@@ -493,8 +504,10 @@ void tile_setup(soma_handle* h) {
                 : h->tile_threads == 768 ? tile_attr_p<768>(P, h->tile_smem) : tile_attr_p<512>(P, h->tile_smem);
   if (e != cudaSuccess) { cudaGetLastError(); return no("cudaFuncSetAttribute(max dynamic shared memory) failed"); }
   h->tile_ready = true;
-  // automatic choice: tiles pay off when there are several rounds of them over the SMs
-  h->tile_auto = h->n_tiles >= 4u * (uint32_t)h->sm_count;
+  // automatic choice: the fused kernel.  With its chunks handed out in chain-list order (see
+  // launch_fused_p) it is the fastest path measured on every config (cfg4: 1.12 ms against 1.64 ms for
+  // either windowed kernel, profiles/); the windowed kernels stay selectable as paths 3 and 4.
+  h->tile_auto = false;
   h->tile_why[0] = 0;
 }
 
@@ -503,6 +516,7 @@ int launch_tile_pn(soma_handle* h) {
   TileArgs A{};
   A.S = step_args(h);
   A.slot_meta = h->slot_meta();
+  A.slot_k = h->slot_k();
   A.T = h->T;
   A.wx = h->te[0]; A.ey = h->te[1]; A.ez = h->te[2];
   A.cy = h->tc[1]; A.cz = h->tc[2];
@@ -523,8 +537,10 @@ int launch_tile_pn(soma_handle* h) {
   const CUtensorMap& tmc = h->tm_counts[h->pad_cur];
   h->counts_in_pad = true;
   const bool multi = h->n_patterns > 1;
+  const bool sweep = h->path != 3;                 // path 3 keeps the first column-sweep kernel (soma_tile.cuh) for comparison
 #define SOMA_LAUNCH_TILE(MULTI, FAST) \
-  tile_step_kernel<P, MULTI, NT, FAST><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc)
+  do { if (sweep) sweep_step_kernel<P, MULTI, NT, FAST><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc); \
+       else tile_step_kernel<P, MULTI, NT, FAST><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc); } while (0)
   if (h->tile_fast) { if (multi) SOMA_LAUNCH_TILE(true, true); else SOMA_LAUNCH_TILE(false, true); }
   else              { if (multi) SOMA_LAUNCH_TILE(true, false); else SOMA_LAUNCH_TILE(false, false); }
 #undef SOMA_LAUNCH_TILE
@@ -535,9 +551,12 @@ int launch_tile_pn(soma_handle* h) {
 template <int NT>
 int launch_tile_n(soma_handle* h) {
   switch (fused_lanes(h->N)) {
+#ifndef SOMA_MIN_BUILD
     case 1: return launch_tile_pn<1, NT>(h);   case 2: return launch_tile_pn<2, NT>(h);
     case 4: return launch_tile_pn<4, NT>(h);   case 8: return launch_tile_pn<8, NT>(h);
-    case 16: return launch_tile_pn<16, NT>(h); case 32: return launch_tile_pn<32, NT>(h);
+    case 32: return launch_tile_pn<32, NT>(h);
+#endif
+    case 16: return launch_tile_pn<16, NT>(h);
   }
   return fail(h, SOMA_EINVAL, "tiled path does not support this beads_per_chain");
 }
@@ -584,7 +603,8 @@ int resort(soma_handle* h, int kind) {
       h->B, h->N, h->sort_bins(), h->sort_key(), h->sort_rank(),
       h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->pos(dst, 0), h->pos(dst, 1), h->pos(dst, 2),
       h->slot_chain(src), h->slot_pattern(src), h->slot_chain(dst), h->slot_pattern(dst),
-      kind == 2 ? h->meta_src() : nullptr, kind == 2 ? h->slot_meta() : nullptr);
+      kind == 2 ? h->meta_src() : nullptr, kind == 2 ? h->slot_meta() : nullptr,
+      kind == 2 ? h->slot_k() : nullptr, kind == 2 ? h->tile_K : 1u);
   h->launches += 3;
   CU(h, cudaGetLastError());
   h->live = dst;
@@ -772,7 +792,8 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   // chains are kept sorted by position when the system is large enough for it to matter
   h->resort_interval = h->n_chains >= 4096 ? 64 : 0;
   h->fused_blocks_per_sm = 3;
-  h->fused_waves = 1;
+  h->fused_chunk = 224;
+  h->fused_persistent = 0;
   h->tc[0] = 64; h->tc[1] = 8; h->tc[2] = 8;
   h->th[0] = h->th[1] = h->th[2] = 8;
   h->tile_slice = 2;
@@ -907,8 +928,8 @@ const char* soma_last_error(const soma_t* h) { return h ? h->err : g_last_error;
 int soma_set_option(soma_t* h, const char* name, int64_t value) {
   if (!h || !name) return fail(h, SOMA_EINVAL, "NULL argument");
   if (!std::strcmp(name, "path")) {
-    if (value < 0 || value > 3) return fail(h, SOMA_EINVAL, "path must be 0, 1, 2 or 3");
-    if (value == 3 && !h->tile_ready) {
+    if (value < 0 || value > 4) return fail(h, SOMA_EINVAL, "path must be 0, 1, 2, 3 or 4");
+    if (value >= 3 && !h->tile_ready) {
       char buf[160];
       snprintf(buf, sizeof buf, "tiled path unavailable: %s", h->tile_why);
       return fail(h, SOMA_EINVAL, buf);
@@ -959,7 +980,7 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
           (k < 3 ? h->tc[k] : h->th[k - 3]) = (uint32_t)value;
         }
         tile_setup(h);
-        if (!h->tile_ready && h->path == 3) h->path = 0;
+        if (!h->tile_ready && h->path >= 3) h->path = 0;
         return SOMA_OK;                      // soma_get_counters()[3] tells whether tiles are usable now
       }
   }
@@ -974,9 +995,14 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     h->tile_fast = false;
     return SOMA_OK;
   }
-  if (!std::strcmp(name, "fused_waves")) {
-    if (value < 1 || value > 1024) return fail(h, SOMA_EINVAL, "fused_waves must be in [1, 1024]");
-    h->fused_waves = (int)value;
+  if (!std::strcmp(name, "fused_persistent")) {
+    if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "fused_persistent must be 0 or 1");
+    h->fused_persistent = (int)value;
+    return SOMA_OK;
+  }
+  if (!std::strcmp(name, "fused_chunk")) {
+    if (value < 1 || value > (1 << 20)) return fail(h, SOMA_EINVAL, "fused_chunk must be in [1, 2^20]");
+    h->fused_chunk = (int)value;
     return SOMA_OK;
   }
   return fail(h, SOMA_EINVAL, "unknown option name");
@@ -985,7 +1011,7 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
 int soma_get_counters(const soma_t* h, uint64_t* out) {
   if (!h || !out) return SOMA_EINVAL;
   out[0] = h->launches; out[1] = h->steps_done; out[2] = h->resorts;
-  out[3] = use_tile(h) ? 3 : (use_fused(h) ? 2 : 1);
+  out[3] = use_tile(h) ? (h->path == 3 ? 3 : 4) : (use_fused(h) ? 2 : 1);
   return SOMA_OK;
 }
 

@@ -130,9 +130,7 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
   const uint32_t sub = lane / P;                              // which of the warp's chains
   const uint32_t wpb = blockDim.x >> 5;
   const uint64_t n_groups = ((uint64_t)A.n_chains + G - 1) / G;
-  const uint64_t g_begin = (uint64_t)blockIdx.x * groups_per_block;
-  uint64_t g_end = g_begin + groups_per_block;
-  if (g_end > n_groups) g_end = n_groups;
+  const uint64_t n_chunks = (n_groups + groups_per_block - 1) / groups_per_block;
   unsigned n_acc = 0;
 
   // bead types of this lane (loop-invariant when every chain has the same pattern)
@@ -142,6 +140,14 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
     type0 = tt & 0xffu; type1 = tt >> 8;
   }
 
+  // Chunks of `groups_per_block` consecutive warp groups are dealt out to the resident blocks in
+  // turn, so that at any moment the whole grid works on one contiguous stretch of the position-sorted
+  // chain list: the omega values and density counters that stretch touches (a few MB) stay in L2,
+  // which one contiguous run per block (every block in a different part of the box) does not allow.
+  for (uint64_t chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
+  const uint64_t g_begin = chunk * groups_per_block;
+  uint64_t g_end = g_begin + groups_per_block;
+  if (g_end > n_groups) g_end = n_groups;
   for (uint64_t wg = g_begin + (threadIdx.x >> 5); wg < g_end; wg += wpb) {
     const uint64_t slot64 = wg * G + sub;
     const bool live = slot64 < A.n_chains;
@@ -188,6 +194,7 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
       atomicAdd(A.counts_next + (size_t)type0 * A.cells + cell_e, 1u);
       atomicAdd(A.counts_next + (size_t)type1 * A.cells + cell_o, 1u);
     }
+  }
   }
   // accepted-move count: warp reduce, one atomic per warp
 #pragma unroll
@@ -324,7 +331,8 @@ chain_permute_kernel(uint64_t B, uint32_t N, const uint32_t* __restrict__ bin_st
                      float* __restrict__ dx, float* __restrict__ dy, float* __restrict__ dz,
                      const uint32_t* __restrict__ s_chain, const uint8_t* __restrict__ s_pat,
                      uint32_t* __restrict__ d_chain, uint8_t* __restrict__ d_pat,
-                     const float4* __restrict__ s_meta, float4* __restrict__ d_meta /* both may be null */) {
+                     const float4* __restrict__ s_meta, float4* __restrict__ d_meta /* both may be null */,
+                     uint16_t* __restrict__ d_k /* may be null */, uint32_t K) {
   const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= B) return;
   const uint32_t s = (uint32_t)(j / N), i = (uint32_t)(j % N);
@@ -334,6 +342,7 @@ chain_permute_kernel(uint64_t B, uint32_t N, const uint32_t* __restrict__ bin_st
   if (i == 0) {
     d_chain[d] = s_chain[s]; d_pat[d] = s_pat[s];
     if (d_meta) d_meta[d] = s_meta[s];
+    if (d_k) d_k[d] = (uint16_t)((key[s] >> 1) % K);       // tile sort key = 2 (unit K + slice) + e
   }
 }
 

@@ -184,6 +184,7 @@ constexpr uint32_t kSweepAuxBytes = 4096;
 struct TileArgs {
   StepArgs S;                 // omega = linear field (slow path); counts_next is not used by this kernel
   const float4* __restrict__ slot_meta;     // [n] per slot: floor offsets x, y, z and the chain id (bits)
+  const uint16_t* __restrict__ slot_k;      // [n] per slot: slice index of the chain inside its unit (soma_sweep.cuh)
   uint32_t* __restrict__ counts_pad;        // [T][px][py][pz] ghost-padded density grid this step bins into
   const uint32_t* __restrict__ bin_start;   // [2 K n_units + 1]: per unit and slice, compact chains then extended ones
   uint32_t px, py, pz;        // padded dims: padded coordinate q holds cell (q - halo) mod n
@@ -241,7 +242,7 @@ __device__ __forceinline__ bool tile_move(const TileArgs& A, const LaneCtx& C, c
                                           const float* __restrict__ omega_t,
                                           float& rx, float& ry, float& rz, uint32_t& addr, bool& in,
                                           float lx, float ly, float lz, float& q_l,
-                                          float qx, float qy, float qz, float& q_r, float h) {
+                                          float qx, float qy, float qz, float& q_r, float h, bool force_out = false) {
   const Words4 w = philox_tail(A.S.keys, L, c0_1);
   const float tx = trial_axis<FAST>(C, rx, w.w0);
   const float ty = trial_axis<FAST>(C, ry, w.w1);
@@ -253,7 +254,7 @@ __device__ __forceinline__ bool tile_move(const TileArgs& A, const LaneCtx& C, c
   const float dql = __fsub_rn(ql_new, q_l), dqr = __fsub_rn(qr_new, q_r);
   const float dq = EVEN ? __fmaf_rn(h, dql, dqr) : __fmaf_rn(h, dqr, dql);
   uint32_t addr_new;
-  const bool in_new = win_addr<FAST>(C.g, tx, ty, tz, offx, offy, offz, p_f, seam_f, base_t_d, addr_new);
+  const bool in_new = win_addr<FAST>(C.g, tx, ty, tz, offx, offy, offz, p_f, seam_f, base_t_d, addr_new) && !force_out;
   float w_new, w_old;
   if (__any_sync(0xffffffffu, !(in_new && in))) {                  // rare, warp-uniform
     w_new = in_new ? lds_f32(addr_new) : omega_outside(omega_t, A.S.grid, tx, ty, tz);

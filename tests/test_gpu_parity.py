@@ -16,7 +16,8 @@ from helpers import assert_same_state, gpu_system, lockstep
 
 pytestmark = pytest.mark.gpu
 
-FUSED, GENERIC, TILED = 2, 1, 3
+FUSED, GENERIC, TILED, SWEEP = 2, 1, 3, 4
+TILED_PATHS = (TILED, SWEEP)      # 3: first column-sweep kernel (soma_tile.cuh), 4: swept-window kernel (soma_sweep.cuh)
 
 
 def _run_both(s, steps_list, path, **kw):
@@ -190,8 +191,9 @@ TILE_CASES = {
 }
 
 
+@pytest.mark.parametrize("TILED", TILED_PATHS)
 @pytest.mark.parametrize("case", sorted(TILE_CASES))
-def test_tiled_path_parity_after_1_and_10_steps(case):
+def test_tiled_path_parity_after_1_and_10_steps(case, TILED):
     make, opts = TILE_CASES[case]
     s = make()
     o = oracle.Oracle.from_system(s)
@@ -207,8 +209,9 @@ def test_tiled_path_parity_after_1_and_10_steps(case):
         assert g.counters()["path"] == TILED
 
 
+@pytest.mark.parametrize("TILED", TILED_PATHS)
 @pytest.mark.parametrize("interval", [0, 1, 3])
-def test_tiled_path_with_drift_and_resorts(interval):
+def test_tiled_path_with_drift_and_resorts(interval, TILED):
     """40 steps: without re-sorting the chains drift out of their tiles (fallback path); with
     frequent re-sorting the slot order keeps changing.  The trajectory may not depend on either."""
     s = _scaled(4, 6000, (16, 16, 16))
@@ -229,7 +232,7 @@ def test_switching_paths_mid_run_keeps_the_trajectory():
     o.mc_steps(8)
     with gpu_system(s, path=FUSED, options=SMALL_TILES) as g:
         g.load_state(s.x, s.y, s.z)
-        for path in (FUSED, TILED, GENERIC, TILED, FUSED, TILED, TILED, GENERIC):
+        for path in (FUSED, TILED, GENERIC, SWEEP, FUSED, SWEEP, TILED, GENERIC):
             g.set_option("path", path)
             g.mc_steps(1)
         assert_same_state(g, o, "path switched every step")
