@@ -138,9 +138,7 @@ const char *soma_last_error(const soma_t *h);
  *                     steps (0 = never; default 64 for >= 4096 chains, else 0); results are
  *                     independent of it (the random stream is keyed by the logical chain id)
  *   "resort_now"      re-order once, now (value ignored)
- *   "fused_chunk"     warp groups (32 beads-pairs each) per block of the fused kernel (default 224);
- *   "fused_persistent" 1 = one resident wave of "fused_blocks_per_sm" blocks per SM takes the chunks
- *                     cyclically, 0 (default) = one block per chunk in launch order (tuning)
+ *   "fused_chunk"     warp groups (32 bead pairs each) per block of the fused kernel (default 224; tuning)
  * Errors: SOMA_EINVAL (unknown name / unsupported value). */
 int soma_set_option(soma_t *h, const char *name, int64_t value);
 

@@ -173,7 +173,7 @@ struct soma_handle {
   // options
   int path;              // 0 auto, 1 generic, 2 fused
   int64_t resort_interval;      // re-order the chains every k steps (0 = never)
-  int fused_blocks_per_sm, fused_chunk, fused_persistent;
+  int fused_chunk;              // warp groups per block of the fused kernel
   // tiled kernel (soma_tile.cuh)
   bool tile_grid_ok;            // the grid allows tiles at all
   bool tile_ready;              // geometry + tensor maps are set up for the current options
@@ -350,15 +350,10 @@ int launch_fused_p(soma_handle* h) {
   constexpr int G = 32 / P;
   const uint64_t n_groups = (h->n_chains + G - 1) / G;           // warps of work
   const unsigned bs = 256, wpb = bs / 32;
-  // chunks of fused_chunk warp groups (a multiple of the warps per block), dealt out cyclically to
-  // at most one resident wave of blocks
-  const uint64_t resident = (uint64_t)h->sm_count * h->fused_blocks_per_sm;
+  // chunks of fused_chunk warp groups (a multiple of the warps per block)
   uint64_t gpb = ((uint64_t)h->fused_chunk + wpb - 1) / wpb * wpb;
   const uint64_t n_chunks = (n_groups + gpb - 1) / gpb;
-  // fused_persistent = 1: one resident wave of blocks takes the chunks cyclically; 0 (default): one
-  // block per chunk, handed out in order by the hardware block scheduler as blocks retire -- the
-  // dynamic order keeps the blocks closer together in the chain list (measured: 1.12 vs 1.23 ms on cfg4)
-  const uint64_t blocks = (h->fused_persistent && n_chunks > resident) ? resident : n_chunks;
+  const uint64_t blocks = n_chunks;                // one block per chunk, in chain-list order
   const bool multi = h->n_patterns > 1;
 #define SOMA_LAUNCH_FUSED(POW2, MULTI) \
   fused_step_kernel<P, POW2, MULTI><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb)
@@ -791,9 +786,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->path = 0;
   // chains are kept sorted by position when the system is large enough for it to matter
   h->resort_interval = h->n_chains >= 4096 ? 64 : 0;
-  h->fused_blocks_per_sm = 3;
   h->fused_chunk = 224;
-  h->fused_persistent = 0;
   h->tc[0] = 64; h->tc[1] = 8; h->tc[2] = 8;
   h->th[0] = h->th[1] = h->th[2] = 8;
   h->tile_slice = 2;
@@ -956,11 +949,6 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
     return resort(h, use_tile(h) ? 2 : 1);
   }
-  if (!std::strcmp(name, "fused_blocks_per_sm")) {
-    if (value < 1 || value > 32) return fail(h, SOMA_EINVAL, "fused_blocks_per_sm must be in [1, 32]");
-    h->fused_blocks_per_sm = (int)value;
-    return SOMA_OK;
-  }
   {
     static const char* const tn[9] = {"tile_cx", "tile_cy", "tile_cz", "tile_hx", "tile_hy", "tile_hz", "tile_threads",
                                       "tile_slice", "tile_ring"};
@@ -993,11 +981,6 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
   if (!std::strcmp(name, "tile_fast")) {               // 0: use the general arithmetic even where the shortcuts apply
     if (value != 0) return fail(h, SOMA_EINVAL, "tile_fast can only be switched off");
     h->tile_fast = false;
-    return SOMA_OK;
-  }
-  if (!std::strcmp(name, "fused_persistent")) {
-    if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "fused_persistent must be 0 or 1");
-    h->fused_persistent = (int)value;
     return SOMA_OK;
   }
   if (!std::strcmp(name, "fused_chunk")) {

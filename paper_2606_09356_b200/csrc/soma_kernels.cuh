@@ -121,8 +121,11 @@ bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint64_t B, const float* __res
 // kept sorted by position -- the omega gathers of a block stay inside a small neighbourhood that
 // the L1 keeps, and the atomics of concurrently running blocks fall into a bounded part of L2.
 // ---------------------------------------------------------------------------------------------
+#ifndef SOMA_FUSED_MIN_BLOCKS
+#define SOMA_FUSED_MIN_BLOCKS 4      /* 62 registers: 4 blocks per SM; measured best on cfg4 (3: 1.61 ms, 4: 1.13, 5: 1.16, 6: 1.28) */
+#endif
 template <int P, bool POW2, bool MULTI_PAT>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, SOMA_FUSED_MIN_BLOCKS)
 fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
   constexpr int G = 32 / P;                                   // chains per warp
   const uint32_t lane = threadIdx.x & 31u;
@@ -130,7 +133,6 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
   const uint32_t sub = lane / P;                              // which of the warp's chains
   const uint32_t wpb = blockDim.x >> 5;
   const uint64_t n_groups = ((uint64_t)A.n_chains + G - 1) / G;
-  const uint64_t n_chunks = (n_groups + groups_per_block - 1) / groups_per_block;
   unsigned n_acc = 0;
 
   // bead types of this lane (loop-invariant when every chain has the same pattern)
@@ -140,23 +142,35 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
     type0 = tt & 0xffu; type1 = tt >> 8;
   }
 
-  // Chunks of `groups_per_block` consecutive warp groups are dealt out to the resident blocks in
-  // turn, so that at any moment the whole grid works on one contiguous stretch of the position-sorted
-  // chain list: the omega values and density counters that stretch touches (a few MB) stay in L2,
-  // which one contiguous run per block (every block in a different part of the box) does not allow.
-  for (uint64_t chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
-  const uint64_t g_begin = chunk * groups_per_block;
+  // Every block takes one chunk of `groups_per_block` consecutive warp groups.  The hardware hands
+  // the blocks out in launch order as earlier ones retire, so at any moment the whole grid works on
+  // one contiguous stretch of the position-sorted chain list: the omega values and density counters
+  // that stretch touches (a few MB) stay in L2, which one long run per block (every block in a
+  // different part of the box) does not allow.
+  const uint64_t g_begin = (uint64_t)blockIdx.x * groups_per_block;
   uint64_t g_end = g_begin + groups_per_block;
   if (g_end > n_groups) g_end = n_groups;
+  // positions and chain id of the warp's next group are fetched one iteration ahead
+  float2 Xn = make_float2(0.f, 0.f), Yn = Xn, Zn = Xn;
+  uint32_t chain_n = 0;
+  auto fetch = [&](uint64_t wg) {
+    const uint64_t s64 = wg * G + sub;
+    const uint32_t sl = s64 < A.n_chains ? (uint32_t)s64 : 0u;
+    const uint64_t jj = (uint64_t)sl * A.N + 2u * l;
+    Xn = *reinterpret_cast<const float2*>(A.x + jj);
+    Yn = *reinterpret_cast<const float2*>(A.y + jj);
+    Zn = *reinterpret_cast<const float2*>(A.z + jj);
+    chain_n = A.slot_chain[sl];
+  };
+  if (g_begin + (threadIdx.x >> 5) < g_end) fetch(g_begin + (threadIdx.x >> 5));
   for (uint64_t wg = g_begin + (threadIdx.x >> 5); wg < g_end; wg += wpb) {
     const uint64_t slot64 = wg * G + sub;
     const bool live = slot64 < A.n_chains;
     const uint32_t slot = live ? (uint32_t)slot64 : 0u;       // dead lanes shadow slot 0, never store
     const uint64_t j = (uint64_t)slot * A.N + 2u * l;
-    const float2 X = *reinterpret_cast<const float2*>(A.x + j);
-    const float2 Y = *reinterpret_cast<const float2*>(A.y + j);
-    const float2 Z = *reinterpret_cast<const float2*>(A.z + j);
-    const uint32_t chain = A.slot_chain[slot];
+    const float2 X = Xn, Y = Yn, Z = Zn;
+    const uint32_t chain = chain_n;
+    if (wg + wpb < g_end) fetch(wg + wpb);
     if (MULTI_PAT) {
       const uint16_t tt = *reinterpret_cast<const uint16_t*>(A.patterns + (uint32_t)A.slot_pattern[slot] * A.N + 2u * l);
       type0 = tt & 0xffu; type1 = tt >> 8;
@@ -194,7 +208,6 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
       atomicAdd(A.counts_next + (size_t)type0 * A.cells + cell_e, 1u);
       atomicAdd(A.counts_next + (size_t)type1 * A.cells + cell_o, 1u);
     }
-  }
   }
   // accepted-move count: warp reduce, one atomic per warp
 #pragma unroll
