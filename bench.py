@@ -30,6 +30,10 @@ if ROOT not in sys.path:
 
 import numpy as np
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one fused_step_kernel launch on cfg4, from the committed
+# ncu --set full capture profiles/r1_ncu_cfg4_fused_final.txt (1.777933 + 1.627542 GB)
+NCU_TRAFFIC_CFG4_FUSED = 3.405475e9
+
 METRIC = "attempted bead moves/s"
 UNIT = "moves/s"
 
@@ -261,6 +265,7 @@ def run_ours(args):
     kt = g.kernel_times()
     g.set_option("kernel_timing", 0)
     launches = g.counters()["launches"] - c0["launches"]
+    g_path = g.counters()["path"]
     ms, moves = aggregate_over_ranks(local_ms, float(B) * args.steps, dev)
     value = moves / (ms * 1e-3)
 
@@ -286,9 +291,15 @@ def run_ours(args):
     n_t = max(1, kt["steps"])
     move_ms, omega_ms = kt["move_bin_ms"] / n_t, kt["omega_ms"] / n_t
     achieved = ab["move_bin_kernel"] / (move_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "fused_step_kernel (rows a1+a2+a3+a5)" if launches == 2 * args.steps else "move+bin kernels",
+    path_now = g_path
+    kname = {1: "half_sweep_kernel x2 + bin_kernel (rows a1+a2+a3+a5)", 2: "fused_step_kernel (rows a1+a2+a3+a5)",
+             3: "tile_step_kernel (rows a1+a2+a3+a5)", 4: "sweep_step_kernel (rows a1+a2+a3+a5)"}[path_now]
+    traffic = args.traffic
+    if traffic is None and path_now == 2 and args.config == 4:
+        traffic = NCU_TRAFFIC_CFG4_FUSED
+    roofline = {"bound": "hbm", "kernel": kname,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": args.traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": ab["move_bin_kernel"],
+                "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": ab["move_bin_kernel"],
                 "kernel_ms": move_ms, "omega_kernel_ms": omega_ms,
                 "omega_kernel_frac": ab["omega_kernel"] / (omega_ms * 1e-3) / 1e9 / peak if omega_ms > 0 else None,
                 "step_frac": ab["step"] / (local_ms / args.steps * 1e-3) / 1e9 / peak,
@@ -329,7 +340,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: 134 M beads)")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--path", type=int, default=0, help="library kernel path: 0 auto, 1 generic, 2 fused")
+    ap.add_argument("--path", type=int, default=0, help="library kernel path: 0 auto (fused), 1 generic, 2 fused, 3/4 windowed kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
