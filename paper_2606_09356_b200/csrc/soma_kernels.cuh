@@ -157,9 +157,10 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
     const uint64_t s64 = wg * G + sub;
     const uint32_t sl = s64 < A.n_chains ? (uint32_t)s64 : 0u;
     const uint64_t jj = (uint64_t)sl * A.N + 2u * l;
-    Xn = *reinterpret_cast<const float2*>(A.x + jj);
-    Yn = *reinterpret_cast<const float2*>(A.y + jj);
-    Zn = *reinterpret_cast<const float2*>(A.z + jj);
+    // positions are streamed (read once, written once): keep them from evicting omega out of L1
+    Xn = __ldcs(reinterpret_cast<const float2*>(A.x + jj));
+    Yn = __ldcs(reinterpret_cast<const float2*>(A.y + jj));
+    Zn = __ldcs(reinterpret_cast<const float2*>(A.z + jj));
     chain_n = A.slot_chain[sl];
   };
   if (g_begin + (threadIdx.x >> 5) < g_end) fetch(g_begin + (threadIdx.x >> 5));
@@ -202,9 +203,9 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
       n_acc += (acc && live) ? 1u : 0u;
     }
     if (live) {
-      *reinterpret_cast<float2*>(A.x + j) = make_float2(ex, ox);
-      *reinterpret_cast<float2*>(A.y + j) = make_float2(ey, oy);
-      *reinterpret_cast<float2*>(A.z + j) = make_float2(ez, oz);
+      __stcs(reinterpret_cast<float2*>(A.x + j), make_float2(ex, ox));
+      __stcs(reinterpret_cast<float2*>(A.y + j), make_float2(ey, oy));
+      __stcs(reinterpret_cast<float2*>(A.z + j), make_float2(ez, oz));
       atomicAdd(A.counts_next + (size_t)type0 * A.cells + cell_e, 1u);
       atomicAdd(A.counts_next + (size_t)type1 * A.cells + cell_o, 1u);
     }
