@@ -355,8 +355,12 @@ int launch_fused_p(soma_handle* h) {
   const uint64_t n_chunks = (n_groups + gpb - 1) / gpb;
   const uint64_t blocks = n_chunks;                // one block per chunk, in chain-list order
   const bool multi = h->n_patterns > 1;
-#define SOMA_LAUNCH_FUSED(POW2, MULTI) \
-  fused_step_kernel<P, POW2, MULTI><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb)
+  const bool fast = h->tile_fast && h->pow2;       // exact one-FFMA shortcuts apply (see fused_move)
+#define SOMA_LAUNCH_FUSED(POW2, MULTI)                                                                          \
+  do {                                                                                                          \
+    if (fast && POW2) fused_step_kernel<P, POW2, MULTI, POW2><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb); \
+    else fused_step_kernel<P, POW2, MULTI, false><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb);    \
+  } while (0)
   if (h->pow2) { if (multi) SOMA_LAUNCH_FUSED(true, true); else SOMA_LAUNCH_FUSED(true, false); }
   else         { if (multi) SOMA_LAUNCH_FUSED(false, true); else SOMA_LAUNCH_FUSED(false, false); }
 #undef SOMA_LAUNCH_FUSED

@@ -65,6 +65,58 @@ __device__ __forceinline__ bool move_bead(const StepArgs& A, uint32_t chain, uin
   return acc;
 }
 
+// The move of the fused kernel: the same arithmetic with the loop-invariant work taken out.
+//  * Philox rounds 1-3 are partially folded per lane (PhiloxLane, soma_device.cuh);
+//  * the squared lengths of the bead's two bonds are carried along (q_l, q_r; on return the lengths
+//    after the move) instead of being recomputed, and a missing neighbour contributes
+//    h * (finite) = 0 (h = 0 or 1) -- one fp32 add as in DESIGN.md section 2 step 5.4;
+//  * FAST (a and all inv_h powers of two, inv_h >= 1, power-of-two grid): a tmap(w) = 2a h + a(2^-23 - 1)
+//    is exact in one FFMA, and r inv_h is exact so the floor is one FFMA.RD;
+//  * the decision comes from one FFMA on the hardware logarithm with a guard band (metropolis_accept_fma).
+struct FusedConst { float a2, ac; uint32_t u0; };   // 2a, a(2^-23 - 1), hi(M1 step) ^ k0[0]
+
+template <bool POW2, bool FAST>
+__device__ __forceinline__ uint32_t cell_of_fused(const Grid& g, float x, float y, float z) {
+  if (POW2 && FAST) {
+    const uint32_t ix = __float_as_uint(__fmaf_rd(x, g.inv_hx, kFloorMagic)) & (g.nx - 1u);
+    const uint32_t iy = __float_as_uint(__fmaf_rd(y, g.inv_hy, kFloorMagic)) & (g.ny - 1u);
+    const uint32_t iz = __float_as_uint(__fmaf_rd(z, g.inv_hz, kFloorMagic)) & (g.nz - 1u);
+    return (ix * g.ny + iy) * g.nz + iz;
+  }
+  return cell_of<POW2>(g, x, y, z);
+}
+
+template <bool FAST>
+__device__ __forceinline__ float trial_axis_fused(const StepArgs& A, const FusedConst& F, float r, uint32_t w) {
+  if (FAST) {
+    const float h = __fadd_rn(__uint_as_float(0x3f800000u | (w >> 9)), -1.0f);
+    return __fadd_rn(r, __fmaf_rn(F.a2, h, F.ac));
+  }
+  return __fadd_rn(r, __fmul_rn(A.a, tmap(w)));
+}
+
+template <bool POW2, bool FAST, bool EVEN>
+__device__ __forceinline__ bool fused_move(const StepArgs& A, const FusedConst& F, const PhiloxLane& L, uint32_t c0_1,
+                                           const float* __restrict__ omega_t,
+                                           float& rx, float& ry, float& rz, uint32_t& cell,
+                                           float lx, float ly, float lz, float& q_l,
+                                           float qx, float qy, float qz, float& q_r, float h) {
+  const Words4 w = philox_tail(A.keys, L, c0_1);
+  const float tx = trial_axis_fused<FAST>(A, F, rx, w.w0);
+  const float ty = trial_axis_fused<FAST>(A, F, ry, w.w1);
+  const float tz = trial_axis_fused<FAST>(A, F, rz, w.w2);
+  const float ql_new = bond_sq(tx, ty, tz, lx, ly, lz);
+  const float qr_new = bond_sq(tx, ty, tz, qx, qy, qz);
+  const float dql = __fsub_rn(ql_new, q_l), dqr = __fsub_rn(qr_new, q_r);
+  const float dq = EVEN ? __fmaf_rn(h, dql, dqr) : __fmaf_rn(h, dqr, dql);
+  const uint32_t cell_new = cell_of_fused<POW2, FAST>(A.grid, tx, ty, tz);
+  const float dw = __fsub_rn(__ldg(omega_t + cell_new), __ldg(omega_t + cell));
+  const float dE = __fmaf_rn(A.kb, dq, dw);
+  const bool acc = metropolis_accept_fma(dE, w.w3);
+  if (acc) { rx = tx; ry = ty; rz = tz; cell = cell_new; q_l = ql_new; q_r = qr_new; }
+  return acc;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Generic path: one thread per bead of the given parity.
 // ---------------------------------------------------------------------------------------------
@@ -124,7 +176,7 @@ bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint64_t B, const float* __res
 #ifndef SOMA_FUSED_MIN_BLOCKS
 #define SOMA_FUSED_MIN_BLOCKS 4      /* 62 registers: 4 blocks per SM; measured best on cfg4 (3: 1.61 ms, 4: 1.13, 5: 1.16, 6: 1.28) */
 #endif
-template <int P, bool POW2, bool MULTI_PAT>
+template <int P, bool POW2, bool MULTI_PAT, bool FAST>
 __global__ void __launch_bounds__(256, SOMA_FUSED_MIN_BLOCKS)
 fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
   constexpr int G = 32 / P;                                   // chains per warp
@@ -135,6 +187,14 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
   const uint64_t n_groups = ((uint64_t)A.n_chains + G - 1) / G;
   unsigned n_acc = 0;
 
+  const float hl = l > 0 ? 1.0f : 0.0f, hr = l + 1 < P ? 1.0f : 0.0f;    // does the left / right cross-lane neighbour exist
+  FusedConst F;
+  F.a2 = __fmul_rn(2.0f, A.a);
+  F.ac = __fmul_rn(A.a, -0.99999988079071044921875f);                    // a (2^-23 - 1): exact when a is a power of two
+  const uint64_t m1 = (uint64_t)kPhiloxM1 * A.ctr2;
+  F.u0 = (uint32_t)(m1 >> 32) ^ A.keys.k0[0];
+  const PhiloxLane L0 = philox_lane(A.keys, (uint32_t)m1, 2u * l, A.ctr3_base);
+  const PhiloxLane L1 = philox_lane(A.keys, (uint32_t)m1, 2u * l + 1u, A.ctr3_base | 1u);
   // bead types of this lane (loop-invariant when every chain has the same pattern)
   uint32_t type0 = 0, type1 = 0;
   if (!MULTI_PAT) {
@@ -181,16 +241,20 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
 
     float ex = X.x, ey = Y.x, ez = Z.x;                       // even bead 2l
     float ox = X.y, oy = Y.y, oz = Z.y;                       // odd bead 2l+1
-    uint32_t cell_e = cell_of<POW2>(A.grid, ex, ey, ez);
-    uint32_t cell_o = cell_of<POW2>(A.grid, ox, oy, oz);
+    uint32_t cell_e = cell_of_fused<POW2, FAST>(A.grid, ex, ey, ez);
+    uint32_t cell_o = cell_of_fused<POW2, FAST>(A.grid, ox, oy, oz);
+    const uint32_t c0_1 = F.u0 ^ chain;
 
-    // half-sweep 0: even bead; left neighbour = odd bead of lane l-1, right neighbour = own odd bead
+    // half-sweep 0: even bead; left neighbour = odd bead of lane l-1, right neighbour = own odd bead.
+    // qA = |even - odd|^2, qB = |odd of lane l-1 - even|^2
+    const float lx = __shfl_up_sync(0xffffffffu, ox, 1, P);
+    const float ly = __shfl_up_sync(0xffffffffu, oy, 1, P);
+    const float lz = __shfl_up_sync(0xffffffffu, oz, 1, P);
+    float qA = bond_sq(ex, ey, ez, ox, oy, oz);
+    float qB = bond_sq(ex, ey, ez, lx, ly, lz);
     {
-      const float lx = __shfl_up_sync(0xffffffffu, ox, 1, P);
-      const float ly = __shfl_up_sync(0xffffffffu, oy, 1, P);
-      const float lz = __shfl_up_sync(0xffffffffu, oz, 1, P);
-      const bool acc = move_bead<POW2>(A, chain, 2u * l, 0u, om0, ex, ey, ez, cell_e,
-                                       l > 0, lx, ly, lz, true, ox, oy, oz);
+      const bool acc = fused_move<POW2, FAST, true>(A, F, L0, c0_1, om0, ex, ey, ez, cell_e,
+                                                    lx, ly, lz, qB, ox, oy, oz, qA, hl);
       n_acc += (acc && live) ? 1u : 0u;
     }
     // half-sweep 1: odd bead; left = own even bead (new), right = even bead of lane l+1 (new)
@@ -198,8 +262,9 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
       const float qx = __shfl_down_sync(0xffffffffu, ex, 1, P);
       const float qy = __shfl_down_sync(0xffffffffu, ey, 1, P);
       const float qz = __shfl_down_sync(0xffffffffu, ez, 1, P);
-      const bool acc = move_bead<POW2>(A, chain, 2u * l + 1u, 1u, om1, ox, oy, oz, cell_o,
-                                       true, ex, ey, ez, l + 1 < P, qx, qy, qz);
+      float qR = __shfl_down_sync(0xffffffffu, qB, 1, P);
+      const bool acc = fused_move<POW2, FAST, false>(A, F, L1, c0_1, om1, ox, oy, oz, cell_o,
+                                                     ex, ey, ez, qA, qx, qy, qz, qR, hr);
       n_acc += (acc && live) ? 1u : 0u;
     }
     if (live) {

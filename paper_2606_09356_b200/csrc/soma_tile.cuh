@@ -72,65 +72,6 @@ __device__ __forceinline__ void reds_inc(uint32_t addr) {
   asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(addr) : "memory");
 }
 
-// ---- Philox4x32-10 with the loop-invariant part of the first three rounds folded ---------------
-// Counter of a move = (bead i, chain c, step, parity | domain<<8 | step_hi<<16).  Only c differs
-// between the moves a lane makes, and it enters through round 1 as c0' = u0 ^ c, so for every lane
-// and parity the values below are fixed for the whole kernel (derivation in DESIGN.md section 7):
-//   LC = lo(M0 i) ^ k1[1]                       (xor-ed onto hi(M0 c0') in round 2)
-//   LD = lo(M1 c2') ^ k0[2],  c2' = hi(M0 i) ^ ctr3 ^ k1[0]
-//   LE = hi(M0 c0'') ^ k1[2], c0'' = hi(M1 c2') ^ u1 ^ k0[1]
-//   LF = lo(M0 c0'')
-// which leaves 16 wide multiplies and 18 xors per move instead of 20 + 20.
-struct PhiloxLane { uint32_t LC, LD, LE, LF; };
-
-__device__ __forceinline__ PhiloxLane philox_lane(const PhiloxKeys& K, uint32_t u1, uint32_t i, uint32_t ctr3) {
-  const uint64_t p0 = (uint64_t)kPhiloxM0 * i;
-  const uint32_t c2_1 = (uint32_t)(p0 >> 32) ^ ctr3 ^ K.k1[0];
-  const uint64_t p1 = (uint64_t)kPhiloxM1 * c2_1;
-  const uint32_t c0_2 = (uint32_t)(p1 >> 32) ^ u1 ^ K.k0[1];
-  const uint64_t q0 = (uint64_t)kPhiloxM0 * c0_2;
-  PhiloxLane L;
-  L.LC = (uint32_t)p0 ^ K.k1[1];
-  L.LD = (uint32_t)p1 ^ K.k0[2];
-  L.LE = (uint32_t)(q0 >> 32) ^ K.k1[2];
-  L.LF = (uint32_t)q0;
-  return L;
-}
-
-// c0_1 = u0 ^ chain, u0 = hi(M1 step) ^ k0[0]
-__device__ __forceinline__ Words4 philox_tail(const PhiloxKeys& K, const PhiloxLane& L, uint32_t c0_1) {
-  const uint64_t r2 = (uint64_t)kPhiloxM0 * c0_1;                       // round 2
-  const uint32_t c2_2 = (uint32_t)(r2 >> 32) ^ L.LC;
-  const uint64_t r3 = (uint64_t)kPhiloxM1 * c2_2;                       // round 3
-  uint32_t c0 = (uint32_t)(r3 >> 32) ^ L.LD;
-  uint32_t c1 = (uint32_t)r3;
-  uint32_t c2 = L.LE ^ (uint32_t)r2;
-  uint32_t c3 = L.LF;
-#pragma unroll
-  for (int r = 3; r < 10; ++r) {
-    const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;
-    const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
-    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ K.k0[r];
-    c1 = (uint32_t)p1;
-    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ K.k1[r];
-    c3 = (uint32_t)p0;
-  }
-  return Words4{c0, c1, c2, c3};
-}
-
-// ---- Metropolis decision, one fused multiply-add from the hardware logarithm --------------------
-// m = lg2(u 2^24) ln2 + dE = dE + ln u + 24 ln2 up to ~1e-5.  accept iff fl(dE + lnu) <= 0
-// (DESIGN.md section 2 step 5.6); m outside [T - band, T + band] decides that exactly (this
-// includes dE <= 0: then the exact rule accepts, and either m < T - band or the slow path runs).
-constexpr float kLn2 = 0.693147182464599609375f;
-constexpr float kLnT = 16.6355323791503906250f;            // 24 ln 2
-__device__ __forceinline__ bool metropolis_accept_fma(float dE, uint32_t w3) {
-  const float m = __fmaf_rn(lg2_approx(umap_int(w3)), kLn2, dE);
-  bool acc = m < kLnT - kLnBand;
-  if (!acc && m <= kLnT + kLnBand) acc = __fadd_rn(dE, lnu_exact(umap(w3))) <= 0.0f;
-  return acc;
-}
-
 // ---- window-local cell ---------------------------------------------------------------------------
 // A chain group works inside a WINDOW of the grid: wx x ey x ez cells whose omega values and
 // density counters sit in shared memory, slab by slab along x (a slab = one x layer, [T][ey][ez]),
