@@ -75,6 +75,7 @@ def lib() -> C.CDLL:
             "oracle_set_density": (None, [vp, u32p]),
             "oracle_get_omega": (None, [vp, f32p]),
             "oracle_set_omega": (None, [vp, f32p]),
+            "oracle_set_external_field": (None, [vp, f32p]),
             "oracle_get_step": (C.c_uint64, [vp]),
             "oracle_set_step": (None, [vp, C.c_uint64]),
             "oracle_cell_index": (C.c_uint64, [vp, C.c_float, C.c_float, C.c_float]),
@@ -209,6 +210,14 @@ class Oracle:
     def set_omega(self, omega):
         omega = np.ascontiguousarray(omega, dtype=np.float32).reshape(self.T, self.Cells)
         lib().oracle_set_omega(self._h, _p(omega, C.c_float))
+
+    def set_external_field(self, ext):
+        """ext [T][C] in kT per bead, added to omega (R21); None removes it."""
+        if ext is None:
+            lib().oracle_set_external_field(self._h, None)
+        else:
+            ext = np.ascontiguousarray(ext, dtype=np.float32).reshape(self.T, self.Cells)
+            lib().oracle_set_external_field(self._h, _p(ext, C.c_float))
 
     @property
     def step(self) -> int:

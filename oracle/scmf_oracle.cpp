@@ -102,6 +102,7 @@ struct Oracle {
   std::vector<float> x, y, z;           // [B], index c*N+i, unwrapped (R7)
   std::vector<uint32_t> counts;         // [T][C], cell = (ix*ny+iy)*nz+iz (R12)
   std::vector<float> omega;             // [T][C]
+  std::vector<float> ext;               // [T][C] external field (empty = none), R21
   uint64_t t;                           // absolute step index
   bool loaded;
 };
@@ -138,6 +139,8 @@ void bin(Oracle& o) {
 
 // DESIGN.md section 2 step 3 (NS part 3; R2 formula):
 //   phi_s(c) = n_s(c) * C/B;  omega_t(c) = (1/N) * ( kappaN*(sum_s phi_s - 1) + sum_{s != t} chiN_ts * phi_s ).
+// With an external field ("umbrella potential"; R21):
+//   omega_t(c) = fl32( fl32(invN * acc) + ext_t(c) ),  ext in kT per bead.
 void compute_omega(Oracle& o) {
   std::vector<float> phi(o.T);
   for (uint64_t c = 0; c < o.C; ++c) {
@@ -151,7 +154,8 @@ void compute_omega(Oracle& o) {
       float acc = p;
       for (uint32_t s = 0; s < o.T; ++s)
         if (s != t) acc = fmaf(o.chiN[(size_t)t * o.T + s], phi[s], acc);
-      o.omega[(size_t)t * o.C + c] = o.invN * acc;
+      const float w = o.invN * acc;
+      o.omega[(size_t)t * o.C + c] = o.ext.empty() ? w : w + o.ext[(size_t)t * o.C + c];
     }
   }
 }
@@ -382,6 +386,12 @@ void oracle_set_omega(void* h, const float* omega) {
   std::memcpy(o.omega.data(), omega, o.omega.size() * sizeof(float));
 }
 uint64_t oracle_get_step(void* h) { return static_cast<Oracle*>(h)->t; }
+// external field [T][C] (nullptr = none); omega is recomputed from the current densities
+void oracle_set_external_field(void* h, const float* ext) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (ext) o.ext.assign(ext, ext + (size_t)o.T * o.C); else o.ext.clear();
+  if (o.loaded) compute_omega(o);
+}
 void oracle_set_step(void* h, uint64_t t) { static_cast<Oracle*>(h)->t = t; }
 
 uint64_t oracle_cell_index(void* h, float x, float y, float z) {

@@ -168,3 +168,46 @@ def test_load_state_bins_and_computes_omega():
     om = o.omega()
     assert np.allclose(om[0], want0, rtol=0, atol=5e-6)
     assert np.allclose(om[1], want1, rtol=0, atol=5e-6)
+
+
+# ---- external field (R21) ------------------------------------------
+
+def test_external_field_boltzmann_occupancy_of_single_bead_molecules():
+    """Single-bead molecules (N = 1) without interactions in a cell-wise constant external field are
+    independent Metropolis walkers with stationary density proportional to exp(-ext(cell)): after a
+    burn-in the cell occupancies are one multinomial draw from those weights (chi^2, 63 dof)."""
+    from scipy import stats
+    n, grid, box = 200_000, (4, 4, 4), (2.0, 2.0, 2.0)
+    s = si.custom_system(n, 1, 1, [[0]], None, [[0.0]], 0.0, grid, box, seed=77)
+    rng = np.random.default_rng(5)
+    ext = rng.uniform(0.0, 2.0, size=(1, 64)).astype(np.float32)
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    o.set_external_field(ext)
+    assert np.array_equal(o.omega(), ext)                       # no interactions: omega is the field itself
+    o.mc_steps(120)
+    counts = o.density().reshape(-1).astype(np.float64)
+    p = np.exp(-ext.astype(np.float64).reshape(-1))
+    p /= p.sum()
+    chi2 = float(((counts - n * p) ** 2 / (n * p)).sum())
+    assert chi2 < stats.chi2.ppf(1 - 1e-4, df=63), chi2
+    # the field matters: against uniform weights the same counts are wildly off
+    assert float(((counts - n / 64) ** 2 / (n / 64)).sum()) > 50 * 63
+
+
+def test_external_field_adds_to_omega_in_fp32_and_can_be_removed():
+    s = si.make_system(si.config(0))
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    base = o.omega().copy()
+    ext = np.random.default_rng(9).normal(0.0, 0.7, size=base.shape).astype(np.float32)
+    o.set_external_field(ext)
+    assert np.array_equal(o.omega().view(np.uint32), (base + ext).view(np.uint32))   # one fp32 add per cell
+    o.mc_steps(2)                                                # the field persists across steps
+    o2 = oracle.Oracle.from_system(s)
+    o2.load_state(*o.positions(), step0=2)
+    assert np.array_equal(o.omega() - o2.omega(), (o2.omega() + ext) - o2.omega())
+    o.set_external_field(None)
+    assert np.array_equal(o.omega().view(np.uint32), o2.omega().view(np.uint32))
+    o.set_external_field(np.zeros_like(ext))                     # a zero field changes nothing, bit for bit
+    assert np.array_equal(o.omega().view(np.uint32), o2.omega().view(np.uint32))
