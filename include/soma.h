@@ -107,6 +107,14 @@ int soma_get_positions(soma_t *h, float *x, float *y, float *z, int ptrs_are_dev
 /* Current field omega, [T][cells] fp32 (helper; not in north_star's list). */
 int soma_get_omega(soma_t *h, float *omega, int ptr_is_device);
 
+/* External field (the SOMA side of the paper's "umbrella potential"
+ * equilibration; reading R21): ext [T][cells] fp32, in kT per bead, same
+ * layout as omega.  From now on omega_t(c) = fl32(fl32(invN * acc) + ext_t(c)) -- DESIGN.md section 2
+ * step 3 plus one fp32 add.  The array is copied (host arrays: before the call returns); omega of
+ * the current configuration is recomputed at once if a state is loaded, so the next step sees the
+ * field.  ext == NULL removes it.  It survives soma_load_state.  Errors: SOMA_ECUDA. */
+int soma_set_external_field(soma_t *h, const float *ext, int ptr_is_device);
+
 /* Absolute step index (step0 + steps done). */
 int soma_get_step(soma_t *h, uint64_t *step);
 

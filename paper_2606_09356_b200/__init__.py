@@ -26,7 +26,7 @@ LIB_PATH: Path = _build.LIB_PATH
 # every symbol include/soma.h declares (tests check the library exports exactly these)
 EXPORTS = (
     "soma_workspace_bytes", "soma_create", "soma_load_state", "soma_mc_steps", "soma_get_density",
-    "soma_get_positions", "soma_get_omega", "soma_get_step", "soma_destroy", "soma_last_error",
+    "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_get_step", "soma_destroy", "soma_last_error",
     "soma_set_option", "soma_get_counters", "soma_get_kernel_times", "soma_debug_half_sweep", "soma_debug_finish_step",
     "soma_debug_set_omega", "soma_debug_philox", "soma_debug_maps", "soma_debug_accept",
     "soma_debug_cell_index",
@@ -85,6 +85,7 @@ def load_library() -> C.CDLL:
             "soma_get_density": (i32, [vp, vp, i32]),
             "soma_get_positions": (i32, [vp, vp, vp, vp, i32]),
             "soma_get_omega": (i32, [vp, vp, i32]),
+            "soma_set_external_field": (i32, [vp, vp, i32]),
             "soma_get_step": (i32, [vp, C.POINTER(u64)]),
             "soma_destroy": (i32, [vp]),
             "soma_last_error": (C.c_char_p, [vp]),
@@ -180,6 +181,16 @@ def soma_get_positions(h, x, y, z):
 def soma_get_omega(h, out):
     _check(load_library().soma_get_omega(h, _ptr(out), _is_device(out)), h)
     return out
+
+
+def soma_set_external_field(h, ext):
+    """ext: [T][cells] fp32 numpy array or CUDA tensor, or None to remove the field."""
+    if ext is None:
+        _check(load_library().soma_set_external_field(h, None, 0), h)
+        return
+    if isinstance(ext, np.ndarray):
+        ext = np.ascontiguousarray(ext, dtype=np.float32)
+    _check(load_library().soma_set_external_field(h, _ptr(ext), _is_device(ext)), h)
 
 
 def soma_get_step(h) -> int:
@@ -327,6 +338,9 @@ class Soma:
 
     def omega(self) -> np.ndarray:
         return soma_get_omega(self._h, np.empty((self.T, self.cells), dtype=np.float32))
+
+    def set_external_field(self, ext):
+        soma_set_external_field(self._h, ext)
 
     @property
     def step(self) -> int:

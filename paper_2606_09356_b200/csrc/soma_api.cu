@@ -25,6 +25,7 @@ struct Layout {            // byte offsets into the workspace
   uint64_t pos[2][3];      // two position sets (x,y,z): the live one and a staging / re-order target
   uint64_t counts[2];      // [T][C] uint32, double-buffered
   uint64_t omega;          // [T][C] fp32
+  uint64_t ext;            // [T][C] fp32 external field (used once soma_set_external_field has set one)
   uint64_t slot_chain[2];  // [n] uint32: logical chain id of every slot (second copy: re-order target)
   uint64_t slot_pattern[2];// [n] uint8
   uint64_t patterns;       // [n_patterns][N] uint8
@@ -77,6 +78,7 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
     for (int d = 0; d < 3; ++d) { L.pos[s][d] = off; off += align_up(B * 4); }
   for (int s = 0; s < 2; ++s) { L.counts[s] = off; off += align_up(TC * 4); }
   L.omega = off; off += align_up(TC * 4);
+  L.ext = off; off += align_up(TC * 4);
   for (int s = 0; s < 2; ++s) { L.slot_chain[s] = off; off += align_up(n * 4); }
   for (int s = 0; s < 2; ++s) { L.slot_pattern[s] = off; off += align_up(n); }
   L.patterns = off; off += align_up(pat_bytes);
@@ -167,6 +169,7 @@ struct soma_handle {
   uint64_t range_check_interval;
   // state
   bool loaded;
+  bool has_ext;          // an external field is set (soma_set_external_field)
   bool identity_order;   // slot_chain is the identity
   uint64_t step;
   int sm_count;
@@ -207,6 +210,7 @@ struct soma_handle {
   float* pos(int set, int d) const { return reinterpret_cast<float*>(ws + L.pos[set][d]); }
   uint32_t* counts(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts[s]); }
   float* omega() const { return reinterpret_cast<float*>(ws + L.omega); }
+  float* ext() const { return reinterpret_cast<float*>(ws + L.ext); }
   uint32_t* slot_chain(int s) const { return reinterpret_cast<uint32_t*>(ws + L.slot_chain[s]); }
   uint8_t* slot_pattern(int s) const { return reinterpret_cast<uint8_t*>(ws + L.slot_pattern[s]); }
   uint32_t* slot_chain() const { return slot_chain(live); }
@@ -314,6 +318,7 @@ int launch_omega(soma_handle* h) {
   A.counts = h->counts(h->cur);
   A.counts_to_zero = h->counts(h->cur ^ 1);
   A.omega = h->omega();
+  A.ext = h->has_ext ? h->ext() : nullptr;
   if (use_tile(h)) {            // also fills the ghost-padded copy the tiles are loaded from
     PadGeom pg{h->pad[0], h->pad[1], h->pad[2], h->th[0], h->th[1], h->th[2]};
     const unsigned g = blocks_for((uint64_t)h->pad[0] * h->pad[1] * h->pad[2], 256);
@@ -902,6 +907,23 @@ int soma_get_positions(soma_t* h, float* x, float* y, float* z, int dev) {
     CU(h, cudaMemcpyAsync(dst[d], h->pos(set, d), h->B * 4,
                           dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
   if (!dev) CU(h, cudaStreamSynchronize(h->stream));
+  return SOMA_OK;
+}
+
+int soma_set_external_field(soma_t* h, const float* ext, int dev) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (ext) {
+    CU(h, cudaMemcpyAsync(h->ext(), ext, (size_t)h->cells * h->T * 4,
+                          dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+    if (!dev) CU(h, cudaStreamSynchronize(h->stream));           // the caller may reuse its buffer
+  }
+  h->has_ext = ext != nullptr;
+  if (h->loaded) {                                               // omega of the current densities, with the new field
+    if (h->counts_in_pad) return fail(h, SOMA_ESTATE, "internal: densities not folded");
+    h->omega_custom = false;
+    if ((rc = launch_omega(h)) != SOMA_OK) return rc;
+  }
   return SOMA_OK;
 }
 

@@ -292,6 +292,7 @@ struct OmegaArgs {
   const uint32_t* __restrict__ counts;       // [T][C] fresh counts
   uint32_t* __restrict__ counts_to_zero;     // [T][C] buffer for the next step (may be null)
   float* __restrict__ omega;                 // [T][C]
+  const float* __restrict__ ext;             // [T][C] external field added to omega (R21), or null
 };
 
 template <int T_>
@@ -318,7 +319,8 @@ omega_kernel(OmegaArgs A) {
 #pragma unroll
       for (uint32_t s = 0; s < (T_ > 0 ? T_ : kMaxTypes); ++s)
         if (s < T && s != t) acc = __fmaf_rn(A.chiN[t * T + s], phi[s], acc);
-      A.omega[(size_t)t * A.cells + c] = __fmul_rn(A.invN, acc);
+      const float w = __fmul_rn(A.invN, acc);
+      A.omega[(size_t)t * A.cells + c] = A.ext ? __fadd_rn(w, A.ext[(size_t)t * A.cells + c]) : w;
     }
   }
 }

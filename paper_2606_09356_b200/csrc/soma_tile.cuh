@@ -563,7 +563,8 @@ omega_pad_kernel(OmegaArgs A, Grid grid, PadGeom pg, float* __restrict__ omega_p
 #pragma unroll
       for (uint32_t s = 0; s < (T_ > 0 ? T_ : kMaxTypes); ++s)
         if (s < T && s != t) acc = __fmaf_rn(A.chiN[t * T + s], phi[s], acc);
-      const float w = __fmul_rn(A.invN, acc);
+      float w = __fmul_rn(A.invN, acc);
+      if (A.ext) w = __fadd_rn(w, A.ext[(size_t)t * A.cells + c]);
       omega_pad[(size_t)t * pcells + p] = w;
       if (interior) A.omega[(size_t)t * A.cells + c] = w;
     }

@@ -253,3 +253,41 @@ def test_tiled_path_is_refused_where_it_cannot_run():
         g.set_option("path", TILED)
         g.set_option("tile_hz", 3)                                           # window 10 cells along z: not a multiple of 4 -> tiles off
         assert g.counters()["path"] != TILED
+
+
+# ---- external field: omega = interaction part + ext, every kernel path -----
+
+@pytest.mark.parametrize("path", [FUSED, GENERIC, TILED, SWEEP])
+def test_external_field_parity(path):
+    s = _scaled(4, 6000, (16, 16, 16))
+    ext = np.random.default_rng(31).normal(0.0, 0.8, size=(2, 16 ** 3)).astype(np.float32)
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    o.set_external_field(ext)
+    with gpu_system(s, path=path, options=SMALL_TILES if path in TILED_PATHS else None) as g:
+        g.load_state(s.x, s.y, s.z)
+        g.set_external_field(ext)
+        assert np.array_equal(g.omega().view(np.uint32), o.omega().view(np.uint32))
+        assert g.mc_steps(5, want_accepted=True) == o.mc_steps(5)
+        assert_same_state(g, o, f"external field, path {path}, 5 steps")
+        g.load_state(*g.positions(), step0=5)                     # the field survives a reload
+        assert np.array_equal(g.omega().view(np.uint32), o.omega().view(np.uint32))
+        g.set_external_field(None)
+        o.set_external_field(None)
+        assert g.mc_steps(3, want_accepted=True) == o.mc_steps(3)
+        assert_same_state(g, o, f"external field removed, path {path}")
+
+
+def test_external_field_single_bead_molecules_on_device():
+    """N = 1 (generic path): the oracle's Boltzmann pin, run on the GPU and compared bit for bit."""
+    s = si.custom_system(20000, 1, 1, [[0]], None, [[0.0]], 0.0, (4, 4, 4), (2.0, 2.0, 2.0), seed=78)
+    ext = np.random.default_rng(6).uniform(0.0, 2.0, size=(1, 64)).astype(np.float32)
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    o.set_external_field(ext)
+    with gpu_system(s) as g:
+        g.load_state(s.x, s.y, s.z)
+        import torch
+        g.set_external_field(torch.from_numpy(ext).cuda())        # device pointer in
+        assert g.mc_steps(40, want_accepted=True) == o.mc_steps(40)
+        assert_same_state(g, o, "N=1 in an external field")
