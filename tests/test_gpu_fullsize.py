@@ -51,3 +51,23 @@ def test_cfg4_full_size_one_step_bit_exact_then_invariants():
         assert np.array_equal(hist, dens[t].reshape(-1).astype(np.int64))
     # beads move by less than the half-width per step and axis
     assert float(np.abs(x - s.x).max()) < 10 * w.move_halfwidth
+
+
+@pytest.mark.parametrize("cfg,steps", [(1, 10), (2, 10), (3, 2)])
+def test_full_size_configs_bit_exact(cfg, steps):
+    """configs[1..3] at BASELINE.json's full sizes on the default kernel path (cfg1, cfg3: N = 64, one
+    chain per warp; cfg3: two chain patterns), whole state against the oracle after `steps` MC steps."""
+    w = si.config(cfg)
+    s = si.make_system(w)
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    acc_o = o.mc_steps(steps)
+    with gpu_system(s) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert g.mc_steps(steps, want_accepted=True) == acc_o
+        gx, gy, gz = g.positions()
+        ox, oy, oz = o.positions()
+        assert np.array_equal(gx, ox) and np.array_equal(gy, oy) and np.array_equal(gz, oz)
+        assert np.array_equal(g.density(), o.density())
+        assert np.array_equal(g.omega().view(np.uint32), o.omega().view(np.uint32))
+    o.close()
