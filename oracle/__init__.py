@@ -76,6 +76,7 @@ def lib() -> C.CDLL:
             "oracle_get_omega": (None, [vp, f32p]),
             "oracle_set_omega": (None, [vp, f32p]),
             "oracle_set_external_field": (None, [vp, f32p]),
+            "oracle_generate_state": (C.c_int, [vp, C.c_uint64, C.c_uint64]),
             "oracle_get_step": (C.c_uint64, [vp]),
             "oracle_set_step": (None, [vp, C.c_uint64]),
             "oracle_cell_index": (C.c_uint64, [vp, C.c_float, C.c_float, C.c_float]),
@@ -156,6 +157,10 @@ class Oracle:
         x, y, z = (np.ascontiguousarray(v, dtype=np.float32) for v in (x, y, z))
         assert x.size == y.size == z.size == self.B
         lib().oracle_load_state(self._h, _p(x, C.c_float), _p(y, C.c_float), _p(z, C.c_float), int(step0))
+
+    def generate_state(self, gen_seed: int, step0: int = 0):
+        """Gaussian random-walk initial state by the recipe of DESIGN.md R22, then bin + omega."""
+        lib().oracle_generate_state(self._h, int(gen_seed), int(step0))
 
     def mc_steps(self, n: int) -> int:
         return int(lib().oracle_mc_steps(self._h, int(n)))

@@ -392,6 +392,44 @@ void oracle_set_external_field(void* h, const float* ext) {
   if (ext) o.ext.assign(ext, ext + (size_t)o.T * o.C); else o.ext.clear();
   if (o.loaded) compute_omega(o);
 }
+// Initial state on the device's recipe ("generating bead
+// coordinates"; R22, the configs' "Gaussian random-walk chains, bond components ~N(0, b^2/3),
+// first bead uniform in the box"): for chain c, bead i draw (w0..w3) = Philox4x32-10(counter =
+// (i, c, 0, 1 << 8), key = gen_seed)  -- domain 1, so no draw collides with a Monte-Carlo move's --
+// and U(w) = (w + 0.5) 2^-32 in double.  Bead 0: r_d = box_d * U(w_d).  Bead i >= 1: Box-Muller,
+// g0 = sqrt(-2 ln U(w0)) cos(2 pi U(w1)), g1 = the same with sin, g2 = sqrt(-2 ln U(w2)) cos(2 pi U(w3));
+// r_d(i) = r_d(i-1) + (b / sqrt 3) g_d, accumulated in double; every stored coordinate is the double
+// rounded once to fp32.  Then DESIGN.md section 2 step 4 with these positions.
+int oracle_generate_state(void* h, uint64_t gen_seed, uint64_t step0) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const uint32_t key[2] = {(uint32_t)gen_seed, (uint32_t)(gen_seed >> 32)};
+  const double sigma = (double)o.b / std::sqrt(3.0), two_pi = 6.283185307179586;
+  auto U = [](uint32_t w) { return ((double)w + 0.5) * 0x1p-32; };
+  for (uint64_t c = 0; c < o.n_chains; ++c) {
+    double r[3] = {0.0, 0.0, 0.0};
+    for (uint32_t i = 0; i < o.N; ++i) {
+      const uint32_t ctr[4] = {i, (uint32_t)c, 0u, 1u << 8};
+      uint32_t w[4];
+      philox4x32_10(ctr, key, w);
+      if (i == 0) {
+        for (int d = 0; d < 3; ++d) r[d] = (double)o.box[d] * U(w[d]);
+      } else {
+        const double ra = std::sqrt(-2.0 * std::log(U(w[0]))), rb = std::sqrt(-2.0 * std::log(U(w[2])));
+        r[0] += sigma * (ra * std::cos(two_pi * U(w[1])));
+        r[1] += sigma * (ra * std::sin(two_pi * U(w[1])));
+        r[2] += sigma * (rb * std::cos(two_pi * U(w[3])));
+      }
+      const uint64_t j = c * o.N + i;
+      o.x[j] = (float)r[0]; o.y[j] = (float)r[1]; o.z[j] = (float)r[2];
+    }
+  }
+  o.t = step0;
+  bin(o);
+  compute_omega(o);
+  o.loaded = true;
+  return 0;
+}
+
 void oracle_set_step(void* h, uint64_t t) { static_cast<Oracle*>(h)->t = t; }
 
 uint64_t oracle_cell_index(void* h, float x, float y, float z) {
