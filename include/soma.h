@@ -92,6 +92,19 @@ int soma_create(const soma_params *p, void *cuda_stream, soma_t **out);
 int soma_load_state(soma_t *h, const float *x, const float *y, const float *z, uint64_t step0,
                     int ptrs_are_device);
 
+/* Generate the initial state on the device instead of loading one (
+ * the paper moved "generating bead coordinates" to the GPU; reading R22):
+ * Gaussian random-walk chains as BASELINE.json `configs` describe them -- first bead uniform in the
+ * box, bond components N(0, b^2/3), unwrapped.  Draws: Philox4x32-10, key = gen_seed, counter =
+ * (bead, chain, 0, 1 << 8) (domain 1: disjoint from the Monte-Carlo stream whatever the seeds);
+ * U(w) = (w + 0.5) 2^-32; bead 0 at box_d * U(w_d); bead i >= 1 at the previous bead plus
+ * (b / sqrt 3) * (Box-Muller pair of (w0, w1), first of the pair of (w2, w3)), accumulated in double,
+ * each coordinate rounded once to fp32.  Then exactly what soma_load_state does with those positions
+ * (absolute step = step0, densities, omega).  Double-precision log/sin/cos differ in the last bit
+ * between math libraries, so two implementations agree to 1 fp32 ulp on a ~1e-8 fraction of the
+ * coordinates and bit for bit on the rest.  Errors: SOMA_EINVAL (step0 >= 2^48), SOMA_ECUDA. */
+int soma_generate_state(soma_t *h, uint64_t gen_seed, uint64_t step0);
+
 /* DESIGN.md section 2 step 6, `n_steps` times: half-sweep(even), half-sweep(odd), bin, omega,
  * step += 1.  `accepted` (host pointer, may be NULL) receives the number of accepted moves of this
  * call; passing it synchronises the stream, passing NULL keeps the call asynchronous.

@@ -26,7 +26,7 @@ LIB_PATH: Path = _build.LIB_PATH
 # every symbol include/soma.h declares (tests check the library exports exactly these)
 EXPORTS = (
     "soma_workspace_bytes", "soma_create", "soma_load_state", "soma_mc_steps", "soma_get_density",
-    "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_get_step", "soma_destroy", "soma_last_error",
+    "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_generate_state", "soma_get_step", "soma_destroy", "soma_last_error",
     "soma_set_option", "soma_get_counters", "soma_get_kernel_times", "soma_debug_half_sweep", "soma_debug_finish_step",
     "soma_debug_set_omega", "soma_debug_philox", "soma_debug_maps", "soma_debug_accept",
     "soma_debug_cell_index",
@@ -86,6 +86,7 @@ def load_library() -> C.CDLL:
             "soma_get_positions": (i32, [vp, vp, vp, vp, i32]),
             "soma_get_omega": (i32, [vp, vp, i32]),
             "soma_set_external_field": (i32, [vp, vp, i32]),
+            "soma_generate_state": (i32, [vp, u64, u64]),
             "soma_get_step": (i32, [vp, C.POINTER(u64)]),
             "soma_destroy": (i32, [vp]),
             "soma_last_error": (C.c_char_p, [vp]),
@@ -191,6 +192,10 @@ def soma_set_external_field(h, ext):
     if isinstance(ext, np.ndarray):
         ext = np.ascontiguousarray(ext, dtype=np.float32)
     _check(load_library().soma_set_external_field(h, _ptr(ext), _is_device(ext)), h)
+
+
+def soma_generate_state(h, gen_seed: int, step0: int = 0):
+    _check(load_library().soma_generate_state(h, int(gen_seed), int(step0)), h)
 
 
 def soma_get_step(h) -> int:
@@ -320,6 +325,9 @@ class Soma:
 
     def load_state(self, x, y, z, step0: int = 0):
         soma_load_state(self._h, x, y, z, step0)
+
+    def generate_state(self, gen_seed: int, step0: int = 0):
+        soma_generate_state(self._h, gen_seed, step0)
 
     def mc_steps(self, n: int, want_accepted: bool = False):
         return soma_mc_steps(self._h, n, want_accepted)

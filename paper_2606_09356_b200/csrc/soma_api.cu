@@ -151,7 +151,7 @@ struct soma_handle {
   uint32_t N, T, n_patterns, cells;
   Grid grid;
   bool pow2;
-  float a, kb, dens_scale, invN, kappaN;
+  float a, kb, dens_scale, invN, kappaN, b, box[3];
   float chiN[kMaxTypes * kMaxTypes];
   uint64_t seed;
   // device
@@ -744,6 +744,8 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->grid.inv_hz = (float)p->grid[2] / p->box[2];
   h->pow2 = is_pow2(p->grid[0]) && is_pow2(p->grid[1]) && is_pow2(p->grid[2]);
   h->a = p->move_halfwidth;
+  h->b = p->b;
+  for (int d = 0; d < 3; ++d) h->box[d] = p->box[d];
   h->kb = 1.5f / (p->b * p->b);
   h->dens_scale = (float)((double)h->cells / (double)h->B);
   h->invN = 1.0f / (float)h->N;
@@ -815,16 +817,10 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   return SOMA_OK;
 }
 
-int soma_load_state(soma_t* h, const float* x, const float* y, const float* z, uint64_t step0, int dev) {
-  int rc = check(h);
-  if (rc != SOMA_OK) return rc;
-  if (!x || !y || !z) return fail(h, SOMA_EINVAL, "position pointer is NULL");
-  if (step0 >= (1ull << 48)) return fail(h, SOMA_EINVAL, "step0 must be < 2^48");
-  const cudaMemcpyKind kind = dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-  h->live = 0;
-  h->loaded = false;
-  const float* src[3] = {x, y, z};
-  for (int d = 0; d < 3; ++d) CU(h, cudaMemcpyAsync(h->pos(0, d), src[d], h->B * 4, kind, h->stream));
+namespace {
+// DESIGN.md section 2 step 4 for positions already in set 0: slot tables, bin(), omega(), range check, re-ordering
+int finish_load(soma_handle* h, uint64_t step0) {
+  int rc;
   // slot s holds chain s again
   iota_kernel<<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>((uint32_t)h->n_chains, h->slot_chain(0));
   h->launches++;
@@ -845,6 +841,38 @@ int soma_load_state(soma_t* h, const float* x, const float* y, const float* z, u
     if ((rc = resort(h, use_tile(h) ? 2 : 1)) != SOMA_OK) return rc;
   h->loaded = true;
   return SOMA_OK;
+}
+}  // namespace
+
+int soma_load_state(soma_t* h, const float* x, const float* y, const float* z, uint64_t step0, int dev) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!x || !y || !z) return fail(h, SOMA_EINVAL, "position pointer is NULL");
+  if (step0 >= (1ull << 48)) return fail(h, SOMA_EINVAL, "step0 must be < 2^48");
+  const cudaMemcpyKind kind = dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  h->live = 0;
+  h->loaded = false;
+  const float* src[3] = {x, y, z};
+  for (int d = 0; d < 3; ++d) CU(h, cudaMemcpyAsync(h->pos(0, d), src[d], h->B * 4, kind, h->stream));
+  return finish_load(h, step0);
+}
+
+int soma_generate_state(soma_t* h, uint64_t gen_seed, uint64_t step0) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (step0 >= (1ull << 48)) return fail(h, SOMA_EINVAL, "step0 must be < 2^48");
+  h->live = 0;
+  h->loaded = false;
+  GenArgs G{};
+  G.n_chains = (uint32_t)h->n_chains; G.N = h->N;
+  G.k0 = (uint32_t)gen_seed; G.k1 = (uint32_t)(gen_seed >> 32);
+  for (int d = 0; d < 3; ++d) G.box[d] = (double)h->box[d];
+  G.sigma = (double)h->b / std::sqrt(3.0);
+  G.x = h->pos(0, 0); G.y = h->pos(0, 1); G.z = h->pos(0, 2);
+  generate_state_kernel<<<blocks_for(h->n_chains, 128), 128, 0, h->stream>>>(G);
+  h->launches++;
+  CU(h, cudaGetLastError());
+  return finish_load(h, step0);
 }
 
 int soma_mc_steps(soma_t* h, uint32_t n_steps, uint64_t* accepted) {

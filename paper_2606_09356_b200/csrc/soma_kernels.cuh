@@ -437,6 +437,43 @@ range_check_kernel(Grid grid, uint64_t B, const float* __restrict__ x, const flo
   if (!(m < kCellCoordLimit)) *range_flag = 1u;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Initial state on the device (R22): Gaussian random-walk
+// chains, first bead uniform in the box.  One thread per chain; draws keyed by (bead, chain) in
+// Philox domain 1; double-precision Box-Muller and accumulation, one rounding to fp32 per coordinate.
+// ---------------------------------------------------------------------------------------------
+struct GenArgs {
+  uint32_t n_chains, N;
+  uint32_t k0, k1;                 // generator seed, low and high word
+  double box[3];
+  double sigma;                    // b / sqrt(3)
+  float* __restrict__ x; float* __restrict__ y; float* __restrict__ z;
+};
+
+__device__ __forceinline__ double unit_open(uint32_t w) { return ((double)w + 0.5) * 0x1p-32; }
+
+__global__ void __launch_bounds__(128)
+generate_state_kernel(GenArgs G) {
+  const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= G.n_chains) return;
+  const double two_pi = 6.283185307179586;
+  double r0 = 0.0, r1 = 0.0, r2 = 0.0;
+  const uint64_t j0 = (uint64_t)c * G.N;
+  for (uint32_t i = 0; i < G.N; ++i) {
+    const Words4 w = philox4x32_10(i, c, 0u, 1u << 8, G.k0, G.k1);
+    if (i == 0) {
+      r0 = G.box[0] * unit_open(w.w0); r1 = G.box[1] * unit_open(w.w1); r2 = G.box[2] * unit_open(w.w2);
+    } else {
+      const double ra = sqrt(-2.0 * log(unit_open(w.w0))), rb = sqrt(-2.0 * log(unit_open(w.w2)));
+      const double t1 = two_pi * unit_open(w.w1), t3 = two_pi * unit_open(w.w3);
+      r0 = __dadd_rn(r0, __dmul_rn(G.sigma, __dmul_rn(ra, cos(t1))));
+      r1 = __dadd_rn(r1, __dmul_rn(G.sigma, __dmul_rn(ra, sin(t1))));
+      r2 = __dadd_rn(r2, __dmul_rn(G.sigma, __dmul_rn(rb, cos(t3))));
+    }
+    G.x[j0 + i] = (float)r0; G.y[j0 + i] = (float)r1; G.z[j0 + i] = (float)r2;
+  }
+}
+
 // ---- data movement helpers ----
 // dst[slot_chain[s]*N + i] = src[s*N + i]  (slot order -> caller's chain order), one thread per bead
 __global__ void __launch_bounds__(256)
