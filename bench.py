@@ -31,8 +31,8 @@ if ROOT not in sys.path:
 import numpy as np
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one fused_step_kernel launch on cfg4, from the committed
-# ncu --set full capture profiles/r1_ncu_cfg4_fused_final.txt (1.777933 + 1.627542 GB)
-NCU_TRAFFIC_CFG4_FUSED = 3.405475e9
+# ncu --set full capture profiles/r1_ncu_cfg4_fused_final.txt (1.773020 + 1.625843 GB)
+NCU_TRAFFIC_CFG4_FUSED = 3.398863e9
 
 METRIC = "attempted bead moves/s"
 UNIT = "moves/s"
@@ -307,8 +307,8 @@ def run_ours(args):
                 "bytes_per_move": ab["step"] / B}
     if path_now == 2 and args.config == 4:
         # not measured live: from the committed ncu capture of this kernel (profiles/r1_ncu_cfg4_fused_final.txt)
-        roofline["limiter"] = {"unit": "L2 (LTS) sector throughput", "l2_sectors_per_launch": 401.06e6,
-                               "achieved_bytes_per_cycle": 5993, "cap_bytes_per_cycle": 6300,
+        roofline["limiter"] = {"unit": "L2 (LTS) sector throughput", "l2_sectors_per_launch": 397.29e6,
+                               "achieved_bytes_per_cycle": 5980, "cap_bytes_per_cycle": 6300,
                                "cap_source": "B300_MICROARCH.md 'LTS throughput cap ~6300 B/cyc full-chip'",
                                "note": "DRAM traffic equals the algorithmic bytes (x1.015); the kernel sits at 95 % of the L2 sector cap"}
 
