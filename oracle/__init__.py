@@ -77,6 +77,7 @@ def lib() -> C.CDLL:
             "oracle_set_omega": (None, [vp, f32p]),
             "oracle_set_external_field": (None, [vp, f32p]),
             "oracle_generate_state": (C.c_int, [vp, C.c_uint64, C.c_uint64]),
+            "oracle_validate": (None, [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]),
             "oracle_get_step": (C.c_uint64, [vp]),
             "oracle_set_step": (None, [vp, C.c_uint64]),
             "oracle_cell_index": (C.c_uint64, [vp, C.c_float, C.c_float, C.c_float]),
@@ -161,6 +162,14 @@ class Oracle:
     def generate_state(self, gen_seed: int, step0: int = 0):
         """Gaussian random-walk initial state by the recipe of DESIGN.md R22, then bin + omega."""
         lib().oracle_generate_state(self._h, int(gen_seed), int(step0))
+
+    def validate(self) -> dict:
+        """Non-finite coordinates, density totals, largest and mean squared bond length of the state."""
+        out = (C.c_uint64 * 10)()
+        bond = (C.c_double * 2)()
+        lib().oracle_validate(self._h, out, bond)
+        return {"nonfinite": int(out[0]), "density_total": int(out[1]), "density_per_type": [int(out[2 + t]) for t in range(self.T)],
+                "max_bond_sq": float(bond[0]), "mean_bond_sq": float(bond[1])}
 
     def mc_steps(self, n: int) -> int:
         return int(lib().oracle_mc_steps(self._h, int(n)))

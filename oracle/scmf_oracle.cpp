@@ -430,6 +430,35 @@ int oracle_generate_state(void* h, uint64_t gen_seed, uint64_t step0) {
   return 0;
 }
 
+// Validation of a state (the paper's "validation functions"):
+// out[0] = coordinates that are NaN or infinite; out[1] = total of the density grids;
+// out[2 + t] = beads of type t in the grids (t < 8); bond[0] = largest squared bond length (fp32, the
+// pinned operation order of step 5.4), bond[1] = mean squared bond length (accumulated in double).
+void oracle_validate(void* h, uint64_t* out, double* bond) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  uint64_t bad = 0;
+  for (uint64_t j = 0; j < o.B; ++j)
+    bad += (std::isfinite(o.x[j]) ? 0 : 1) + (std::isfinite(o.y[j]) ? 0 : 1) + (std::isfinite(o.z[j]) ? 0 : 1);
+  out[0] = bad;
+  out[1] = 0;
+  for (uint32_t t = 0; t < 8; ++t) out[2 + t] = 0;
+  for (uint32_t t = 0; t < o.T; ++t)
+    for (uint64_t c = 0; c < o.C; ++c) { out[2 + t] += o.counts[(size_t)t * o.C + c]; out[1] += o.counts[(size_t)t * o.C + c]; }
+  float qmax = 0.0f;
+  double qsum = 0.0;
+  uint64_t nb = 0;
+  for (uint64_t c = 0; c < o.n_chains; ++c)
+    for (uint32_t i = 0; i + 1 < o.N; ++i) {
+      const uint64_t j = c * o.N + i;
+      const float q = bond_sq(o.x[j], o.y[j], o.z[j], o.x[j + 1], o.y[j + 1], o.z[j + 1]);
+      if (q > qmax) qmax = q;
+      qsum += (double)q;
+      ++nb;
+    }
+  bond[0] = (double)qmax;
+  bond[1] = nb ? qsum / (double)nb : 0.0;
+}
+
 void oracle_set_step(void* h, uint64_t t) { static_cast<Oracle*>(h)->t = t; }
 
 uint64_t oracle_cell_index(void* h, float x, float y, float z) {

@@ -56,3 +56,27 @@ def test_generated_state_is_deterministic_keyed_and_off_the_move_stream():
     w_mc = oracle.philox4x32_10([0, 0, 0, 0], [7, 0])
     assert not np.array_equal(w_gen, w_mc)
     assert x[0, 0] == np.float32(8.0 * ((float(w_gen[0]) + 0.5) * 2.0 ** -32))
+
+
+def test_validate_reports_what_it_should():
+    """Pins of the validation report: hand-made states with known answers."""
+    s = si.custom_system(3, 4, 2, [[0, 0, 1, 1]], None, [[0, 5], [5, 0]], 10.0, (4, 4, 4), (2.0, 2.0, 2.0), seed=3)
+    o = oracle.Oracle.from_system(s)
+    x = np.array([0, 1, 1, 1,   0, 0, 0, 0,   0.5, 0.5, 0.5, 2.5], dtype=np.float32)   # bonds: 1,0,0 | 0,0,0 | 0,0,2
+    y = np.zeros(12, dtype=np.float32)
+    z = np.zeros(12, dtype=np.float32)
+    y[7] = 1.5                                                                          # chain 1: last bond = 1.5
+    o.load_state(x, y, z)
+    v = o.validate()
+    assert v["nonfinite"] == 0 and v["density_total"] == 12 and v["density_per_type"] == [6, 6]
+    assert v["max_bond_sq"] == 4.0
+    assert v["mean_bond_sq"] == pytest_approx((1.0 + 2.25 + 4.0) / 9.0)
+    x[5] = np.nan
+    z[0] = np.inf
+    o.set_beads([5, 0], x[[5, 0]], y[[5, 0]], z[[5, 0]])
+    assert o.validate()["nonfinite"] == 2
+
+
+def pytest_approx(v):
+    import pytest
+    return pytest.approx(v, rel=1e-12)
