@@ -105,6 +105,19 @@ int soma_load_state(soma_t *h, const float *x, const float *y, const float *z, u
  * coordinates and bit for bit on the rest.  Errors: SOMA_EINVAL (step0 >= 2^48), SOMA_ECUDA. */
 int soma_generate_state(soma_t *h, uint64_t gen_seed, uint64_t step0);
 
+/* Validation report of the current state (the paper's "validation functions", moved to the GPU
+ * together with the generation of the coordinates): computed on the device in one
+ * pass over the positions and one over the density grids; synchronises the stream. */
+typedef struct soma_validation {
+  uint64_t n_nonfinite;           /* coordinates that are NaN or infinite                          */
+  uint64_t density_total;         /* sum of all density grids; must equal B                        */
+  uint64_t density_per_type[8];   /* beads of each type in the grids                               */
+  float    max_bond_sq;           /* largest squared bond length (fp32, operation order of step 5.4) */
+  uint32_t ok;                    /* 1 iff n_nonfinite == 0 and density_total == B                 */
+  double   mean_bond_sq;          /* mean squared bond length, accumulated in double (0 if N == 1); b^2 at equilibrium */
+} soma_validation;
+int soma_validate_state(soma_t *h, soma_validation *out);
+
 /* DESIGN.md section 2 step 6, `n_steps` times: half-sweep(even), half-sweep(odd), bin, omega,
  * step += 1.  `accepted` (host pointer, may be NULL) receives the number of accepted moves of this
  * call; passing it synchronises the stream, passing NULL keeps the call asynchronous.

@@ -26,7 +26,7 @@ LIB_PATH: Path = _build.LIB_PATH
 # every symbol include/soma.h declares (tests check the library exports exactly these)
 EXPORTS = (
     "soma_workspace_bytes", "soma_create", "soma_load_state", "soma_mc_steps", "soma_get_density",
-    "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_generate_state", "soma_get_step", "soma_destroy", "soma_last_error",
+    "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_generate_state", "soma_validate_state", "soma_get_step", "soma_destroy", "soma_last_error",
     "soma_set_option", "soma_get_counters", "soma_get_kernel_times", "soma_debug_half_sweep", "soma_debug_finish_step",
     "soma_debug_set_omega", "soma_debug_philox", "soma_debug_maps", "soma_debug_accept",
     "soma_debug_cell_index",
@@ -64,6 +64,12 @@ class soma_params(C.Structure):
     ]
 
 
+class soma_validation(C.Structure):
+    """Mirror of `struct soma_validation` in include/soma.h."""
+    _fields_ = [("n_nonfinite", C.c_uint64), ("density_total", C.c_uint64), ("density_per_type", C.c_uint64 * 8),
+                ("max_bond_sq", C.c_float), ("ok", C.c_uint32), ("mean_bond_sq", C.c_double)]
+
+
 _lib: Optional[C.CDLL] = None
 
 
@@ -87,6 +93,7 @@ def load_library() -> C.CDLL:
             "soma_get_omega": (i32, [vp, vp, i32]),
             "soma_set_external_field": (i32, [vp, vp, i32]),
             "soma_generate_state": (i32, [vp, u64, u64]),
+            "soma_validate_state": (i32, [vp, C.POINTER(soma_validation)]),
             "soma_get_step": (i32, [vp, C.POINTER(u64)]),
             "soma_destroy": (i32, [vp]),
             "soma_last_error": (C.c_char_p, [vp]),
@@ -196,6 +203,14 @@ def soma_set_external_field(h, ext):
 
 def soma_generate_state(h, gen_seed: int, step0: int = 0):
     _check(load_library().soma_generate_state(h, int(gen_seed), int(step0)), h)
+
+
+def soma_validate_state(h) -> dict:
+    v = soma_validation()
+    _check(load_library().soma_validate_state(h, C.byref(v)), h)
+    return {"nonfinite": int(v.n_nonfinite), "density_total": int(v.density_total),
+            "density_per_type": [int(t) for t in v.density_per_type], "max_bond_sq": float(v.max_bond_sq),
+            "mean_bond_sq": float(v.mean_bond_sq), "ok": bool(v.ok)}
 
 
 def soma_get_step(h) -> int:
@@ -328,6 +343,9 @@ class Soma:
 
     def generate_state(self, gen_seed: int, step0: int = 0):
         soma_generate_state(self._h, gen_seed, step0)
+
+    def validate(self) -> dict:
+        return soma_validate_state(self._h)
 
     def mc_steps(self, n: int, want_accepted: bool = False):
         return soma_mc_steps(self._h, n, want_accepted)

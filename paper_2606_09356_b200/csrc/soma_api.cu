@@ -32,6 +32,7 @@ struct Layout {            // byte offsets into the workspace
   uint64_t pattern0;       // [n] uint8: pattern id of every chain in the caller's order
   uint64_t accepted;       // uint64
   uint64_t range_flag;     // uint32
+  uint64_t validate;       // 11 x 8 bytes: report of soma_validate_state
   uint64_t sort_key;       // [n] uint32
   uint64_t sort_rank;      // [n] uint32
   uint64_t sort_bins;      // [2 n_bins_max + 2] uint32: bin counts, then bin starts (= tile_start)
@@ -85,6 +86,7 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   L.pattern0 = off; off += align_up(n);
   L.accepted = off; off += align_up(8);
   L.range_flag = off; off += align_up(4);
+  L.validate = off; off += align_up(88);
   L.sort_key = off; off += align_up(n * 4);
   L.sort_rank = off; off += align_up(n * 4);
   L.sort_bins = off; off += align_up(n_bins * 4);
@@ -952,6 +954,36 @@ int soma_set_external_field(soma_t* h, const float* ext, int dev) {
     h->omega_custom = false;
     if ((rc = launch_omega(h)) != SOMA_OK) return rc;
   }
+  return SOMA_OK;
+}
+
+int soma_validate_state(soma_t* h, soma_validation* out) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!out) return fail(h, SOMA_EINVAL, "out is NULL");
+  if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
+  unsigned long long* report = reinterpret_cast<unsigned long long*>(h->ws + h->L.validate);
+  double* bond_sum = reinterpret_cast<double*>(report + 10);
+  CU(h, cudaMemsetAsync(report, 0, 11 * 8, h->stream));
+  validate_positions_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
+      h->B, h->N, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2), report, bond_sum);
+  const unsigned gx = blocks_for(h->cells, 256) < 1024u ? blocks_for(h->cells, 256) : 1024u;
+  validate_density_kernel<<<dim3(gx, h->T), 256, 0, h->stream>>>(h->cells, h->T, h->counts(h->cur), report);
+  h->launches += 2;
+  CU(h, cudaGetLastError());
+  unsigned long long host[11];
+  CU(h, cudaMemcpyAsync(host, report, sizeof host, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  std::memset(out, 0, sizeof *out);
+  out->n_nonfinite = host[0];
+  for (uint32_t t = 0; t < h->T; ++t) { out->density_per_type[t] = host[1 + t]; out->density_total += host[1 + t]; }
+  const uint32_t qbits = (uint32_t)host[9];
+  std::memcpy(&out->max_bond_sq, &qbits, 4);
+  double sum;
+  std::memcpy(&sum, &host[10], 8);
+  const uint64_t n_bonds = h->n_chains * (uint64_t)(h->N - 1);
+  out->mean_bond_sq = n_bonds ? sum / (double)n_bonds : 0.0;
+  out->ok = (out->n_nonfinite == 0 && out->density_total == h->B) ? 1u : 0u;
   return SOMA_OK;
 }
 

@@ -474,6 +474,48 @@ generate_state_kernel(GenArgs G) {
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Validation of the current state (the paper's "validation functions").
+// report[0] = non-finite coordinates, report[1 + t] = beads of type t in the density grids,
+// report[9] = bit pattern of the largest squared bond length, bond_sum = sum of squared bond lengths.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+validate_positions_kernel(uint64_t B, uint32_t N, const float* __restrict__ x, const float* __restrict__ y,
+                          const float* __restrict__ z, unsigned long long* __restrict__ report, double* __restrict__ bond_sum) {
+  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned bad = 0;
+  float q = 0.0f;
+  if (j < B) {
+    const float px = x[j], py = y[j], pz = z[j];
+    bad = (isfinite(px) ? 0u : 1u) + (isfinite(py) ? 0u : 1u) + (isfinite(pz) ? 0u : 1u);
+    if ((uint32_t)(j % N) + 1u < N) q = bond_sq(px, py, pz, x[j + 1], y[j + 1], z[j + 1]);   // bond (i, i+1) of the same chain
+  }
+  // NaN never wins a maximum taken on bit patterns of non-negative floats; it is counted in `bad`
+  float qm = q == q ? q : 0.0f;
+  double qs = q == q ? (double)q : 0.0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    qm = fmaxf(qm, __shfl_xor_sync(0xffffffffu, qm, o));
+    qs += __shfl_xor_sync(0xffffffffu, qs, o);
+  }
+  if ((threadIdx.x & 31u) == 0) {
+    if (bad) atomicAdd(report, (unsigned long long)bad);
+    atomicMax(report + 9, (unsigned long long)__float_as_uint(qm));
+    atomicAdd(bond_sum, qs);
+  }
+}
+
+__global__ void __launch_bounds__(256)
+validate_density_kernel(uint32_t cells, uint32_t T, const uint32_t* __restrict__ counts, unsigned long long* __restrict__ report) {
+  const uint32_t t = blockIdx.y;
+  unsigned long long sum = 0;
+  for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < cells; c += gridDim.x * blockDim.x) sum += counts[(size_t)t * cells + c];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+  if ((threadIdx.x & 31u) == 0 && sum) atomicAdd(report + 1 + t, sum);
+}
+
 // ---- data movement helpers ----
 // dst[slot_chain[s]*N + i] = src[s*N + i]  (slot order -> caller's chain order), one thread per bead
 __global__ void __launch_bounds__(256)

@@ -68,3 +68,30 @@ def test_generate_full_size_cfg4_statistics_and_speed():
         assert abs((d * d).mean() - b * b / 3) < 4 * math.sqrt(2.0 / d.size) * b * b / 3
     print(f"soma_generate_state, cfg4: {dt * 1e3:.1f} ms incl. binning, omega and the chain re-ordering")
     assert dt < 1.0
+
+
+@pytest.mark.parametrize("cfg,n,grid", [(4, 20000, (32, 32, 16)), (3, 5001, (32, 16, 16))])
+def test_validate_state_matches_the_oracle(cfg, n, grid):
+    s = si.make_system(si.scaled(si.config(cfg), n, grid))
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s) as g:
+        g.load_state(s.x, s.y, s.z)
+        for steps in (0, 3):
+            if steps:
+                g.mc_steps(steps)
+                o.mc_steps(steps)
+            vg, vo = g.validate(), o.validate()
+            assert vg["ok"] and vg["nonfinite"] == vo["nonfinite"] == 0
+            assert vg["density_total"] == vo["density_total"] == s.workload.n_beads
+            assert vg["density_per_type"][: s.workload.n_types] == vo["density_per_type"]
+            assert vg["max_bond_sq"] == np.float32(vo["max_bond_sq"])                    # fp32 maximum: exact
+            assert vg["mean_bond_sq"] == pytest.approx(vo["mean_bond_sq"], rel=1e-12)   # double sums in another order
+
+
+def test_validate_single_bead_molecules_have_no_bonds():
+    s = si.custom_system(5000, 1, 1, [[0]], None, [[0.0]], 0.0, (8, 8, 8), (4.0, 4.0, 4.0), seed=79)
+    with gpu_system(s) as g:
+        g.load_state(s.x, s.y, s.z)
+        v = g.validate()
+    assert v["ok"] and v["density_total"] == 5000 and v["max_bond_sq"] == 0.0 and v["mean_bond_sq"] == 0.0
