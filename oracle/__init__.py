@@ -77,6 +77,7 @@ def lib() -> C.CDLL:
             "oracle_set_omega": (None, [vp, f32p]),
             "oracle_set_external_field": (None, [vp, f32p]),
             "oracle_generate_state": (C.c_int, [vp, C.c_uint64, C.c_uint64]),
+            "oracle_set_singles": (C.c_int, [vp, C.POINTER(C.c_uint64)]),
             "oracle_validate": (None, [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]),
             "oracle_get_step": (C.c_uint64, [vp]),
             "oracle_set_step": (None, [vp, C.c_uint64]),
@@ -123,7 +124,7 @@ class Oracle:
     """One SCMF system held by the CPU oracle."""
 
     def __init__(self, n_chains, N, n_types, type_patterns, chain_pattern, b, chiN, kappaN,
-                 grid, box, move_halfwidth, seed):
+                 grid, box, move_halfwidth, seed, n_single=None):
         self.n_chains, self.N, self.T = int(n_chains), int(N), int(n_types)
         self.B = self.n_chains * self.N
         self.grid = tuple(int(g) for g in grid)
@@ -139,13 +140,18 @@ class Oracle:
             float(kappaN), _p(g, C.c_uint32), _p(bx, C.c_float), float(move_halfwidth), int(seed))
         if not self._h:
             raise ValueError("oracle_create rejected the parameters")
+        if n_single is not None:                     # single-bead molecules per type, stored after the chains (R23)
+            ns = np.ascontiguousarray(n_single, dtype=np.uint64).reshape(self.T)
+            if lib().oracle_set_singles(self._h, _p(ns, C.c_uint64)) != 0:
+                raise ValueError("too many molecules")
+            self.B += int(ns.sum())
 
     @classmethod
     def from_system(cls, s) -> "Oracle":
         """`s` is a scmf_inputs.System (duck-typed; this package imports nothing of it)."""
         w = s.workload
         return cls(w.n_chains, w.N, w.n_types, s.type_patterns, s.chain_pattern, w.b, s.chiN,
-                   w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed)
+                   w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed, n_single=getattr(s, "n_single", None))
 
     def close(self):
         if getattr(self, "_h", None):

@@ -103,6 +103,10 @@ struct Oracle {
   std::vector<uint32_t> counts;         // [T][C], cell = (ix*ny+iy)*nz+iz (R12)
   std::vector<float> omega;             // [T][C]
   std::vector<float> ext;               // [T][C] external field (empty = none), R21
+  // single-bead molecules (R23): n_single[t] of type t, stored after the chains in x, y, z,
+  // type 0 first; molecule m has the logical chain id n_chains + m and bead index 0
+  std::vector<uint64_t> n_single;       // [T] (empty = none)
+  uint64_t S = 0;                       // their total
   uint64_t t;                           // absolute step index
   bool loaded;
 };
@@ -126,9 +130,19 @@ inline uint64_t cell_index(const Oracle& o, float rx, float ry, float rz) {
   return ((uint64_t)g[0] * o.grid[1] + (uint64_t)g[1]) * o.grid[2] + (uint64_t)g[2];
 }
 
+inline uint32_t single_type(const Oracle& o, uint64_t m) {
+  uint32_t t = 0;
+  while (m >= o.n_single[t]) { m -= o.n_single[t]; ++t; }
+  return t;
+}
+
 // DESIGN.md section 2 step 2 (NS part 2; R9 nearest-grid-point assignment): integer counts.
 void bin(Oracle& o) {
   std::fill(o.counts.begin(), o.counts.end(), 0u);
+  for (uint64_t m = 0; m < o.S; ++m) {
+    const uint64_t j = o.n_chains * o.N + m;
+    o.counts[(size_t)single_type(o, m) * o.C + cell_index(o, o.x[j], o.y[j], o.z[j])] += 1u;
+  }
   for (uint64_t c = 0; c < o.n_chains; ++c)
     for (uint32_t i = 0; i < o.N; ++i) {
       const uint64_t j = c * o.N + i;
@@ -240,6 +254,26 @@ inline int trial_move(Oracle& o, uint64_t c, uint32_t i, uint32_t parity, double
   return 0;
 }
 
+// The move of single-bead molecule m (R23): bead index 0 of logical chain n_chains + m, in
+// half-sweep 0; no bonds, so dE = fma(kb, 0, dw) = dw = omega_t(new cell) - omega_t(old cell).
+inline int trial_move_single(Oracle& o, uint64_t m, double* margin64) {
+  const uint32_t ctr[4] = {0u, (uint32_t)(o.n_chains + m), (uint32_t)o.t,
+                           0u | (RNG_DOMAIN_MOVE << 8) | ((uint32_t)(o.t >> 32) << 16)};
+  const uint32_t key[2] = {(uint32_t)o.seed, (uint32_t)(o.seed >> 32)};
+  uint32_t w[4];
+  philox4x32_10(ctr, key, w);
+  const uint64_t j = o.n_chains * o.N + m;
+  const float nx = o.x[j] + o.a * tmap(w[0]), ny = o.y[j] + o.a * tmap(w[1]), nz = o.z[j] + o.a * tmap(w[2]);
+  const float u = umap(w[3]);
+  const size_t tb = (size_t)single_type(o, m) * o.C;
+  const float w_new = o.omega[tb + cell_index(o, nx, ny, nz)], w_old = o.omega[tb + cell_index(o, o.x[j], o.y[j], o.z[j])];
+  const float dE = fmaf(o.kb, 0.0f, w_new - w_old);
+  const float mg = dE + lnu32(u);
+  if (margin64) *margin64 = ((double)w_new - (double)w_old) + std::log((double)u);
+  if (mg <= 0.0f) { o.x[j] = nx; o.y[j] = ny; o.z[j] = nz; return 1; }
+  return 0;
+}
+
 // order: 0 ascending, 1 descending, 2 = caller-supplied permutation of the same-parity bead list
 // (R5: same-parity beads of a linear chain share no bond and omega is frozen, so the
 // visiting order within a half-sweep is immaterial; tests check that bit for bit).
@@ -249,6 +283,13 @@ uint64_t half_sweep(Oracle& o, uint32_t parity, int order, const uint64_t* perm,
   if (order == 2) {
     for (uint64_t k = 0; k < n_perm; ++k) {
       const uint64_t j = perm[k];
+      if (j >= o.n_chains * o.N) {                       // a single-bead molecule: half-sweep 0 only
+        if (parity != 0) continue;
+        const int acc = trial_move_single(o, j - o.n_chains * o.N, margins ? &margins[j] : nullptr);
+        if (accept_mask) accept_mask[j] = (uint8_t)acc;
+        accepted += (uint64_t)acc;
+        continue;
+      }
       const uint64_t c = j / o.N;
       const uint32_t i = (uint32_t)(j % o.N);
       if ((i & 1u) != parity) continue;
@@ -270,6 +311,14 @@ uint64_t half_sweep(Oracle& o, uint32_t parity, int order, const uint64_t* perm,
       accepted += (uint64_t)acc;
     }
   }
+  if (parity == 0)
+    for (uint64_t mm = 0; mm < o.S; ++mm) {
+      const uint64_t m = order == 0 ? mm : o.S - 1 - mm;
+      const uint64_t j = o.n_chains * o.N + m;
+      const int acc = trial_move_single(o, m, margins ? &margins[j] : nullptr);
+      if (accept_mask) accept_mask[j] = (uint8_t)acc;
+      accepted += (uint64_t)acc;
+    }
   return accepted;
 }
 
@@ -386,6 +435,20 @@ void oracle_set_omega(void* h, const float* omega) {
   std::memcpy(o.omega.data(), omega, o.omega.size() * sizeof(float));
 }
 uint64_t oracle_get_step(void* h) { return static_cast<Oracle*>(h)->t; }
+// single-bead molecules: n_single[T] (call right after oracle_create, before any state is loaded)
+int oracle_set_singles(void* h, const uint64_t* n_single) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  o.n_single.assign(n_single, n_single + o.T);
+  o.S = 0;
+  for (uint32_t t = 0; t < o.T; ++t) o.S += o.n_single[t];
+  if (o.n_chains + o.S >= (1ull << 32)) return -1;
+  o.B = o.n_chains * o.N + o.S;
+  o.dens_scale = (float)((double)o.C / (double)o.B);
+  o.x.assign(o.B, 0.0f); o.y.assign(o.B, 0.0f); o.z.assign(o.B, 0.0f);
+  o.loaded = false;
+  return 0;
+}
+
 // external field [T][C] (nullptr = none); omega is recomputed from the current densities
 void oracle_set_external_field(void* h, const float* ext) {
   Oracle& o = *static_cast<Oracle*>(h);
@@ -422,6 +485,15 @@ int oracle_generate_state(void* h, uint64_t gen_seed, uint64_t step0) {
       const uint64_t j = c * o.N + i;
       o.x[j] = (float)r[0]; o.y[j] = (float)r[1]; o.z[j] = (float)r[2];
     }
+  }
+  for (uint64_t m = 0; m < o.S; ++m) {                 // single-bead molecules: the bead-0 rule with chain id n_chains + m
+    const uint32_t ctr[4] = {0u, (uint32_t)(o.n_chains + m), 0u, 1u << 8};
+    uint32_t w[4];
+    philox4x32_10(ctr, key, w);
+    const uint64_t j = o.n_chains * o.N + m;
+    o.x[j] = (float)((double)o.box[0] * U(w[0]));
+    o.y[j] = (float)((double)o.box[1] * U(w[1]));
+    o.z[j] = (float)((double)o.box[2] * U(w[2]));
   }
   o.t = step0;
   bin(o);

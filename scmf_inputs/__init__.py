@@ -66,6 +66,7 @@ class System:
     y: np.ndarray
     z: np.ndarray
     extra: dict = field(default_factory=dict)
+    n_single: Optional[np.ndarray] = None    # uint64 [T]: single-bead molecules per type, stored after the chains
 
     @property
     def n_patterns(self) -> int:
@@ -75,8 +76,12 @@ class System:
         """uint8 [n_chains*N] type of every bead (harness-side bookkeeping only)."""
         w = self.workload
         if self.chain_pattern is None:
-            return np.tile(self.type_patterns[0], w.n_chains)
-        return self.type_patterns[self.chain_pattern].reshape(-1)
+            t = np.tile(self.type_patterns[0], w.n_chains)
+        else:
+            t = self.type_patterns[self.chain_pattern].reshape(-1)
+        if self.n_single is not None:
+            t = np.concatenate([t, np.repeat(np.arange(w.n_types, dtype=np.uint8), self.n_single.astype(np.int64))])
+        return t
 
 
 # BASELINE.json configs[0..4]; cell size b/2 everywhere, so box = grid / 2.
@@ -152,7 +157,7 @@ def make_system(w: Workload, chunk_chains: int = 1 << 20) -> System:
 
 def custom_system(n_chains: int, N: int, n_types: int, type_patterns, chain_pattern, chiN,
                   kappaN: float, grid, box, seed: int, b: float = 1.0,
-                  move_halfwidth: float = 0.5, name: str = "custom") -> System:
+                  move_halfwidth: float = 0.5, name: str = "custom", n_single=None) -> System:
     """Arbitrary architecture (edge-case tests): explicit patterns and a full chiN matrix."""
     w = Workload(name, n_chains, N, n_types, "custom", tuple(int(g) for g in grid),
                  tuple(float(v) for v in box), 0.0, float(kappaN), seed=seed, steps=1, b=b,
@@ -164,7 +169,12 @@ def custom_system(n_chains: int, N: int, n_types: int, type_patterns, chain_patt
         steps = rng.standard_normal((n_chains, N)) * sigma
         steps[:, 0] = rng.random(n_chains) * box[d]
         out.append(np.cumsum(steps, axis=1).reshape(-1).astype(np.float32))
+    ns = None
+    if n_single is not None:                     # single-bead molecules: uniform in the box, appended after the chains
+        ns = np.ascontiguousarray(n_single, dtype=np.uint64).reshape(n_types)
+        for d in range(3):
+            out[d] = np.concatenate([out[d], (rng.random(int(ns.sum())) * box[d]).astype(np.float32)])
     pats = np.ascontiguousarray(np.asarray(type_patterns, dtype=np.uint8).reshape(-1, N))
     cp = None if chain_pattern is None else np.ascontiguousarray(chain_pattern, dtype=np.uint8)
     chi = np.ascontiguousarray(np.asarray(chiN, dtype=np.float32).reshape(n_types, n_types))
-    return System(w, pats, cp, chi, out[0], out[1], out[2])
+    return System(w, pats, cp, chi, out[0], out[1], out[2], n_single=ns)

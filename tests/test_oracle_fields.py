@@ -211,3 +211,67 @@ def test_external_field_adds_to_omega_in_fp32_and_can_be_removed():
     assert np.array_equal(o.omega().view(np.uint32), o2.omega().view(np.uint32))
     o.set_external_field(np.zeros_like(ext))                     # a zero field changes nothing, bit for bit
     assert np.array_equal(o.omega().view(np.uint32), o2.omega().view(np.uint32))
+
+
+# ---- single-bead molecules next to chains (R23) --------------------
+
+def _mixture(n_chains=300, n_single=(500, 0, 1200), seed=21, chi=None, kappaN=0.0, grid=(4, 4, 4), box=(2.0, 2.0, 2.0)):
+    chi = np.zeros((3, 3)) if chi is None else chi
+    return si.custom_system(n_chains, 8, 3, [[0, 0, 0, 0, 1, 1, 1, 1]], None, chi, kappaN, grid, box, seed=seed, n_single=n_single)
+
+
+def test_single_bead_molecules_are_counted_by_type_and_normalise_the_density():
+    s = _mixture()
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    d = o.density()
+    assert d[0].sum() == 300 * 4 + 500 and d[1].sum() == 300 * 4 and d[2].sum() == 1200
+    B = 300 * 8 + 1700
+    assert o.constants()["dens_scale"] == np.float32(64 / B)              # phi normalised by ALL beads (R10)
+    # histogram of the returned positions, type by type
+    x, y, z = o.positions()
+    cells = [o.cell_index(a, b_, c) for a, b_, c in zip(x, y, z)]
+    types = s.bead_types()
+    for t in range(3):
+        assert np.array_equal(np.bincount(np.asarray(cells)[types == t], minlength=64), d[t])
+    o.mc_steps(3)
+    assert o.density().sum() == B
+
+
+def test_single_bead_molecules_follow_the_boltzmann_weights_of_their_own_field():
+    """Non-interacting mixture in an external field that differs by type: the solvent species (type 2)
+    equilibrates to exp(-ext_2), untouched by the chains and by the other species' field."""
+    from scipy import stats
+    s = _mixture(n_chains=50, n_single=(20000, 0, 150000), seed=22)
+    ext = np.random.default_rng(8).uniform(0.0, 1.5, size=(3, 64)).astype(np.float32)
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    o.set_external_field(ext)
+    o.mc_steps(120)
+    x, y, z = o.positions()
+    types = s.bead_types()
+    nN = 50 * 8
+    for t, n in ((0, 20000), (2, 150000)):
+        sel = np.flatnonzero(types == t)
+        sel = sel[sel >= nN]                                              # the single-bead molecules of that type
+        cells = np.array([o.cell_index(x[j], y[j], z[j]) for j in sel])
+        counts = np.bincount(cells, minlength=64).astype(np.float64)
+        p = np.exp(-ext[t].astype(np.float64)); p /= p.sum()
+        chi2 = float(((counts - n * p) ** 2 / (n * p)).sum())
+        assert chi2 < stats.chi2.ppf(1 - 1e-4, df=63), (t, chi2)
+
+
+def test_single_bead_moves_are_order_independent_and_use_their_own_stream():
+    s = _mixture(chi=np.array([[0, 8, 3], [8, 0, 5], [3, 5, 0.0]]), kappaN=20.0, seed=23)
+    a = oracle.Oracle.from_system(s); a.load_state(s.x, s.y, s.z)
+    b = oracle.Oracle.from_system(s); b.load_state(s.x, s.y, s.z)
+    a.half_sweep(0, order=0); b.half_sweep(0, order=1)
+    assert all(np.array_equal(u, v) for u, v in zip(a.positions(), b.positions()))
+    # molecule m draws the stream of (bead 0, chain n_chains + m): check one trial position by hand
+    c = oracle.Oracle.from_system(s); c.load_state(s.x, s.y, s.z)
+    j = 300 * 8 + 7
+    w = oracle.philox4x32_10([0, 300 + 7, 0, 0], [s.workload.seed & 0xffffffff, s.workload.seed >> 32])
+    want = np.float32(s.x[j]) + np.float32(0.5) * np.float32(oracle.tmap(int(w[0])))
+    c.set_omega(np.zeros((3, 64), np.float32))                            # dE = 0: every move is accepted
+    c.half_sweep(0)
+    assert c.positions()[0][j] == want
