@@ -73,6 +73,12 @@ typedef struct soma_params {
                                    256-byte aligned, must outlive the handle), or NULL = the
                                    library allocates with cudaMalloc                            */
   uint64_t workspace_bytes;     /* size of `workspace` (ignored when workspace == NULL)         */
+  const uint64_t *n_single;     /* host [T] or NULL: single-bead molecules of each type next to the
+                                   chains (solvent species, DESIGN.md
+                                   R23).  They are stored AFTER the chains in every position array
+                                   (type 0 first), so B = n_chains*N + sum(n_single); molecule m is
+                                   bead 0 of logical chain n_chains + m for the random stream, moves
+                                   in half-sweep 0 and has no bonds.  n_chains + sum < 2^32.     */
 } soma_params;
 
 /* Device bytes a handle for `p` needs (positions x2, grids, chain tables).  0 on invalid `p`. */

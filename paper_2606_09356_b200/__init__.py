@@ -61,6 +61,7 @@ class soma_params(C.Structure):
         ("seed", C.c_uint64),
         ("workspace", C.c_void_p),
         ("workspace_bytes", C.c_uint64),
+        ("n_single", C.c_void_p),
     ]
 
 
@@ -134,7 +135,7 @@ def _is_device(a) -> int:
 # ---- the C entry points, same names ------------------------------------------------------------
 
 def make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN, kappaN,
-                grid, box, move_halfwidth, seed):
+                grid, box, move_halfwidth, seed, n_single=None):
     """Build a soma_params plus the numpy arrays it points to (keep the tuple alive until create)."""
     pats = np.ascontiguousarray(type_patterns, dtype=np.uint8)
     n_patterns = 1 if pats.ndim < 2 else int(pats.shape[0])     # validation is the library's job
@@ -150,7 +151,9 @@ def make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern
     p.box = (C.c_float * 3)(*[float(v) for v in box])
     p.seed = int(seed)
     p.workspace, p.workspace_bytes = None, 0
-    return p, (pats, cp, chi)
+    ns = None if n_single is None else np.ascontiguousarray(n_single, dtype=np.uint64)
+    p.n_single = None if ns is None else ns.ctypes.data
+    return p, (pats, cp, chi, ns)
 
 
 def soma_workspace_bytes(p: soma_params) -> int:
@@ -292,16 +295,16 @@ class Soma:
     """One SCMF system on the current CUDA device.  Device memory and stream come from PyTorch."""
 
     def __init__(self, n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN,
-                 kappaN, grid, box, move_halfwidth, seed, stream=None, lend_workspace: bool = True):
+                 kappaN, grid, box, move_halfwidth, seed, stream=None, lend_workspace: bool = True, n_single=None):
         import torch
         if not torch.cuda.is_available():
             raise SomaError(SOMA_ECUDA, "no CUDA device: this package has no CPU fallback")
         self.n_chains, self.N, self.T = int(n_chains), int(beads_per_chain), int(n_types)
-        self.B = self.n_chains * self.N
+        self.B = self.n_chains * self.N + (0 if n_single is None else int(np.asarray(n_single, dtype=np.uint64).sum()))
         self.grid = tuple(int(g) for g in grid)
         self.cells = self.grid[0] * self.grid[1] * self.grid[2]
         p, keep = make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN,
-                              kappaN, grid, box, move_halfwidth, seed)
+                              kappaN, grid, box, move_halfwidth, seed, n_single=n_single)
         self._workspace = None
         if lend_workspace:
             nbytes = soma_workspace_bytes(p)
@@ -318,7 +321,7 @@ class Soma:
         """`s` is a scmf_inputs.System (duck-typed)."""
         w = s.workload
         return cls(w.n_chains, w.N, w.n_types, s.type_patterns, s.chain_pattern, w.b, s.chiN,
-                   w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed, **kw)
+                   w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed, n_single=getattr(s, "n_single", None), **kw)
 
     def close(self):
         if getattr(self, "_h", None):

@@ -26,6 +26,7 @@ struct Layout {            // byte offsets into the workspace
   uint64_t counts[2];      // [T][C] uint32, double-buffered
   uint64_t omega;          // [T][C] fp32
   uint64_t ext;            // [T][C] fp32 external field (used once soma_set_external_field has set one)
+  uint64_t single[3];      // [S] fp32 each: positions of the single-bead molecules (never re-ordered)
   uint64_t slot_chain[2];  // [n] uint32: logical chain id of every slot (second copy: re-order target)
   uint64_t slot_pattern[2];// [n] uint8
   uint64_t patterns;       // [n_patterns][N] uint8
@@ -72,7 +73,7 @@ bool tile_capable_grid(const uint32_t grid[3]) {      // power-of-two axes, at l
 }
 
 // n_bins: entries of the sort_bins array (see sort_bins_capacity)
-Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins, uint64_t pad_words) {
+Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins, uint64_t pad_words, uint64_t S) {
   Layout L{};
   uint64_t off = 0;
   for (int s = 0; s < 2; ++s)
@@ -80,6 +81,7 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   for (int s = 0; s < 2; ++s) { L.counts[s] = off; off += align_up(TC * 4); }
   L.omega = off; off += align_up(TC * 4);
   L.ext = off; off += align_up(TC * 4);
+  for (int d = 0; d < 3; ++d) { L.single[d] = off; off += align_up(S * 4); }
   for (int s = 0; s < 2; ++s) { L.slot_chain[s] = off; off += align_up(n * 4); }
   for (int s = 0; s < 2; ++s) { L.slot_pattern[s] = off; off += align_up(n); }
   L.patterns = off; off += align_up(pat_bytes);
@@ -121,6 +123,14 @@ const char* validate(const soma_params* p) {
     if (cells >= (1ull << 32)) return "too many cells";
   }
   if (cells * p->n_types >= (1ull << 32)) return "n_types * cells must be < 2^32";
+  if (p->n_single) {
+    uint64_t S = 0;
+    for (uint32_t t = 0; t < p->n_types; ++t) {
+      if (p->n_single[t] >= (1ull << 32)) return "n_single[t] must be < 2^32";
+      S += p->n_single[t];
+    }
+    if (p->n_chains + S >= (1ull << 32)) return "n_chains + single-bead molecules must be < 2^32";
+  }
   const uint64_t npat = (uint64_t)p->n_patterns * p->beads_per_chain;
   for (uint64_t k = 0; k < npat; ++k)
     if (p->type_patterns[k] >= p->n_types) return "type_patterns holds a type >= n_types";
@@ -149,7 +159,9 @@ int fused_lanes(uint32_t N) {   // P = N/2 if the fused kernel supports N, else 
 
 struct soma_handle {
   // problem
-  uint64_t n_chains, B;
+  uint64_t n_chains, B;          // B = n_chains * N: beads in chains
+  uint64_t S, Btot;              // single-bead molecules (R23) and all beads
+  uint32_t single_start[kMaxTypes + 1];
   uint32_t N, T, n_patterns, cells;
   Grid grid;
   bool pow2;
@@ -213,6 +225,7 @@ struct soma_handle {
   uint32_t* counts(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts[s]); }
   float* omega() const { return reinterpret_cast<float*>(ws + L.omega); }
   float* ext() const { return reinterpret_cast<float*>(ws + L.ext); }
+  float* single(int d) const { return reinterpret_cast<float*>(ws + L.single[d]); }
   uint32_t* slot_chain(int s) const { return reinterpret_cast<uint32_t*>(ws + L.slot_chain[s]); }
   uint8_t* slot_pattern(int s) const { return reinterpret_cast<uint8_t*>(ws + L.slot_pattern[s]); }
   uint32_t* slot_chain() const { return slot_chain(live); }
@@ -294,6 +307,26 @@ int launch_half_sweep(soma_handle* h, uint32_t parity) {
   return SOMA_OK;
 }
 
+// Single-bead molecules: trial moves (half-sweep 0) and / or binning into `counts` -- the linear grid,
+// or the ghost-padded grid the windowed kernels flush into (padded = true).
+int launch_singles(soma_handle* h, bool do_move, bool do_bin, uint32_t* counts, bool padded, bool check_range = false) {
+  if (h->S == 0) return SOMA_OK;
+  SingleArgs A{};
+  A.S = step_args(h);
+  A.n_total = (uint32_t)h->S; A.T = h->T;
+  for (int t = 0; t <= kMaxTypes; ++t) A.start[t] = h->single_start[t];
+  A.x = h->single(0); A.y = h->single(1); A.z = h->single(2);
+  A.counts = counts;
+  if (padded) { A.px = h->pad[0]; A.py = h->pad[1]; A.pz = h->pad[2]; A.hx = h->th[0]; A.hy = h->th[1]; A.hz = h->th[2]; }
+  A.range_flag = check_range ? h->range_flag() : nullptr;
+  A.do_move = do_move; A.do_bin = do_bin;
+  if (h->pow2) singles_kernel<true><<<blocks_for(h->S, 256), 256, 0, h->stream>>>(A);
+  else singles_kernel<false><<<blocks_for(h->S, 256), 256, 0, h->stream>>>(A);
+  h->launches++;
+  CU(h, cudaGetLastError());
+  return SOMA_OK;
+}
+
 int launch_bin(soma_handle* h, uint32_t* counts, bool check_range = false) {
   uint32_t* flag = check_range ? h->range_flag() : nullptr;
   if (h->pow2)
@@ -306,7 +339,7 @@ int launch_bin(soma_handle* h, uint32_t* counts, bool check_range = false) {
         h->slot_pattern(), h->patterns(), counts, flag);
   h->launches++;
   CU(h, cudaGetLastError());
-  return SOMA_OK;
+  return launch_singles(h, false, true, counts, false, check_range);
 }
 
 // omega from counts(cur); zero counts(cur^1) for the next step's binning.
@@ -665,12 +698,15 @@ int one_step(soma_handle* h) {
   if (timed) timing_mark(h);
   if (tiled) {
     if ((rc = launch_tile(h)) != SOMA_OK) return rc;             // a1 + a2 + a3 (+a5), tiled
+    if ((rc = launch_singles(h, true, true, h->counts_pad(h->pad_cur), true)) != SOMA_OK) return rc;
   } else if (use_fused(h)) {
     if ((rc = launch_fused(h)) != SOMA_OK) return rc;            // a1 + a2 + a3 (+a5)
+    if ((rc = launch_singles(h, true, true, h->counts(h->cur ^ 1), false)) != SOMA_OK) return rc;
   } else {
     if ((rc = launch_half_sweep(h, 0)) != SOMA_OK) return rc;    // a1
+    if ((rc = launch_singles(h, true, false, nullptr, false)) != SOMA_OK) return rc;   // a1, single-bead molecules
     if ((rc = launch_half_sweep(h, 1)) != SOMA_OK) return rc;    // a2
-    if ((rc = launch_bin(h, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;   // a3
+    if ((rc = launch_bin(h, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;   // a3 (chains and single-bead molecules)
   }
   h->cur ^= 1;
   if (timed) timing_mark(h);
@@ -709,7 +745,9 @@ uint64_t soma_workspace_bytes(const soma_params* p) {
   const uint64_t B = p->n_chains * p->beads_per_chain;
   const uint64_t TC = (uint64_t)p->grid[0] * p->grid[1] * p->grid[2] * p->n_types;
   const uint64_t pad_words = tile_capable_grid(p->grid) ? omega_pad_cells_max(p->grid) * p->n_types : 0;
-  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bins_capacity(p->grid), pad_words).total;
+  uint64_t S = 0;
+  if (p->n_single) for (uint32_t t = 0; t < p->n_types; ++t) S += p->n_single[t];
+  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bins_capacity(p->grid), pad_words, S).total;
 }
 
 int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
@@ -739,6 +777,13 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->stream = static_cast<cudaStream_t>(cuda_stream);
   h->n_chains = p->n_chains; h->N = p->beads_per_chain; h->T = p->n_types; h->n_patterns = p->n_patterns;
   h->B = h->n_chains * h->N;
+  h->S = 0;
+  for (uint32_t t = 0; t < h->T; ++t) {
+    h->single_start[t] = (uint32_t)h->S;
+    if (p->n_single) h->S += p->n_single[t];
+  }
+  for (uint32_t t = h->T; t <= (uint32_t)kMaxTypes; ++t) h->single_start[t] = (uint32_t)h->S;
+  h->Btot = h->B + h->S;
   h->cells = p->grid[0] * p->grid[1] * p->grid[2];
   h->grid.nx = p->grid[0]; h->grid.ny = p->grid[1]; h->grid.nz = p->grid[2];
   h->grid.inv_hx = (float)p->grid[0] / p->box[0];
@@ -749,7 +794,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->b = p->b;
   for (int d = 0; d < 3; ++d) h->box[d] = p->box[d];
   h->kb = 1.5f / (p->b * p->b);
-  h->dens_scale = (float)((double)h->cells / (double)h->B);
+  h->dens_scale = (float)((double)h->cells / (double)h->Btot);
   h->invN = 1.0f / (float)h->N;
   h->kappaN = p->kappaN;
   for (uint32_t k = 0; k < h->T * h->T; ++k) h->chiN[k] = p->chiN[k];
@@ -758,7 +803,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->tile_grid_ok = tile_capable_grid(p->grid);
   h->sort_bins_cap = sort_bins_capacity(p->grid);
   h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, h->sort_bins_cap,
-                     h->tile_grid_ok ? omega_pad_cells_max(p->grid) * h->T : 0);
+                     h->tile_grid_ok ? omega_pad_cells_max(p->grid) * h->T : 0, h->S);
   if (p->workspace) {
     if (p->workspace_bytes < h->L.total || (reinterpret_cast<uintptr_t>(p->workspace) % kAlign)) {
       free_handle(h);
@@ -856,6 +901,8 @@ int soma_load_state(soma_t* h, const float* x, const float* y, const float* z, u
   h->loaded = false;
   const float* src[3] = {x, y, z};
   for (int d = 0; d < 3; ++d) CU(h, cudaMemcpyAsync(h->pos(0, d), src[d], h->B * 4, kind, h->stream));
+  if (h->S)
+    for (int d = 0; d < 3; ++d) CU(h, cudaMemcpyAsync(h->single(d), src[d] + h->B, h->S * 4, kind, h->stream));
   return finish_load(h, step0);
 }
 
@@ -874,6 +921,12 @@ int soma_generate_state(soma_t* h, uint64_t gen_seed, uint64_t step0) {
   generate_state_kernel<<<blocks_for(h->n_chains, 128), 128, 0, h->stream>>>(G);
   h->launches++;
   CU(h, cudaGetLastError());
+  if (h->S) {
+    generate_singles_kernel<<<blocks_for(h->S, 256), 256, 0, h->stream>>>(
+        (uint32_t)h->S, (uint32_t)h->n_chains, G.k0, G.k1, G.box[0], G.box[1], G.box[2], h->single(0), h->single(1), h->single(2));
+    h->launches++;
+    CU(h, cudaGetLastError());
+  }
   return finish_load(h, step0);
 }
 
@@ -889,6 +942,11 @@ int soma_mc_steps(soma_t* h, uint32_t n_steps, uint64_t* accepted) {
           h->grid, h->B, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2), h->range_flag());
       h->launches++;
       CU(h, cudaGetLastError());
+      if (h->S) {
+        range_check_kernel<<<blocks_for(h->S, 256), 256, 0, h->stream>>>(h->grid, h->S, h->single(0), h->single(1), h->single(2), h->range_flag());
+        h->launches++;
+        CU(h, cudaGetLastError());
+      }
       if ((rc = verify_range(h)) != SOMA_OK) return rc;
     }
     if ((rc = one_step(h)) != SOMA_OK) return rc;
@@ -936,6 +994,10 @@ int soma_get_positions(soma_t* h, float* x, float* y, float* z, int dev) {
   for (int d = 0; d < 3; ++d)
     CU(h, cudaMemcpyAsync(dst[d], h->pos(set, d), h->B * 4,
                           dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+  if (h->S)
+    for (int d = 0; d < 3; ++d)
+      CU(h, cudaMemcpyAsync(dst[d] + h->B, h->single(d), h->S * 4,
+                            dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
   if (!dev) CU(h, cudaStreamSynchronize(h->stream));
   return SOMA_OK;
 }
@@ -967,6 +1029,10 @@ int soma_validate_state(soma_t* h, soma_validation* out) {
   CU(h, cudaMemsetAsync(report, 0, 11 * 8, h->stream));
   validate_positions_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
       h->B, h->N, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2), report, bond_sum);
+  if (h->S) {      // N = 1 in the kernel: no bonds, only the finiteness test
+    validate_positions_kernel<<<blocks_for(h->S, 256), 256, 0, h->stream>>>(h->S, 1u, h->single(0), h->single(1), h->single(2), report, bond_sum);
+    h->launches++;
+  }
   const unsigned gx = blocks_for(h->cells, 256) < 1024u ? blocks_for(h->cells, 256) : 1024u;
   validate_density_kernel<<<dim3(gx, h->T), 256, 0, h->stream>>>(h->cells, h->T, h->counts(h->cur), report);
   h->launches += 2;
@@ -983,7 +1049,7 @@ int soma_validate_state(soma_t* h, soma_validation* out) {
   std::memcpy(&sum, &host[10], 8);
   const uint64_t n_bonds = h->n_chains * (uint64_t)(h->N - 1);
   out->mean_bond_sq = n_bonds ? sum / (double)n_bonds : 0.0;
-  out->ok = (out->n_nonfinite == 0 && out->density_total == h->B) ? 1u : 0u;
+  out->ok = (out->n_nonfinite == 0 && out->density_total == h->Btot) ? 1u : 0u;
   return SOMA_OK;
 }
 
@@ -1111,6 +1177,7 @@ int soma_debug_half_sweep(soma_t* h, uint32_t parity, uint64_t* accepted) {
   if (parity > 1) return fail(h, SOMA_EINVAL, "parity must be 0 or 1");
   CU(h, cudaMemsetAsync(h->accepted(), 0, 8, h->stream));
   if ((rc = launch_half_sweep(h, parity)) != SOMA_OK) return rc;
+  if (parity == 0 && (rc = launch_singles(h, true, false, nullptr, false)) != SOMA_OK) return rc;
   if (accepted) {
     unsigned long long v = 0;
     CU(h, cudaMemcpyAsync(&v, h->accepted(), 8, cudaMemcpyDeviceToHost, h->stream));

@@ -438,6 +438,72 @@ range_check_kernel(Grid grid, uint64_t B, const float* __restrict__ x, const flo
 }
 
 // ---------------------------------------------------------------------------------------------
+// Single-bead molecules next to the chains (solvent species, R23):
+// molecule m = bead 0 of logical chain n_chains + m, moved in half-sweep 0, no bonds, so
+// dE = fma(kb, 0, dw) = omega_t(new cell) - omega_t(old cell).  One thread per molecule; positions in
+// their own arrays (never re-ordered), type by the per-type start table.
+// ---------------------------------------------------------------------------------------------
+struct SingleArgs {
+  StepArgs S;                       // grid, cells, a, kb, keys, ctr2, ctr3_base, omega, accepted; n_chains = first logical id
+  uint32_t n_total, T;
+  uint32_t start[kMaxTypes + 1];    // molecules of type t are [start[t], start[t+1])
+  float* __restrict__ x; float* __restrict__ y; float* __restrict__ z;
+  uint32_t* __restrict__ counts;    // grid to bin into: linear [T][C], or ghost-padded [T][px][py][pz] if px != 0
+  uint32_t px, py, pz, hx, hy, hz;
+  uint32_t* __restrict__ range_flag;  // may be null
+  int do_move, do_bin;
+};
+
+template <bool POW2>
+__global__ void __launch_bounds__(256)
+singles_kernel(SingleArgs A) {
+  const uint32_t m = blockIdx.x * blockDim.x + threadIdx.x;
+  bool acc = false;
+  if (m < A.n_total) {
+    uint32_t type = 0;
+    while (m >= A.start[type + 1]) ++type;
+    float rx = A.x[m], ry = A.y[m], rz = A.z[m];
+    const Grid& G = A.S.grid;
+    if (A.range_flag) {
+      const float mm = fmaxf(fabsf(__fmul_rn(rx, G.inv_hx)), fmaxf(fabsf(__fmul_rn(ry, G.inv_hy)), fabsf(__fmul_rn(rz, G.inv_hz))));
+      if (!(mm < kCellCoordLimit)) *A.range_flag = 1u;
+    }
+    if (A.do_move) {
+      const Words4 w = philox4x32_10(0u, A.S.n_chains + m, A.S.ctr2, A.S.ctr3_base, A.S.keys);
+      const Trial t = trial_position(rx, ry, rz, A.S.a, w);
+      const float* om = A.S.omega + (size_t)type * A.S.cells;
+      const float dw = __fsub_rn(__ldg(om + cell_of<POW2>(G, t.x, t.y, t.z)), __ldg(om + cell_of<POW2>(G, rx, ry, rz)));
+      acc = metropolis_accept(__fmaf_rn(A.S.kb, 0.0f, dw), w.w3);
+      if (acc) { rx = t.x; ry = t.y; rz = t.z; A.x[m] = rx; A.y[m] = ry; A.z[m] = rz; }
+    }
+    if (A.do_bin) {
+      if (A.px) {                                        // ghost-padded grid of the windowed kernels: the interior image
+        const uint32_t gx = wrap<POW2>(__float2int_rd(__fmul_rn(rx, G.inv_hx)), G.nx);
+        const uint32_t gy = wrap<POW2>(__float2int_rd(__fmul_rn(ry, G.inv_hy)), G.ny);
+        const uint32_t gz = wrap<POW2>(__float2int_rd(__fmul_rn(rz, G.inv_hz)), G.nz);
+        atomicAdd(A.counts + ((size_t)(type * A.px + gx + A.hx) * A.py + gy + A.hy) * A.pz + gz + A.hz, 1u);
+      } else {
+        atomicAdd(A.counts + (size_t)type * A.S.cells + cell_of<POW2>(G, rx, ry, rz), 1u);
+      }
+    }
+  }
+  const unsigned n_acc = __popc(__ballot_sync(0xffffffffu, acc));
+  if ((threadIdx.x & 31u) == 0 && n_acc) atomicAdd(A.S.accepted, (unsigned long long)n_acc);
+}
+
+// single-bead molecules of the generated initial state: the bead-0 rule with chain id n_chains + m
+__global__ void __launch_bounds__(256)
+generate_singles_kernel(uint32_t n_total, uint32_t first_id, uint32_t k0, uint32_t k1, double bx, double by, double bz,
+                        float* __restrict__ x, float* __restrict__ y, float* __restrict__ z) {
+  const uint32_t m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= n_total) return;
+  const Words4 w = philox4x32_10(0u, first_id + m, 0u, 1u << 8, k0, k1);
+  x[m] = (float)(bx * (((double)w.w0 + 0.5) * 0x1p-32));
+  y[m] = (float)(by * (((double)w.w1 + 0.5) * 0x1p-32));
+  z[m] = (float)(bz * (((double)w.w2 + 0.5) * 0x1p-32));
+}
+
+// ---------------------------------------------------------------------------------------------
 // Initial state on the device (R22): Gaussian random-walk
 // chains, first bead uniform in the box.  One thread per chain; draws keyed by (bead, chain) in
 // Philox domain 1; double-precision Box-Muller and accumulation, one rounding to fp32 per coordinate.

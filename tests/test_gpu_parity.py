@@ -291,3 +291,39 @@ def test_external_field_single_bead_molecules_on_device():
         g.set_external_field(torch.from_numpy(ext).cuda())        # device pointer in
         assert g.mc_steps(40, want_accepted=True) == o.mc_steps(40)
         assert_same_state(g, o, "N=1 in an external field")
+
+
+# ---- single-bead molecules next to the chains (R23) ----------------
+
+def _mixture(n_chains=3000, N=32, n_single=(7000, 0, 11000), grid=(16, 16, 16), seed=51):
+    chi = np.array([[0, 18, 6], [18, 0, 9], [6, 9, 0.0]])
+    pat = [[0] * (N // 2) + [1] * (N - N // 2)]
+    return si.custom_system(n_chains, N, 3, pat, None, chi, 40.0, grid, tuple(g / 2 for g in grid), seed=seed, n_single=n_single)
+
+
+@pytest.mark.parametrize("path", [FUSED, GENERIC, TILED, SWEEP])
+def test_mixture_of_chains_and_single_bead_molecules(path):
+    s = _mixture()
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s, path=path, options=SMALL_TILES if path in TILED_PATHS else None) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert_same_state(g, o, f"mixture loaded, path {path}")
+        done = 0
+        for upto in (1, 10):
+            assert g.mc_steps(upto - done, want_accepted=True) == o.mc_steps(upto - done)
+            done = upto
+            assert_same_state(g, o, f"mixture, path {path}, {upto} steps")
+        v = g.validate()
+        assert v["ok"] and v["density_per_type"][:3] == o.validate()["density_per_type"]
+
+
+def test_mixture_generic_chain_length_lockstep_and_generated_state():
+    s = _mixture(n_chains=900, N=5, n_single=(0, 4000, 1), grid=(8, 8, 8), seed=52)       # odd N: generic kernels
+    o = oracle.Oracle.from_system(s)
+    o.generate_state(99)
+    with gpu_system(s) as g:
+        g.generate_state(99)
+        assert all(np.array_equal(a, b_) for a, b_ in zip(g.positions(), o.positions()))
+        assert g.mc_steps(6, want_accepted=True) == o.mc_steps(6)
+        assert_same_state(g, o, "generated mixture, 6 steps")
