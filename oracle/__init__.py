@@ -78,6 +78,10 @@ def lib() -> C.CDLL:
             "oracle_set_external_field": (None, [vp, f32p]),
             "oracle_generate_state": (C.c_int, [vp, C.c_uint64, C.c_uint64]),
             "oracle_set_singles": (C.c_int, [vp, C.POINTER(C.c_uint64)]),
+            "oracle_set_smc": (None, [vp, C.c_float]),
+            "oracle_smc_margin": (C.c_float, [vp, C.c_uint64, C.c_float, C.c_float, C.c_float]),
+            "oracle_smc_draws": (None, [vp, C.c_uint64, C.c_uint32, C.c_uint32, C.POINTER(C.c_double)]),
+            "oracle_det_functions": (None, [C.c_double, C.POINTER(C.c_double)]),
             "oracle_validate": (None, [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]),
             "oracle_get_step": (C.c_uint64, [vp]),
             "oracle_set_step": (None, [vp, C.c_uint64]),
@@ -118,6 +122,13 @@ def lnu(u) -> np.ndarray:
     out = np.empty_like(u)
     lib().oracle_lnu_array(_p(u, C.c_float), _p(out, C.c_float), u.size)
     return out
+
+
+def det_functions(x: float):
+    """(det_log(x), sin(2 pi x), cos(2 pi x)) of the library-free routines behind the normal deviates (R24)."""
+    out = (C.c_double * 3)()
+    lib().oracle_det_functions(float(x), out)
+    return float(out[0]), float(out[1]), float(out[2])
 
 
 class Oracle:
@@ -168,6 +179,18 @@ class Oracle:
     def generate_state(self, gen_seed: int, step0: int = 0):
         """Gaussian random-walk initial state by the recipe of DESIGN.md R22, then bin + omega."""
         lib().oracle_generate_state(self._h, int(gen_seed), int(step0))
+
+    def set_smc(self, A: float):
+        """A > 0: bond-force-biased moves with mobility A (R24); 0: uniform moves."""
+        lib().oracle_set_smc(self._h, float(A))
+
+    def smc_margin(self, bead: int, nx, ny, nz) -> float:
+        return float(lib().oracle_smc_margin(self._h, int(bead), float(nx), float(ny), float(nz)))
+
+    def smc_draws(self, chain: int, bead: int, parity: int):
+        out = (C.c_double * 4)()
+        lib().oracle_smc_draws(self._h, int(chain), int(bead), int(parity), out)
+        return [float(v) for v in out]
 
     def validate(self) -> dict:
         """Non-finite coordinates, density totals, largest and mean squared bond length of the state."""

@@ -105,6 +105,8 @@ struct Oracle {
   std::vector<float> ext;               // [T][C] external field (empty = none), R21
   // single-bead molecules (R23): n_single[t] of type t, stored after the chains in x, y, z,
   // type 0 first; molecule m has the logical chain id n_chains + m and bead index 0
+  float smcA = 0.0f;                    // > 0: bond-force-biased moves with mobility A (R24), 0: uniform moves
+  float gA = 0.0f, sq2A = 0.0f, inv4A = 0.0f;   // fl(A * 2 kb), (float)sqrt(2 A), (float)(1 / (4 A))
   std::vector<uint64_t> n_single;       // [T] (empty = none)
   uint64_t S = 0;                       // their total
   uint64_t t;                           // absolute step index
@@ -231,8 +233,110 @@ inline double delta_energy_f64(const Oracle& o, uint64_t c, uint32_t i, float nx
   return (double)o.kb * dq + dw;
 }
 
+// ---- standard normal deviates with no library function in them (R24) -------------------
+// Box-Muller in double from U = (w + 0.5) 2^-32, with the logarithm and the sine / cosine written out
+// as fixed sequences of IEEE operations (+, *, /, fma, sqrt), so that any conforming implementation
+// produces the same bits.  Accuracy ~1e-15, far below what the fp32 result keeps.
+inline double det_log(double x) {                       // x in (0, 1]
+  uint64_t bits; std::memcpy(&bits, &x, 8);
+  int e = (int)((bits >> 52) & 0x7ff) - 1023;
+  bits = (bits & 0x000fffffffffffffull) | 0x3ff0000000000000ull;
+  double m; std::memcpy(&m, &bits, 8);                  // m in [1, 2)
+  if (m > 1.4142135623730951) { m = m * 0.5; e += 1; }  // m in (sqrt 1/2, sqrt 2]
+  const double sq = (m - 1.0) / (m + 1.0), z = sq * sq; // log m = 2 atanh(sq) = 2 sq (1 + z/3 + z^2/5 + ...)
+  double p = 1.0 / 27.0;
+  p = std::fma(p, z, 1.0 / 25.0); p = std::fma(p, z, 1.0 / 23.0); p = std::fma(p, z, 1.0 / 21.0);
+  p = std::fma(p, z, 1.0 / 19.0); p = std::fma(p, z, 1.0 / 17.0); p = std::fma(p, z, 1.0 / 15.0);
+  p = std::fma(p, z, 1.0 / 13.0); p = std::fma(p, z, 1.0 / 11.0); p = std::fma(p, z, 1.0 / 9.0);
+  p = std::fma(p, z, 1.0 / 7.0);  p = std::fma(p, z, 1.0 / 5.0);  p = std::fma(p, z, 1.0 / 3.0);
+  const double lm = std::fma(2.0 * sq, z * p, 2.0 * sq);
+  return std::fma((double)e, 0.6931471805599453, lm);
+}
+inline void det_sincos_2pi(double u, double* sn, double* cs) {   // sin, cos of 2 pi u, u in (0, 1)
+  const double t = u * 4.0;                              // quarter turns
+  const double k = std::floor(t + 0.5);
+  const double r = (t - k) * 1.5707963267948966, z = r * r;   // r in [-pi/4, pi/4]
+  double ps = -1.0 / 355687428096000.0;                  // sin r = r (1 - z/3! + z^2/5! - ... - z^8/17!)
+  ps = std::fma(ps, z, 1.0 / 1307674368000.0); ps = std::fma(ps, z, -1.0 / 6227020800.0);
+  ps = std::fma(ps, z, 1.0 / 39916800.0);      ps = std::fma(ps, z, -1.0 / 362880.0);
+  ps = std::fma(ps, z, 1.0 / 5040.0);          ps = std::fma(ps, z, -1.0 / 120.0);
+  ps = std::fma(ps, z, 1.0 / 6.0);
+  const double s0 = std::fma(-r * z, ps, r);
+  double pc = 1.0 / 20922789888000.0;                    // cos r = 1 - z/2! + z^2/4! - ... + z^8/16!
+  pc = std::fma(pc, z, -1.0 / 87178291200.0); pc = std::fma(pc, z, 1.0 / 479001600.0);
+  pc = std::fma(pc, z, -1.0 / 3628800.0);     pc = std::fma(pc, z, 1.0 / 40320.0);
+  pc = std::fma(pc, z, -1.0 / 720.0);         pc = std::fma(pc, z, 1.0 / 24.0);
+  pc = std::fma(pc, z, -0.5);
+  const double c0 = std::fma(pc, z, 1.0);
+  const int q = (int)k & 3;                              // rotate by k quarter turns
+  *sn = q == 0 ? s0 : q == 1 ? c0 : q == 2 ? -s0 : -c0;
+  *cs = q == 0 ? c0 : q == 1 ? -s0 : q == 2 ? -c0 : s0;
+}
+inline double unit32(uint32_t w) { return ((double)w + 0.5) * 0x1p-32; }
+
+// Bond-force-biased ("smart Monte Carlo") trial move of bead (c, i), R24 (PAPER.md:41, :77:
+// "bond-force-biased Monte-Carlo", "biased trial moves").  S = sum over the bonded neighbours of
+// (r - r_j) (i-1 first), so the bonded force is F = -2 kb S.  Proposal r' = r + A F + sqrt(2A) xi:
+//   dr_d = fma(-gA, S_d, sq2A * xi_d),  r'_d = r_d + dr_d,  gA = fl(A * fl(2 kb)).
+// With S' the same sum at r', qf = |dr + gA S|^2 (forward), qr = |dr - gA S'|^2 (reverse), each
+// fma(z,z, fma(y,y, x*x)); margin m = fma(inv4A, qr - qf, dE) + lnu, dE as for uniform moves; accept iff m <= 0.
+// xi_0, xi_1 = Box-Muller pair of words (w0, w1) of the move's Philox call (domain 0); xi_2 = cosine
+// member of the pair of words (v0, v1) of a second call with domain 2; u from w3 as before.
+inline int trial_move_smc(Oracle& o, uint64_t c, uint32_t i, uint32_t parity, double* margin64) {
+  const uint32_t hi = (uint32_t)(o.t >> 32) << 16;
+  const uint32_t ctr[4] = {i, (uint32_t)c, (uint32_t)o.t, parity | (RNG_DOMAIN_MOVE << 8) | hi};
+  const uint32_t ctr2[4] = {i, (uint32_t)c, (uint32_t)o.t, parity | (2u << 8) | hi};
+  const uint32_t key[2] = {(uint32_t)o.seed, (uint32_t)(o.seed >> 32)};
+  uint32_t w[4], v[4];
+  philox4x32_10(ctr, key, w);
+  philox4x32_10(ctr2, key, v);
+  double sn, cs, sn2, cs2;
+  const double ra = std::sqrt(-2.0 * det_log(unit32(w[0])));
+  det_sincos_2pi(unit32(w[1]), &sn, &cs);
+  const double rb = std::sqrt(-2.0 * det_log(unit32(v[0])));
+  det_sincos_2pi(unit32(v[1]), &sn2, &cs2);
+  const float xi[3] = {(float)(ra * cs), (float)(ra * sn), (float)(rb * cs2)};
+  const float u = umap(w[3]);
+  const uint64_t j = c * o.N + i;
+  const float r[3] = {o.x[j], o.y[j], o.z[j]};
+  float S[3] = {0.0f, 0.0f, 0.0f};
+  bool have = false;
+  for (int side = 0; side < 2; ++side) {
+    if (side == 0 && i == 0) continue;
+    if (side == 1 && i + 1 >= o.N) continue;
+    const uint64_t k = side == 0 ? j - 1 : j + 1;
+    const float s3[3] = {r[0] - o.x[k], r[1] - o.y[k], r[2] - o.z[k]};
+    for (int d = 0; d < 3; ++d) S[d] = have ? S[d] + s3[d] : s3[d];
+    have = true;
+  }
+  float dr[3], n[3];
+  for (int d = 0; d < 3; ++d) { dr[d] = fmaf(-o.gA, S[d], o.sq2A * xi[d]); n[d] = r[d] + dr[d]; }
+  float S2[3] = {0.0f, 0.0f, 0.0f};
+  have = false;
+  for (int side = 0; side < 2; ++side) {
+    if (side == 0 && i == 0) continue;
+    if (side == 1 && i + 1 >= o.N) continue;
+    const uint64_t k = side == 0 ? j - 1 : j + 1;
+    const float s3[3] = {n[0] - o.x[k], n[1] - o.y[k], n[2] - o.z[k]};
+    for (int d = 0; d < 3; ++d) S2[d] = have ? S2[d] + s3[d] : s3[d];
+    have = true;
+  }
+  float a[3], b_[3];
+  for (int d = 0; d < 3; ++d) { a[d] = fmaf(o.gA, S[d], dr[d]); b_[d] = fmaf(-o.gA, S2[d], dr[d]); }
+  const float qf = fmaf(a[2], a[2], fmaf(a[1], a[1], a[0] * a[0]));
+  const float qr = fmaf(b_[2], b_[2], fmaf(b_[1], b_[1], b_[0] * b_[0]));
+  const float dE = delta_energy(o, c, i, n[0], n[1], n[2]);
+  const float meff = fmaf(o.inv4A, qr - qf, dE);
+  const float m = meff + lnu32(u);
+  if (margin64)
+    *margin64 = delta_energy_f64(o, c, i, n[0], n[1], n[2]) + ((double)qr - (double)qf) * (double)o.inv4A + std::log((double)u);
+  if (m <= 0.0f) { o.x[j] = n[0]; o.y[j] = n[1]; o.z[j] = n[2]; return 1; }
+  return 0;
+}
+
 // One Metropolis trial move of bead (c, i) (DESIGN.md section 2 step 5).  Returns 1 if accepted.
 inline int trial_move(Oracle& o, uint64_t c, uint32_t i, uint32_t parity, double* margin64) {
+  if (o.smcA > 0.0f) return trial_move_smc(o, c, i, parity, margin64);
   const uint32_t ctr[4] = {i, (uint32_t)c, (uint32_t)o.t,
                            parity | (RNG_DOMAIN_MOVE << 8) | ((uint32_t)(o.t >> 32) << 16)};
   const uint32_t key[2] = {(uint32_t)o.seed, (uint32_t)(o.seed >> 32)};
@@ -435,6 +539,59 @@ void oracle_set_omega(void* h, const float* omega) {
   std::memcpy(o.omega.data(), omega, o.omega.size() * sizeof(float));
 }
 uint64_t oracle_get_step(void* h) { return static_cast<Oracle*>(h)->t; }
+// move type: A > 0 = bond-force-biased moves with mobility A (R24), 0 = uniform moves
+void oracle_set_smc(void* h, float A) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  o.smcA = A;
+  o.gA = A * (2.0f * o.kb);
+  o.sq2A = (float)std::sqrt(2.0 * (double)A);
+  o.inv4A = A > 0.0f ? (float)(1.0 / (4.0 * (double)A)) : 0.0f;
+}
+// the normal deviates of a move, for the tests: out[0..2] = xi, out[3] = u
+void oracle_smc_draws(void* h, uint64_t c, uint32_t i, uint32_t parity, double* out) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const uint32_t hi = (uint32_t)(o.t >> 32) << 16;
+  const uint32_t ctr[4] = {i, (uint32_t)c, (uint32_t)o.t, parity | hi}, ctr2[4] = {i, (uint32_t)c, (uint32_t)o.t, parity | (2u << 8) | hi};
+  const uint32_t key[2] = {(uint32_t)o.seed, (uint32_t)(o.seed >> 32)};
+  uint32_t w[4], v[4];
+  philox4x32_10(ctr, key, w); philox4x32_10(ctr2, key, v);
+  double sn, cs, sn2, cs2;
+  const double ra = std::sqrt(-2.0 * det_log(unit32(w[0])));
+  det_sincos_2pi(unit32(w[1]), &sn, &cs);
+  const double rb = std::sqrt(-2.0 * det_log(unit32(v[0])));
+  det_sincos_2pi(unit32(v[1]), &sn2, &cs2);
+  out[0] = ra * cs; out[1] = ra * sn; out[2] = rb * cs2; out[3] = (double)umap(w[3]);
+}
+// fma(inv4A, qr - qf, dE) of moving bead `bead` to (nx, ny, nz): the bond-force-biased margin without ln u
+float oracle_smc_margin(void* h, uint64_t bead, float nx, float ny, float nz) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const uint64_t c = bead / o.N, j = bead;
+  const uint32_t i = (uint32_t)(bead % o.N);
+  const float r[3] = {o.x[j], o.y[j], o.z[j]}, n[3] = {nx, ny, nz};
+  float S[3] = {0, 0, 0}, S2[3] = {0, 0, 0};
+  bool have = false;
+  for (int side = 0; side < 2; ++side) {
+    if (side == 0 && i == 0) continue;
+    if (side == 1 && i + 1 >= o.N) continue;
+    const uint64_t k = side == 0 ? j - 1 : j + 1;
+    const float nb[3] = {o.x[k], o.y[k], o.z[k]};
+    for (int d = 0; d < 3; ++d) {
+      S[d] = have ? S[d] + (r[d] - nb[d]) : r[d] - nb[d];
+      S2[d] = have ? S2[d] + (n[d] - nb[d]) : n[d] - nb[d];
+    }
+    have = true;
+  }
+  float a[3], b_[3];
+  for (int d = 0; d < 3; ++d) { const float dr = n[d] - r[d]; a[d] = fmaf(o.gA, S[d], dr); b_[d] = fmaf(-o.gA, S2[d], dr); }
+  const float qf = fmaf(a[2], a[2], fmaf(a[1], a[1], a[0] * a[0]));
+  const float qr = fmaf(b_[2], b_[2], fmaf(b_[1], b_[1], b_[0] * b_[0]));
+  return fmaf(o.inv4A, qr - qf, delta_energy(o, c, i, nx, ny, nz));
+}
+void oracle_det_functions(double x, double* out) {       // out = {det_log(x), sin(2 pi x), cos(2 pi x)}
+  out[0] = det_log(x);
+  det_sincos_2pi(x, &out[1], &out[2]);
+}
+
 // single-bead molecules: n_single[T] (call right after oracle_create, before any state is loaded)
 int oracle_set_singles(void* h, const uint64_t* n_single) {
   Oracle& o = *static_cast<Oracle*>(h);
