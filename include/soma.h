@@ -63,7 +63,12 @@ typedef struct soma_params {
   float b;                      /* bond length; harmonic bonds with k = 3/(2 b^2) kT (DESIGN R1)  */
   float kappaN;                 /* kappa*N, incompressibility                                     */
   float move_halfwidth;         /* a: trial displacement uniform in the cube (-a, a)^3           */
-  float reserved1;              /* must be 0                                                    */
+  float smc_mobility;           /* A >= 0.  0: unbiased uniform trial moves (the configs' move).  A > 0:
+                                   bond-force-biased ("smart Monte Carlo") moves, the move the paper's
+                                   mc_polymer_iteration performs (SURVEY.md section 8(f) row
+                                   f1; R24): r' = r + A F_bonded(r) + sqrt(2A) xi, xi standard normal,
+                                   accepted with min(1, e^-dE T(r'->r)/T(r->r')); move_halfwidth is then
+                                   unused.  Runs on the generic kernels (any N).  Units: length^2/kT  */
   uint32_t grid[3];             /* cells per axis                                               */
   uint32_t reserved2;           /* must be 0                                                    */
   float box[3];                 /* periodic box lengths; cell size = box/grid                   */

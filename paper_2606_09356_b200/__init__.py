@@ -53,7 +53,7 @@ class soma_params(C.Structure):
         ("b", C.c_float),
         ("kappaN", C.c_float),
         ("move_halfwidth", C.c_float),
-        ("reserved1", C.c_float),
+        ("smc_mobility", C.c_float),
         ("grid", C.c_uint32 * 3),
         ("reserved2", C.c_uint32),
         ("box", C.c_float * 3),
@@ -135,7 +135,7 @@ def _is_device(a) -> int:
 # ---- the C entry points, same names ------------------------------------------------------------
 
 def make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN, kappaN,
-                grid, box, move_halfwidth, seed, n_single=None):
+                grid, box, move_halfwidth, seed, n_single=None, smc_mobility=0.0):
     """Build a soma_params plus the numpy arrays it points to (keep the tuple alive until create)."""
     pats = np.ascontiguousarray(type_patterns, dtype=np.uint8)
     n_patterns = 1 if pats.ndim < 2 else int(pats.shape[0])     # validation is the library's job
@@ -147,6 +147,7 @@ def make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern
     p.chain_pattern = None if cp is None else cp.ctypes.data
     p.chiN = chi.ctypes.data
     p.b, p.kappaN, p.move_halfwidth = float(b), float(kappaN), float(move_halfwidth)
+    p.smc_mobility = float(smc_mobility)
     p.grid = (C.c_uint32 * 3)(*[int(g) for g in grid])
     p.box = (C.c_float * 3)(*[float(v) for v in box])
     p.seed = int(seed)
@@ -295,7 +296,7 @@ class Soma:
     """One SCMF system on the current CUDA device.  Device memory and stream come from PyTorch."""
 
     def __init__(self, n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN,
-                 kappaN, grid, box, move_halfwidth, seed, stream=None, lend_workspace: bool = True, n_single=None):
+                 kappaN, grid, box, move_halfwidth, seed, stream=None, lend_workspace: bool = True, n_single=None, smc_mobility=0.0):
         import torch
         if not torch.cuda.is_available():
             raise SomaError(SOMA_ECUDA, "no CUDA device: this package has no CPU fallback")
@@ -304,7 +305,7 @@ class Soma:
         self.grid = tuple(int(g) for g in grid)
         self.cells = self.grid[0] * self.grid[1] * self.grid[2]
         p, keep = make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN,
-                              kappaN, grid, box, move_halfwidth, seed, n_single=n_single)
+                              kappaN, grid, box, move_halfwidth, seed, n_single=n_single, smc_mobility=smc_mobility)
         self._workspace = None
         if lend_workspace:
             nbytes = soma_workspace_bytes(p)

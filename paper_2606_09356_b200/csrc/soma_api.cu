@@ -109,7 +109,8 @@ const char* validate(const soma_params* p) {
   if (p->beads_per_chain == 0 || p->beads_per_chain > 65535) return "beads_per_chain must be in [1, 65535]";
   if (p->n_types == 0 || p->n_types > (uint32_t)kMaxTypes) return "n_types must be in [1, 8]";
   if (p->n_patterns == 0 || p->n_patterns > 256) return "n_patterns must be in [1, 256]";
-  if (p->reserved0 || p->reserved1 != 0.0f || p->reserved2 || p->reserved3 != 0.0f) return "reserved fields must be 0";
+  if (p->reserved0 || p->reserved2 || p->reserved3 != 0.0f) return "reserved fields must be 0";
+  if (!(p->smc_mobility >= 0.0f) || p->smc_mobility > 1e6f) return "smc_mobility must be in [0, 1e6]";
   if (!p->type_patterns) return "type_patterns is NULL";
   if (!p->chiN) return "chiN is NULL";
   if (!(p->b > 0.0f)) return "b must be > 0";
@@ -166,6 +167,7 @@ struct soma_handle {
   Grid grid;
   bool pow2;
   float a, kb, dens_scale, invN, kappaN, b, box[3];
+  float smcA, gA, sq2A, inv4A;   // bond-force-biased moves (R24); smcA = 0: uniform moves
   float chiN[kMaxTypes * kMaxTypes];
   uint64_t seed;
   // device
@@ -280,6 +282,7 @@ StepArgs step_args(const soma_handle* h) {
   A.N = h->N;
   A.a = h->a;
   A.kb = h->kb;
+  A.gA = h->gA; A.sq2A = h->sq2A; A.inv4A = h->inv4A;
   A.keys = h->keys;
   A.ctr2 = (uint32_t)h->step;
   A.ctr3_base = (0u << 8) | ((uint32_t)(h->step >> 32) << 16);   // domain 0 = MC move
@@ -422,11 +425,11 @@ int launch_fused(soma_handle* h) {
 }
 
 bool use_fused(const soma_handle* h) {
-  if (h->path == 1) return false;
+  if (h->path == 1 || h->smcA > 0.0f) return false;      // bond-force-biased moves run on the generic kernels
   return fused_lanes(h->N) != 0;
 }
 bool use_tile(const soma_handle* h) {
-  if (!h->tile_ready || h->omega_custom) return false;
+  if (!h->tile_ready || h->omega_custom || h->smcA > 0.0f) return false;
   return h->path == 3 || h->path == 4 || (h->path == 0 && h->tile_auto);
 }
 
@@ -794,6 +797,10 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->b = p->b;
   for (int d = 0; d < 3; ++d) h->box[d] = p->box[d];
   h->kb = 1.5f / (p->b * p->b);
+  h->smcA = p->smc_mobility;
+  h->gA = h->smcA * (2.0f * h->kb);
+  h->sq2A = (float)std::sqrt(2.0 * (double)h->smcA);
+  h->inv4A = h->smcA > 0.0f ? (float)(1.0 / (4.0 * (double)h->smcA)) : 0.0f;
   h->dens_scale = (float)((double)h->cells / (double)h->Btot);
   h->invN = 1.0f / (float)h->N;
   h->kappaN = p->kappaN;

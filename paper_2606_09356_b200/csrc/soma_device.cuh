@@ -156,6 +156,57 @@ __device__ __forceinline__ bool metropolis_accept_fma(float dE, uint32_t w3) {
   return acc;
 }
 
+// ---- standard normal deviates for the bond-force-biased move (R24) -------------------
+// Box-Muller in double with the logarithm and sine / cosine spelled out in IEEE operations only
+// (add, mul, div, fma, sqrt -- each correctly rounded on any conforming implementation), so the
+// deviates do not depend on a math library.  Written from the definition in DESIGN.md R24.
+__device__ __forceinline__ double ln_ieee(double x) {               // x in (0, 1]
+  long long bits = __double_as_longlong(x);
+  int e = (int)((bits >> 52) & 0x7ff) - 1023;
+  double m = __longlong_as_double((bits & 0x000fffffffffffffLL) | 0x3ff0000000000000LL);   // [1, 2)
+  if (m > 1.4142135623730951) { m = __dmul_rn(m, 0.5); e += 1; }
+  const double q = __ddiv_rn(__dadd_rn(m, -1.0), __dadd_rn(m, 1.0)), z = __dmul_rn(q, q);
+  double p = 1.0 / 27.0;
+  p = __fma_rn(p, z, 1.0 / 25.0); p = __fma_rn(p, z, 1.0 / 23.0); p = __fma_rn(p, z, 1.0 / 21.0);
+  p = __fma_rn(p, z, 1.0 / 19.0); p = __fma_rn(p, z, 1.0 / 17.0); p = __fma_rn(p, z, 1.0 / 15.0);
+  p = __fma_rn(p, z, 1.0 / 13.0); p = __fma_rn(p, z, 1.0 / 11.0); p = __fma_rn(p, z, 1.0 / 9.0);
+  p = __fma_rn(p, z, 1.0 / 7.0);  p = __fma_rn(p, z, 1.0 / 5.0);  p = __fma_rn(p, z, 1.0 / 3.0);
+  const double q2 = __dmul_rn(2.0, q);
+  const double lm = __fma_rn(q2, __dmul_rn(z, p), q2);
+  return __fma_rn((double)e, 0.6931471805599453, lm);
+}
+__device__ __forceinline__ void sincos_2pi_ieee(double u, double& sn, double& cs) {   // u in (0, 1)
+  const double t = __dmul_rn(u, 4.0);
+  const double k = floor(__dadd_rn(t, 0.5));
+  const double r = __dmul_rn(__dadd_rn(t, -k), 1.5707963267948966), z = __dmul_rn(r, r);
+  double ps = -1.0 / 355687428096000.0;
+  ps = __fma_rn(ps, z, 1.0 / 1307674368000.0); ps = __fma_rn(ps, z, -1.0 / 6227020800.0);
+  ps = __fma_rn(ps, z, 1.0 / 39916800.0);      ps = __fma_rn(ps, z, -1.0 / 362880.0);
+  ps = __fma_rn(ps, z, 1.0 / 5040.0);          ps = __fma_rn(ps, z, -1.0 / 120.0);
+  ps = __fma_rn(ps, z, 1.0 / 6.0);
+  const double s0 = __fma_rn(__dmul_rn(-r, z), ps, r);
+  double pc = 1.0 / 20922789888000.0;
+  pc = __fma_rn(pc, z, -1.0 / 87178291200.0); pc = __fma_rn(pc, z, 1.0 / 479001600.0);
+  pc = __fma_rn(pc, z, -1.0 / 3628800.0);     pc = __fma_rn(pc, z, 1.0 / 40320.0);
+  pc = __fma_rn(pc, z, -1.0 / 720.0);         pc = __fma_rn(pc, z, 1.0 / 24.0);
+  pc = __fma_rn(pc, z, -0.5);
+  const double c0 = __fma_rn(pc, z, 1.0);
+  const int qd = (int)k & 3;
+  sn = qd == 0 ? s0 : qd == 1 ? c0 : qd == 2 ? -s0 : -c0;
+  cs = qd == 0 ? c0 : qd == 1 ? -s0 : qd == 2 ? -c0 : s0;
+}
+__device__ __forceinline__ double unit32(uint32_t w) { return __dmul_rn(__dadd_rn((double)w, 0.5), 0x1p-32); }
+
+// xi[0..2]: deviates of a move from the words of its two Philox calls (domain 0: w, domain 2: v)
+__device__ __forceinline__ void smc_deviates(const Words4& w, const Words4& v, float& x0, float& x1, float& x2) {
+  double sn, cs, sn2, cs2;
+  const double ra = sqrt(__dmul_rn(-2.0, ln_ieee(unit32(w.w0))));
+  sincos_2pi_ieee(unit32(w.w1), sn, cs);
+  const double rb = sqrt(__dmul_rn(-2.0, ln_ieee(unit32(v.w0))));
+  sincos_2pi_ieee(unit32(v.w1), sn2, cs2);
+  x0 = (float)__dmul_rn(ra, cs); x1 = (float)__dmul_rn(ra, sn); x2 = (float)__dmul_rn(rb, cs2);
+}
+
 // ---- geometry ----
 struct Grid {
   uint32_t nx, ny, nz;          // cells per axis

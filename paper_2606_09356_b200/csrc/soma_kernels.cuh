@@ -27,6 +27,7 @@ struct StepArgs {
   uint32_t N;                 // beads per chain
   float a;                    // trial half-width
   float kb;                   // 1.5f/(b*b)
+  float gA, sq2A, inv4A;      // bond-force-biased moves (R24): fl(A * 2 kb), (float)sqrt(2A), (float)(1/(4A)); gA = 0: uniform moves
   PhiloxKeys keys;            // round keys of (seed lo, seed hi)
   uint32_t ctr2;              // (uint32) step
   uint32_t ctr3_base;         // domain << 8 | (uint32)(step >> 32) << 16; parity is or-ed in
@@ -62,6 +63,54 @@ __device__ __forceinline__ bool move_bead(const StepArgs& A, uint32_t chain, uin
   const float dE = __fmaf_rn(A.kb, dq, dw);
   const bool acc = metropolis_accept(dE, w.w3);
   if (acc) { rx = t.x; ry = t.y; rz = t.z; cell = cell_new; }
+  return acc;
+}
+
+// Bond-force-biased move (R24): proposal r' = r + A F + sqrt(2A) xi with the bonded force
+// F = -2 kb S, S = sum over the bonded neighbours of (r - r_j); margin = dE + (qr - qf)/(4A) + ln u.
+template <bool POW2>
+__device__ __forceinline__ bool move_bead_smc(const StepArgs& A, uint32_t chain, uint32_t i, uint32_t parity,
+                                              const float* __restrict__ omega_t,
+                                              float& rx, float& ry, float& rz, uint32_t& cell,
+                                              bool has_l, float lx, float ly, float lz,
+                                              bool has_r, float qx, float qy, float qz) {
+  const Words4 w = philox4x32_10(i, chain, A.ctr2, A.ctr3_base | parity, A.keys);
+  const Words4 v = philox4x32_10(i, chain, A.ctr2, A.ctr3_base | parity | (2u << 8), A.keys);
+  float x0, x1, x2;
+  smc_deviates(w, v, x0, x1, x2);
+  float Sx = 0.f, Sy = 0.f, Sz = 0.f;
+  if (has_l) { Sx = __fsub_rn(rx, lx); Sy = __fsub_rn(ry, ly); Sz = __fsub_rn(rz, lz); }
+  if (has_r) {
+    const float ax = __fsub_rn(rx, qx), ay = __fsub_rn(ry, qy), az = __fsub_rn(rz, qz);
+    Sx = has_l ? __fadd_rn(Sx, ax) : ax; Sy = has_l ? __fadd_rn(Sy, ay) : ay; Sz = has_l ? __fadd_rn(Sz, az) : az;
+  }
+  const float dx = __fmaf_rn(-A.gA, Sx, __fmul_rn(A.sq2A, x0));
+  const float dy = __fmaf_rn(-A.gA, Sy, __fmul_rn(A.sq2A, x1));
+  const float dz = __fmaf_rn(-A.gA, Sz, __fmul_rn(A.sq2A, x2));
+  const float tx = __fadd_rn(rx, dx), ty = __fadd_rn(ry, dy), tz = __fadd_rn(rz, dz);
+  float Tx = 0.f, Ty = 0.f, Tz = 0.f, dq = 0.0f;
+  if (has_l) {
+    Tx = __fsub_rn(tx, lx); Ty = __fsub_rn(ty, ly); Tz = __fsub_rn(tz, lz);
+    dq = __fsub_rn(bond_sq(tx, ty, tz, lx, ly, lz), bond_sq(rx, ry, rz, lx, ly, lz));
+  }
+  if (has_r) {
+    const float ax = __fsub_rn(tx, qx), ay = __fsub_rn(ty, qy), az = __fsub_rn(tz, qz);
+    Tx = has_l ? __fadd_rn(Tx, ax) : ax; Ty = has_l ? __fadd_rn(Ty, ay) : ay; Tz = has_l ? __fadd_rn(Tz, az) : az;
+    const float dqr = __fsub_rn(bond_sq(tx, ty, tz, qx, qy, qz), bond_sq(rx, ry, rz, qx, qy, qz));
+    dq = has_l ? __fadd_rn(dq, dqr) : dqr;
+  }
+  const float ax_ = __fmaf_rn(A.gA, Sx, dx), ay_ = __fmaf_rn(A.gA, Sy, dy), az_ = __fmaf_rn(A.gA, Sz, dz);
+  const float bx_ = __fmaf_rn(-A.gA, Tx, dx), by_ = __fmaf_rn(-A.gA, Ty, dy), bz_ = __fmaf_rn(-A.gA, Tz, dz);
+  const float qf = __fmaf_rn(az_, az_, __fmaf_rn(ay_, ay_, __fmul_rn(ax_, ax_)));
+  const float qr = __fmaf_rn(bz_, bz_, __fmaf_rn(by_, by_, __fmul_rn(bx_, bx_)));
+  const uint32_t cell_new = cell_of<POW2>(A.grid, tx, ty, tz);
+  const float dw = __fsub_rn(__ldg(omega_t + cell_new), __ldg(omega_t + cell));
+  const float dE = __fmaf_rn(A.kb, dq, dw);
+  const float meff = __fmaf_rn(A.inv4A, __fsub_rn(qr, qf), dE);
+  // accept iff fl(meff + lnu) <= 0: the general decision routine without its dE <= 0 shortcut argument
+  // (meff <= 0 still implies acceptance, since lnu <= 0)
+  const bool acc = metropolis_accept(meff, w.w3);
+  if (acc) { rx = tx; ry = ty; rz = tz; cell = cell_new; }
   return acc;
 }
 
@@ -138,8 +187,10 @@ half_sweep_kernel(StepArgs A, uint32_t parity, uint32_t n_par /* beads of this p
     if (has_l) { lx = A.x[j - 1]; ly = A.y[j - 1]; lz = A.z[j - 1]; }
     if (has_r) { qx = A.x[j + 1]; qy = A.y[j + 1]; qz = A.z[j + 1]; }
     uint32_t cell = cell_of<POW2>(A.grid, rx, ry, rz);
-    acc = move_bead<POW2>(A, chain, i, parity, A.omega + (size_t)type * A.cells, rx, ry, rz, cell,
-                          has_l, lx, ly, lz, has_r, qx, qy, qz);
+    acc = A.gA > 0.0f ? move_bead_smc<POW2>(A, chain, i, parity, A.omega + (size_t)type * A.cells, rx, ry, rz, cell,
+                                            has_l, lx, ly, lz, has_r, qx, qy, qz)
+                      : move_bead<POW2>(A, chain, i, parity, A.omega + (size_t)type * A.cells, rx, ry, rz, cell,
+                                        has_l, lx, ly, lz, has_r, qx, qy, qz);
     if (acc) { A.x[j] = rx; A.y[j] = ry; A.z[j] = rz; }
   }
   const unsigned n_acc = __popc(__ballot_sync(0xffffffffu, acc));

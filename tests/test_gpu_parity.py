@@ -327,3 +327,28 @@ def test_mixture_generic_chain_length_lockstep_and_generated_state():
         assert all(np.array_equal(a, b_) for a, b_ in zip(g.positions(), o.positions()))
         assert g.mc_steps(6, want_accepted=True) == o.mc_steps(6)
         assert_same_state(g, o, "generated mixture, 6 steps")
+
+
+# ---- bond-force-biased moves (R24) -----------------------------------
+
+@pytest.mark.parametrize("case", ["cfg0_full", "cfg4_scaled", "cfg3_scaled_N64", "N5_T3_mixture"])
+def test_bond_force_biased_moves_parity(case):
+    A = 0.05
+    if case == "cfg0_full":
+        s = si.make_system(si.config(0))
+    elif case == "cfg4_scaled":
+        s = _scaled(4, 4097, (16, 16, 16))
+    elif case == "cfg3_scaled_N64":
+        s = _scaled(3, 2049, (16, 16, 16))
+    else:
+        s = _mixture(n_chains=900, N=5, n_single=(0, 2000, 300), grid=(8, 8, 8), seed=53)
+    o = oracle.Oracle.from_system(s)
+    o.set_smc(A)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s, smc_mobility=A) as g:
+        g.load_state(s.x, s.y, s.z)
+        done = 0
+        for upto in (1, 10):
+            assert g.mc_steps(upto - done, want_accepted=True) == o.mc_steps(upto - done)
+            done = upto
+            assert_same_state(g, o, f"{case}, bond-force-biased moves, {upto} steps")
