@@ -241,7 +241,7 @@ def run_ours(args):
     out_pos = [torch.empty(B, dtype=torch.float32).pin_memory() for _ in range(3)]
     out_den = torch.empty((w.n_types, w.n_cells), dtype=torch.int32).pin_memory()
     stream = torch.cuda.current_stream()
-    g = soma.Soma.from_system(s)
+    g = soma.Soma.from_system(s, smc_mobility=args.smc_mobility)
     if args.path:
         g.set_option("path", args.path)
     clocks = ClockSampler(local_rank)
@@ -319,7 +319,8 @@ def run_ours(args):
         "config": {"workload": w.name, "n_chains": w.n_chains, "beads_per_chain": w.N, "beads": B, "grid": list(w.grid),
                    "chiN": w.chiN, "kappaN": w.kappaN, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": f"inputs larger than L2: positions {12 * B / 1e6:.0f} MB + grids {12 * w.n_types * w.n_cells / 1e6:.0f} MB per step",
-                   "mc_steps_per_s": world * args.steps / (ms * 1e-3)},
+                   "mc_steps_per_s": world * args.steps / (ms * 1e-3),
+                   **({"moves": f"bond-force-biased, A = {args.smc_mobility}"} if args.smc_mobility > 0 else {})},
         "clocks": clk, "gpu_launches": int(launches),
         "e2e": {"value": e2e_moves / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 12 * B / S,
                 "d2h_bytes_per_step": (12 * B + 4 * w.n_types * w.n_cells) / S, "mc_steps": S, "ms": e2e_ms,
@@ -348,6 +349,8 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--path", type=int, default=0, help="library kernel path: 0 auto (fused), 1 generic, 2 fused, 3/4 windowed kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--smc-mobility", type=float, default=0.0,
+                    help="A > 0: bond-force-biased moves (DESIGN.md R24) instead of the configs' uniform moves; not the headline metric")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
     args = ap.parse_args()

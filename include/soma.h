@@ -68,7 +68,7 @@ typedef struct soma_params {
                                    mc_polymer_iteration performs (SURVEY.md section 8(f) row
                                    f1; R24): r' = r + A F_bonded(r) + sqrt(2A) xi, xi standard normal,
                                    accepted with min(1, e^-dE T(r'->r)/T(r->r')); move_halfwidth is then
-                                   unused.  Runs on the generic kernels (any N).  Units: length^2/kT  */
+                                   unused.  Runs on the fused or the generic kernels (not the windowed ones).  Units: length^2/kT  */
   uint32_t grid[3];             /* cells per axis                                               */
   uint32_t reserved2;           /* must be 0                                                    */
   float box[3];                 /* periodic box lengths; cell size = box/grid                   */

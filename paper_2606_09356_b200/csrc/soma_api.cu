@@ -401,7 +401,8 @@ int launch_fused_p(soma_handle* h) {
   const bool fast = h->tile_fast && h->pow2;       // exact one-FFMA shortcuts apply (see fused_move)
 #define SOMA_LAUNCH_FUSED(POW2, MULTI)                                                                          \
   do {                                                                                                          \
-    if (fast && POW2) fused_step_kernel<P, POW2, MULTI, POW2><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb); \
+    if (h->smcA > 0.0f) fused_step_kernel<P, POW2, MULTI, false, true><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb); \
+    else if (fast && POW2) fused_step_kernel<P, POW2, MULTI, POW2><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb); \
     else fused_step_kernel<P, POW2, MULTI, false><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb);    \
   } while (0)
   if (h->pow2) { if (multi) SOMA_LAUNCH_FUSED(true, true); else SOMA_LAUNCH_FUSED(true, false); }
@@ -425,7 +426,7 @@ int launch_fused(soma_handle* h) {
 }
 
 bool use_fused(const soma_handle* h) {
-  if (h->path == 1 || h->smcA > 0.0f) return false;      // bond-force-biased moves run on the generic kernels
+  if (h->path == 1) return false;
   return fused_lanes(h->N) != 0;
 }
 bool use_tile(const soma_handle* h) {

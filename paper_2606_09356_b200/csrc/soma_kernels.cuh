@@ -227,8 +227,10 @@ bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint64_t B, const float* __res
 #ifndef SOMA_FUSED_MIN_BLOCKS
 #define SOMA_FUSED_MIN_BLOCKS 4      /* 62 registers: 4 blocks per SM; measured best on cfg4 (3: 1.61 ms, 4: 1.13, 5: 1.16, 6: 1.28) */
 #endif
-template <int P, bool POW2, bool MULTI_PAT, bool FAST>
-__global__ void __launch_bounds__(256, SOMA_FUSED_MIN_BLOCKS)
+// SMC: bond-force-biased moves (R24) instead of uniform ones; their double-precision normal
+// deviates need more registers, so that variant runs 2 blocks per SM.
+template <int P, bool POW2, bool MULTI_PAT, bool FAST, bool SMC = false>
+__global__ void __launch_bounds__(256, SMC ? 2 : SOMA_FUSED_MIN_BLOCKS)
 fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
   constexpr int G = 32 / P;                                   // chains per warp
   const uint32_t lane = threadIdx.x & 31u;
@@ -303,7 +305,10 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
     const float lz = __shfl_up_sync(0xffffffffu, oz, 1, P);
     float qA = bond_sq(ex, ey, ez, ox, oy, oz);
     float qB = bond_sq(ex, ey, ez, lx, ly, lz);
-    {
+    if (SMC) {
+      const bool acc = move_bead_smc<POW2>(A, chain, 2u * l, 0u, om0, ex, ey, ez, cell_e, l > 0, lx, ly, lz, true, ox, oy, oz);
+      n_acc += (acc && live) ? 1u : 0u;
+    } else {
       const bool acc = fused_move<POW2, FAST, true>(A, F, L0, c0_1, om0, ex, ey, ez, cell_e,
                                                     lx, ly, lz, qB, ox, oy, oz, qA, hl);
       n_acc += (acc && live) ? 1u : 0u;
@@ -314,8 +319,9 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
       const float qy = __shfl_down_sync(0xffffffffu, ey, 1, P);
       const float qz = __shfl_down_sync(0xffffffffu, ez, 1, P);
       float qR = __shfl_down_sync(0xffffffffu, qB, 1, P);
-      const bool acc = fused_move<POW2, FAST, false>(A, F, L1, c0_1, om1, ox, oy, oz, cell_o,
-                                                     ex, ey, ez, qA, qx, qy, qz, qR, hr);
+      const bool acc = SMC ? move_bead_smc<POW2>(A, chain, 2u * l + 1u, 1u, om1, ox, oy, oz, cell_o, true, ex, ey, ez, l + 1 < P, qx, qy, qz)
+                           : fused_move<POW2, FAST, false>(A, F, L1, c0_1, om1, ox, oy, oz, cell_o,
+                                                           ex, ey, ez, qA, qx, qy, qz, qR, hr);
       n_acc += (acc && live) ? 1u : 0u;
     }
     if (live) {

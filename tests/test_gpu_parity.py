@@ -331,8 +331,9 @@ def test_mixture_generic_chain_length_lockstep_and_generated_state():
 
 # ---- bond-force-biased moves (R24) -----------------------------------
 
+@pytest.mark.parametrize("path", [FUSED, GENERIC])
 @pytest.mark.parametrize("case", ["cfg0_full", "cfg4_scaled", "cfg3_scaled_N64", "N5_T3_mixture"])
-def test_bond_force_biased_moves_parity(case):
+def test_bond_force_biased_moves_parity(case, path):
     A = 0.05
     if case == "cfg0_full":
         s = si.make_system(si.config(0))
@@ -345,7 +346,10 @@ def test_bond_force_biased_moves_parity(case):
     o = oracle.Oracle.from_system(s)
     o.set_smc(A)
     o.load_state(s.x, s.y, s.z)
-    with gpu_system(s, smc_mobility=A) as g:
+    if case == "N5_T3_mixture" and path == FUSED:
+        pytest.skip("odd N: generic kernels only")
+    with gpu_system(s, path=path, smc_mobility=A) as g:
+        assert g.counters()["path"] == path
         g.load_state(s.x, s.y, s.z)
         done = 0
         for upto in (1, 10):
