@@ -71,3 +71,21 @@ def test_full_size_configs_bit_exact(cfg, steps):
         assert np.array_equal(g.density(), o.density())
         assert np.array_equal(g.omega().view(np.uint32), o.omega().view(np.uint32))
     o.close()
+
+
+def test_cfg2_full_size_bond_force_biased_moves_bit_exact():
+    """configs[2] at full size (16.8 M beads) with the paper's bond-force-biased moves (R24) on
+    the fused kernel: 33.6 M Gaussian-driven moves, every coordinate bit-identical to the oracle."""
+    w = si.config(2)
+    s = si.make_system(w)
+    o = oracle.Oracle.from_system(s)
+    o.set_smc(0.05)
+    o.load_state(s.x, s.y, s.z)
+    acc_o = o.mc_steps(2)
+    with gpu_system(s, smc_mobility=0.05) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert g.mc_steps(2, want_accepted=True) == acc_o
+        for a, b_ in zip(g.positions(), o.positions()):
+            assert np.array_equal(a, b_)
+        assert np.array_equal(g.density(), o.density())
+    o.close()
