@@ -234,45 +234,46 @@ inline double delta_energy_f64(const Oracle& o, uint64_t c, uint32_t i, float nx
 }
 
 // ---- standard normal deviates with no library function in them (R24) -------------------
-// Box-Muller in double from U = (w + 0.5) 2^-32, with the logarithm and the sine / cosine written out
-// as fixed sequences of IEEE operations (+, *, /, fma, sqrt), so that any conforming implementation
-// produces the same bits.  Accuracy ~1e-15, far below what the fp32 result keeps.
-inline double det_log(double x) {                       // x in (0, 1]
-  uint64_t bits; std::memcpy(&bits, &x, 8);
-  int e = (int)((bits >> 52) & 0x7ff) - 1023;
-  bits = (bits & 0x000fffffffffffffull) | 0x3ff0000000000000ull;
-  double m; std::memcpy(&m, &bits, 8);                  // m in [1, 2)
-  if (m > 1.4142135623730951) { m = m * 0.5; e += 1; }  // m in (sqrt 1/2, sqrt 2]
-  const double sq = (m - 1.0) / (m + 1.0), z = sq * sq; // log m = 2 atanh(sq) = 2 sq (1 + z/3 + z^2/5 + ...)
-  double p = 1.0 / 27.0;
-  p = std::fma(p, z, 1.0 / 25.0); p = std::fma(p, z, 1.0 / 23.0); p = std::fma(p, z, 1.0 / 21.0);
-  p = std::fma(p, z, 1.0 / 19.0); p = std::fma(p, z, 1.0 / 17.0); p = std::fma(p, z, 1.0 / 15.0);
-  p = std::fma(p, z, 1.0 / 13.0); p = std::fma(p, z, 1.0 / 11.0); p = std::fma(p, z, 1.0 / 9.0);
-  p = std::fma(p, z, 1.0 / 7.0);  p = std::fma(p, z, 1.0 / 5.0);  p = std::fma(p, z, 1.0 / 3.0);
-  const double lm = std::fma(2.0 * sq, z * p, 2.0 * sq);
-  return std::fma((double)e, 0.6931471805599453, lm);
+// Box-Muller in fp32 from U = ((w >> 9) + 0.5) 2^-23 (exact in fp32), with the logarithm and the
+// sine / cosine written out as fixed sequences of IEEE fp32 operations (+, *, /, fma, sqrt), so that
+// any conforming implementation produces the same bits.  Accuracy ~2e-7, the resolution of the fp32
+// positions the deviates are added to.
+inline float det_log(float x) {                         // x in (0, 1]
+  uint32_t bits; std::memcpy(&bits, &x, 4);
+  int e = (int)((bits >> 23) & 0xff) - 127;
+  bits = (bits & 0x007fffffu) | 0x3f800000u;
+  float m; std::memcpy(&m, &bits, 4);                   // m in [1, 2)
+  if (m > 1.41421354f) { m = m * 0.5f; e += 1; }        // m in (sqrt 1/2, sqrt 2]
+  const float sq = (m - 1.0f) / (m + 1.0f), z = sq * sq; // log m = 2 atanh(sq) = 2 sq (1 + z/3 + z^2/5 + ...)
+  float p = 1.0f / 11.0f;
+  p = fmaf(p, z, 1.0f / 9.0f); p = fmaf(p, z, 1.0f / 7.0f); p = fmaf(p, z, 1.0f / 5.0f); p = fmaf(p, z, 1.0f / 3.0f);
+  const float lm = fmaf(2.0f * sq, z * p, 2.0f * sq);
+  return fmaf((float)e, 0.693147182f, lm);
 }
-inline void det_sincos_2pi(double u, double* sn, double* cs) {   // sin, cos of 2 pi u, u in (0, 1)
-  const double t = u * 4.0;                              // quarter turns
-  const double k = std::floor(t + 0.5);
-  const double r = (t - k) * 1.5707963267948966, z = r * r;   // r in [-pi/4, pi/4]
-  double ps = -1.0 / 355687428096000.0;                  // sin r = r (1 - z/3! + z^2/5! - ... - z^8/17!)
-  ps = std::fma(ps, z, 1.0 / 1307674368000.0); ps = std::fma(ps, z, -1.0 / 6227020800.0);
-  ps = std::fma(ps, z, 1.0 / 39916800.0);      ps = std::fma(ps, z, -1.0 / 362880.0);
-  ps = std::fma(ps, z, 1.0 / 5040.0);          ps = std::fma(ps, z, -1.0 / 120.0);
-  ps = std::fma(ps, z, 1.0 / 6.0);
-  const double s0 = std::fma(-r * z, ps, r);
-  double pc = 1.0 / 20922789888000.0;                    // cos r = 1 - z/2! + z^2/4! - ... + z^8/16!
-  pc = std::fma(pc, z, -1.0 / 87178291200.0); pc = std::fma(pc, z, 1.0 / 479001600.0);
-  pc = std::fma(pc, z, -1.0 / 3628800.0);     pc = std::fma(pc, z, 1.0 / 40320.0);
-  pc = std::fma(pc, z, -1.0 / 720.0);         pc = std::fma(pc, z, 1.0 / 24.0);
-  pc = std::fma(pc, z, -0.5);
-  const double c0 = std::fma(pc, z, 1.0);
+inline void det_sincos_2pi(float u, float* sn, float* cs) {   // sin, cos of 2 pi u, u in (0, 1)
+  const float t = u * 4.0f;                              // quarter turns
+  const float k = floorf(t + 0.5f);
+  const float r = (t - k) * 1.57079637f, z = r * r;      // r in [-pi/4, pi/4]
+  float ps = 1.0f / 362880.0f;                           // sin r = r (1 - z/3! + z^2/5! - z^3/7! + z^4/9!)
+  ps = fmaf(ps, z, -1.0f / 5040.0f); ps = fmaf(ps, z, 1.0f / 120.0f); ps = fmaf(ps, z, -1.0f / 6.0f);
+  const float s0 = fmaf(r * z, ps, r);
+  float pc = -1.0f / 3628800.0f;                         // cos r = 1 - z/2! + z^2/4! - z^3/6! + z^4/8! - z^5/10!
+  pc = fmaf(pc, z, 1.0f / 40320.0f); pc = fmaf(pc, z, -1.0f / 720.0f); pc = fmaf(pc, z, 1.0f / 24.0f); pc = fmaf(pc, z, -0.5f);
+  const float c0 = fmaf(pc, z, 1.0f);
   const int q = (int)k & 3;                              // rotate by k quarter turns
   *sn = q == 0 ? s0 : q == 1 ? c0 : q == 2 ? -s0 : -c0;
   *cs = q == 0 ? c0 : q == 1 ? -s0 : q == 2 ? -c0 : s0;
 }
-inline double unit32(uint32_t w) { return ((double)w + 0.5) * 0x1p-32; }
+inline float unit23(uint32_t w) { return ((float)(w >> 9) + 0.5f) * 0x1p-23f; }
+// xi[0..2] of a move from the words of its two Philox calls (domain 0: w, domain 2: v)
+inline void smc_deviates(const uint32_t* w, const uint32_t* v, float* xi) {
+  float sn, cs, sn2, cs2;
+  const float ra = sqrtf(-2.0f * det_log(unit23(w[0])));
+  det_sincos_2pi(unit23(w[1]), &sn, &cs);
+  const float rb = sqrtf(-2.0f * det_log(unit23(v[0])));
+  det_sincos_2pi(unit23(v[1]), &sn2, &cs2);
+  xi[0] = ra * cs; xi[1] = ra * sn; xi[2] = rb * cs2;
+}
 
 // Bond-force-biased ("smart Monte Carlo") trial move of bead (c, i), R24 (PAPER.md:41, :77:
 // "bond-force-biased Monte-Carlo", "biased trial moves").  S = sum over the bonded neighbours of
@@ -280,7 +281,7 @@ inline double unit32(uint32_t w) { return ((double)w + 0.5) * 0x1p-32; }
 //   dr_d = fma(-gA, S_d, sq2A * xi_d),  r'_d = r_d + dr_d,  gA = fl(A * fl(2 kb)).
 // With S' the same sum at r', qf = |dr + gA S|^2 (forward), qr = |dr - gA S'|^2 (reverse), each
 // fma(z,z, fma(y,y, x*x)); margin m = fma(inv4A, qr - qf, dE) + lnu, dE as for uniform moves; accept iff m <= 0.
-// xi_0, xi_1 = Box-Muller pair of words (w0, w1) of the move's Philox call (domain 0); xi_2 = cosine
+// xi_0, xi_1 = fp32 Box-Muller pair of words (w0, w1) of the move's Philox call (domain 0); xi_2 = cosine
 // member of the pair of words (v0, v1) of a second call with domain 2; u from w3 as before.
 inline int trial_move_smc(Oracle& o, uint64_t c, uint32_t i, uint32_t parity, double* margin64) {
   const uint32_t hi = (uint32_t)(o.t >> 32) << 16;
@@ -290,12 +291,8 @@ inline int trial_move_smc(Oracle& o, uint64_t c, uint32_t i, uint32_t parity, do
   uint32_t w[4], v[4];
   philox4x32_10(ctr, key, w);
   philox4x32_10(ctr2, key, v);
-  double sn, cs, sn2, cs2;
-  const double ra = std::sqrt(-2.0 * det_log(unit32(w[0])));
-  det_sincos_2pi(unit32(w[1]), &sn, &cs);
-  const double rb = std::sqrt(-2.0 * det_log(unit32(v[0])));
-  det_sincos_2pi(unit32(v[1]), &sn2, &cs2);
-  const float xi[3] = {(float)(ra * cs), (float)(ra * sn), (float)(rb * cs2)};
+  float xi[3];
+  smc_deviates(w, v, xi);
   const float u = umap(w[3]);
   const uint64_t j = c * o.N + i;
   const float r[3] = {o.x[j], o.y[j], o.z[j]};
@@ -555,12 +552,9 @@ void oracle_smc_draws(void* h, uint64_t c, uint32_t i, uint32_t parity, double* 
   const uint32_t key[2] = {(uint32_t)o.seed, (uint32_t)(o.seed >> 32)};
   uint32_t w[4], v[4];
   philox4x32_10(ctr, key, w); philox4x32_10(ctr2, key, v);
-  double sn, cs, sn2, cs2;
-  const double ra = std::sqrt(-2.0 * det_log(unit32(w[0])));
-  det_sincos_2pi(unit32(w[1]), &sn, &cs);
-  const double rb = std::sqrt(-2.0 * det_log(unit32(v[0])));
-  det_sincos_2pi(unit32(v[1]), &sn2, &cs2);
-  out[0] = ra * cs; out[1] = ra * sn; out[2] = rb * cs2; out[3] = (double)umap(w[3]);
+  float xi[3];
+  smc_deviates(w, v, xi);
+  out[0] = xi[0]; out[1] = xi[1]; out[2] = xi[2]; out[3] = (double)umap(w[3]);
 }
 // fma(inv4A, qr - qf, dE) of moving bead `bead` to (nx, ny, nz): the bond-force-biased margin without ln u
 float oracle_smc_margin(void* h, uint64_t bead, float nx, float ny, float nz) {
@@ -587,9 +581,11 @@ float oracle_smc_margin(void* h, uint64_t bead, float nx, float ny, float nz) {
   const float qr = fmaf(b_[2], b_[2], fmaf(b_[1], b_[1], b_[0] * b_[0]));
   return fmaf(o.inv4A, qr - qf, delta_energy(o, c, i, nx, ny, nz));
 }
-void oracle_det_functions(double x, double* out) {       // out = {det_log(x), sin(2 pi x), cos(2 pi x)}
-  out[0] = det_log(x);
-  det_sincos_2pi(x, &out[1], &out[2]);
+void oracle_det_functions(double x, double* out) {       // out = {det_log(x), sin(2 pi x), cos(2 pi x)}, fp32 routines
+  float sn, cs;
+  out[0] = det_log((float)x);
+  det_sincos_2pi((float)x, &sn, &cs);
+  out[1] = sn; out[2] = cs;
 }
 
 // single-bead molecules: n_single[T] (call right after oracle_create, before any state is loaded)

@@ -157,54 +157,45 @@ __device__ __forceinline__ bool metropolis_accept_fma(float dE, uint32_t w3) {
 }
 
 // ---- standard normal deviates for the bond-force-biased move (R24) -------------------
-// Box-Muller in double with the logarithm and sine / cosine spelled out in IEEE operations only
-// (add, mul, div, fma, sqrt -- each correctly rounded on any conforming implementation), so the
-// deviates do not depend on a math library.  Written from the definition in DESIGN.md R24.
-__device__ __forceinline__ double ln_ieee(double x) {               // x in (0, 1]
-  long long bits = __double_as_longlong(x);
-  int e = (int)((bits >> 52) & 0x7ff) - 1023;
-  double m = __longlong_as_double((bits & 0x000fffffffffffffLL) | 0x3ff0000000000000LL);   // [1, 2)
-  if (m > 1.4142135623730951) { m = __dmul_rn(m, 0.5); e += 1; }
-  const double q = __ddiv_rn(__dadd_rn(m, -1.0), __dadd_rn(m, 1.0)), z = __dmul_rn(q, q);
-  double p = 1.0 / 27.0;
-  p = __fma_rn(p, z, 1.0 / 25.0); p = __fma_rn(p, z, 1.0 / 23.0); p = __fma_rn(p, z, 1.0 / 21.0);
-  p = __fma_rn(p, z, 1.0 / 19.0); p = __fma_rn(p, z, 1.0 / 17.0); p = __fma_rn(p, z, 1.0 / 15.0);
-  p = __fma_rn(p, z, 1.0 / 13.0); p = __fma_rn(p, z, 1.0 / 11.0); p = __fma_rn(p, z, 1.0 / 9.0);
-  p = __fma_rn(p, z, 1.0 / 7.0);  p = __fma_rn(p, z, 1.0 / 5.0);  p = __fma_rn(p, z, 1.0 / 3.0);
-  const double q2 = __dmul_rn(2.0, q);
-  const double lm = __fma_rn(q2, __dmul_rn(z, p), q2);
-  return __fma_rn((double)e, 0.6931471805599453, lm);
+// fp32 Box-Muller from U = ((w >> 9) + 0.5) 2^-23 with the logarithm and sine / cosine spelled out
+// in IEEE fp32 operations only (add, mul, div, fma, sqrt -- each correctly rounded on any conforming
+// implementation), so the deviates do not depend on a math library.  Written from DESIGN.md R24.
+__device__ __forceinline__ float ln_ieee(float x) {                  // x in (0, 1]
+  const uint32_t bits = __float_as_uint(x);
+  int e = (int)((bits >> 23) & 0xffu) - 127;
+  float m = __uint_as_float((bits & 0x007fffffu) | 0x3f800000u);   // [1, 2)
+  if (m > 1.41421354f) { m = __fmul_rn(m, 0.5f); e += 1; }
+  const float q = __fdiv_rn(__fadd_rn(m, -1.0f), __fadd_rn(m, 1.0f)), z = __fmul_rn(q, q);
+  float p = 1.0f / 11.0f;
+  p = __fmaf_rn(p, z, 1.0f / 9.0f); p = __fmaf_rn(p, z, 1.0f / 7.0f); p = __fmaf_rn(p, z, 1.0f / 5.0f); p = __fmaf_rn(p, z, 1.0f / 3.0f);
+  const float q2 = __fmul_rn(2.0f, q);
+  const float lm = __fmaf_rn(q2, __fmul_rn(z, p), q2);
+  return __fmaf_rn((float)e, 0.693147182f, lm);
 }
-__device__ __forceinline__ void sincos_2pi_ieee(double u, double& sn, double& cs) {   // u in (0, 1)
-  const double t = __dmul_rn(u, 4.0);
-  const double k = floor(__dadd_rn(t, 0.5));
-  const double r = __dmul_rn(__dadd_rn(t, -k), 1.5707963267948966), z = __dmul_rn(r, r);
-  double ps = -1.0 / 355687428096000.0;
-  ps = __fma_rn(ps, z, 1.0 / 1307674368000.0); ps = __fma_rn(ps, z, -1.0 / 6227020800.0);
-  ps = __fma_rn(ps, z, 1.0 / 39916800.0);      ps = __fma_rn(ps, z, -1.0 / 362880.0);
-  ps = __fma_rn(ps, z, 1.0 / 5040.0);          ps = __fma_rn(ps, z, -1.0 / 120.0);
-  ps = __fma_rn(ps, z, 1.0 / 6.0);
-  const double s0 = __fma_rn(__dmul_rn(-r, z), ps, r);
-  double pc = 1.0 / 20922789888000.0;
-  pc = __fma_rn(pc, z, -1.0 / 87178291200.0); pc = __fma_rn(pc, z, 1.0 / 479001600.0);
-  pc = __fma_rn(pc, z, -1.0 / 3628800.0);     pc = __fma_rn(pc, z, 1.0 / 40320.0);
-  pc = __fma_rn(pc, z, -1.0 / 720.0);         pc = __fma_rn(pc, z, 1.0 / 24.0);
-  pc = __fma_rn(pc, z, -0.5);
-  const double c0 = __fma_rn(pc, z, 1.0);
+__device__ __forceinline__ void sincos_2pi_ieee(float u, float& sn, float& cs) {   // u in (0, 1)
+  const float t = __fmul_rn(u, 4.0f);
+  const float k = floorf(__fadd_rn(t, 0.5f));
+  const float r = __fmul_rn(__fadd_rn(t, -k), 1.57079637f), z = __fmul_rn(r, r);
+  float ps = 1.0f / 362880.0f;
+  ps = __fmaf_rn(ps, z, -1.0f / 5040.0f); ps = __fmaf_rn(ps, z, 1.0f / 120.0f); ps = __fmaf_rn(ps, z, -1.0f / 6.0f);
+  const float s0 = __fmaf_rn(__fmul_rn(r, z), ps, r);
+  float pc = -1.0f / 3628800.0f;
+  pc = __fmaf_rn(pc, z, 1.0f / 40320.0f); pc = __fmaf_rn(pc, z, -1.0f / 720.0f); pc = __fmaf_rn(pc, z, 1.0f / 24.0f); pc = __fmaf_rn(pc, z, -0.5f);
+  const float c0 = __fmaf_rn(pc, z, 1.0f);
   const int qd = (int)k & 3;
   sn = qd == 0 ? s0 : qd == 1 ? c0 : qd == 2 ? -s0 : -c0;
   cs = qd == 0 ? c0 : qd == 1 ? -s0 : qd == 2 ? -c0 : s0;
 }
-__device__ __forceinline__ double unit32(uint32_t w) { return __dmul_rn(__dadd_rn((double)w, 0.5), 0x1p-32); }
+__device__ __forceinline__ float unit23(uint32_t w) { return __fmul_rn(__fadd_rn((float)(w >> 9), 0.5f), 0x1p-23f); }
 
 // xi[0..2]: deviates of a move from the words of its two Philox calls (domain 0: w, domain 2: v)
 __device__ __forceinline__ void smc_deviates(const Words4& w, const Words4& v, float& x0, float& x1, float& x2) {
-  double sn, cs, sn2, cs2;
-  const double ra = sqrt(__dmul_rn(-2.0, ln_ieee(unit32(w.w0))));
-  sincos_2pi_ieee(unit32(w.w1), sn, cs);
-  const double rb = sqrt(__dmul_rn(-2.0, ln_ieee(unit32(v.w0))));
-  sincos_2pi_ieee(unit32(v.w1), sn2, cs2);
-  x0 = (float)__dmul_rn(ra, cs); x1 = (float)__dmul_rn(ra, sn); x2 = (float)__dmul_rn(rb, cs2);
+  float sn, cs, sn2, cs2;
+  const float ra = __fsqrt_rn(__fmul_rn(-2.0f, ln_ieee(unit23(w.w0))));
+  sincos_2pi_ieee(unit23(w.w1), sn, cs);
+  const float rb = __fsqrt_rn(__fmul_rn(-2.0f, ln_ieee(unit23(v.w0))));
+  sincos_2pi_ieee(unit23(v.w1), sn2, cs2);
+  x0 = __fmul_rn(ra, cs); x1 = __fmul_rn(ra, sn); x2 = __fmul_rn(rb, cs2);
 }
 
 // ---- geometry ----

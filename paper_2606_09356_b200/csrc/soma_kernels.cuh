@@ -227,8 +227,8 @@ bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint64_t B, const float* __res
 #ifndef SOMA_FUSED_MIN_BLOCKS
 #define SOMA_FUSED_MIN_BLOCKS 4      /* 62 registers: 4 blocks per SM; measured best on cfg4 (3: 1.61 ms, 4: 1.13, 5: 1.16, 6: 1.28) */
 #endif
-// SMC: bond-force-biased moves (R24) instead of uniform ones; their double-precision normal
-// deviates need more registers: that variant runs 3 blocks per SM (80 registers; measured 2 / 3 / 4 blocks = 3.19 / 2.87 / 2.92 ms on cfg4).
+// SMC: bond-force-biased moves (R24) instead of uniform ones; their normal
+// deviates need more registers: that variant runs 3 blocks per SM (80 registers; measured 3 / 4 blocks = 2.02 / 2.13 ms on cfg4).
 template <int P, bool POW2, bool MULTI_PAT, bool FAST, bool SMC = false>
 __global__ void __launch_bounds__(256, SMC ? 3 : SOMA_FUSED_MIN_BLOCKS)
 fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
