@@ -321,8 +321,9 @@ class Soma:
     def from_system(cls, s, **kw) -> "Soma":
         """`s` is a scmf_inputs.System (duck-typed)."""
         w = s.workload
+        kw.setdefault("n_single", getattr(s, "n_single", None))
         return cls(w.n_chains, w.N, w.n_types, s.type_patterns, s.chain_pattern, w.b, s.chiN,
-                   w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed, n_single=getattr(s, "n_single", None), **kw)
+                   w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed, **kw)
 
     def close(self):
         if getattr(self, "_h", None):

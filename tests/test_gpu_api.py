@@ -169,3 +169,30 @@ def test_launch_counter_counts_kernels(small):
         before = g.counters()
         g.mc_steps(5)
         assert g.counters()["launches"] - before["launches"] == 5 * 4   # even, odd, bin, omega
+
+
+def test_error_codes_of_the_calls_beyond_the_six(soma, small):
+    s = small
+    lib = soma.load_library()
+    with gpu_system(s) as g:
+        h = g._h
+        v = soma.soma_validation()
+        assert lib.soma_validate_state(h, C.byref(v)) == soma.SOMA_ESTATE          # nothing loaded yet
+        assert lib.soma_validate_state(h, None) == soma.SOMA_EINVAL
+        assert lib.soma_generate_state(h, 1, 1 << 48) == soma.SOMA_EINVAL
+        ext = np.full((2, 512), 0.25, dtype=np.float32)
+        g.set_external_field(ext)                                                   # allowed before a state exists ...
+        g.load_state(s.x, s.y, s.z)
+        o = oracle.Oracle.from_system(s)
+        o.load_state(s.x, s.y, s.z)
+        o.set_external_field(ext)
+        assert np.array_equal(g.omega().view(np.uint32), o.omega().view(np.uint32))   # ... and applied by the load
+    # parameter validation at create: negative mobility, too many molecules
+    for bad in (dict(smc_mobility=-1.0), dict(n_single=np.array([1 << 33, 0], dtype=np.uint64))):
+        with pytest.raises(soma.SomaError) as e:
+            soma.Soma.from_system(s, **bad)
+        assert e.value.code == soma.SOMA_EINVAL
+    # the windowed kernels do not implement the bond-force-biased move: the library falls back to the fused kernel
+    with gpu_system(si.make_system(si.scaled(si.config(4), 8192, (32, 32, 32))), smc_mobility=0.05) as g:
+        g.set_option("path", 4)
+        assert g.counters()["path"] == 2
