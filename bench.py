@@ -244,6 +244,9 @@ def run_ours(args):
     g = soma.Soma.from_system(s, smc_mobility=args.smc_mobility)
     if args.path:
         g.set_option("path", args.path)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        g.set_option(k, int(v))
     clocks = ClockSampler(local_rank)
 
     # ---- device-resident timing: K steps after W warm-up steps --------------------------------
@@ -292,8 +295,8 @@ def run_ours(args):
     move_ms, omega_ms = kt["move_bin_ms"] / n_t, kt["omega_ms"] / n_t
     achieved = ab["move_bin_kernel"] / (move_ms * 1e-3) / 1e9
     path_now = g_path
-    kname = {1: "half_sweep_kernel x2 + bin_kernel (rows a1+a2+a3+a5)", 2: "fused_step_kernel (rows a1+a2+a3+a5)",
-             3: "tile_step_kernel (rows a1+a2+a3+a5)", 4: "sweep_step_kernel (rows a1+a2+a3+a5)"}[path_now]
+    kname = {1: "half_sweep_kernel x2 + bin_kernel (rows a1+a2+a3+a5)", 2: "lean_step_kernel (rows a1+a2+a3+a5)",
+             3: "lean_step_kernel, bead counts in shared-memory windows (rows a1+a2+a3+a5)"}[path_now]
     traffic = args.traffic
     if traffic is None and path_now == 2 and args.config == 4:
         traffic = NCU_TRAFFIC_CFG4_FUSED
@@ -348,8 +351,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: 134 M beads)")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--path", type=int, default=0, help="library kernel path: 0 auto (fused), 1 generic, 2 fused, 3/4 windowed kernels")
+    ap.add_argument("--path", type=int, default=0, help="library kernel path: 0 auto, 1 generic, 2 fused, 3 fused with windowed counts")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=INT", help="soma_set_option(NAME, INT) before the run (tuning)")
     ap.add_argument("--smc-mobility", type=float, default=0.0,
                     help="A > 0: bond-force-biased moves (DESIGN.md R24) instead of the configs' uniform moves; not the headline metric")
     ap.add_argument("--traffic", type=float, default=None,

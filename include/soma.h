@@ -68,7 +68,7 @@ typedef struct soma_params {
                                    mc_polymer_iteration performs (SURVEY.md section 8(f) row
                                    f1; R24): r' = r + A F_bonded(r) + sqrt(2A) xi, xi standard normal,
                                    accepted with min(1, e^-dE T(r'->r)/T(r->r')); move_halfwidth is then
-                                   unused.  Runs on the fused or the generic kernels (not the windowed ones).  Units: length^2/kT  */
+                                   unused.  Runs on the general fused or the generic kernels.  Units: length^2/kT  */
   uint32_t grid[3];             /* cells per axis                                               */
   uint32_t reserved2;           /* must be 0                                                    */
   float box[3];                 /* periodic box lengths; cell size = box/grid                   */
@@ -165,18 +165,19 @@ const char *soma_last_error(const soma_t *h);
 /* Tuning / test switches.  Names:
  *   "path"            0 = automatic (the fused kernel where N allows it, else the generic ones),
  *                     1 = generic kernels (4 launches/step, any N),
- *                     2 = fused chain-in-registers kernel (N = 2P, P a power of two <= 32; else EINVAL),
- *                     3 = first windowed kernel (soma_tile.cuh): omega and density slabs of a column in a
- *                         shared-memory ring, moved by TMA (as 2, plus: power-of-two grid axes >= 16
- *                         and >= the window; else EINVAL),
- *                     4 = swept-window kernel (soma_sweep.cuh): the same data flow with a branch-free
- *                         body for chains inside their window (same conditions as 3)
- *   "tile_cx"         segment length along x in cells (default 64); "tile_cy|cz" column core (8, 8);
- *   "tile_hx|hy|hz"   halo in cells (8, 8, 8); "tile_slice" cells per x slice (2); "tile_ring" ring
- *                     slots (0 = as many as fit); "tile_margin" (1) chains with a bead this close to a
- *                     window face sort behind the others; "tile_fast" 0 = general arithmetic only;
- *   "tile_threads"    512, 768 or 1024 threads per CTA of the windowed kernels.  A combination they
- *                     cannot use switches them off (see soma_get_counters [3])
+ *                     2 = fused chain-in-registers kernel (N = 2P, P a power of two <= 32; else EINVAL).
+ *                         Where the geometry allows it -- power-of-two grid, cell size a power of two
+ *                         <= 1, move half-width a power of two, uniform moves -- this is the lean kernel
+ *                         of soma_lean.cuh, else the general one of soma_kernels.cuh,
+ *                     3 = the lean kernel with one block per tile of the box, bead counts in a
+ *                         shared-memory window (tile + halo) added to the density grid by bulk reduce-adds
+ *                         (conditions of the lean kernel, plus: tiles divide the grid, window <= grid and
+ *                         <= 56 KB, z extents multiples of 4 cells; else EINVAL)
+ *   "win_cx|cy|cz"    tile core in cells (default 8, 8, 8); "win_hx|hy|hz" halo in cells (4, 4, 4).  A
+ *                     combination path 3 cannot use switches it off (see soma_get_counters [3])
+ *   "win_auto"        1 = path 0 takes path 3 where it can run, 0 = path 0 takes path 2
+ *   "fused_lean"      0 = path 2 always runs the general fused kernel (default 1)
+ *   "fused_carveout"  preferred shared-memory carve-out of the fused kernel in percent (-1 = driver default; tuning)
  *   "kernel_timing"   1 = record CUDA events on the handle's stream around the kernels of every step
  *                     (read them with soma_get_kernel_times), 0 = off (default)
  *   "resort_interval" re-order the chains in memory by position at soma_load_state and then every k
@@ -188,7 +189,7 @@ const char *soma_last_error(const soma_t *h);
 int soma_set_option(soma_t *h, const char *name, int64_t value);
 
 /* Counters since soma_create: [0] kernels launched by this library, [1] MC steps done,
- * [2] chain re-orderings done; [3] the kernel path the next step will take (1, 2, 3 or 4).
+ * [2] chain re-orderings done; [3] the kernel path the next step will take (1, 2 or 3).
  * `out` is a host pointer to 4 uint64. */
 int soma_get_counters(const soma_t *h, uint64_t *out);
 
@@ -211,10 +212,13 @@ int soma_debug_set_omega(soma_t *h, const float *omega);
  * philox: ctr [n][4], key [2] -> out [n][4];  maps: words [n] -> tmap [n], u [n], lnu [n] (lnu by the
  * kernel's slow path, i.e. the value it uses when a move is near the threshold), lnu_fast [n] (may
  * be NULL; the hardware-logarithm value that decides every move outside the +-1e-4 band);
- * accept: dE [n], words [n] -> decision [n] (0/1) by the kernel's full fast+slow accept routine. */
+ * accept: dE [n], words [n] -> decision [n] (0/1) by the kernel's full fast+slow accept routine
+ * (generic kernels); accept_fma: the same rule by the routine of the fused kernels (one FFMA on the
+ * hardware logarithm, guard band, exact logarithm inside the band). */
 int soma_debug_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
 int soma_debug_maps(const uint32_t *words, float *tmap, float *u, float *lnu, float *lnu_fast, uint64_t n);
 int soma_debug_accept(const float *dE, const uint32_t *words, uint8_t *decision, uint64_t n);
+int soma_debug_accept_fma(const float *dE, const uint32_t *words, uint8_t *decision, uint64_t n);
 /* Cell index of host positions under the handle's grid/box. */
 int soma_debug_cell_index(soma_t *h, const float *x, const float *y, const float *z, uint32_t *cell,
                           uint64_t n);

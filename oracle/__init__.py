@@ -82,6 +82,7 @@ def lib() -> C.CDLL:
             "oracle_smc_margin": (C.c_float, [vp, C.c_uint64, C.c_float, C.c_float, C.c_float]),
             "oracle_smc_draws": (None, [vp, C.c_uint64, C.c_uint32, C.c_uint32, C.POINTER(C.c_double)]),
             "oracle_det_functions": (None, [C.c_double, C.POINTER(C.c_double)]),
+            "oracle_det_functions_n": (None, [f32p, C.c_uint64, f32p, f32p, f32p]),
             "oracle_validate": (None, [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]),
             "oracle_get_step": (C.c_uint64, [vp]),
             "oracle_set_step": (None, [vp, C.c_uint64]),
@@ -129,6 +130,14 @@ def det_functions(x: float):
     out = (C.c_double * 3)()
     lib().oracle_det_functions(float(x), out)
     return float(out[0]), float(out[1]), float(out[2])
+
+
+def det_functions_n(x: np.ndarray):
+    """det_functions over an array of fp32 arguments: (log, sin 2 pi x, cos 2 pi x) as fp32 arrays."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    lg, sn, cs = (np.empty(x.size, dtype=np.float32) for _ in range(3))
+    lib().oracle_det_functions_n(_p(x, C.c_float), x.size, _p(lg, C.c_float), _p(sn, C.c_float), _p(cs, C.c_float))
+    return lg, sn, cs
 
 
 class Oracle:

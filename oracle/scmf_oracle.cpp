@@ -587,6 +587,13 @@ void oracle_det_functions(double x, double* out) {       // out = {det_log(x), s
   det_sincos_2pi((float)x, &sn, &cs);
   out[1] = sn; out[2] = cs;
 }
+// the same for n arguments at once (test plumbing: lets the pin visit every argument the deviates can take)
+void oracle_det_functions_n(const float* x, uint64_t n, float* lg, float* sn, float* cs) {
+  for (uint64_t k = 0; k < n; ++k) {
+    lg[k] = det_log(x[k]);
+    det_sincos_2pi(x[k], &sn[k], &cs[k]);
+  }
+}
 
 // single-bead molecules: n_single[T] (call right after oracle_create, before any state is loaded)
 int oracle_set_singles(void* h, const uint64_t* n_single) {

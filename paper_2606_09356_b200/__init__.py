@@ -29,7 +29,7 @@ EXPORTS = (
     "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_generate_state", "soma_validate_state", "soma_get_step", "soma_destroy", "soma_last_error",
     "soma_set_option", "soma_get_counters", "soma_get_kernel_times", "soma_debug_half_sweep", "soma_debug_finish_step",
     "soma_debug_set_omega", "soma_debug_philox", "soma_debug_maps", "soma_debug_accept",
-    "soma_debug_cell_index",
+    "soma_debug_accept_fma", "soma_debug_cell_index",
 )
 
 
@@ -107,6 +107,7 @@ def load_library() -> C.CDLL:
             "soma_debug_philox": (i32, [vp, vp, vp, u64]),
             "soma_debug_maps": (i32, [vp, vp, vp, vp, vp, u64]),
             "soma_debug_accept": (i32, [vp, vp, vp, u64]),
+            "soma_debug_accept_fma": (i32, [vp, vp, vp, u64]),
             "soma_debug_cell_index": (i32, [vp, vp, vp, vp, vp, u64]),
         }
         for name, (res, args) in sig.items():
@@ -280,6 +281,15 @@ def soma_debug_accept(dE: np.ndarray, words: np.ndarray) -> np.ndarray:
     assert dE.size == words.size
     out = np.empty(dE.size, dtype=np.uint8)
     _check(load_library().soma_debug_accept(dE.ctypes.data, words.ctypes.data, out.ctypes.data, dE.size))
+    return out
+
+
+def soma_debug_accept_fma(dE: np.ndarray, words: np.ndarray) -> np.ndarray:
+    dE = np.ascontiguousarray(dE, dtype=np.float32).reshape(-1)
+    words = np.ascontiguousarray(words, dtype=np.uint32).reshape(-1)
+    assert dE.size == words.size
+    out = np.empty(dE.size, dtype=np.uint8)
+    _check(load_library().soma_debug_accept_fma(dE.ctypes.data, words.ctypes.data, out.ctypes.data, dE.size))
     return out
 
 

@@ -10,7 +10,7 @@
 #include <string>
 #include <vector>
 
-#include "soma_sweep.cuh"
+#include "soma_lean.cuh"
 
 using namespace soma;
 
@@ -36,12 +36,7 @@ struct Layout {            // byte offsets into the workspace
   uint64_t validate;       // 11 x 8 bytes: report of soma_validate_state
   uint64_t sort_key;       // [n] uint32
   uint64_t sort_rank;      // [n] uint32
-  uint64_t sort_bins;      // [2 n_bins_max + 2] uint32: bin counts, then bin starts (= tile_start)
-  uint64_t slot_meta;      // [n] float4: per slot floor offsets + chain id, written by the tile sort
-  uint64_t meta_src;       // [n] float4: the same in the order before the sort (scratch)
-  uint64_t slot_k;         // [n] uint16: slice index of every slot's chain (swept-window kernel)
-  uint64_t omega_pad;      // [T][pad cells] fp32: ghost-padded omega for the tile loads (0 bytes if unused)
-  uint64_t counts_pad[2];  // [T][pad cells] uint32: ghost-padded density grids the tiles flush into
+  uint64_t sort_bins;      // [n_bins + 1] uint32: bin counts, then (scanned) bin starts
   uint64_t total;
 };
 
@@ -53,27 +48,8 @@ uint64_t sort_bin_count(const uint32_t grid[3]) {
   return n;
 }
 
-// entries of the bin array: the cube bins of the plain re-ordering, or 2 bins per (unit, slice) of the sweep
-uint64_t sort_bins_capacity(const uint32_t grid[3]) {
-  const uint64_t a = sort_bin_count(grid) + 2, b = (uint64_t)grid[0] * grid[1] * grid[2] / 8 + 2;
-  return a > b ? a : b;
-}
-
-// the ghost-padded omega copy is sized for the largest tile the options allow
-constexpr uint32_t kMaxTileCore = 32, kMaxTileHalo = 16;
-uint64_t omega_pad_cells_max(const uint32_t grid[3]) {
-  uint64_t n = 1;
-  for (int d = 0; d < 3; ++d) n *= (uint64_t)grid[d] + kMaxTileCore + 2 * kMaxTileHalo + 3;
-  return n;
-}
-bool tile_capable_grid(const uint32_t grid[3]) {      // power-of-two axes, at least 16 cells each
-  for (int d = 0; d < 3; ++d)
-    if (grid[d] < 16 || (grid[d] & (grid[d] - 1))) return false;
-  return true;
-}
-
-// n_bins: entries of the sort_bins array (see sort_bins_capacity)
-Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins, uint64_t pad_words, uint64_t S) {
+// n_bins: entries of the sort_bins array
+Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins, uint64_t S) {
   Layout L{};
   uint64_t off = 0;
   for (int s = 0; s < 2; ++s)
@@ -92,11 +68,6 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   L.sort_key = off; off += align_up(n * 4);
   L.sort_rank = off; off += align_up(n * 4);
   L.sort_bins = off; off += align_up(n_bins * 4);
-  L.slot_meta = off; off += align_up(n * 16);
-  L.meta_src = off; off += align_up(n * 16);
-  L.slot_k = off; off += align_up(n * 2);
-  L.omega_pad = off; off += align_up(pad_words * 4);
-  for (int s = 0; s < 2; ++s) { L.counts_pad[s] = off; off += align_up(pad_words * 4); }
   L.total = off;
   return L;
 }
@@ -193,27 +164,17 @@ struct soma_handle {
   int path;              // 0 auto, 1 generic, 2 fused
   int64_t resort_interval;      // re-order the chains every k steps (0 = never)
   int fused_chunk;              // warp groups per block of the fused kernel
-  // tiled kernel (soma_tile.cuh)
-  bool tile_grid_ok;            // the grid allows tiles at all
-  bool tile_ready;              // geometry + tensor maps are set up for the current options
-  uint32_t tc[3], th[3];        // tile core and halo in cells
-  int tile_threads;             // 512, 768 or 1024
-  bool tile_fast;               // inv_h a power of two >= 1 on every axis and a a power of two
-  uint32_t tile_margin;         // chains with a bead this close to a window face sort behind the others
-  uint32_t tile_slice, tile_ring_opt;   // slice width in cells; ring slots (0 = as many as fit)
-  uint32_t tile_lseg, tile_K, tile_R, tile_slab_bytes, tile_slab_stride, tile_aux_offset;
-  uint64_t sort_bins_cap;       // entries of the sort_bins array
-  uint32_t te[3], tm[3], n_tiles, pad[3];
-  size_t tile_smem;
-  uint32_t tile_counts_offset;
-  CUtensorMap tm_omega, tm_counts[2];
-  int sorted_kind;              // bins the slots are currently sorted by: 0 none, 1 cubes of 4 cells, 2 tiles
-  bool tile_auto;               // path 0 picks the tiled kernel
-  bool pad_valid;               // the ghost-padded omega copy matches the linear field
-  int pad_cur;                  // padded density grid the next tiled step bins into (zeroed)
-  bool counts_in_pad;           // the last move kernel binned into counts_pad(pad_cur), not into the linear grid
-  bool omega_custom;            // omega was overwritten by soma_debug_set_omega (tiles off until the next load)
-  char tile_why[96];            // why tiles are unavailable ("" if they are)
+  int fused_carveout;           // preferred shared-memory carve-out of the fused kernel in percent (-1: driver default)
+  bool fast_arith;              // inv_h a power of two >= 1 on every axis and a a power of two: the one-FFMA shortcuts are exact
+  int sorted_kind;              // bins the slots are currently sorted by: 0 none, 1 cubes of 4 cells, 2 tiles of the windowed-count kernel
+  // lean kernel (soma_lean.cuh) and its windowed-count variant
+  int fused_lean;               // use lean_step_kernel where it applies (option, default 1)
+  int lean_threads;             // threads per block of the lean kernel: 256, 512 or 1024
+  uint32_t wc[3], wh[3];        // tile core and halo in cells (options win_c*, win_h*)
+  uint32_t ww[3], nt[3], n_tiles;   // window = core + 2 halo; tiles per axis
+  size_t win_smem;
+  bool win_ready, win_auto;     // geometry is valid for this system; path 0 picks the windowed variant
+  char win_why[96];             // why the windowed variant is unavailable ("" if it is available)
   // counters
   uint64_t launches, steps_done, resorts;
   // per-kernel timing ("kernel_timing" option): event triples (before moves, after moves+bin, after omega)
@@ -236,11 +197,6 @@ struct soma_handle {
   uint32_t* sort_key() const { return reinterpret_cast<uint32_t*>(ws + L.sort_key); }
   uint32_t* sort_rank() const { return reinterpret_cast<uint32_t*>(ws + L.sort_rank); }
   uint32_t* sort_bins() const { return reinterpret_cast<uint32_t*>(ws + L.sort_bins); }
-  float* omega_pad() const { return reinterpret_cast<float*>(ws + L.omega_pad); }
-  float4* slot_meta() const { return reinterpret_cast<float4*>(ws + L.slot_meta); }
-  float4* meta_src() const { return reinterpret_cast<float4*>(ws + L.meta_src); }
-  uint16_t* slot_k() const { return reinterpret_cast<uint16_t*>(ws + L.slot_k); }
-  uint32_t* counts_pad(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts_pad[s]); }
   uint8_t* patterns() const { return reinterpret_cast<uint8_t*>(ws + L.patterns); }
   uint8_t* pattern0() const { return reinterpret_cast<uint8_t*>(ws + L.pattern0); }
   unsigned long long* accepted() const { return reinterpret_cast<unsigned long long*>(ws + L.accepted); }
@@ -310,9 +266,8 @@ int launch_half_sweep(soma_handle* h, uint32_t parity) {
   return SOMA_OK;
 }
 
-// Single-bead molecules: trial moves (half-sweep 0) and / or binning into `counts` -- the linear grid,
-// or the ghost-padded grid the windowed kernels flush into (padded = true).
-int launch_singles(soma_handle* h, bool do_move, bool do_bin, uint32_t* counts, bool padded, bool check_range = false) {
+// Single-bead molecules: trial moves (half-sweep 0) and / or binning into `counts`.
+int launch_singles(soma_handle* h, bool do_move, bool do_bin, uint32_t* counts, bool check_range = false) {
   if (h->S == 0) return SOMA_OK;
   SingleArgs A{};
   A.S = step_args(h);
@@ -320,7 +275,6 @@ int launch_singles(soma_handle* h, bool do_move, bool do_bin, uint32_t* counts, 
   for (int t = 0; t <= kMaxTypes; ++t) A.start[t] = h->single_start[t];
   A.x = h->single(0); A.y = h->single(1); A.z = h->single(2);
   A.counts = counts;
-  if (padded) { A.px = h->pad[0]; A.py = h->pad[1]; A.pz = h->pad[2]; A.hx = h->th[0]; A.hy = h->th[1]; A.hz = h->th[2]; }
   A.range_flag = check_range ? h->range_flag() : nullptr;
   A.do_move = do_move; A.do_bin = do_bin;
   if (h->pow2) singles_kernel<true><<<blocks_for(h->S, 256), 256, 0, h->stream>>>(A);
@@ -342,12 +296,10 @@ int launch_bin(soma_handle* h, uint32_t* counts, bool check_range = false) {
         h->slot_pattern(), h->patterns(), counts, flag);
   h->launches++;
   CU(h, cudaGetLastError());
-  return launch_singles(h, false, true, counts, false, check_range);
+  return launch_singles(h, false, true, counts, check_range);
 }
 
 // omega from counts(cur); zero counts(cur^1) for the next step's binning.
-bool use_tile(const soma_handle* h);
-
 int launch_omega(soma_handle* h) {
   OmegaArgs A{};
   A.cells = h->cells; A.T = h->T;
@@ -357,38 +309,119 @@ int launch_omega(soma_handle* h) {
   A.counts_to_zero = h->counts(h->cur ^ 1);
   A.omega = h->omega();
   A.ext = h->has_ext ? h->ext() : nullptr;
-  if (use_tile(h)) {            // also fills the ghost-padded copy the tiles are loaded from
-    PadGeom pg{h->pad[0], h->pad[1], h->pad[2], h->th[0], h->th[1], h->th[2]};
-    const unsigned g = blocks_for((uint64_t)h->pad[0] * h->pad[1] * h->pad[2], 256);
-    const uint32_t* in = h->counts_in_pad ? h->counts_pad(h->pad_cur) : nullptr;   // fold the tiles' ghost layers
-    uint32_t* out = h->counts(h->cur);
-    uint32_t* zero = h->counts_pad(h->pad_cur ^ 1);
-    switch (h->T) {
-      case 1: omega_pad_kernel<1><<<g, 256, 0, h->stream>>>(A, h->grid, pg, h->omega_pad(), in, out, zero); break;
-      case 2: omega_pad_kernel<2><<<g, 256, 0, h->stream>>>(A, h->grid, pg, h->omega_pad(), in, out, zero); break;
-      case 3: omega_pad_kernel<3><<<g, 256, 0, h->stream>>>(A, h->grid, pg, h->omega_pad(), in, out, zero); break;
-      default: omega_pad_kernel<0><<<g, 256, 0, h->stream>>>(A, h->grid, pg, h->omega_pad(), in, out, zero); break;
-    }
-    if (h->counts_in_pad) h->pad_cur ^= 1;       // the grid just folded is zeroed by the NEXT omega pass
-    h->counts_in_pad = false;
-    h->pad_valid = true;
-  } else {
-    h->pad_valid = false;
-    const unsigned g = blocks_for(h->cells, 256);
-    switch (h->T) {
-      case 1: omega_kernel<1><<<g, 256, 0, h->stream>>>(A); break;
-      case 2: omega_kernel<2><<<g, 256, 0, h->stream>>>(A); break;
-      case 3: omega_kernel<3><<<g, 256, 0, h->stream>>>(A); break;
-      default: omega_kernel<0><<<g, 256, 0, h->stream>>>(A); break;
-    }
+  const unsigned g = blocks_for(h->cells, 256);
+  switch (h->T) {
+    case 1: omega_kernel<1><<<g, 256, 0, h->stream>>>(A); break;
+    case 2: omega_kernel<2><<<g, 256, 0, h->stream>>>(A); break;
+    case 3: omega_kernel<3><<<g, 256, 0, h->stream>>>(A); break;
+    default: omega_kernel<0><<<g, 256, 0, h->stream>>>(A); break;
   }
   h->launches++;
   CU(h, cudaGetLastError());
   return SOMA_OK;
 }
 
+bool lean_ok(const soma_handle* h) {
+  return h->fused_lean && h->fast_arith && h->pow2 && h->smcA == 0.0f && fused_lanes(h->N) != 0;
+}
+bool use_win(const soma_handle* h) {
+  if (!h->win_ready || !lean_ok(h) || h->path == 1) return false;
+  return h->path == 3 || (h->path == 0 && h->win_auto);
+}
+
+// Geometry of the windowed-count variant from the options.  Leaves win_ready false (with the reason
+// in h->win_why) when it cannot run; that is not an error.
+void win_setup(soma_handle* h) {
+  h->win_ready = false;
+  if (h->sorted_kind == 2) h->sorted_kind = 0;          // the tile table belongs to the old geometry
+  auto no = [&](const char* why) { snprintf(h->win_why, sizeof h->win_why, "%s", why); };
+  if (!lean_ok(h)) return no("needs a power-of-two grid, power-of-two cell size >= 1/b-unit and move half-width, uniform moves, N = 2P");
+  const uint32_t n[3] = {h->grid.nx, h->grid.ny, h->grid.nz};
+  uint64_t tiles = 1, words = h->T;
+  for (int d = 0; d < 3; ++d) {
+    if (h->wc[d] < kSortBinEdge || h->wc[d] > n[d] || n[d] % h->wc[d]) return no("tile core must be >= 4 cells and divide the grid");
+    h->ww[d] = h->wc[d] + 2 * h->wh[d];
+    if (h->ww[d] > n[d]) return no("window (core + 2 halo) is larger than the grid");
+    h->nt[d] = n[d] / h->wc[d];
+    tiles *= h->nt[d];
+    words *= h->ww[d];
+  }
+  if (h->wc[2] % 4 || h->wh[2] % 4 || n[2] % 4) return no("tile core and halo along z must be multiples of 4 cells");
+  if (words * 4 > 160 * 1024) return no("window does not fit in shared memory (160 KB per block)");
+  h->n_tiles = (uint32_t)tiles;
+  h->win_smem = (size_t)words * 4;
+  h->win_why[0] = 0;
+  h->win_ready = true;
+}
+
+template <int P, bool MULTI, bool WIN, int NT>
+void launch_lean_k(soma_handle* h, LeanArgs& A) {
+  constexpr int G = 32 / P;
+  auto* k = lean_step_kernel<P, MULTI, WIN, NT>;
+  if (WIN) {
+    if (h->win_smem > 48 * 1024) cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->win_smem);
+    k<<<h->n_tiles, NT, h->win_smem, h->stream>>>(A);
+  } else {
+    const uint64_t n_groups = (h->n_chains + G - 1) / G;
+    const uint64_t wpb = NT / 32;
+    const uint64_t gpb = ((uint64_t)h->fused_chunk * (NT / 256) + wpb - 1) / wpb * wpb;   // fused_chunk is per 256 threads
+    A.groups_per_block = (uint32_t)gpb;
+    if (h->fused_carveout >= 0) cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, h->fused_carveout);
+    k<<<(unsigned)((n_groups + gpb - 1) / gpb), NT, 0, h->stream>>>(A);
+  }
+}
+template <int P, int NT>
+int launch_lean_pn(soma_handle* h, LeanArgs& A, bool win) {
+  const bool multi = h->n_patterns > 1;
+  if (win) { if (multi) launch_lean_k<P, true, true, NT>(h, A); else launch_lean_k<P, false, true, NT>(h, A); }
+  else     { if (multi) launch_lean_k<P, true, false, NT>(h, A); else launch_lean_k<P, false, false, NT>(h, A); }
+  h->launches++;
+  CU(h, cudaGetLastError());
+  return SOMA_OK;
+}
+
+template <int P>
+int launch_lean_p(soma_handle* h) {
+  LeanArgs A{};
+  A.inv_hx = h->grid.inv_hx; A.inv_hy = h->grid.inv_hy; A.inv_hz = h->grid.inv_hz;
+  A.mx = h->grid.nx - 1; A.my = h->grid.ny - 1; A.mz = h->grid.nz - 1;
+  A.ny = h->grid.ny; A.nz = h->grid.nz;
+  A.cells = h->cells;
+  A.n_chains = (uint32_t)h->n_chains;
+  A.a2 = 2.0f * h->a;
+  A.ac = h->a * -0.99999988079071044921875f;       // a (2^-23 - 1), exact: a is a power of two
+  A.kb = h->kb;
+  A.keys = h->keys;
+  const uint64_t m1 = (uint64_t)kPhiloxM1 * (uint32_t)h->step;
+  A.u0 = (uint32_t)(m1 >> 32) ^ h->keys.k0[0];
+  A.u1 = (uint32_t)m1;
+  A.ctr3_base = (0u << 8) | ((uint32_t)(h->step >> 32) << 16);   // domain 0 = MC move
+  A.x = h->pos(h->live, 0); A.y = h->pos(h->live, 1); A.z = h->pos(h->live, 2);
+  A.omega = h->omega();
+  A.counts_next = h->counts(h->cur ^ 1);
+  A.slot_chain = h->slot_chain();
+  A.slot_pattern = h->slot_pattern();
+  A.patterns = h->patterns();
+  A.accepted = h->accepted();
+  A.T = h->T;
+  const bool win = use_win(h);
+  if (win) {
+    A.tile_start = h->sort_bins();
+    A.tcx = h->wc[0]; A.tcy = h->wc[1]; A.tcz = h->wc[2];
+    A.hx = h->wh[0]; A.hy = h->wh[1]; A.hz = h->wh[2];
+    A.wx = h->ww[0]; A.wy = h->ww[1]; A.wz = h->ww[2];
+    A.nty = h->nt[1]; A.ntz = h->nt[2];
+  }
+  switch (h->lean_threads) {
+    case 256: return launch_lean_pn<P, 256>(h, A, win);
+    case 512: return launch_lean_pn<P, 512>(h, A, win);
+    default: return launch_lean_pn<P, 1024>(h, A, win);
+  }
+}
+
 template <int P>
 int launch_fused_p(soma_handle* h) {
+  if (lean_ok(h)) return launch_lean_p<P>(h);
   const StepArgs A = step_args(h);
   constexpr int G = 32 / P;
   const uint64_t n_groups = (h->n_chains + G - 1) / G;           // warps of work
@@ -398,9 +431,11 @@ int launch_fused_p(soma_handle* h) {
   const uint64_t n_chunks = (n_groups + gpb - 1) / gpb;
   const uint64_t blocks = n_chunks;                // one block per chunk, in chain-list order
   const bool multi = h->n_patterns > 1;
-  const bool fast = h->tile_fast && h->pow2;       // exact one-FFMA shortcuts apply (see fused_move)
+  const bool fast = h->fast_arith && h->pow2;      // exact one-FFMA shortcuts apply (see fused_move)
 #define SOMA_LAUNCH_FUSED(POW2, MULTI)                                                                          \
   do {                                                                                                          \
+    if (h->fused_carveout >= 0 && fast && POW2)                                                                 \
+      cudaFuncSetAttribute(fused_step_kernel<P, POW2, MULTI, POW2>, cudaFuncAttributePreferredSharedMemoryCarveout, h->fused_carveout); \
     if (h->smcA > 0.0f) fused_step_kernel<P, POW2, MULTI, false, true><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb); \
     else if (fast && POW2) fused_step_kernel<P, POW2, MULTI, POW2><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb); \
     else fused_step_kernel<P, POW2, MULTI, false><<<(unsigned)blocks, bs, 0, h->stream>>>(A, (uint32_t)gpb);    \
@@ -429,225 +464,36 @@ bool use_fused(const soma_handle* h) {
   if (h->path == 1) return false;
   return fused_lanes(h->N) != 0;
 }
-bool use_tile(const soma_handle* h) {
-  if (!h->tile_ready || h->omega_custom || h->smcA > 0.0f) return false;
-  return h->path == 3 || h->path == 4 || (h->path == 0 && h->tile_auto);
-}
-
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-// 4-D tensor map over a [T][X][Y][Z] array (Z fastest) with a [T][ex][ey][ez] box
-bool encode_map(EncodeTiledFn enc, CUtensorMap* tm, CUtensorMapDataType dt, void* base, uint32_t T, const uint32_t dims[3],
-                const uint32_t box[3]) {
-  const cuuint64_t gdim[4] = {dims[2], dims[1], dims[0], T};
-  const cuuint64_t gstr[3] = {(cuuint64_t)dims[2] * 4, (cuuint64_t)dims[2] * dims[1] * 4, (cuuint64_t)dims[2] * dims[1] * dims[0] * 4};
-  const cuuint32_t bdim[4] = {box[2], box[1], box[0], T};
-  const cuuint32_t estr[4] = {1, 1, 1, 1};
-  return enc(tm, dt, 4, base, gdim, gstr, bdim, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
-template <int P, int NT>
-cudaError_t tile_attr(size_t smem) {
-  cudaError_t e = cudaFuncSetAttribute(tile_step_kernel<P, false, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, true, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, false, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(tile_step_kernel<P, true, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_step_kernel<P, false, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_step_kernel<P, true, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_step_kernel<P, false, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_step_kernel<P, true, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  return e;
-}
-template <int NT>
-cudaError_t tile_attr_p(int P, size_t smem) {
-  switch (P) {
-#ifndef SOMA_MIN_BUILD      /* development builds instantiate N = 32 only */
-    case 1: return tile_attr<1, NT>(smem);   case 2: return tile_attr<2, NT>(smem);
-    case 4: return tile_attr<4, NT>(smem);   case 8: return tile_attr<8, NT>(smem);
-    case 32: return tile_attr<32, NT>(smem);
-#endif
-    case 16: return tile_attr<16, NT>(smem);
-  }
-  return cudaErrorInvalidValue;
-}
-
-// Derive the tile geometry from the options and build the tensor maps.  Leaves tile_ready false
-// (with the reason in h->tile_why) when tiles cannot be used; that is not an error.
-void tile_setup(soma_handle* h) {
-  h->tile_ready = false;
-  h->tile_auto = false;
-  h->pad_valid = false;
-  if (h->sorted_kind == 2) h->sorted_kind = 0;       // the per-slot floor offsets belong to the old geometry
-  auto no = [&](const char* why) { snprintf(h->tile_why, sizeof h->tile_why, "%s", why); };
-  if (!h->tile_grid_ok) return no("grid axes must be powers of two >= 16");
-  const int P = fused_lanes(h->N);
-  if (!P) return no("beads_per_chain must be 2P, P a power of two <= 32");
-  const uint32_t n[3] = {h->grid.nx, h->grid.ny, h->grid.nz};
-  // x: segments of tc[0] cells swept in slices; y, z: column cores tc[1] x tc[2]
-  if (h->tile_slice < 1 || h->tile_slice > 16) return no("tile_slice must be in [1, 16]");
-  uint32_t Lseg = h->tc[0] < n[0] ? h->tc[0] : n[0];
-  if (Lseg < h->tile_slice || (Lseg & (Lseg - 1)) || Lseg % h->tile_slice) return no("segment length must be a power of two and a multiple of the slice");
-  if (Lseg / h->tile_slice > kMaxSlices) return no("too many slices per segment");
-  for (int d = 1; d < 3; ++d)
-    if (h->tc[d] < 4 || h->tc[d] > kMaxTileCore) return no("column core must be in [4, 32] cells");
-  for (int d = 0; d < 3; ++d)
-    if (h->th[d] > kMaxTileHalo) return no("halo must be <= 16 cells");
-  h->te[0] = h->tile_slice + 2 * h->th[0];
-  h->te[1] = h->tc[1] + 2 * h->th[1];
-  h->te[2] = h->tc[2] + 2 * h->th[2];
-  uint64_t nt = 1;
-  for (int d = 0; d < 3; ++d) {
-    const uint32_t core = d == 0 ? Lseg : h->tc[d];
-    if (h->te[d] > n[d]) return no("window (core + 2 halo) is larger than the grid");
-    h->tm[d] = (n[d] + core - 1) / core;
-    h->pad[d] = h->tm[d] * core + 2 * h->th[d];
-    if (h->pad[d] > 2 * n[d]) return no("padded grid would hold a cell three times");
-    nt *= h->tm[d];
-  }
-  if (h->tc[2] % 4 || h->te[2] % 4) return no("column core and extent along z must be multiples of 4 cells");
-  h->pad[2] = (h->pad[2] + 3u) / 4u * 4u;
-  h->tile_lseg = Lseg;
-  h->tile_K = Lseg / h->tile_slice;
-  if (2 * nt * h->tile_K + 1 > h->sort_bins_cap) return no("too many units");
-  h->n_tiles = (uint32_t)nt;
-  h->tile_slab_bytes = h->T * h->te[1] * h->te[2] * 4;
-  h->tile_slab_stride = (h->tile_slab_bytes + 127u) / 128u * 128u;
-  const uint32_t smem_max = 227u * 1024u;
-  uint32_t R = (smem_max - kSweepAuxBytes) / (2u * h->tile_slab_stride);
-  if (R > kMaxRing) R = kMaxRing;
-  if (R > Lseg + 2 * h->th[0]) R = Lseg + 2 * h->th[0];
-  if (h->tile_ring_opt) { if (h->tile_ring_opt > R) return no("tile_ring does not fit in shared memory"); R = h->tile_ring_opt; }
-  if (R < h->te[0]) return no("the ring cannot hold one window (slice + 2 hx slabs)");
-  if ((uint64_t)R * h->tile_slab_stride >= (1u << 22)) return no("ring too large");
-  h->tile_R = R;
-  h->tile_counts_offset = R * h->tile_slab_stride;
-  h->tile_aux_offset = 2u * R * h->tile_slab_stride;
-  h->tile_smem = (size_t)h->tile_aux_offset + kSweepAuxBytes;
-  void* fn = nullptr;
-  cudaDriverEntryPointQueryResult q;
-  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) {
-    cudaGetLastError();
-    return no("cuTensorMapEncodeTiled is not available");
-  }
-  EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(fn);
-  const uint32_t box[3] = {1, h->te[1], h->te[2]};                    // one slab: [T][1][ey][ez]
-  if (!encode_map(enc, &h->tm_omega, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, h->omega_pad(), h->T, h->pad, box)) return no("tensor map (omega) rejected");
-  for (int s = 0; s < 2; ++s)
-    if (!encode_map(enc, &h->tm_counts[s], CU_TENSOR_MAP_DATA_TYPE_UINT32, h->counts_pad(s), h->T, h->pad, box)) return no("tensor map (counts) rejected");
-  // both padded density grids start zeroed; from here on the omega pass keeps them so
-  const size_t pad_bytes = (size_t)h->pad[0] * h->pad[1] * h->pad[2] * h->T * 4;
-  if (cudaMemsetAsync(h->counts_pad(0), 0, pad_bytes, h->stream) != cudaSuccess ||
-      cudaMemsetAsync(h->counts_pad(1), 0, pad_bytes, h->stream) != cudaSuccess) { cudaGetLastError(); return no("cudaMemsetAsync failed"); }
-  h->pad_cur = 0;
-  h->counts_in_pad = false;
-  cudaError_t e = h->tile_threads == 1024 ? tile_attr_p<1024>(P, h->tile_smem)
-                : h->tile_threads == 768 ? tile_attr_p<768>(P, h->tile_smem) : tile_attr_p<512>(P, h->tile_smem);
-  if (e != cudaSuccess) { cudaGetLastError(); return no("cudaFuncSetAttribute(max dynamic shared memory) failed"); }
-  h->tile_ready = true;
-  // automatic choice: the fused kernel.  With its chunks handed out in chain-list order (see
-  // launch_fused_p) it is the fastest path measured on every config (cfg4: 1.12 ms against 1.64 ms for
-  // either windowed kernel, profiles/); the windowed kernels stay selectable as paths 3 and 4.
-  h->tile_auto = false;
-  h->tile_why[0] = 0;
-}
-
-template <int P, int NT>
-int launch_tile_pn(soma_handle* h) {
-  TileArgs A{};
-  A.S = step_args(h);
-  A.slot_meta = h->slot_meta();
-  A.slot_k = h->slot_k();
-  A.T = h->T;
-  A.wx = h->te[0]; A.ey = h->te[1]; A.ez = h->te[2];
-  A.cy = h->tc[1]; A.cz = h->tc[2];
-  A.hx = h->th[0]; A.hy = h->th[1]; A.hz = h->th[2];
-  A.slice = h->tile_slice; A.R = h->tile_R; A.K = h->tile_K; A.Lseg = h->tile_lseg;
-  A.mtz = h->tm[2]; A.nseg = h->tm[0]; A.n_units = h->n_tiles;
-  A.slab_bytes = h->tile_slab_bytes; A.slab_stride = h->tile_slab_stride;
-  A.counts_offset = h->tile_counts_offset; A.aux_offset = h->tile_aux_offset;
-  A.bin_start = h->sort_bins();
-  A.counts_pad = h->counts_pad(h->pad_cur);
-  A.px = h->pad[0]; A.py = h->pad[1]; A.pz = h->pad[2];
-  const uint64_t m1 = (uint64_t)kPhiloxM1 * A.S.ctr2;
-  A.philox_u0 = (uint32_t)(m1 >> 32) ^ h->keys.k0[0];
-  A.philox_u1 = (uint32_t)m1;
-  A.a2 = 2.0f * h->a;
-  A.ac = h->a * -0.99999988079071044921875f;      // a (2^-23 - 1), exact when a is a power of two
-  const unsigned grid = (unsigned)(h->n_tiles < (uint32_t)h->sm_count ? h->n_tiles : (uint32_t)h->sm_count);
-  const CUtensorMap& tmc = h->tm_counts[h->pad_cur];
-  h->counts_in_pad = true;
-  const bool multi = h->n_patterns > 1;
-  const bool sweep = h->path != 3;                 // path 3 keeps the first column-sweep kernel (soma_tile.cuh) for comparison
-#define SOMA_LAUNCH_TILE(MULTI, FAST) \
-  do { if (sweep) sweep_step_kernel<P, MULTI, NT, FAST><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc); \
-       else tile_step_kernel<P, MULTI, NT, FAST><<<grid, NT, h->tile_smem, h->stream>>>(A, h->tm_omega, tmc); } while (0)
-  if (h->tile_fast) { if (multi) SOMA_LAUNCH_TILE(true, true); else SOMA_LAUNCH_TILE(false, true); }
-  else              { if (multi) SOMA_LAUNCH_TILE(true, false); else SOMA_LAUNCH_TILE(false, false); }
-#undef SOMA_LAUNCH_TILE
-  h->launches++;
-  CU(h, cudaGetLastError());
-  return SOMA_OK;
-}
-template <int NT>
-int launch_tile_n(soma_handle* h) {
-  switch (fused_lanes(h->N)) {
-#ifndef SOMA_MIN_BUILD
-    case 1: return launch_tile_pn<1, NT>(h);   case 2: return launch_tile_pn<2, NT>(h);
-    case 4: return launch_tile_pn<4, NT>(h);   case 8: return launch_tile_pn<8, NT>(h);
-    case 32: return launch_tile_pn<32, NT>(h);
-#endif
-    case 16: return launch_tile_pn<16, NT>(h);
-  }
-  return fail(h, SOMA_EINVAL, "tiled path does not support this beads_per_chain");
-}
-int launch_tile(soma_handle* h) {
-  return h->tile_threads == 1024 ? launch_tile_n<1024>(h) : h->tile_threads == 768 ? launch_tile_n<768>(h) : launch_tile_n<512>(h);
-}
-
 // Re-order the chains in memory by the coarse bin of their centre of mass (counting sort on the
-// device).  kind 1: cubes of kSortBinEdge cells; kind 2: the tiles of the tiled kernel, whose
-// tile_start table is the scanned bin array.
+// device).  kind 1: cubes of kSortBinEdge cells; kind 2: the tiles of the windowed-count kernel
+// (numbered z fastest), whose tile_start table is the scanned bin array.
 int resort(soma_handle* h, int kind) {
   const int src = h->live, dst = h->live ^ 1;
+  SortArgs S{};
+  S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
   uint32_t n_bins;
   if (kind == 2) {
-    TileSortArgs S{};
-    S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
-    S.cy = h->tc[1]; S.cz = h->tc[2];
-    S.hx = h->th[0]; S.hy = h->th[1]; S.hz = h->th[2];
-    S.wx = h->te[0]; S.ey = h->te[1]; S.ez = h->te[2];
-    S.slice = h->tile_slice; S.K = h->tile_K; S.Lseg = h->tile_lseg; S.mtz = h->tm[2]; S.nseg = h->tm[0];
-    S.margin = h->tile_margin;
-    n_bins = 2u * h->n_tiles * h->tile_K;
-    CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
-    tile_key_kernel<<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
-        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->slot_chain(src), h->sort_bins(), h->sort_key(),
-        h->sort_rank(), h->meta_src());
+    S.cbx = h->wc[0]; S.cby = h->wc[1]; S.cbz = h->wc[2];
+    S.ncy = h->grid.ny / h->wc[1]; S.ncz = h->grid.nz / h->wc[2];
+    n_bins = h->n_tiles;
   } else {
-    SortArgs S{};
-    S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
     S.cbx = S.cby = S.cbz = kSortBinEdge;
     S.ncy = (h->grid.ny + kSortBinEdge - 1) / kSortBinEdge;
     S.ncz = (h->grid.nz + kSortBinEdge - 1) / kSortBinEdge;
     n_bins = h->n_bins;
-    CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
-    if (h->pow2)
-      chain_key_kernel<true><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
-          S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
-    else
-      chain_key_kernel<false><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
-          S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
   }
+  CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
+  if (h->pow2)
+    chain_key_kernel<true><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
+        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
+  else
+    chain_key_kernel<false><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
+        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
   bin_scan_kernel<<<1, 1024, 0, h->stream>>>(n_bins + 1, h->sort_bins());      // entry n_bins becomes the total
   chain_permute_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
       h->B, h->N, h->sort_bins(), h->sort_key(), h->sort_rank(),
       h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->pos(dst, 0), h->pos(dst, 1), h->pos(dst, 2),
-      h->slot_chain(src), h->slot_pattern(src), h->slot_chain(dst), h->slot_pattern(dst),
-      kind == 2 ? h->meta_src() : nullptr, kind == 2 ? h->slot_meta() : nullptr,
-      kind == 2 ? h->slot_k() : nullptr, kind == 2 ? h->tile_K : 1u);
+      h->slot_chain(src), h->slot_pattern(src), h->slot_chain(dst), h->slot_pattern(dst));
   h->launches += 3;
   CU(h, cudaGetLastError());
   h->live = dst;
@@ -690,25 +536,20 @@ cudaEvent_t timing_mark(soma_handle* h) {
 
 int one_step(soma_handle* h) {
   int rc;
-  const bool tiled = use_tile(h);
-  const int kind = tiled ? 2 : 1;
-  // the tiled kernel needs the slots sorted by tile; otherwise sorting is an optimisation
-  if (tiled && !h->pad_valid)                                    // path switched after the last omega pass
-    if ((rc = launch_omega(h)) != SOMA_OK) return rc;
-  if ((tiled && h->sorted_kind != 2) ||
+  const bool win = use_win(h);
+  const int kind = win ? 2 : 1;
+  // the windowed-count kernel needs the slots sorted by tile; otherwise sorting is an optimisation
+  if ((win && h->sorted_kind != 2) ||
       (h->resort_interval > 0 && (h->steps_since_sort >= (uint64_t)h->resort_interval || h->sorted_kind != kind)))
     if ((rc = resort(h, kind)) != SOMA_OK) return rc;
   const bool timed = h->timing && h->ev_used + 3 <= 3 * kMaxTimedSteps;
   if (timed) timing_mark(h);
-  if (tiled) {
-    if ((rc = launch_tile(h)) != SOMA_OK) return rc;             // a1 + a2 + a3 (+a5), tiled
-    if ((rc = launch_singles(h, true, true, h->counts_pad(h->pad_cur), true)) != SOMA_OK) return rc;
-  } else if (use_fused(h)) {
+  if (use_fused(h)) {
     if ((rc = launch_fused(h)) != SOMA_OK) return rc;            // a1 + a2 + a3 (+a5)
-    if ((rc = launch_singles(h, true, true, h->counts(h->cur ^ 1), false)) != SOMA_OK) return rc;
+    if ((rc = launch_singles(h, true, true, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;
   } else {
     if ((rc = launch_half_sweep(h, 0)) != SOMA_OK) return rc;    // a1
-    if ((rc = launch_singles(h, true, false, nullptr, false)) != SOMA_OK) return rc;   // a1, single-bead molecules
+    if ((rc = launch_singles(h, true, false, nullptr)) != SOMA_OK) return rc;   // a1, single-bead molecules
     if ((rc = launch_half_sweep(h, 1)) != SOMA_OK) return rc;    // a2
     if ((rc = launch_bin(h, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;   // a3 (chains and single-bead molecules)
   }
@@ -748,10 +589,9 @@ uint64_t soma_workspace_bytes(const soma_params* p) {
   if (bad) { fail(nullptr, SOMA_EINVAL, bad); return 0; }
   const uint64_t B = p->n_chains * p->beads_per_chain;
   const uint64_t TC = (uint64_t)p->grid[0] * p->grid[1] * p->grid[2] * p->n_types;
-  const uint64_t pad_words = tile_capable_grid(p->grid) ? omega_pad_cells_max(p->grid) * p->n_types : 0;
   uint64_t S = 0;
   if (p->n_single) for (uint32_t t = 0; t < p->n_types; ++t) S += p->n_single[t];
-  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bins_capacity(p->grid), pad_words, S).total;
+  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bin_count(p->grid) + 2, S).total;
 }
 
 int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
@@ -808,10 +648,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   for (uint32_t k = 0; k < h->T * h->T; ++k) h->chiN[k] = p->chiN[k];
   h->seed = p->seed;
   h->n_bins = (uint32_t)sort_bin_count(p->grid);
-  h->tile_grid_ok = tile_capable_grid(p->grid);
-  h->sort_bins_cap = sort_bins_capacity(p->grid);
-  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, h->sort_bins_cap,
-                     h->tile_grid_ok ? omega_pad_cells_max(p->grid) * h->T : 0, h->S);
+  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, sort_bin_count(p->grid) + 2, h->S);
   if (p->workspace) {
     if (p->workspace_bytes < h->L.total || (reinterpret_cast<uintptr_t>(p->workspace) % kAlign)) {
       free_handle(h);
@@ -853,18 +690,17 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   // chains are kept sorted by position when the system is large enough for it to matter
   h->resort_interval = h->n_chains >= 4096 ? 64 : 0;
   h->fused_chunk = 224;
-  h->tc[0] = 64; h->tc[1] = 8; h->tc[2] = 8;
-  h->th[0] = h->th[1] = h->th[2] = 8;
-  h->tile_slice = 2;
-  h->tile_ring_opt = 0;
-  h->tile_threads = 768;
-  h->tile_margin = 1;
+  h->fused_carveout = -1;
+  h->fused_lean = 1;
+  h->lean_threads = 256;
+  h->wc[0] = h->wc[1] = h->wc[2] = 8;
+  h->wh[0] = h->wh[1] = h->wh[2] = 4;
   {
     auto pow2f = [](float v) { int e; return v > 0.0f && std::frexp(v, &e) == 0.5f && e > -100 && e < 100; };
-    h->tile_fast = pow2f(h->a) && pow2f(h->grid.inv_hx) && pow2f(h->grid.inv_hy) && pow2f(h->grid.inv_hz) &&
+    h->fast_arith = pow2f(h->a) && pow2f(h->grid.inv_hx) && pow2f(h->grid.inv_hy) && pow2f(h->grid.inv_hz) &&
                    h->grid.inv_hx >= 1.0f && h->grid.inv_hy >= 1.0f && h->grid.inv_hz >= 1.0f;
   }
-  tile_setup(h);
+  win_setup(h);
   const double cells_per_step = (double)h->a * (double)fmaxf(h->grid.inv_hx, fmaxf(h->grid.inv_hy, h->grid.inv_hz));
   const double k = cells_per_step > 0.0 ? 2097152.0 / cells_per_step : 1e18;
   h->range_check_interval = k >= 1e18 ? (1ull << 60) : (k < 1.0 ? 1ull : (uint64_t)k);
@@ -891,9 +727,8 @@ int finish_load(soma_handle* h, uint64_t step0) {
   if ((rc = verify_range(h)) != SOMA_OK) return rc;     // synchronises: the caller may reuse its buffers
   h->steps_since_sort = 0;
   h->sorted_kind = 0;
-  h->omega_custom = false;
-  if (use_tile(h) || h->resort_interval > 0)
-    if ((rc = resort(h, use_tile(h) ? 2 : 1)) != SOMA_OK) return rc;
+  if (use_win(h) || h->resort_interval > 0)
+    if ((rc = resort(h, use_win(h) ? 2 : 1)) != SOMA_OK) return rc;
   h->loaded = true;
   return SOMA_OK;
 }
@@ -1020,8 +855,6 @@ int soma_set_external_field(soma_t* h, const float* ext, int dev) {
   }
   h->has_ext = ext != nullptr;
   if (h->loaded) {                                               // omega of the current densities, with the new field
-    if (h->counts_in_pad) return fail(h, SOMA_ESTATE, "internal: densities not folded");
-    h->omega_custom = false;
     if ((rc = launch_omega(h)) != SOMA_OK) return rc;
   }
   return SOMA_OK;
@@ -1081,10 +914,10 @@ const char* soma_last_error(const soma_t* h) { return h ? h->err : g_last_error;
 int soma_set_option(soma_t* h, const char* name, int64_t value) {
   if (!h || !name) return fail(h, SOMA_EINVAL, "NULL argument");
   if (!std::strcmp(name, "path")) {
-    if (value < 0 || value > 4) return fail(h, SOMA_EINVAL, "path must be 0, 1, 2, 3 or 4");
-    if (value >= 3 && !h->tile_ready) {
+    if (value < 0 || value > 3) return fail(h, SOMA_EINVAL, "path must be 0, 1, 2 or 3");
+    if (value == 3 && !h->win_ready) {
       char buf[160];
-      snprintf(buf, sizeof buf, "tiled path unavailable: %s", h->tile_why);
+      snprintf(buf, sizeof buf, "windowed path unavailable: %s", h->win_why);
       return fail(h, SOMA_EINVAL, buf);
     }
     if (value == 2 && !fused_lanes(h->N))
@@ -1107,45 +940,44 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     int rc = check(h);
     if (rc != SOMA_OK) return rc;
     if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
-    return resort(h, use_tile(h) ? 2 : 1);
+    return resort(h, use_win(h) ? 2 : 1);
   }
   {
-    static const char* const tn[9] = {"tile_cx", "tile_cy", "tile_cz", "tile_hx", "tile_hy", "tile_hz", "tile_threads",
-                                      "tile_slice", "tile_ring"};
-    for (int k = 0; k < 9; ++k)
-      if (!std::strcmp(name, tn[k])) {
-        if (k == 6) {
-          if (value != 512 && value != 768 && value != 1024) return fail(h, SOMA_EINVAL, "tile_threads must be 512, 768 or 1024");
-          h->tile_threads = (int)value;
-        } else if (k == 7) {
-          if (value < 1 || value > 16) return fail(h, SOMA_EINVAL, "tile_slice must be in [1, 16]");
-          h->tile_slice = (uint32_t)value;
-        } else if (k == 8) {
-          if (value < 0 || value > (int64_t)kMaxRing) return fail(h, SOMA_EINVAL, "tile_ring must be in [0, 32]");
-          h->tile_ring_opt = (uint32_t)value;
-        } else {
-          if (value < 0 || value > 4096) return fail(h, SOMA_EINVAL, "tile size out of range");
-          (k < 3 ? h->tc[k] : h->th[k - 3]) = (uint32_t)value;
-        }
-        tile_setup(h);
-        if (!h->tile_ready && h->path >= 3) h->path = 0;
-        return SOMA_OK;                      // soma_get_counters()[3] tells whether tiles are usable now
+    static const char* const wn[6] = {"win_cx", "win_cy", "win_cz", "win_hx", "win_hy", "win_hz"};
+    for (int k = 0; k < 6; ++k)
+      if (!std::strcmp(name, wn[k])) {
+        if (value < 0 || value > 4096) return fail(h, SOMA_EINVAL, "window size out of range");
+        (k < 3 ? h->wc[k] : h->wh[k - 3]) = (uint32_t)value;
+        win_setup(h);
+        if (!h->win_ready && h->path == 3) h->path = 0;
+        return SOMA_OK;                      // soma_get_counters()[3] tells whether the windowed path is in use now
       }
   }
-  if (!std::strcmp(name, "tile_margin")) {
-    if (value < 0 || value > 16) return fail(h, SOMA_EINVAL, "tile_margin must be in [0, 16]");
-    h->tile_margin = (uint32_t)value;
-    if (h->sorted_kind == 2) h->sorted_kind = 0;
+  if (!std::strcmp(name, "fused_lean")) {              // 0: the general fused kernel even where the lean one applies
+    if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "fused_lean must be 0 or 1");
+    h->fused_lean = (int)value;
+    win_setup(h);
+    if (!h->win_ready && h->path == 3) h->path = 0;
     return SOMA_OK;
   }
-  if (!std::strcmp(name, "tile_fast")) {               // 0: use the general arithmetic even where the shortcuts apply
-    if (value != 0) return fail(h, SOMA_EINVAL, "tile_fast can only be switched off");
-    h->tile_fast = false;
+  if (!std::strcmp(name, "lean_threads")) {
+    if (value != 256 && value != 512 && value != 1024) return fail(h, SOMA_EINVAL, "lean_threads must be 256, 512 or 1024");
+    h->lean_threads = (int)value;
+    return SOMA_OK;
+  }
+  if (!std::strcmp(name, "win_auto")) {                // does path 0 pick the windowed-count kernel where it can run
+    if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "win_auto must be 0 or 1");
+    h->win_auto = value != 0;
     return SOMA_OK;
   }
   if (!std::strcmp(name, "fused_chunk")) {
     if (value < 1 || value > (1 << 20)) return fail(h, SOMA_EINVAL, "fused_chunk must be in [1, 2^20]");
     h->fused_chunk = (int)value;
+    return SOMA_OK;
+  }
+  if (!std::strcmp(name, "fused_carveout")) {
+    if (value < -1 || value > 100) return fail(h, SOMA_EINVAL, "fused_carveout must be in [-1, 100]");
+    h->fused_carveout = (int)value;
     return SOMA_OK;
   }
   return fail(h, SOMA_EINVAL, "unknown option name");
@@ -1154,7 +986,7 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
 int soma_get_counters(const soma_t* h, uint64_t* out) {
   if (!h || !out) return SOMA_EINVAL;
   out[0] = h->launches; out[1] = h->steps_done; out[2] = h->resorts;
-  out[3] = use_tile(h) ? (h->path == 3 ? 3 : 4) : (use_fused(h) ? 2 : 1);
+  out[3] = use_win(h) ? 3 : (use_fused(h) ? 2 : 1);
   return SOMA_OK;
 }
 
@@ -1185,7 +1017,7 @@ int soma_debug_half_sweep(soma_t* h, uint32_t parity, uint64_t* accepted) {
   if (parity > 1) return fail(h, SOMA_EINVAL, "parity must be 0 or 1");
   CU(h, cudaMemsetAsync(h->accepted(), 0, 8, h->stream));
   if ((rc = launch_half_sweep(h, parity)) != SOMA_OK) return rc;
-  if (parity == 0 && (rc = launch_singles(h, true, false, nullptr, false)) != SOMA_OK) return rc;
+  if (parity == 0 && (rc = launch_singles(h, true, false, nullptr)) != SOMA_OK) return rc;
   if (accepted) {
     unsigned long long v = 0;
     CU(h, cudaMemcpyAsync(&v, h->accepted(), 8, cudaMemcpyDeviceToHost, h->stream));
@@ -1212,8 +1044,6 @@ int soma_debug_set_omega(soma_t* h, const float* omega) {
   if (!omega) return fail(h, SOMA_EINVAL, "omega is NULL");
   CU(h, cudaMemcpyAsync(h->omega(), omega, (size_t)h->cells * h->T * 4, cudaMemcpyHostToDevice, h->stream));
   CU(h, cudaStreamSynchronize(h->stream));
-  h->omega_custom = true;
-  h->pad_valid = false;
   return SOMA_OK;
 }
 
@@ -1270,6 +1100,19 @@ int soma_debug_accept(const float* dE, const uint32_t* words, uint8_t* decision,
   CUG(cudaMemcpy(e.p, dE, n * 4, cudaMemcpyHostToDevice));
   CUG(cudaMemcpy(w.p, words, n * 4, cudaMemcpyHostToDevice));
   debug_accept_kernel<<<blocks_for(n, 256), 256>>>(n, (const float*)e.p, (const uint32_t*)w.p, (uint8_t*)d.p);
+  CUG(cudaGetLastError());
+  CUG(cudaMemcpy(decision, d.p, n, cudaMemcpyDeviceToHost));
+  return SOMA_OK;
+}
+
+int soma_debug_accept_fma(const float* dE, const uint32_t* words, uint8_t* decision, uint64_t n) {
+  if (!dE || !words || !decision) return fail(nullptr, SOMA_EINVAL, "NULL argument");
+  if (n == 0) return SOMA_OK;
+  DevBuf e, w, d;
+  CUG(e.alloc(n * 4)); CUG(w.alloc(n * 4)); CUG(d.alloc(n));
+  CUG(cudaMemcpy(e.p, dE, n * 4, cudaMemcpyHostToDevice));
+  CUG(cudaMemcpy(w.p, words, n * 4, cudaMemcpyHostToDevice));
+  debug_accept_fma_kernel<<<blocks_for(n, 256), 256>>>(n, (const float*)e.p, (const uint32_t*)w.p, (uint8_t*)d.p);
   CUG(cudaGetLastError());
   CUG(cudaMemcpy(decision, d.p, n, cudaMemcpyDeviceToHost));
   return SOMA_OK;

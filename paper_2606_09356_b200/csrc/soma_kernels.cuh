@@ -468,20 +468,14 @@ chain_permute_kernel(uint64_t B, uint32_t N, const uint32_t* __restrict__ bin_st
                      const float* __restrict__ sx, const float* __restrict__ sy, const float* __restrict__ sz,
                      float* __restrict__ dx, float* __restrict__ dy, float* __restrict__ dz,
                      const uint32_t* __restrict__ s_chain, const uint8_t* __restrict__ s_pat,
-                     uint32_t* __restrict__ d_chain, uint8_t* __restrict__ d_pat,
-                     const float4* __restrict__ s_meta, float4* __restrict__ d_meta /* both may be null */,
-                     uint16_t* __restrict__ d_k /* may be null */, uint32_t K) {
+                     uint32_t* __restrict__ d_chain, uint8_t* __restrict__ d_pat) {
   const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= B) return;
   const uint32_t s = (uint32_t)(j / N), i = (uint32_t)(j % N);
   const uint32_t d = bin_start[key[s]] + rank[s];
   const uint64_t k = (uint64_t)d * N + i;
   dx[k] = sx[j]; dy[k] = sy[j]; dz[k] = sz[j];
-  if (i == 0) {
-    d_chain[d] = s_chain[s]; d_pat[d] = s_pat[s];
-    if (d_meta) d_meta[d] = s_meta[s];
-    if (d_k) d_k[d] = (uint16_t)((key[s] >> 1) % K);       // tile sort key = 2 (unit K + slice) + e
-  }
+  if (i == 0) { d_chain[d] = s_chain[s]; d_pat[d] = s_pat[s]; }
 }
 
 // sets *range_flag if a bead's cell coordinate is NaN or beyond kCellCoordLimit (see floor_bits)
@@ -505,8 +499,7 @@ struct SingleArgs {
   uint32_t n_total, T;
   uint32_t start[kMaxTypes + 1];    // molecules of type t are [start[t], start[t+1])
   float* __restrict__ x; float* __restrict__ y; float* __restrict__ z;
-  uint32_t* __restrict__ counts;    // grid to bin into: linear [T][C], or ghost-padded [T][px][py][pz] if px != 0
-  uint32_t px, py, pz, hx, hy, hz;
+  uint32_t* __restrict__ counts;    // grid to bin into: [T][C]
   uint32_t* __restrict__ range_flag;  // may be null
   int do_move, do_bin;
 };
@@ -533,16 +526,7 @@ singles_kernel(SingleArgs A) {
       acc = metropolis_accept(__fmaf_rn(A.S.kb, 0.0f, dw), w.w3);
       if (acc) { rx = t.x; ry = t.y; rz = t.z; A.x[m] = rx; A.y[m] = ry; A.z[m] = rz; }
     }
-    if (A.do_bin) {
-      if (A.px) {                                        // ghost-padded grid of the windowed kernels: the interior image
-        const uint32_t gx = wrap<POW2>(__float2int_rd(__fmul_rn(rx, G.inv_hx)), G.nx);
-        const uint32_t gy = wrap<POW2>(__float2int_rd(__fmul_rn(ry, G.inv_hy)), G.ny);
-        const uint32_t gz = wrap<POW2>(__float2int_rd(__fmul_rn(rz, G.inv_hz)), G.nz);
-        atomicAdd(A.counts + ((size_t)(type * A.px + gx + A.hx) * A.py + gy + A.hy) * A.pz + gz + A.hz, 1u);
-      } else {
-        atomicAdd(A.counts + (size_t)type * A.S.cells + cell_of<POW2>(G, rx, ry, rz), 1u);
-      }
-    }
+    if (A.do_bin) atomicAdd(A.counts + (size_t)type * A.S.cells + cell_of<POW2>(G, rx, ry, rz), 1u);
   }
   const unsigned n_acc = __popc(__ballot_sync(0xffffffffu, acc));
   if ((threadIdx.x & 31u) == 0 && n_acc) atomicAdd(A.S.accepted, (unsigned long long)n_acc);
@@ -677,6 +661,12 @@ __global__ void debug_accept_kernel(uint64_t n, const float* dE, const uint32_t*
   const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= n) return;
   out[k] = metropolis_accept(dE[k], words[k]) ? 1 : 0;
+}
+// the decision routine of the fused kernels (one FFMA on the hardware logarithm + guard band)
+__global__ void debug_accept_fma_kernel(uint64_t n, const float* dE, const uint32_t* words, uint8_t* out) {
+  const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  out[k] = metropolis_accept_fma(dE[k], words[k]) ? 1 : 0;
 }
 template <bool POW2>
 __global__ void debug_cell_kernel(Grid g, uint64_t n, const float* x, const float* y, const float* z, uint32_t* out) {

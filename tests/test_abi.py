@@ -75,8 +75,7 @@ def test_workspace_bytes_and_validation(soma):
     nbytes = soma.soma_workspace_bytes(p)
     B, TC = 256 * 32, 2 * 16 ** 3
     assert nbytes >= 2 * 3 * 4 * B + 3 * 4 * TC + 5 * 256          # two position sets, two count grids, omega, tables
-    pad = 3 * 2 * 4 * (16 + 32 + 2 * 16 + 3) ** 3                     # ghost-padded omega + two density grids for the tiled kernel
-    assert nbytes < 2 * (2 * 3 * 4 * B + 3 * 4 * TC) + pad + 32 * 256
+    assert nbytes < 2 * (2 * 3 * 4 * B + 4 * 4 * TC) + 40 * 256   # + external field, sort scratch, alignment
     bad = [
         dict(n_chains=0), dict(beads_per_chain=0), dict(n_types=9), dict(b=0.0), dict(grid=(16, 0, 16)),
         dict(box=(8.0, -1.0, 8.0)), dict(chiN=np.array([[0, 20], [19, 0]], dtype=np.float32)),

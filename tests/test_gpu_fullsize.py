@@ -11,31 +11,38 @@ from helpers import gpu_system
 pytestmark = pytest.mark.gpu
 
 
-def test_cfg4_full_size_one_step_bit_exact_then_invariants():
+def _compare_full_state(g, o, what):
+    gx, gy, gz = g.positions()
+    ox, oy, oz = o.positions()
+    for name, a, b_ in (("x", gx, ox), ("y", gy, oy), ("z", gz, oz)):
+        assert np.array_equal(a, b_), f"{what}: {name} differs in {(a != b_).sum()} beads"    # bit-identical: no decision flipped
+    del gx, gy, gz, ox, oy, oz
+    assert np.array_equal(g.density(), o.density()), what
+    assert np.array_equal(g.omega().view(np.uint32), o.omega().view(np.uint32)), what
+
+
+def test_cfg4_full_size_after_1_and_10_steps_bit_exact():
+    """`north_star`: "compared with the oracle ... after 1 and after 10 MC steps" -- at the headline size, in
+    the launch configuration bench.py times (path 0), with the chain re-ordering inside the run (every 4
+    steps here, so that two fall into the ten steps; bench.py's default is every 64).  Ten oracle steps of
+    134 M beads take ~200 s on one core."""
     w = si.config(4)
     s = si.make_system(w)
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
-    acc_o = o.mc_steps(1)
-    ox, oy, oz = o.positions()
-    dens_o, om_o = o.density(), o.omega()
-    o.close()
-    with gpu_system(s) as g:                              # path 0 = what bench.py runs
+    with gpu_system(s, options=dict(resort_interval=4)) as g:    # path 0 = what bench.py runs
         g.load_state(s.x, s.y, s.z)
-        acc_g = g.mc_steps(1, want_accepted=True)
-        gx, gy, gz = g.positions()
-        assert acc_g == acc_o
-        for a, b_ in ((gx, ox), (gy, oy), (gz, oz)):
-            assert np.array_equal(a, b_)                  # bit-identical: no decision flipped among 134 M moves
-        del ox, oy, oz
-        assert np.array_equal(g.density(), dens_o)
-        assert np.array_equal(g.omega().view(np.uint32), om_o.view(np.uint32))
-        # nine more steps (one chain re-ordering is not due yet; force one to cover it at this size)
-        g.mc_steps(4)
-        g.set_option("resort_now", 1)
-        g.mc_steps(5)
+        acc_o = o.mc_steps(1)
+        assert g.mc_steps(1, want_accepted=True) == acc_o
+        _compare_full_state(g, o, "cfg4 after 1 step")
+        r0 = g.counters()["resorts"]
+        acc_o = o.mc_steps(9)
+        assert g.mc_steps(9, want_accepted=True) == acc_o
+        assert g.counters()["resorts"] >= r0 + 2
+        _compare_full_state(g, o, "cfg4 after 10 steps")
         x, y, z = g.positions()
         dens = g.density()
+    o.close()
     assert int(dens.sum()) == w.n_beads
     types = s.bead_types()
     for t in range(w.n_types):
@@ -53,23 +60,42 @@ def test_cfg4_full_size_one_step_bit_exact_then_invariants():
     assert float(np.abs(x - s.x).max()) < 10 * w.move_halfwidth
 
 
-@pytest.mark.parametrize("cfg,steps", [(1, 10), (2, 10), (3, 2)])
+@pytest.mark.parametrize("path", [2, 3])
+def test_cfg4_full_size_one_step_on_both_fused_variants(path):
+    """Whichever of the two variants of the lean kernel path 0 does not pick, at full size for one step."""
+    w = si.config(4)
+    s = si.make_system(w)
+    with gpu_system(s, path=path) as g:
+        if g.counters()["path"] == gpu_default_path(s):
+            pytest.skip("this is path 0's choice, covered by the 10-step test")
+        o = oracle.Oracle.from_system(s)
+        o.load_state(s.x, s.y, s.z)
+        g.load_state(s.x, s.y, s.z)
+        assert g.mc_steps(1, want_accepted=True) == o.mc_steps(1)
+        _compare_full_state(g, o, f"cfg4 path {path} after 1 step")
+        o.close()
+
+
+def gpu_default_path(s):
+    with gpu_system(s) as g:
+        return g.counters()["path"]
+
+
+@pytest.mark.parametrize("cfg,steps", [(1, 10), (2, 10), (3, 10)])
 def test_full_size_configs_bit_exact(cfg, steps):
     """configs[1..3] at BASELINE.json's full sizes on the default kernel path (cfg1, cfg3: N = 64, one
-    chain per warp; cfg3: two chain patterns), whole state against the oracle after `steps` MC steps."""
+    chain per warp; cfg3: two chain patterns), whole state against the oracle after 1 and after `steps`
+    MC steps, one chain re-ordering inside the run."""
     w = si.config(cfg)
     s = si.make_system(w)
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
-    acc_o = o.mc_steps(steps)
-    with gpu_system(s) as g:
+    with gpu_system(s, options=dict(resort_interval=6)) as g:
         g.load_state(s.x, s.y, s.z)
-        assert g.mc_steps(steps, want_accepted=True) == acc_o
-        gx, gy, gz = g.positions()
-        ox, oy, oz = o.positions()
-        assert np.array_equal(gx, ox) and np.array_equal(gy, oy) and np.array_equal(gz, oz)
-        assert np.array_equal(g.density(), o.density())
-        assert np.array_equal(g.omega().view(np.uint32), o.omega().view(np.uint32))
+        assert g.mc_steps(1, want_accepted=True) == o.mc_steps(1)
+        _compare_full_state(g, o, f"cfg{cfg} after 1 step")
+        assert g.mc_steps(steps - 1, want_accepted=True) == o.mc_steps(steps - 1)
+        _compare_full_state(g, o, f"cfg{cfg} after {steps} steps")
     o.close()
 
 

@@ -16,8 +16,7 @@ from helpers import assert_same_state, gpu_system, lockstep
 
 pytestmark = pytest.mark.gpu
 
-FUSED, GENERIC, TILED, SWEEP = 2, 1, 3, 4
-TILED_PATHS = (TILED, SWEEP)      # 3: first column-sweep kernel (soma_tile.cuh), 4: swept-window kernel (soma_sweep.cuh)
+FUSED, GENERIC, WINDOWED = 2, 1, 3      # 3: the lean kernel with bead counts in shared-memory windows (soma_lean.cuh)
 
 
 def _run_both(s, steps_list, path, **kw):
@@ -157,72 +156,100 @@ def test_large_seed_step_and_chain_ids_reach_the_counter():
         assert not np.array_equal(g2.positions()[0], o.positions()[0])
 
 
-# ---- the tiled kernel (x-sweep over columns: omega and density slabs in a shared-memory ring, TMA in and out)
-# Small windows on small grids so that the oracle stays fast while the run still covers many units,
-# windows that wrap around every periodic face, partial last columns (core not dividing the grid),
-# ring slots reused several times per sweep, beads outside their window (global-memory slow path)
-# and drift between re-sorts.  tile_cx = segment length along x, tile_cy/cz = column core,
-# tile_h* = halo, tile_slice = cells per slice, tile_ring = ring slots (0: as many as fit).
+# ---- the windowed-count variant of the lean kernel (path 3): one block per tile of the box, bead counts
+# in a shared-memory window (tile + halo) that is bulk-reduce-added into the global grid.  Small windows on
+# small grids so that the oracle stays fast while the run still covers many tiles, windows that wrap
+# around every periodic face, empty tiles, beads outside their window (global atomics) and drift
+# between re-sorts.  win_c* = tile core, win_h* = halo, in cells.
 
-SMALL_TILES = dict(tile_cx=4, tile_cy=4, tile_cz=4, tile_hx=2, tile_hy=2, tile_hz=2)          # 6x8x8 windows, most chains stick out
-ODD_TILES = dict(tile_cx=16, tile_cy=5, tile_cz=8, tile_hx=3, tile_hy=4, tile_hz=6, tile_slice=4, tile_ring=11)   # cores not dividing the grid, ring = one window + 1
-WIDE_HALO = dict(tile_cx=8, tile_cy=4, tile_cz=4, tile_hx=5, tile_hy=6, tile_hz=6, tile_slice=1)   # 11x16x16 windows: nearly all beads inside
-TIGHT_RING = dict(tile_cx=32, tile_cy=4, tile_cz=4, tile_hx=3, tile_hy=4, tile_hz=2, tile_slice=2, tile_ring=8)   # ring = exactly one window: no load-ahead
+SMALL_WIN = dict(win_cx=4, win_cy=4, win_cz=4, win_hx=2, win_hy=2, win_hz=4)          # 8x8x12 windows, many beads stick out
+NO_HALO = dict(win_cx=4, win_cy=8, win_cz=4, win_hx=0, win_hy=0, win_hz=0)            # window = core: most beads outside
+WIDE_WIN = dict(win_cx=8, win_cy=4, win_cz=8, win_hx=4, win_hy=6, win_hz=4)           # 16x16x16 windows (the whole 16^3 grid: wraps everywhere)
 
-TILE_CASES = {
-    "cfg0_full_small_tiles": (lambda: si.make_system(si.config(0)), SMALL_TILES),
-    "cfg0_full_wide_halo": (lambda: si.make_system(si.config(0)), WIDE_HALO),
-    "cfg1_scaled_T1_N64": (lambda: _scaled(1, 4099, (16, 16, 16)), SMALL_TILES),
-    "cfg2_scaled_odd_tiles": (lambda: _scaled(2, 8193, (32, 16, 32)), ODD_TILES),
-    "cfg3_scaled_blend_N64": (lambda: _scaled(3, 4098, (32, 16, 16)), WIDE_HALO),
-    "cfg4_scaled_default_tiles": (lambda: _scaled(4, 16385, (32, 32, 32)), {}),                 # 8x8 columns + 8, slices of 2: the bench shape
-    "cfg4_scaled_tight_ring": (lambda: _scaled(4, 16385, (32, 32, 16)), TIGHT_RING),
-    "cfg2_scaled_general_arithmetic": (lambda: _scaled(2, 8193, (32, 16, 32)), dict(SMALL_TILES, tile_fast=0, tile_margin=0)),
-    "cfg4_scaled_threads_512": (lambda: _scaled(4, 16385, (32, 32, 16)), dict(WIDE_HALO, tile_threads=512)),
-    "cfg4_scaled_threads_768": (lambda: _scaled(4, 16385, (32, 32, 16)), dict(SMALL_TILES, tile_threads=768)),
+WIN_CASES = {
+    "cfg0_full_small_win": (lambda: si.make_system(si.config(0)), SMALL_WIN),
+    "cfg0_full_wide_win": (lambda: si.make_system(si.config(0)), WIDE_WIN),
+    "cfg0_full_no_halo": (lambda: si.make_system(si.config(0)), NO_HALO),
+    "cfg1_scaled_T1_N64": (lambda: _scaled(1, 4099, (16, 16, 16)), SMALL_WIN),
+    "cfg2_scaled": (lambda: _scaled(2, 8193, (32, 16, 32)), WIDE_WIN),
+    "cfg3_scaled_blend_N64": (lambda: _scaled(3, 4098, (32, 16, 16)), SMALL_WIN),
+    "cfg4_scaled_default_win": (lambda: _scaled(4, 16385, (32, 32, 32)), {}),           # 8^3 tiles + 4: the bench shape
+    "cfg4_scaled_noncubic": (lambda: _scaled(4, 16385, (32, 32, 16)), dict(win_cx=16, win_cy=8, win_cz=4, win_hx=2, win_hy=4, win_hz=4)),
     "T3_three_patterns": (lambda: _custom(900, 32, 3, [[0] * 10 + [1] * 12 + [2] * 10, [2] * 32, [1] * 16 + [0] * 16],
                                           np.arange(900) % 3, [[0, 12, 5], [12, 0, 21], [5, 21, 0]], 35.0, (16, 32, 16), (8.0, 16.0, 8.0), 41),
-                          SMALL_TILES),
-    "N2": (lambda: _custom(3001, 2, 2, [[0, 1]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 42), SMALL_TILES),
-    "N8": (lambda: _custom(1517, 8, 2, [[0, 0, 0, 1, 1, 1, 1, 0]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 43), SMALL_TILES),
-    "one_chain": (lambda: _custom(1, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (16, 16, 16), (8, 8, 8), 44), SMALL_TILES),
-    "big_moves_unit_cells": (lambda: _custom(700, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (16, 16, 32), (11.2, 14.0, 25.6), 45,
-                                             b=0.7, move_halfwidth=0.9), WIDE_HALO),
+                          SMALL_WIN),
+    "N2": (lambda: _custom(3001, 2, 2, [[0, 1]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 42), SMALL_WIN),
+    "N8": (lambda: _custom(1517, 8, 2, [[0, 0, 0, 1, 1, 1, 1, 0]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 43), SMALL_WIN),
+    "one_chain": (lambda: _custom(1, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (16, 16, 16), (8, 8, 8), 44), SMALL_WIN),   # all tiles but one empty
+    "T8_sparse": (lambda: _custom(300, 16, 8, [[0, 1, 2, 3, 4, 5, 6, 7] * 2], None,
+                                  (np.arange(64).reshape(8, 8) + np.arange(64).reshape(8, 8).T) * (1 - np.eye(8)) * 0.3, 25.0,
+                                  (8, 8, 8), (4, 4, 4), 46), dict(win_cx=4, win_cy=4, win_cz=4, win_hx=1, win_hy=1, win_hz=0)),
 }
 
 
-@pytest.mark.parametrize("TILED", TILED_PATHS)
-@pytest.mark.parametrize("case", sorted(TILE_CASES))
-def test_tiled_path_parity_after_1_and_10_steps(case, TILED):
-    make, opts = TILE_CASES[case]
+@pytest.mark.parametrize("case", sorted(WIN_CASES))
+def test_windowed_count_path_parity_after_1_and_10_steps(case):
+    make, opts = WIN_CASES[case]
     s = make()
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
-    with gpu_system(s, path=TILED, options=opts) as g:
-        assert g.counters()["path"] == TILED
+    with gpu_system(s, path=WINDOWED, options=opts) as g:
+        assert g.counters()["path"] == WINDOWED
         g.load_state(s.x, s.y, s.z)
         done = 0
         for upto in (1, 10):
             assert g.mc_steps(upto - done, want_accepted=True) == o.mc_steps(upto - done)
             done = upto
-            assert_same_state(g, o, f"{case} tiled after {upto} steps")
-        assert g.counters()["path"] == TILED
+            assert_same_state(g, o, f"{case} windowed after {upto} steps")
+        assert g.counters()["path"] == WINDOWED
 
 
-@pytest.mark.parametrize("TILED", TILED_PATHS)
+@pytest.mark.parametrize("path", [FUSED, WINDOWED])
 @pytest.mark.parametrize("interval", [0, 1, 3])
-def test_tiled_path_with_drift_and_resorts(interval, TILED):
-    """40 steps: without re-sorting the chains drift out of their tiles (fallback path); with
-    frequent re-sorting the slot order keeps changing.  The trajectory may not depend on either."""
+def test_drift_and_resorts_do_not_change_the_trajectory(interval, path):
+    """40 steps: without re-sorting the chains drift out of their tiles (global atomics); with frequent
+    re-sorting the slot order keeps changing.  The trajectory may not depend on either.  (Path 2 is the
+    kernel bench.py times: its periodic re-ordering is compared with the oracle here.)"""
     s = _scaled(4, 6000, (16, 16, 16))
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
     acc_o = o.mc_steps(40)
-    with gpu_system(s, path=TILED, options=dict(SMALL_TILES, resort_interval=interval)) as g:
+    with gpu_system(s, path=path, options=dict(SMALL_WIN, resort_interval=interval)) as g:
         g.load_state(s.x, s.y, s.z)
         assert g.mc_steps(40, want_accepted=True) == acc_o
-        assert_same_state(g, o, f"tiled, resort_interval={interval}")
-        assert g.counters()["resorts"] == (1 if interval == 0 else 1 + (40 - 1) // interval)
+        assert_same_state(g, o, f"path {path}, resort_interval={interval}")
+        first = 1 if (interval or path == WINDOWED) else 0           # path 2 never sorts when the interval is 0
+        assert g.counters()["resorts"] == first + ((40 - 1) // interval if interval else 0)
+
+
+@pytest.mark.parametrize("path", [FUSED, WINDOWED])
+@pytest.mark.parametrize("interval", [1, 3])
+def test_parity_after_1_and_10_steps_with_resorts(interval, path):
+    """The full-state comparison after 1 and 10 steps with the chain re-ordering inside the run."""
+    s = _scaled(4, 16385, (32, 32, 16))
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s, path=path, options=dict(resort_interval=interval)) as g:
+        g.load_state(s.x, s.y, s.z)
+        done = 0
+        for upto in (1, 10):
+            assert g.mc_steps(upto - done, want_accepted=True) == o.mc_steps(upto - done)
+            done = upto
+            assert_same_state(g, o, f"path {path}, resort every {interval}, after {upto} steps")
+        assert g.counters()["resorts"] >= 1 + 9 // interval
+
+
+@pytest.mark.parametrize("lean", [0, 1])
+def test_general_and_lean_fused_kernels_agree_with_the_oracle(lean):
+    """fused_lean = 0 keeps the general fused kernel (any grid, any cell size) on a system where the lean
+    one applies; both must give the oracle's state."""
+    s = _scaled(2, 8193, (16, 16, 16))
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s, path=FUSED, options=dict(fused_lean=lean)) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert g.mc_steps(5, want_accepted=True) == o.mc_steps(5)
+        assert_same_state(g, o, f"fused_lean={lean}")
 
 
 def test_switching_paths_mid_run_keeps_the_trajectory():
@@ -230,41 +257,40 @@ def test_switching_paths_mid_run_keeps_the_trajectory():
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
     o.mc_steps(8)
-    with gpu_system(s, path=FUSED, options=SMALL_TILES) as g:
+    with gpu_system(s, path=FUSED, options=SMALL_WIN) as g:
         g.load_state(s.x, s.y, s.z)
-        for path in (FUSED, TILED, GENERIC, SWEEP, FUSED, SWEEP, TILED, GENERIC):
+        for path in (FUSED, WINDOWED, GENERIC, WINDOWED, FUSED, GENERIC, WINDOWED, FUSED):
             g.set_option("path", path)
             g.mc_steps(1)
         assert_same_state(g, o, "path switched every step")
 
 
-def test_tiled_path_is_refused_where_it_cannot_run():
+def test_windowed_path_is_refused_where_it_cannot_run():
     import paper_2606_09356_b200 as soma
-    for make in (EDGE["T3_npot"], EDGE["N33"], EDGE["one_chain"]):          # non-power-of-two grid, odd N, 1-cell grid
+    for make in (EDGE["T3_npot"], EDGE["N33"], EDGE["one_chain"], EDGE["b_and_a"]):   # non-power-of-two grid, odd N, 1-cell grid, cell size not 2^k
         with gpu_system(make()) as g:
             with pytest.raises(soma.SomaError) as e:
-                g.set_option("path", TILED)
-            assert e.value.code == soma.SOMA_EINVAL and "tiled path unavailable" in str(e.value)
-    with gpu_system(si.make_system(si.config(0))) as g:                      # default 18x24x24 window > 16^3 grid
+                g.set_option("path", WINDOWED)
+            assert e.value.code == soma.SOMA_EINVAL and "windowed path unavailable" in str(e.value)
+    with gpu_system(si.make_system(si.config(0))) as g:                      # default 16^3 window = the 16^3 grid: allowed
+        g.set_option("path", WINDOWED)
+        g.set_option("win_hz", 3)                                            # halo along z not a multiple of 4 -> windows off
+        assert g.counters()["path"] != WINDOWED
+        g.set_option("win_hz", 8)                                            # window larger than the grid
         with pytest.raises(soma.SomaError):
-            g.set_option("path", TILED)
-        g.set_option("tile_cx", 4); g.set_option("tile_cy", 4); g.set_option("tile_cz", 4)
-        g.set_option("tile_hx", 2); g.set_option("tile_hy", 2); g.set_option("tile_hz", 2)
-        g.set_option("path", TILED)
-        g.set_option("tile_hz", 3)                                           # window 10 cells along z: not a multiple of 4 -> tiles off
-        assert g.counters()["path"] != TILED
+            g.set_option("path", WINDOWED)
 
 
 # ---- external field: omega = interaction part + ext, every kernel path -----
 
-@pytest.mark.parametrize("path", [FUSED, GENERIC, TILED, SWEEP])
+@pytest.mark.parametrize("path", [FUSED, GENERIC, WINDOWED])
 def test_external_field_parity(path):
     s = _scaled(4, 6000, (16, 16, 16))
     ext = np.random.default_rng(31).normal(0.0, 0.8, size=(2, 16 ** 3)).astype(np.float32)
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
     o.set_external_field(ext)
-    with gpu_system(s, path=path, options=SMALL_TILES if path in TILED_PATHS else None) as g:
+    with gpu_system(s, path=path, options=SMALL_WIN if path == WINDOWED else None) as g:
         g.load_state(s.x, s.y, s.z)
         g.set_external_field(ext)
         assert np.array_equal(g.omega().view(np.uint32), o.omega().view(np.uint32))
@@ -301,12 +327,12 @@ def _mixture(n_chains=3000, N=32, n_single=(7000, 0, 11000), grid=(16, 16, 16), 
     return si.custom_system(n_chains, N, 3, pat, None, chi, 40.0, grid, tuple(g / 2 for g in grid), seed=seed, n_single=n_single)
 
 
-@pytest.mark.parametrize("path", [FUSED, GENERIC, TILED, SWEEP])
+@pytest.mark.parametrize("path", [FUSED, GENERIC, WINDOWED])
 def test_mixture_of_chains_and_single_bead_molecules(path):
     s = _mixture()
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
-    with gpu_system(s, path=path, options=SMALL_TILES if path in TILED_PATHS else None) as g:
+    with gpu_system(s, path=path, options=SMALL_WIN if path == WINDOWED else None) as g:
         g.load_state(s.x, s.y, s.z)
         assert_same_state(g, o, f"mixture loaded, path {path}")
         done = 0

@@ -73,6 +73,55 @@ def test_uniform_maps_and_lnu_all_2_24_values(soma):
         assert float(tt[0]) == oracle.tmap(w) and float(uu[0]) == oracle.umap(w)
 
 
+def _threshold_sample(rng, n):
+    """(dE, words, lnu): a sample concentrated on the acceptance threshold dE = -lnu."""
+    words = rng.integers(0, 2 ** 32, size=n, dtype=np.uint64).astype(np.uint32)
+    u = ((words >> np.uint32(8)).astype(np.float64) + 1.0) * 2.0 ** -24
+    lnu = oracle.lnu(u.astype(np.float32))
+    dE = np.empty(n, dtype=np.float32)
+    q = n // 4
+    dE[:q] = rng.normal(0.0, 3.0, q).astype(np.float32)                       # generic
+    base = (-lnu[q:3 * q]).astype(np.float32)                                 # on the threshold
+    ulps = rng.integers(-3, 4, size=2 * q)
+    near = base.copy()
+    for s in range(1, 4):
+        near = np.where(ulps >= s, np.nextafter(near, np.float32(np.inf)), near)
+        near = np.where(ulps <= -s, np.nextafter(near, np.float32(-np.inf)), near)
+    dE[q:3 * q] = near
+    dE[3 * q:] = (-lnu[3 * q:] + rng.uniform(-3e-4, 3e-4, n - 3 * q)).astype(np.float32)   # in/around the band
+    dE[:20] = [0.0, -0.0, 1e-30, -1e-30, 1e-8, 17.0, 16.635532, 16.64, 100.0, np.inf, -np.inf, 5e-8, 6e-8, 1.1920929e-07, 2e-7, 3e-7,
+               np.nan, -np.nan, 3.4e38, -3.4e38]
+    return dE, words, lnu
+
+
+def test_fused_kernels_accept_routine_matches_the_definition(soma):
+    """metropolis_accept_fma -- the decision routine of the fused kernels, i.e. of the path bench.py times:
+    one FFMA on the hardware logarithm, a +-1e-4 guard band, the exact logarithm inside it -- against the
+    rule accept iff fl32(dE + lnu) <= 0 (DESIGN.md section 2 step 5.6) on the threshold-concentrated sample,
+    and for EVERY one of the 2^24 values of u at dE = -lnu moved by 0, +-1, +-2, +-3 ulps."""
+    dE, words, lnu = _threshold_sample(np.random.default_rng(6), 1 << 21)
+    got = soma.soma_debug_accept_fma(dE, words)
+    with np.errstate(invalid="ignore"):
+        want = ((dE + lnu).astype(np.float32) <= 0).astype(np.uint8)
+    bad = np.nonzero(got != want)[0]
+    assert bad.size == 0, (bad[:10], dE[bad[:10]], lnu[bad[:10]])
+    k = np.arange(1 << 24, dtype=np.uint32)
+    words = (k << np.uint32(8)) | np.uint32(0x5A)
+    u = ((k.astype(np.float64) + 1.0) * 2.0 ** -24).astype(np.float32)
+    lnu = oracle.lnu(u)
+    n_acc = 0
+    for shift in (0, 1, -1, 2, -2, 3, -3):
+        dE = (-lnu).astype(np.float32)
+        for _ in range(abs(shift)):
+            dE = np.nextafter(dE, np.float32(np.inf if shift > 0 else -np.inf))
+        got = soma.soma_debug_accept_fma(dE, words)
+        want = ((dE + lnu).astype(np.float32) <= 0).astype(np.uint8)
+        bad = np.nonzero(got != want)[0]
+        assert bad.size == 0, (shift, bad[:10], dE[bad[:10]], lnu[bad[:10]])
+        n_acc += int(want.sum())
+    assert 0.3 < n_acc / (7 * (1 << 24)) < 0.7                                # the shifts straddle the threshold
+
+
 def test_accept_decisions_match_the_definition(soma):
     """accept iff fl32(dE + lnu) <= 0 (DESIGN.md section 2 step 5.6), lnu the oracle's.  The sample
     is concentrated on the threshold: dE = -lnu +- a few ulps, where the kernel's fast logarithm

@@ -14,15 +14,24 @@ A = 0.05
 
 
 def test_library_free_log_and_sincos_agree_with_libm():
-    """The fp32 routines behind the deviates, at fp32 accuracy over the whole range of their arguments
-    (U = (k + 0.5) 2^-23, k < 2^23)."""
-    rng = np.random.default_rng(1)
-    ks = np.concatenate([rng.integers(0, 1 << 23, 6000), [0, 1, 2, (1 << 23) - 1, 1 << 21, 1 << 22, 3 << 21]])
-    for k in ks:
-        x = float(np.float32((float(k) + 0.5) * 2.0 ** -23))
-        lg, sn, cs = oracle.det_functions(x)
-        assert abs(lg - math.log(x)) <= 3e-7 * max(1.0, abs(math.log(x))), (x, lg)
-        assert abs(sn - math.sin(2 * math.pi * x)) < 4e-7 and abs(cs - math.cos(2 * math.pi * x)) < 4e-7, x
+    """The fp32 routines behind the deviates against libm in double, at fp32 accuracy, for EVERY argument
+    they can be given: U = (k + 0.5) 2^-23, k = 0 .. 2^23 - 1 (a slip in the exponent split, the quarter-turn
+    rotation or a polynomial coefficient at any single k fails here)."""
+    k = np.arange(1 << 23, dtype=np.float64)
+    x = ((k + 0.5) * 2.0 ** -23).astype(np.float32)
+    assert np.array_equal(x.astype(np.float64), (k + 0.5) * 2.0 ** -23)          # the arguments are exact in fp32
+    lg, sn, cs = oracle.det_functions_n(x)
+    xd = x.astype(np.float64)
+    ref = np.log(xd)
+    err = np.abs(lg.astype(np.float64) - ref) / np.maximum(1.0, np.abs(ref))
+    assert err.max() <= 3e-7, (err.max(), x[err.argmax()])
+    es = np.abs(sn.astype(np.float64) - np.sin(2 * np.pi * xd))
+    ec = np.abs(cs.astype(np.float64) - np.cos(2 * np.pi * xd))
+    assert es.max() < 4e-7 and ec.max() < 4e-7, (es.max(), x[es.argmax()], ec.max(), x[ec.argmax()])
+    # the scalar entry point used elsewhere is the same routine
+    for kk in (0, 1, 2, (1 << 23) - 1, 1 << 21, 1 << 22, 3 << 21, 12345):
+        a = oracle.det_functions(float(x[kk]))
+        assert (np.float32(a[0]), np.float32(a[1]), np.float32(a[2])) == (lg[kk], sn[kk], cs[kk])
 
 
 def test_normal_deviates_are_standard_normal_and_independent():
