@@ -295,8 +295,7 @@ def run_ours(args):
     move_ms, omega_ms = kt["move_bin_ms"] / n_t, kt["omega_ms"] / n_t
     achieved = ab["move_bin_kernel"] / (move_ms * 1e-3) / 1e9
     path_now = g_path
-    kname = {1: "half_sweep_kernel x2 + bin_kernel (rows a1+a2+a3+a5)", 2: "lean_step_kernel (rows a1+a2+a3+a5)",
-             3: "lean_step_kernel, bead counts in shared-memory windows (rows a1+a2+a3+a5)"}[path_now]
+    kname = {1: "half_sweep_kernel x2 + bin_kernel (rows a1+a2+a3+a5)", 2: "lean_step_kernel (rows a1+a2+a3+a5)"}[path_now]
     traffic = args.traffic
     if traffic is None and path_now == 2 and args.config == 4:
         traffic = NCU_TRAFFIC_CFG4_FUSED
@@ -351,7 +350,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: 134 M beads)")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--path", type=int, default=0, help="library kernel path: 0 auto, 1 generic, 2 fused, 3 fused with windowed counts")
+    ap.add_argument("--path", type=int, default=0, help="library kernel path: 0 auto, 1 generic, 2 fused")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=INT", help="soma_set_option(NAME, INT) before the run (tuning)")
     ap.add_argument("--smc-mobility", type=float, default=0.0,

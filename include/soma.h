@@ -168,14 +168,7 @@ const char *soma_last_error(const soma_t *h);
  *                     2 = fused chain-in-registers kernel (N = 2P, P a power of two <= 32; else EINVAL).
  *                         Where the geometry allows it -- power-of-two grid, cell size a power of two
  *                         <= 1, move half-width a power of two, uniform moves -- this is the lean kernel
- *                         of soma_lean.cuh, else the general one of soma_kernels.cuh,
- *                     3 = the lean kernel with one block per tile of the box, bead counts in a
- *                         shared-memory window (tile + halo) added to the density grid by bulk reduce-adds
- *                         (conditions of the lean kernel, plus: tiles divide the grid, window <= grid and
- *                         <= 56 KB, z extents multiples of 4 cells; else EINVAL)
- *   "win_cx|cy|cz"    tile core in cells (default 8, 8, 8); "win_hx|hy|hz" halo in cells (4, 4, 4).  A
- *                     combination path 3 cannot use switches it off (see soma_get_counters [3])
- *   "win_auto"        1 = path 0 takes path 3 where it can run, 0 = path 0 takes path 2
+ *                         of soma_lean.cuh, else the general one of soma_kernels.cuh
  *   "fused_lean"      0 = path 2 always runs the general fused kernel (default 1)
  *   "fused_carveout"  preferred shared-memory carve-out of the fused kernel in percent (-1 = driver default; tuning)
  *   "kernel_timing"   1 = record CUDA events on the handle's stream around the kernels of every step
@@ -185,11 +178,12 @@ const char *soma_last_error(const soma_t *h);
  *                     independent of it (the random stream is keyed by the logical chain id)
  *   "resort_now"      re-order once, now (value ignored)
  *   "fused_chunk"     warp groups (32 bead pairs each) per block of the fused kernel (default 224; tuning)
+ *   "lean_threads"    threads per block of the lean kernel: 256 (default), 512 or 1024 (tuning)
  * Errors: SOMA_EINVAL (unknown name / unsupported value). */
 int soma_set_option(soma_t *h, const char *name, int64_t value);
 
 /* Counters since soma_create: [0] kernels launched by this library, [1] MC steps done,
- * [2] chain re-orderings done; [3] the kernel path the next step will take (1, 2 or 3).
+ * [2] chain re-orderings done; [3] the kernel path the next step will take (1 or 2).
  * `out` is a host pointer to 4 uint64. */
 int soma_get_counters(const soma_t *h, uint64_t *out);
 

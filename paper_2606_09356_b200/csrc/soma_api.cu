@@ -166,15 +166,10 @@ struct soma_handle {
   int fused_chunk;              // warp groups per block of the fused kernel
   int fused_carveout;           // preferred shared-memory carve-out of the fused kernel in percent (-1: driver default)
   bool fast_arith;              // inv_h a power of two >= 1 on every axis and a a power of two: the one-FFMA shortcuts are exact
-  int sorted_kind;              // bins the slots are currently sorted by: 0 none, 1 cubes of 4 cells, 2 tiles of the windowed-count kernel
-  // lean kernel (soma_lean.cuh) and its windowed-count variant
+  bool sorted;                  // the slots are sorted by the cube of 4 cells that holds the chain's centre of mass
+  // lean kernel (soma_lean.cuh)
   int fused_lean;               // use lean_step_kernel where it applies (option, default 1)
   int lean_threads;             // threads per block of the lean kernel: 256, 512 or 1024
-  uint32_t wc[3], wh[3];        // tile core and halo in cells (options win_c*, win_h*)
-  uint32_t ww[3], nt[3], n_tiles;   // window = core + 2 halo; tiles per axis
-  size_t win_smem;
-  bool win_ready, win_auto;     // geometry is valid for this system; path 0 picks the windowed variant
-  char win_why[96];             // why the windowed variant is unavailable ("" if it is available)
   // counters
   uint64_t launches, steps_done, resorts;
   // per-kernel timing ("kernel_timing" option): event triples (before moves, after moves+bin, after omega)
@@ -324,57 +319,20 @@ int launch_omega(soma_handle* h) {
 bool lean_ok(const soma_handle* h) {
   return h->fused_lean && h->fast_arith && h->pow2 && h->smcA == 0.0f && fused_lanes(h->N) != 0;
 }
-bool use_win(const soma_handle* h) {
-  if (!h->win_ready || !lean_ok(h) || h->path == 1) return false;
-  return h->path == 3 || (h->path == 0 && h->win_auto);
-}
-
-// Geometry of the windowed-count variant from the options.  Leaves win_ready false (with the reason
-// in h->win_why) when it cannot run; that is not an error.
-void win_setup(soma_handle* h) {
-  h->win_ready = false;
-  if (h->sorted_kind == 2) h->sorted_kind = 0;          // the tile table belongs to the old geometry
-  auto no = [&](const char* why) { snprintf(h->win_why, sizeof h->win_why, "%s", why); };
-  if (!lean_ok(h)) return no("needs a power-of-two grid, power-of-two cell size >= 1/b-unit and move half-width, uniform moves, N = 2P");
-  const uint32_t n[3] = {h->grid.nx, h->grid.ny, h->grid.nz};
-  uint64_t tiles = 1, words = h->T;
-  for (int d = 0; d < 3; ++d) {
-    if (h->wc[d] < kSortBinEdge || h->wc[d] > n[d] || n[d] % h->wc[d]) return no("tile core must be >= 4 cells and divide the grid");
-    h->ww[d] = h->wc[d] + 2 * h->wh[d];
-    if (h->ww[d] > n[d]) return no("window (core + 2 halo) is larger than the grid");
-    h->nt[d] = n[d] / h->wc[d];
-    tiles *= h->nt[d];
-    words *= h->ww[d];
-  }
-  if (h->wc[2] % 4 || h->wh[2] % 4 || n[2] % 4) return no("tile core and halo along z must be multiples of 4 cells");
-  if (words * 4 > 160 * 1024) return no("window does not fit in shared memory (160 KB per block)");
-  h->n_tiles = (uint32_t)tiles;
-  h->win_smem = (size_t)words * 4;
-  h->win_why[0] = 0;
-  h->win_ready = true;
-}
-
-template <int P, bool MULTI, bool WIN, int NT>
+template <int P, bool MULTI, int NT>
 void launch_lean_k(soma_handle* h, LeanArgs& A) {
   constexpr int G = 32 / P;
-  auto* k = lean_step_kernel<P, MULTI, WIN, NT>;
-  if (WIN) {
-    if (h->win_smem > 48 * 1024) cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->win_smem);
-    k<<<h->n_tiles, NT, h->win_smem, h->stream>>>(A);
-  } else {
-    const uint64_t n_groups = (h->n_chains + G - 1) / G;
-    const uint64_t wpb = NT / 32;
-    const uint64_t gpb = ((uint64_t)h->fused_chunk * (NT / 256) + wpb - 1) / wpb * wpb;   // fused_chunk is per 256 threads
-    A.groups_per_block = (uint32_t)gpb;
-    if (h->fused_carveout >= 0) cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, h->fused_carveout);
-    k<<<(unsigned)((n_groups + gpb - 1) / gpb), NT, 0, h->stream>>>(A);
-  }
+  auto* k = lean_step_kernel<P, MULTI, NT>;
+  const uint64_t n_groups = (h->n_chains + G - 1) / G;
+  const uint64_t wpb = NT / 32;
+  const uint64_t gpb = ((uint64_t)h->fused_chunk * (NT / 256) + wpb - 1) / wpb * wpb;   // fused_chunk is per 256 threads
+  A.groups_per_block = (uint32_t)gpb;
+  if (h->fused_carveout >= 0) cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, h->fused_carveout);
+  k<<<(unsigned)((n_groups + gpb - 1) / gpb), NT, 0, h->stream>>>(A);
 }
 template <int P, int NT>
-int launch_lean_pn(soma_handle* h, LeanArgs& A, bool win) {
-  const bool multi = h->n_patterns > 1;
-  if (win) { if (multi) launch_lean_k<P, true, true, NT>(h, A); else launch_lean_k<P, false, true, NT>(h, A); }
-  else     { if (multi) launch_lean_k<P, true, false, NT>(h, A); else launch_lean_k<P, false, false, NT>(h, A); }
+int launch_lean_pn(soma_handle* h, LeanArgs& A) {
+  if (h->n_patterns > 1) launch_lean_k<P, true, NT>(h, A); else launch_lean_k<P, false, NT>(h, A);
   h->launches++;
   CU(h, cudaGetLastError());
   return SOMA_OK;
@@ -403,19 +361,10 @@ int launch_lean_p(soma_handle* h) {
   A.slot_pattern = h->slot_pattern();
   A.patterns = h->patterns();
   A.accepted = h->accepted();
-  A.T = h->T;
-  const bool win = use_win(h);
-  if (win) {
-    A.tile_start = h->sort_bins();
-    A.tcx = h->wc[0]; A.tcy = h->wc[1]; A.tcz = h->wc[2];
-    A.hx = h->wh[0]; A.hy = h->wh[1]; A.hz = h->wh[2];
-    A.wx = h->ww[0]; A.wy = h->ww[1]; A.wz = h->ww[2];
-    A.nty = h->nt[1]; A.ntz = h->nt[2];
-  }
   switch (h->lean_threads) {
-    case 256: return launch_lean_pn<P, 256>(h, A, win);
-    case 512: return launch_lean_pn<P, 512>(h, A, win);
-    default: return launch_lean_pn<P, 1024>(h, A, win);
+    case 256: return launch_lean_pn<P, 256>(h, A);
+    case 512: return launch_lean_pn<P, 512>(h, A);
+    default: return launch_lean_pn<P, 1024>(h, A);
   }
 }
 
@@ -464,24 +413,16 @@ bool use_fused(const soma_handle* h) {
   if (h->path == 1) return false;
   return fused_lanes(h->N) != 0;
 }
-// Re-order the chains in memory by the coarse bin of their centre of mass (counting sort on the
-// device).  kind 1: cubes of kSortBinEdge cells; kind 2: the tiles of the windowed-count kernel
-// (numbered z fastest), whose tile_start table is the scanned bin array.
-int resort(soma_handle* h, int kind) {
+// Re-order the chains in memory by the coarse bin (cube of kSortBinEdge cells) of their centre of
+// mass: a counting sort on the device.
+int resort(soma_handle* h) {
   const int src = h->live, dst = h->live ^ 1;
   SortArgs S{};
   S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
-  uint32_t n_bins;
-  if (kind == 2) {
-    S.cbx = h->wc[0]; S.cby = h->wc[1]; S.cbz = h->wc[2];
-    S.ncy = h->grid.ny / h->wc[1]; S.ncz = h->grid.nz / h->wc[2];
-    n_bins = h->n_tiles;
-  } else {
-    S.cbx = S.cby = S.cbz = kSortBinEdge;
-    S.ncy = (h->grid.ny + kSortBinEdge - 1) / kSortBinEdge;
-    S.ncz = (h->grid.nz + kSortBinEdge - 1) / kSortBinEdge;
-    n_bins = h->n_bins;
-  }
+  S.cbx = S.cby = S.cbz = kSortBinEdge;
+  S.ncy = (h->grid.ny + kSortBinEdge - 1) / kSortBinEdge;
+  S.ncz = (h->grid.nz + kSortBinEdge - 1) / kSortBinEdge;
+  const uint32_t n_bins = h->n_bins;
   CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
   if (h->pow2)
     chain_key_kernel<true><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
@@ -500,7 +441,7 @@ int resort(soma_handle* h, int kind) {
   h->identity_order = false;
   h->resorts++;
   h->steps_since_sort = 0;
-  h->sorted_kind = kind;
+  h->sorted = true;
   return SOMA_OK;
 }
 
@@ -536,12 +477,8 @@ cudaEvent_t timing_mark(soma_handle* h) {
 
 int one_step(soma_handle* h) {
   int rc;
-  const bool win = use_win(h);
-  const int kind = win ? 2 : 1;
-  // the windowed-count kernel needs the slots sorted by tile; otherwise sorting is an optimisation
-  if ((win && h->sorted_kind != 2) ||
-      (h->resort_interval > 0 && (h->steps_since_sort >= (uint64_t)h->resort_interval || h->sorted_kind != kind)))
-    if ((rc = resort(h, kind)) != SOMA_OK) return rc;
+  if (h->resort_interval > 0 && (h->steps_since_sort >= (uint64_t)h->resort_interval || !h->sorted))
+    if ((rc = resort(h)) != SOMA_OK) return rc;
   const bool timed = h->timing && h->ev_used + 3 <= 3 * kMaxTimedSteps;
   if (timed) timing_mark(h);
   if (use_fused(h)) {
@@ -693,14 +630,11 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->fused_carveout = -1;
   h->fused_lean = 1;
   h->lean_threads = 256;
-  h->wc[0] = h->wc[1] = h->wc[2] = 8;
-  h->wh[0] = h->wh[1] = h->wh[2] = 4;
   {
     auto pow2f = [](float v) { int e; return v > 0.0f && std::frexp(v, &e) == 0.5f && e > -100 && e < 100; };
     h->fast_arith = pow2f(h->a) && pow2f(h->grid.inv_hx) && pow2f(h->grid.inv_hy) && pow2f(h->grid.inv_hz) &&
                    h->grid.inv_hx >= 1.0f && h->grid.inv_hy >= 1.0f && h->grid.inv_hz >= 1.0f;
   }
-  win_setup(h);
   const double cells_per_step = (double)h->a * (double)fmaxf(h->grid.inv_hx, fmaxf(h->grid.inv_hy, h->grid.inv_hz));
   const double k = cells_per_step > 0.0 ? 2097152.0 / cells_per_step : 1e18;
   h->range_check_interval = k >= 1e18 ? (1ull << 60) : (k < 1.0 ? 1ull : (uint64_t)k);
@@ -726,9 +660,9 @@ int finish_load(soma_handle* h, uint64_t step0) {
   if ((rc = launch_omega(h)) != SOMA_OK) return rc;     // also zeroes counts(1)
   if ((rc = verify_range(h)) != SOMA_OK) return rc;     // synchronises: the caller may reuse its buffers
   h->steps_since_sort = 0;
-  h->sorted_kind = 0;
-  if (use_win(h) || h->resort_interval > 0)
-    if ((rc = resort(h, use_win(h) ? 2 : 1)) != SOMA_OK) return rc;
+  h->sorted = false;
+  if (h->resort_interval > 0)
+    if ((rc = resort(h)) != SOMA_OK) return rc;
   h->loaded = true;
   return SOMA_OK;
 }
@@ -914,12 +848,7 @@ const char* soma_last_error(const soma_t* h) { return h ? h->err : g_last_error;
 int soma_set_option(soma_t* h, const char* name, int64_t value) {
   if (!h || !name) return fail(h, SOMA_EINVAL, "NULL argument");
   if (!std::strcmp(name, "path")) {
-    if (value < 0 || value > 3) return fail(h, SOMA_EINVAL, "path must be 0, 1, 2 or 3");
-    if (value == 3 && !h->win_ready) {
-      char buf[160];
-      snprintf(buf, sizeof buf, "windowed path unavailable: %s", h->win_why);
-      return fail(h, SOMA_EINVAL, buf);
-    }
+    if (value < 0 || value > 2) return fail(h, SOMA_EINVAL, "path must be 0, 1 or 2");
     if (value == 2 && !fused_lanes(h->N))
       return fail(h, SOMA_EINVAL, "fused path needs beads_per_chain = 2P, P a power of two <= 32");
     h->path = (int)value;
@@ -940,34 +869,16 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     int rc = check(h);
     if (rc != SOMA_OK) return rc;
     if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
-    return resort(h, use_win(h) ? 2 : 1);
-  }
-  {
-    static const char* const wn[6] = {"win_cx", "win_cy", "win_cz", "win_hx", "win_hy", "win_hz"};
-    for (int k = 0; k < 6; ++k)
-      if (!std::strcmp(name, wn[k])) {
-        if (value < 0 || value > 4096) return fail(h, SOMA_EINVAL, "window size out of range");
-        (k < 3 ? h->wc[k] : h->wh[k - 3]) = (uint32_t)value;
-        win_setup(h);
-        if (!h->win_ready && h->path == 3) h->path = 0;
-        return SOMA_OK;                      // soma_get_counters()[3] tells whether the windowed path is in use now
-      }
+    return resort(h);
   }
   if (!std::strcmp(name, "fused_lean")) {              // 0: the general fused kernel even where the lean one applies
     if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "fused_lean must be 0 or 1");
     h->fused_lean = (int)value;
-    win_setup(h);
-    if (!h->win_ready && h->path == 3) h->path = 0;
     return SOMA_OK;
   }
   if (!std::strcmp(name, "lean_threads")) {
     if (value != 256 && value != 512 && value != 1024) return fail(h, SOMA_EINVAL, "lean_threads must be 256, 512 or 1024");
     h->lean_threads = (int)value;
-    return SOMA_OK;
-  }
-  if (!std::strcmp(name, "win_auto")) {                // does path 0 pick the windowed-count kernel where it can run
-    if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "win_auto must be 0 or 1");
-    h->win_auto = value != 0;
     return SOMA_OK;
   }
   if (!std::strcmp(name, "fused_chunk")) {
@@ -986,7 +897,7 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
 int soma_get_counters(const soma_t* h, uint64_t* out) {
   if (!h || !out) return SOMA_EINVAL;
   out[0] = h->launches; out[1] = h->steps_done; out[2] = h->resorts;
-  out[3] = use_win(h) ? 3 : (use_fused(h) ? 2 : 1);
+  out[3] = use_fused(h) ? 2 : 1;
   return SOMA_OK;
 }
 

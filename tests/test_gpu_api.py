@@ -192,9 +192,6 @@ def test_error_codes_of_the_calls_beyond_the_six(soma, small):
         with pytest.raises(soma.SomaError) as e:
             soma.Soma.from_system(s, **bad)
         assert e.value.code == soma.SOMA_EINVAL
-    # the windowed-count kernel does not implement the bond-force-biased move: path 3 is refused
+    # bond-force-biased moves run on the general fused kernel (path 2) wherever N allows it
     with gpu_system(si.make_system(si.scaled(si.config(4), 8192, (32, 32, 32))), smc_mobility=0.05) as g:
-        with pytest.raises(soma.SomaError) as e:
-            g.set_option("path", 3)
-        assert e.value.code == soma.SOMA_EINVAL
         assert g.counters()["path"] == 2

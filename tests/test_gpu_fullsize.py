@@ -60,27 +60,6 @@ def test_cfg4_full_size_after_1_and_10_steps_bit_exact():
     assert float(np.abs(x - s.x).max()) < 10 * w.move_halfwidth
 
 
-@pytest.mark.parametrize("path", [2, 3])
-def test_cfg4_full_size_one_step_on_both_fused_variants(path):
-    """Whichever of the two variants of the lean kernel path 0 does not pick, at full size for one step."""
-    w = si.config(4)
-    s = si.make_system(w)
-    with gpu_system(s, path=path) as g:
-        if g.counters()["path"] == gpu_default_path(s):
-            pytest.skip("this is path 0's choice, covered by the 10-step test")
-        o = oracle.Oracle.from_system(s)
-        o.load_state(s.x, s.y, s.z)
-        g.load_state(s.x, s.y, s.z)
-        assert g.mc_steps(1, want_accepted=True) == o.mc_steps(1)
-        _compare_full_state(g, o, f"cfg4 path {path} after 1 step")
-        o.close()
-
-
-def gpu_default_path(s):
-    with gpu_system(s) as g:
-        return g.counters()["path"]
-
-
 @pytest.mark.parametrize("cfg,steps", [(1, 10), (2, 10), (3, 10)])
 def test_full_size_configs_bit_exact(cfg, steps):
     """configs[1..3] at BASELINE.json's full sizes on the default kernel path (cfg1, cfg3: N = 64, one

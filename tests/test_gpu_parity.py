@@ -16,7 +16,7 @@ from helpers import assert_same_state, gpu_system, lockstep
 
 pytestmark = pytest.mark.gpu
 
-FUSED, GENERIC, WINDOWED = 2, 1, 3      # 3: the lean kernel with bead counts in shared-memory windows (soma_lean.cuh)
+FUSED, GENERIC = 2, 1
 
 
 def _run_both(s, steps_list, path, **kw):
@@ -156,73 +156,59 @@ def test_large_seed_step_and_chain_ids_reach_the_counter():
         assert not np.array_equal(g2.positions()[0], o.positions()[0])
 
 
-# ---- the windowed-count variant of the lean kernel (path 3): one block per tile of the box, bead counts
-# in a shared-memory window (tile + halo) that is bulk-reduce-added into the global grid.  Small windows on
-# small grids so that the oracle stays fast while the run still covers many tiles, windows that wrap
-# around every periodic face, empty tiles, beads outside their window (global atomics) and drift
-# between re-sorts.  win_c* = tile core, win_h* = halo, in cells.
+# ---- further systems for the lean fused kernel (power-of-two grids, cell size 1/2): several warps per block
+# with ragged tails, non-cubic grids, one to eight types, N = 2 ... 64, a single chain.
 
-SMALL_WIN = dict(win_cx=4, win_cy=4, win_cz=4, win_hx=2, win_hy=2, win_hz=4)          # 8x8x12 windows, many beads stick out
-NO_HALO = dict(win_cx=4, win_cy=8, win_cz=4, win_hx=0, win_hy=0, win_hz=0)            # window = core: most beads outside
-WIDE_WIN = dict(win_cx=8, win_cy=4, win_cz=8, win_hx=4, win_hy=6, win_hz=4)           # 16x16x16 windows (the whole 16^3 grid: wraps everywhere)
-
-WIN_CASES = {
-    "cfg0_full_small_win": (lambda: si.make_system(si.config(0)), SMALL_WIN),
-    "cfg0_full_wide_win": (lambda: si.make_system(si.config(0)), WIDE_WIN),
-    "cfg0_full_no_halo": (lambda: si.make_system(si.config(0)), NO_HALO),
-    "cfg1_scaled_T1_N64": (lambda: _scaled(1, 4099, (16, 16, 16)), SMALL_WIN),
-    "cfg2_scaled": (lambda: _scaled(2, 8193, (32, 16, 32)), WIDE_WIN),
-    "cfg3_scaled_blend_N64": (lambda: _scaled(3, 4098, (32, 16, 16)), SMALL_WIN),
-    "cfg4_scaled_default_win": (lambda: _scaled(4, 16385, (32, 32, 32)), {}),           # 8^3 tiles + 4: the bench shape
-    "cfg4_scaled_noncubic": (lambda: _scaled(4, 16385, (32, 32, 16)), dict(win_cx=16, win_cy=8, win_cz=4, win_hx=2, win_hy=4, win_hz=4)),
-    "T3_three_patterns": (lambda: _custom(900, 32, 3, [[0] * 10 + [1] * 12 + [2] * 10, [2] * 32, [1] * 16 + [0] * 16],
-                                          np.arange(900) % 3, [[0, 12, 5], [12, 0, 21], [5, 21, 0]], 35.0, (16, 32, 16), (8.0, 16.0, 8.0), 41),
-                          SMALL_WIN),
-    "N2": (lambda: _custom(3001, 2, 2, [[0, 1]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 42), SMALL_WIN),
-    "N8": (lambda: _custom(1517, 8, 2, [[0, 0, 0, 1, 1, 1, 1, 0]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 43), SMALL_WIN),
-    "one_chain": (lambda: _custom(1, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (16, 16, 16), (8, 8, 8), 44), SMALL_WIN),   # all tiles but one empty
-    "T8_sparse": (lambda: _custom(300, 16, 8, [[0, 1, 2, 3, 4, 5, 6, 7] * 2], None,
-                                  (np.arange(64).reshape(8, 8) + np.arange(64).reshape(8, 8).T) * (1 - np.eye(8)) * 0.3, 25.0,
-                                  (8, 8, 8), (4, 4, 4), 46), dict(win_cx=4, win_cy=4, win_cz=4, win_hx=1, win_hy=1, win_hz=0)),
+LEAN_CASES = {
+    "cfg1_scaled_T1_N64": lambda: _scaled(1, 4099, (16, 16, 16)),
+    "cfg2_scaled": lambda: _scaled(2, 8193, (32, 16, 32)),
+    "cfg3_scaled_blend_N64": lambda: _scaled(3, 4098, (32, 16, 16)),
+    "cfg4_scaled_noncubic": lambda: _scaled(4, 16385, (32, 32, 16)),
+    "T3_three_patterns": lambda: _custom(900, 32, 3, [[0] * 10 + [1] * 12 + [2] * 10, [2] * 32, [1] * 16 + [0] * 16],
+                                         np.arange(900) % 3, [[0, 12, 5], [12, 0, 21], [5, 21, 0]], 35.0, (16, 32, 16), (8.0, 16.0, 8.0), 41),
+    "N2": lambda: _custom(3001, 2, 2, [[0, 1]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 42),
+    "N8": lambda: _custom(1517, 8, 2, [[0, 0, 0, 1, 1, 1, 1, 0]], None, [[0, 15], [15, 0]], 40.0, (16, 16, 16), (8, 8, 8), 43),
+    "one_chain": lambda: _custom(1, 32, 2, [[0] * 16 + [1] * 16], None, [[0, 20], [20, 0]], 50.0, (16, 16, 16), (8, 8, 8), 44),
+    "T8_sparse": lambda: _custom(300, 16, 8, [[0, 1, 2, 3, 4, 5, 6, 7] * 2], None,
+                                 (np.arange(64).reshape(8, 8) + np.arange(64).reshape(8, 8).T) * (1 - np.eye(8)) * 0.3, 25.0,
+                                 (8, 8, 8), (4, 4, 4), 46),
 }
 
 
-@pytest.mark.parametrize("case", sorted(WIN_CASES))
-def test_windowed_count_path_parity_after_1_and_10_steps(case):
-    make, opts = WIN_CASES[case]
-    s = make()
+@pytest.mark.parametrize("threads", [256, 1024])
+@pytest.mark.parametrize("case", sorted(LEAN_CASES))
+def test_lean_kernel_parity_after_1_and_10_steps(case, threads):
+    s = LEAN_CASES[case]()
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
-    with gpu_system(s, path=WINDOWED, options=opts) as g:
-        assert g.counters()["path"] == WINDOWED
+    with gpu_system(s, path=FUSED, options=dict(lean_threads=threads, fused_chunk=24)) as g:    # small chunks: many blocks, ragged last one
         g.load_state(s.x, s.y, s.z)
         done = 0
         for upto in (1, 10):
             assert g.mc_steps(upto - done, want_accepted=True) == o.mc_steps(upto - done)
             done = upto
-            assert_same_state(g, o, f"{case} windowed after {upto} steps")
-        assert g.counters()["path"] == WINDOWED
+            assert_same_state(g, o, f"{case} lean kernel, {threads} threads, after {upto} steps")
 
 
-@pytest.mark.parametrize("path", [FUSED, WINDOWED])
+@pytest.mark.parametrize("path", [FUSED, GENERIC])
 @pytest.mark.parametrize("interval", [0, 1, 3])
 def test_drift_and_resorts_do_not_change_the_trajectory(interval, path):
-    """40 steps: without re-sorting the chains drift out of their tiles (global atomics); with frequent
+    """40 steps: without re-sorting the chains drift away from their neighbours in memory; with frequent
     re-sorting the slot order keeps changing.  The trajectory may not depend on either.  (Path 2 is the
     kernel bench.py times: its periodic re-ordering is compared with the oracle here.)"""
     s = _scaled(4, 6000, (16, 16, 16))
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
     acc_o = o.mc_steps(40)
-    with gpu_system(s, path=path, options=dict(SMALL_WIN, resort_interval=interval)) as g:
+    with gpu_system(s, path=path, options=dict(resort_interval=interval)) as g:
         g.load_state(s.x, s.y, s.z)
         assert g.mc_steps(40, want_accepted=True) == acc_o
         assert_same_state(g, o, f"path {path}, resort_interval={interval}")
-        first = 1 if (interval or path == WINDOWED) else 0           # path 2 never sorts when the interval is 0
+        first = 1 if interval else 0                                 # never sorted when the interval is 0
         assert g.counters()["resorts"] == first + ((40 - 1) // interval if interval else 0)
 
 
-@pytest.mark.parametrize("path", [FUSED, WINDOWED])
+@pytest.mark.parametrize("path", [FUSED, GENERIC])
 @pytest.mark.parametrize("interval", [1, 3])
 def test_parity_after_1_and_10_steps_with_resorts(interval, path):
     """The full-state comparison after 1 and 10 steps with the chain re-ordering inside the run."""
@@ -257,40 +243,39 @@ def test_switching_paths_mid_run_keeps_the_trajectory():
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
     o.mc_steps(8)
-    with gpu_system(s, path=FUSED, options=SMALL_WIN) as g:
+    with gpu_system(s, path=FUSED) as g:
         g.load_state(s.x, s.y, s.z)
-        for path in (FUSED, WINDOWED, GENERIC, WINDOWED, FUSED, GENERIC, WINDOWED, FUSED):
+        for k, path in enumerate((FUSED, GENERIC, GENERIC, FUSED, FUSED, GENERIC, FUSED, FUSED)):
             g.set_option("path", path)
+            g.set_option("fused_lean", k % 3 != 0)                   # the general fused kernel every third step
             g.mc_steps(1)
         assert_same_state(g, o, "path switched every step")
 
 
-def test_windowed_path_is_refused_where_it_cannot_run():
+def test_path_option_is_validated():
     import paper_2606_09356_b200 as soma
-    for make in (EDGE["T3_npot"], EDGE["N33"], EDGE["one_chain"], EDGE["b_and_a"]):   # non-power-of-two grid, odd N, 1-cell grid, cell size not 2^k
-        with gpu_system(make()) as g:
+    with gpu_system(EDGE["N33"]()) as g:                                     # odd N: no fused kernel
+        with pytest.raises(soma.SomaError) as e:
+            g.set_option("path", FUSED)
+        assert e.value.code == soma.SOMA_EINVAL
+        assert g.counters()["path"] == GENERIC
+    with gpu_system(si.make_system(si.config(0))) as g:
+        for bad in (3, -1):
             with pytest.raises(soma.SomaError) as e:
-                g.set_option("path", WINDOWED)
-            assert e.value.code == soma.SOMA_EINVAL and "windowed path unavailable" in str(e.value)
-    with gpu_system(si.make_system(si.config(0))) as g:                      # default 16^3 window = the 16^3 grid: allowed
-        g.set_option("path", WINDOWED)
-        g.set_option("win_hz", 3)                                            # halo along z not a multiple of 4 -> windows off
-        assert g.counters()["path"] != WINDOWED
-        g.set_option("win_hz", 8)                                            # window larger than the grid
-        with pytest.raises(soma.SomaError):
-            g.set_option("path", WINDOWED)
+                g.set_option("path", bad)
+            assert e.value.code == soma.SOMA_EINVAL
 
 
 # ---- external field: omega = interaction part + ext, every kernel path -----
 
-@pytest.mark.parametrize("path", [FUSED, GENERIC, WINDOWED])
+@pytest.mark.parametrize("path", [FUSED, GENERIC])
 def test_external_field_parity(path):
     s = _scaled(4, 6000, (16, 16, 16))
     ext = np.random.default_rng(31).normal(0.0, 0.8, size=(2, 16 ** 3)).astype(np.float32)
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
     o.set_external_field(ext)
-    with gpu_system(s, path=path, options=SMALL_WIN if path == WINDOWED else None) as g:
+    with gpu_system(s, path=path) as g:
         g.load_state(s.x, s.y, s.z)
         g.set_external_field(ext)
         assert np.array_equal(g.omega().view(np.uint32), o.omega().view(np.uint32))
@@ -327,12 +312,12 @@ def _mixture(n_chains=3000, N=32, n_single=(7000, 0, 11000), grid=(16, 16, 16), 
     return si.custom_system(n_chains, N, 3, pat, None, chi, 40.0, grid, tuple(g / 2 for g in grid), seed=seed, n_single=n_single)
 
 
-@pytest.mark.parametrize("path", [FUSED, GENERIC, WINDOWED])
+@pytest.mark.parametrize("path", [FUSED, GENERIC])
 def test_mixture_of_chains_and_single_bead_molecules(path):
     s = _mixture()
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
-    with gpu_system(s, path=path, options=SMALL_WIN if path == WINDOWED else None) as g:
+    with gpu_system(s, path=path) as g:
         g.load_state(s.x, s.y, s.z)
         assert_same_state(g, o, f"mixture loaded, path {path}")
         done = 0
