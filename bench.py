@@ -30,9 +30,11 @@ if ROOT not in sys.path:
 
 import numpy as np
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one fused_step_kernel launch on cfg4, from the committed
-# ncu --set full capture profiles/r1_ncu_cfg4_fused_final.txt (1.773020 + 1.625843 GB)
-NCU_TRAFFIC_CFG4_FUSED = 3.398863e9
+# ncu counters of the dominant kernel (dram bytes, L2 sectors, ...) are NOT measured by bench.py: they come
+# from the committed table profiles/ncu_counters.csv, one row per (kernel path, config, source hash of the
+# kernels).  A row whose hash is not the hash of the sources this run was built from is stale and ignored.
+NCU_TABLE = os.path.join(ROOT, "profiles", "ncu_counters.csv")
+KERNEL_SOURCES = ("soma_device.cuh", "soma_kernels.cuh", "soma_lean.cuh")
 
 METRIC = "attempted bead moves/s"
 UNIT = "moves/s"
@@ -52,6 +54,64 @@ def algorithmic_bytes(w) -> dict:
         "omega_kernel": 12 * TC,                   # counts read, omega written, other count buffer zeroed
         "step": 24 * B + 20 * TC,
     }
+
+
+def kernel_source_hash() -> str:
+    """First 12 hex digits of the sha256 over the kernel sources: the key that ties an ncu capture to a build."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2606_09356_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:12]
+
+
+def ncu_counters(path: int, config: int, table: str = NCU_TABLE):
+    """Row of profiles/ncu_counters.csv for this (path, config) captured on the current kernel sources, or None."""
+    import csv
+    try:
+        with open(table, newline="") as f:
+            rows = [r for r in csv.DictReader(f)]
+    except OSError:
+        return None
+    key = kernel_source_hash()
+    for r in rows:
+        if int(r["path"]) == path and int(r["config"]) == config and r["source_hash"] == key:
+            return r
+    return None
+
+
+def cpu_info() -> dict:
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.startswith("model name"):
+                    model = ln.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return {"cpu_model": model, "logical_cores": os.cpu_count()}
+
+
+def pin_to_one_core():
+    """Pin this process to the core it runs on (the oracle leg is single-threaded
+    and pinned).  Returns the core, or None where the platform has no affinity call."""
+    try:
+        allowed = sorted(os.sched_getaffinity(0))
+        core = allowed[len(allowed) // 2]
+        os.sched_setaffinity(0, {core})
+        return core, allowed
+    except (AttributeError, OSError):
+        return None, None
+
+
+def unpin(allowed):
+    if allowed:
+        try:
+            os.sched_setaffinity(0, set(allowed))
+        except OSError:
+            pass
 
 
 def measured_peaks() -> tuple[float, str]:
@@ -167,22 +227,49 @@ def sample_workload(w, factor: int):
     return si.scaled(w, w.n_chains // factor, tuple(grid))
 
 
+ORACLE_SAMPLE_FACTOR = 8      # both arms time the oracle on 1/8 of the config (same beads per cell) unless a step count forces less
+
+
+def oracle_sample(w, n_steps: int):
+    """The bounded sample both arms time the oracle on: 1/ORACLE_SAMPLE_FACTOR of the workload at the same
+    beads per cell (a power of two more if n_steps oracle steps of that would take longer than ~100 s at
+    ~120 ns per attempted move).  Returns (sample workload, factor)."""
+    factor = 1
+    while factor < ORACLE_SAMPLE_FACTOR and w.n_chains // (factor * 2) >= 1024:
+        factor *= 2
+    while w.n_beads // factor * 120e-9 * max(1, n_steps) > 100.0 and w.n_chains // (factor * 2) >= 1024:
+        factor *= 2
+    return (sample_workload(w, factor) if factor > 1 else w), factor
+
+
 def time_oracle(system, steps: int, warmup: int = 0, budget_s: float | None = None):
-    """Oracle MC steps on `system`, single-threaded, as it stands.  Returns (seconds, steps timed)."""
+    """Oracle MC steps on `system`, single-threaded and pinned to one core, as it stands.
+    Returns (seconds, steps timed, core)."""
     import oracle
-    o = oracle.Oracle.from_system(system)
-    o.load_state(system.x, system.y, system.z)
-    if warmup:
-        o.mc_steps(warmup)
-    done, t0 = 0, time.perf_counter()
-    while done < steps:
-        o.mc_steps(1)
-        done += 1
-        if budget_s is not None and time.perf_counter() - t0 >= budget_s:
-            break
-    dt = time.perf_counter() - t0
-    o.close()
-    return dt, done
+    core, allowed = pin_to_one_core()
+    try:
+        o = oracle.Oracle.from_system(system)
+        o.load_state(system.x, system.y, system.z)
+        if warmup:
+            o.mc_steps(warmup)
+        done, t0 = 0, time.perf_counter()
+        while done < steps:
+            o.mc_steps(1)
+            done += 1
+            if budget_s is not None and time.perf_counter() - t0 >= budget_s:
+                break
+        dt = time.perf_counter() - t0
+        o.close()
+    finally:
+        unpin(allowed)
+    return dt, done, core
+
+
+def sample_text(w, ws, factor: int) -> str:
+    if factor == 1:
+        return f"the whole of {w.name} ({w.n_beads} beads); every step is one oracle MC step"
+    return (f"{ws.n_chains} chains x {ws.N} beads on a {ws.grid[0]}x{ws.grid[1]}x{ws.grid[2]} grid = 1/{factor} of "
+            f"{w.name} at the same beads per cell; every step is one oracle MC step over that sample")
 
 
 def run_reference(args):
@@ -192,24 +279,18 @@ def run_reference(args):
     if rank != 0:
         return
     w = si.config(args.config)
-    # size the sample so that (K + W) oracle steps take about 90 s at ~120 ns per attempted move
-    target_beads = 90.0 / (120e-9 * max(1, args.steps + args.warmup))
-    factor = 1
-    while w.n_beads // factor > target_beads and w.n_chains // (factor * 2) >= 1024:
-        factor *= 2
-    ws = sample_workload(w, factor) if factor > 1 else w
+    ws, factor = oracle_sample(w, args.steps + args.warmup)
     s = si.make_system(ws)
-    dt, done = time_oracle(s, args.steps, warmup=args.warmup)
+    dt, done, core = time_oracle(s, args.steps, warmup=args.warmup)
     value = ws.n_beads * done / dt
-    sample = (f"{ws.n_chains} chains x {ws.N} beads on a {ws.grid[0]}x{ws.grid[1]}x{ws.grid[2]} grid = 1/{factor} of "
-              f"{w.name} at the same beads per cell; every step is one oracle MC step over that sample")
-    cores = 1
+    sample = sample_text(w, ws, factor)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": done,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / done, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "sample": sample, "mc_steps_per_s": done / dt},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "pinned_core": core, **cpu_info()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -218,6 +299,27 @@ def run_reference(args):
 # --------------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------------
+
+def run_dry(args):
+    """`--dry`: the multi-rank plumbing of run_ours without a GPU (process group on `--backend`, barrier,
+    max-over-ranks time, sum-over-ranks work, rank 0 prints the line) on made-up per-rank timings.  For the
+    CPU tests of the launch path; the line says "dry": true and carries no measurement."""
+    import torch.distributed as dist
+    import scmf_inputs as si
+    rank, _, world = dist_env()
+    if world > 1:
+        dist.init_process_group(args.backend)
+    w = si.config(args.config)
+    barrier()
+    ms, moves = aggregate_over_ranks(10.0 + 5.0 * rank, float(w.n_beads) * args.steps)
+    barrier()
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": moves / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": ms / args.steps, "dry": True, "scaling": "weak",
+                          "config": {"workload": w.name, "parallelism": "replicas only" if world > 1 else "1 gpu"}}))
+    if world > 1:
+        dist.destroy_process_group()
+
 
 def run_ours(args):
     import torch
@@ -231,7 +333,7 @@ def run_ours(args):
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        dist.init_process_group(args.backend, device_id=dev if args.backend == "nccl" else None)
     soma.load_library()                                 # raises if the CUDA library is missing
 
     w = si.config(args.config)
@@ -267,10 +369,32 @@ def run_ours(args):
     local_ms = ev0.elapsed_time(ev1)
     kt = g.kernel_times()
     g.set_option("kernel_timing", 0)
-    launches = g.counters()["launches"] - c0["launches"]
-    g_path = g.counters()["path"]
+    c1 = g.counters()
+    launches = c1["launches"] - c0["launches"]
+    resorts_in_window = c1["resorts"] - c0["resorts"]
+    g_path = c1["path"]
     ms, moves = aggregate_over_ranks(local_ms, float(B) * args.steps, dev)
     value = moves / (ms * 1e-3)
+
+    # ---- the chain re-ordering on its own (it runs every `interval` steps: K decides how many fall into the
+    # window above, so the line also carries a per-step figure that does not depend on K) ---------------
+    interval = 64 if w.n_chains >= 4096 else 0
+    for kv in args.opt:
+        if kv.startswith("resort_interval="):
+            interval = int(kv.split("=")[1])
+    resort_ms = 0.0
+    if interval:
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g.set_option("resort_now", 0)
+        torch.cuda.synchronize()
+        r0.record(stream)
+        for _ in range(3):
+            g.set_option("resort_now", 0)
+        r1.record(stream)
+        torch.cuda.synchronize()
+        resort_ms = r0.elapsed_time(r1) / 3
+    steady_local = (local_ms - resorts_in_window * resort_ms) / args.steps + (resort_ms / interval if interval else 0.0)
+    steady_ms, _ = aggregate_over_ranks(steady_local, 0.0, dev)
 
     # ---- end to end: the config's own run through the C ABI, host buffers in and out -----------
     S = w.steps
@@ -294,26 +418,30 @@ def run_ours(args):
     n_t = max(1, kt["steps"])
     move_ms, omega_ms = kt["move_bin_ms"] / n_t, kt["omega_ms"] / n_t
     achieved = ab["move_bin_kernel"] / (move_ms * 1e-3) / 1e9
-    path_now = g_path
-    kname = {1: "half_sweep_kernel x2 + bin_kernel (rows a1+a2+a3+a5)", 2: "lean_step_kernel (rows a1+a2+a3+a5)"}[path_now]
-    traffic = args.traffic
-    if traffic is None and path_now == 2 and args.config == 4:
-        traffic = NCU_TRAFFIC_CFG4_FUSED
+    kname = {1: "half_sweep_kernel x2 + bin_kernel (rows a1+a2+a3+a5)", 2: "lean_step_kernel (rows a1+a2+a3+a5)"}[g_path]
+    if args.smc_mobility > 0 or (g_path == 2 and any(kv == "fused_lean=0" for kv in args.opt)):
+        kname = kname.replace("lean_step_kernel", "fused_step_kernel")
+    ncu = ncu_counters(g_path, args.config) if args.smc_mobility == 0 and not args.opt else None
     roofline = {"bound": "hbm", "kernel": kname,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": ab["move_bin_kernel"],
+                "traffic": (float(ncu["dram_bytes_read"]) + float(ncu["dram_bytes_write"])) if ncu else None,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": ab["move_bin_kernel"],
                 "kernel_ms": move_ms, "omega_kernel_ms": omega_ms,
                 "omega_kernel_frac": ab["omega_kernel"] / (omega_ms * 1e-3) / 1e9 / peak if omega_ms > 0 else None,
-                "step_frac": ab["step"] / (local_ms / args.steps * 1e-3) / 1e9 / peak,
-                "step_frac_of_8TBps": ab["step"] / (local_ms / args.steps * 1e-3) / 8e12,
+                "step_frac": ab["step"] / (steady_ms * 1e-3) / 1e9 / peak,
+                "step_frac_of_8TBps": ab["step"] / (steady_ms * 1e-3) / 8e12,
+                "target_step_frac_of_8TBps": 0.60, "target_met": ab["step"] / (steady_ms * 1e-3) / 8e12 >= 0.60,
                 "bytes_per_move": ab["step"] / B}
-    if path_now == 2 and args.config == 4:
-        # not measured live: from the committed ncu capture of this kernel (profiles/r1_ncu_cfg4_fused_final.txt)
-        roofline["limiter"] = {"unit": "L2 (LTS) sector throughput", "l2_sectors_per_launch": 397.29e6,
-                               "achieved_bytes_per_cycle": 5980, "cap_bytes_per_cycle": 6300,
-                               "cap_source": "B300_MICROARCH.md 'LTS throughput cap ~6300 B/cyc full-chip'",
-                               "note": "DRAM traffic equals the algorithmic bytes (x1.013); L2 sectors at 95 % of the guide's read cap, LSU wavefronts 72 %, "
-                                       "issue slots 65 %: balanced, see DESIGN.md section 7 for the ablations"}
+    if ncu:
+        roofline["ncu"] = {"source": f"profiles/ncu_counters.csv ({ncu['capture']})", "source_hash": ncu["source_hash"],
+                           "l2_sectors_per_launch": float(ncu["lts_sectors"]),
+                           "warp_instructions_per_launch": float(ncu["inst_executed"]),
+                           "l1tex_to_xbar_request_cycles_pct": float(ncu["l1tex2xbar_req_pct"]),
+                           "lsu_wavefronts_pct": float(ncu["lsu_wavefronts_pct"]),
+                           "issue_active_pct": float(ncu["issue_active_pct"]),
+                           "limiter": ncu["limiter"]}
+    else:
+        roofline["ncu"] = None     # no capture of these kernel sources / this path and config: nothing is quoted
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -324,6 +452,11 @@ def run_ours(args):
                    "l2": f"inputs larger than L2: positions {12 * B / 1e6:.0f} MB + grids {12 * w.n_types * w.n_cells / 1e6:.0f} MB per step",
                    "mc_steps_per_s": world * args.steps / (ms * 1e-3),
                    **({"moves": f"bond-force-biased, A = {args.smc_mobility}"} if args.smc_mobility > 0 else {})},
+        "resort": {"interval_steps": interval, "ms": resort_ms, "in_timed_window": int(resorts_in_window),
+                   "ms_per_step_amortised": resort_ms / interval if interval else 0.0,
+                   "ms_per_step_steady": steady_ms, "moves_per_s_steady": world * B / (steady_ms * 1e-3),
+                   "what": "the chains are re-ordered in memory every interval_steps MC steps; ms_per_step_steady = the timed steps "
+                           "without the re-orderings that fell into the window + one re-ordering per interval_steps, so it does not depend on K"},
         "clocks": clk, "gpu_launches": int(launches),
         "e2e": {"value": e2e_moves / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 12 * B / S,
                 "d2h_bytes_per_step": (12 * B + 4 * w.n_types * w.n_cells) / S, "mc_steps": S, "ms": e2e_ms,
@@ -334,13 +467,29 @@ def run_ours(args):
 
     # ---- the oracle on the host cores, rank 0 at N = 1 only ------------------------------------
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        dt, done = time_oracle(s, steps=4, budget_s=12.0)
-        line["cpu_baseline"] = {"value": B * done / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                "sample": f"{done} full MC step(s) of {w.name} ({B} beads) from the same initial state, {dt:.1f} s"}
+        ws, factor = oracle_sample(w, 4)
+        ss = si.make_system(ws) if factor > 1 else s
+        dt, done, core = time_oracle(ss, steps=4, budget_s=20.0)
+        line["cpu_baseline"] = {"value": ws.n_beads * done / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": sample_text(w, ws, factor) + f"; {done} step(s), {dt:.1f} s",
+                                "pinned_core": core, **cpu_info()}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def relaunch_under_torchrun(n: int) -> int:
+    """`python bench.py --gpus N` without a launcher: start N ranks of this script with torch.distributed.run
+    (one process per GPU, rendezvous on 127.0.0.1) and return its exit code."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -355,13 +504,20 @@ def main():
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=INT", help="soma_set_option(NAME, INT) before the run (tuning)")
     ap.add_argument("--smc-mobility", type=float, default=0.0,
                     help="A > 0: bond-force-biased moves (DESIGN.md R24) instead of the configs' uniform moves; not the headline metric")
-    ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
+    ap.add_argument("--backend", choices=["nccl", "gloo"], default="nccl", help="torch.distributed backend of the barrier / aggregation")
+    ap.add_argument("--dry", action="store_true", help="multi-rank plumbing only, no GPU work (CPU tests)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                   # timing rule: at least 3 warm-up steps
+    world_env = os.environ.get("WORLD_SIZE")
+    if world_env is None and args.gpus > 1 and args.impl == "ours":
+        raise SystemExit(relaunch_under_torchrun(args.gpus))       # one replica per GPU
+    if world_env is not None and int(world_env) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world_env}")
     if args.impl == "reference":
         run_reference(args)
+    elif args.dry:
+        run_dry(args)
     else:
         run_ours(args)
 
