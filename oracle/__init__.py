@@ -77,6 +77,8 @@ def lib() -> C.CDLL:
             "oracle_set_omega": (None, [vp, f32p]),
             "oracle_set_external_field": (None, [vp, f32p]),
             "oracle_generate_state": (C.c_int, [vp, C.c_uint64, C.c_uint64]),
+            "oracle_init_from_density": (C.c_int, [vp, f32p, C.c_uint64, C.c_uint64]),
+            "oracle_set_umbrella": (None, [vp, f32p, C.c_float]),
             "oracle_set_singles": (C.c_int, [vp, C.POINTER(C.c_uint64)]),
             "oracle_set_smc": (None, [vp, C.c_float]),
             "oracle_smc_margin": (C.c_float, [vp, C.c_uint64, C.c_float, C.c_float, C.c_float]),
@@ -188,6 +190,29 @@ class Oracle:
     def generate_state(self, gen_seed: int, step0: int = 0):
         """Gaussian random-walk initial state by the recipe of DESIGN.md R22, then bin + omega."""
         lib().oracle_generate_state(self._h, int(gen_seed), int(step0))
+
+    def init_from_density(self, phi_target, gen_seed: int, step0: int = 0, n_equil_steps: int = 0, umbrella_k: float = 0.0) -> int:
+        """Initial state reproducing the target concentrations phi_target [T][C] (R25), then
+        n_equil_steps MC steps under the umbrella potential of strength umbrella_k, which is removed again.
+        Returns the number of moves accepted during the equilibration."""
+        phi = np.ascontiguousarray(phi_target, dtype=np.float32).reshape(self.T, self.Cells)
+        rc = lib().oracle_init_from_density(self._h, _p(phi, C.c_float), int(gen_seed), int(step0))
+        if rc != 0:
+            raise ValueError({-1: "phi_target holds a negative, NaN or too large value", -2: "a species has zero total target weight"}[rc])
+        acc = 0
+        if n_equil_steps:
+            self.set_umbrella(phi, umbrella_k)
+            acc = self.mc_steps(n_equil_steps)
+            self.set_umbrella(None, 0.0)
+        return acc
+
+    def set_umbrella(self, phi_target, k: float):
+        """Umbrella potential toward phi_target [T][C] with strength k (R25); None switches it off."""
+        if phi_target is None:
+            lib().oracle_set_umbrella(self._h, None, 0.0)
+        else:
+            phi = np.ascontiguousarray(phi_target, dtype=np.float32).reshape(self.T, self.Cells)
+            lib().oracle_set_umbrella(self._h, _p(phi, C.c_float), float(k))
 
     def set_smc(self, A: float):
         """A > 0: bond-force-biased moves with mobility A (R24); 0: uniform moves."""

@@ -103,6 +103,8 @@ struct Oracle {
   std::vector<uint32_t> counts;         // [T][C], cell = (ix*ny+iy)*nz+iz (R12)
   std::vector<float> omega;             // [T][C]
   std::vector<float> ext;               // [T][C] external field (empty = none), R21
+  std::vector<float> phi_target;        // [T][C] target concentrations of the umbrella potential (empty = none), R25
+  float umbrella_k = 0.0f;              // its strength in kT per bead and unit concentration
   // single-bead molecules (R23): n_single[t] of type t, stored after the chains in x, y, z,
   // type 0 first; molecule m has the logical chain id n_chains + m and bead index 0
   float smcA = 0.0f;                    // > 0: bond-force-biased moves with mobility A (R24), 0: uniform moves
@@ -157,6 +159,10 @@ void bin(Oracle& o) {
 //   phi_s(c) = n_s(c) * C/B;  omega_t(c) = (1/N) * ( kappaN*(sum_s phi_s - 1) + sum_{s != t} chiN_ts * phi_s ).
 // With an external field ("umbrella potential"; R21):
 //   omega_t(c) = fl32( fl32(invN * acc) + ext_t(c) ),  ext in kT per bead.
+// With the umbrella potential toward target concentrations phi*_t(c) ("equilibrated using an
+// umbrella potential"; R25: H_umb/kT = (k/2)(B/C) sum_{t,c} (phi_t(c) - phi*_t(c))^2, whose
+// derivative with respect to n_t(c) is k (phi_t(c) - phi*_t(c))), added last:
+//   omega_t(c) = fl32( omega_t(c) + fl32( k * fl32(phi_t(c) - phi*_t(c)) ) ).
 void compute_omega(Oracle& o) {
   std::vector<float> phi(o.T);
   for (uint64_t c = 0; c < o.C; ++c) {
@@ -170,8 +176,10 @@ void compute_omega(Oracle& o) {
       float acc = p;
       for (uint32_t s = 0; s < o.T; ++s)
         if (s != t) acc = fmaf(o.chiN[(size_t)t * o.T + s], phi[s], acc);
-      const float w = o.invN * acc;
-      o.omega[(size_t)t * o.C + c] = o.ext.empty() ? w : w + o.ext[(size_t)t * o.C + c];
+      float w = o.invN * acc;
+      if (!o.ext.empty()) w = w + o.ext[(size_t)t * o.C + c];
+      if (!o.phi_target.empty()) w = w + o.umbrella_k * (phi[t] - o.phi_target[(size_t)t * o.C + c]);
+      o.omega[(size_t)t * o.C + c] = w;
     }
   }
 }
@@ -654,6 +662,117 @@ int oracle_generate_state(void* h, uint64_t gen_seed, uint64_t step0) {
     o.x[j] = (float)((double)o.box[0] * U(w[0]));
     o.y[j] = (float)((double)o.box[1] * U(w[1]));
     o.z[j] = (float)((double)o.box[2] * U(w[2]));
+  }
+  o.t = step0;
+  bin(o);
+  compute_omega(o);
+  o.loaded = true;
+  return 0;
+}
+
+// Umbrella potential toward target concentrations (R25): phi_target [T][C] (nullptr = off).
+// omega of the current densities is recomputed at once.
+void oracle_set_umbrella(void* h, const float* phi_target, float k) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (phi_target) o.phi_target.assign(phi_target, phi_target + (size_t)o.T * o.C); else o.phi_target.clear();
+  o.umbrella_k = phi_target ? k : 0.0f;
+  if (o.loaded) compute_omega(o);
+}
+
+// Initial state that reproduces supplied concentration fields (PAPER.md:119:
+// "Each SOMA simulation begins by generating particle positions that reproduce the supplied concentration
+// fields.  Molecules are placed within half a mean end-to-end distance of their target positions").  The
+// paper gives no rule; R25 is the reading:
+//   Q_t(c) = (uint32) rintf(phi*_t(c) * 65536)                       target concentration on a 2^-16 lattice
+//   W_p(c) = sum_i Q_{type_p(i)}(c)                                  weight of cell c for a chain of pattern p (uint64)
+//   chain c (pattern p): (w0..w3) = Philox(counter (0, c, 0, 3<<8), key = gen_seed),  (v0..) = Philox((1, c, 0, 3<<8));
+//     k = floor( (w0 2^32 + w1) S_p / 2^64 ), S_p = sum_c W_p(c);  target cell = the first cell whose inclusive
+//     prefix sum of W_p exceeds k, i.e. cell c with probability W_p(c)/S_p;  target point r* = (cell
+//     coordinate + (U(w2), U(w3), U(v0))) * (box/grid) in double, U(w) = (w + 0.5) 2^-32;
+//     shape = the Gaussian random walk of DESIGN.md R22 (same domain-1 draws: s_0 = 0, s_i = s_{i-1} + (b/sqrt 3) g(i));
+//     m = (s_0 + s_1 + ... in bead order)/N;  bead i = (float)((r* - m) + s_i): the chain's centre of mass sits at
+//     its target point, so every bead is within about R_e/2 of it.
+//   single-bead molecule m of type t: the same with W = Q_t, chain id n_chains + m, placed at r*.
+// Then DESIGN.md section 2 step 4 with these positions (t = step0).  Returns -1 if a target value is negative,
+// NaN or >= 65536, -2 if a pattern (or single species) that has molecules has zero total weight.
+int oracle_init_from_density(void* h, const float* phi_target, uint64_t gen_seed, uint64_t step0) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const uint32_t key[2] = {(uint32_t)gen_seed, (uint32_t)(gen_seed >> 32)};
+  const double sigma = (double)o.b / std::sqrt(3.0), two_pi = 6.283185307179586;
+  auto U = [](uint32_t w) { return ((double)w + 0.5) * 0x1p-32; };
+  std::vector<uint32_t> Q((size_t)o.T * o.C);
+  for (size_t k = 0; k < Q.size(); ++k) {
+    const float v = phi_target[k];
+    if (!(v >= 0.0f) || !(v < 65536.0f)) return -1;
+    Q[k] = (uint32_t)rintf(v * 65536.0f);
+  }
+  const double hcell[3] = {(double)o.box[0] / (double)o.grid[0], (double)o.box[1] / (double)o.grid[1], (double)o.box[2] / (double)o.grid[2]};
+  std::vector<uint64_t> prefix(o.C);
+  // target point of molecule `id` drawn from the cell weights whose inclusive prefix sums are in `prefix`
+  auto target_point = [&](uint64_t id, double* rstar) {
+    const uint32_t ca[4] = {0u, (uint32_t)id, 0u, 3u << 8}, cb[4] = {1u, (uint32_t)id, 0u, 3u << 8};
+    uint32_t w[4], v[4];
+    philox4x32_10(ca, key, w); philox4x32_10(cb, key, v);
+    const uint64_t u64 = ((uint64_t)w[0] << 32) | w[1];
+    const uint64_t k = (uint64_t)(((unsigned __int128)u64 * prefix[o.C - 1]) >> 64);
+    uint64_t lo = 0, hi = o.C - 1;                        // first cell with prefix > k
+    while (lo < hi) { const uint64_t mid = (lo + hi) / 2; if (prefix[mid] > k) hi = mid; else lo = mid + 1; }
+    const uint64_t iz = lo % o.grid[2], iy = (lo / o.grid[2]) % o.grid[1], ix = lo / ((uint64_t)o.grid[2] * o.grid[1]);
+    rstar[0] = ((double)ix + U(w[2])) * hcell[0];
+    rstar[1] = ((double)iy + U(w[3])) * hcell[1];
+    rstar[2] = ((double)iz + U(v[0])) * hcell[2];
+  };
+  std::vector<double> sx(o.N), sy(o.N), sz(o.N);
+  for (uint32_t p = 0; p < o.n_patterns; ++p) {
+    bool used = false;
+    for (uint64_t c = 0; c < o.n_chains && !used; ++c) used = o.chain_pattern[c] == p;
+    if (!used) continue;
+    uint64_t run = 0;
+    for (uint64_t c = 0; c < o.C; ++c) {
+      uint64_t wgt = 0;
+      for (uint32_t i = 0; i < o.N; ++i) wgt += Q[(size_t)o.type_patterns[(size_t)p * o.N + i] * o.C + c];
+      run += wgt;
+      prefix[c] = run;
+    }
+    if (run == 0) return -2;
+    for (uint64_t c = 0; c < o.n_chains; ++c) {
+      if (o.chain_pattern[c] != p) continue;
+      double rstar[3];
+      target_point(c, rstar);
+      double r[3] = {0.0, 0.0, 0.0}, sum[3] = {0.0, 0.0, 0.0};
+      for (uint32_t i = 0; i < o.N; ++i) {
+        if (i > 0) {
+          const uint32_t ctr[4] = {i, (uint32_t)c, 0u, 1u << 8};
+          uint32_t w[4];
+          philox4x32_10(ctr, key, w);
+          const double ra = std::sqrt(-2.0 * std::log(U(w[0]))), rb = std::sqrt(-2.0 * std::log(U(w[2])));
+          r[0] += sigma * (ra * std::cos(two_pi * U(w[1])));
+          r[1] += sigma * (ra * std::sin(two_pi * U(w[1])));
+          r[2] += sigma * (rb * std::cos(two_pi * U(w[3])));
+        }
+        sx[i] = r[0]; sy[i] = r[1]; sz[i] = r[2];
+        sum[0] += r[0]; sum[1] += r[1]; sum[2] += r[2];
+      }
+      const double base[3] = {rstar[0] - sum[0] / (double)o.N, rstar[1] - sum[1] / (double)o.N, rstar[2] - sum[2] / (double)o.N};
+      for (uint32_t i = 0; i < o.N; ++i) {
+        const uint64_t j = c * o.N + i;
+        o.x[j] = (float)(base[0] + sx[i]); o.y[j] = (float)(base[1] + sy[i]); o.z[j] = (float)(base[2] + sz[i]);
+      }
+    }
+  }
+  uint64_t m0 = 0;
+  for (uint32_t t = 0; t < o.T && o.S; ++t) {
+    if (o.n_single[t] == 0) continue;
+    uint64_t run = 0;
+    for (uint64_t c = 0; c < o.C; ++c) { run += Q[(size_t)t * o.C + c]; prefix[c] = run; }
+    if (run == 0) return -2;
+    for (uint64_t m = m0; m < m0 + o.n_single[t]; ++m) {
+      double rstar[3];
+      target_point(o.n_chains + m, rstar);
+      const uint64_t j = o.n_chains * o.N + m;
+      o.x[j] = (float)rstar[0]; o.y[j] = (float)rstar[1]; o.z[j] = (float)rstar[2];
+    }
+    m0 += o.n_single[t];
   }
   o.t = step0;
   bin(o);
