@@ -116,6 +116,31 @@ int soma_load_state(soma_t *h, const float *x, const float *y, const float *z, u
  * coordinates and bit for bit on the rest.  Errors: SOMA_EINVAL (step0 >= 2^48), SOMA_ECUDA. */
 int soma_generate_state(soma_t *h, uint64_t gen_seed, uint64_t step0);
 
+/* Initial state that reproduces supplied concentration fields, then equilibration under an umbrella
+ * potential (section 3.2: "Each SOMA simulation begins by
+ * generating particle positions that reproduce the supplied concentration fields.  Molecules are placed
+ * within half a mean end-to-end distance of their target positions and equilibrated using an umbrella
+ * potential").  The paper gives no rule; reading R25:
+ *   phi_target [T][cells] fp32 (host or device by `ptr_is_device`), layout of omega, 0 <= value < 65536.
+ *   Q_t(c) = (uint32) rint(phi_target_t(c) 2^16); a chain of pattern p draws its target cell with
+ *   probability W_p(c) / sum W_p, W_p(c) = sum over its beads i of Q_type(i)(c), by inverse CDF on the
+ *   integer prefix sums: k = floor((w0 2^32 + w1) sum W_p / 2^64) for (w0..w3) = Philox4x32-10(counter
+ *   (0, chain, 0, 3 << 8), key = gen_seed); the target point is uniform in that cell (offsets U(w2), U(w3),
+ *   U(v0), (v0..) = Philox((1, chain, 0, 3 << 8)), U(w) = (w + 0.5) 2^-32, in double); the chain is the
+ *   Gaussian random walk of soma_generate_state (same domain-1 draws) translated so that its centre of
+ *   mass sits at the target point, every coordinate rounded once to fp32.  Single-bead molecules of type t:
+ *   weights Q_t, chain id n_chains + m, placed at the target point.  Then soma_load_state's binning and
+ *   omega with step index step0.
+ *   Equilibration: n_equil_steps MC steps (soma_mc_steps) during which
+ *   omega_t(c) = fl32(omega_t(c) + fl32(umbrella_k * fl32(phi_t(c) - phi_target_t(c)))) -- the derivative of
+ *   (umbrella_k / 2)(B / cells) sum (phi - phi_target)^2, added after any external field; afterwards the
+ *   umbrella is removed and omega recomputed.  The step index ends at step0 + n_equil_steps.
+ * Double log/sin/cos as in soma_generate_state: two implementations agree to 1 fp32 ulp on a tiny fraction
+ * of the coordinates.  Errors: SOMA_EINVAL (NULL, bad target value, a molecule species whose target weight
+ * is zero everywhere, step index >= 2^48), SOMA_ECUDA. */
+int soma_init_from_density(soma_t *h, const float *phi_target, int ptr_is_device, uint64_t gen_seed,
+                           uint64_t step0, uint32_t n_equil_steps, float umbrella_k);
+
 /* Validation report of the current state (the paper's "validation functions", moved to the GPU
  * together with the generation of the coordinates): computed on the device in one
  * pass over the positions and one over the density grids; synchronises the stream. */

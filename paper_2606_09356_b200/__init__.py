@@ -26,7 +26,7 @@ LIB_PATH: Path = _build.LIB_PATH
 # every symbol include/soma.h declares (tests check the library exports exactly these)
 EXPORTS = (
     "soma_workspace_bytes", "soma_create", "soma_load_state", "soma_mc_steps", "soma_get_density",
-    "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_generate_state", "soma_validate_state", "soma_get_step", "soma_destroy", "soma_last_error",
+    "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_generate_state", "soma_init_from_density", "soma_validate_state", "soma_get_step", "soma_destroy", "soma_last_error",
     "soma_set_option", "soma_get_counters", "soma_get_kernel_times", "soma_debug_half_sweep", "soma_debug_finish_step",
     "soma_debug_set_omega", "soma_debug_philox", "soma_debug_maps", "soma_debug_accept",
     "soma_debug_accept_fma", "soma_debug_cell_index",
@@ -94,6 +94,7 @@ def load_library() -> C.CDLL:
             "soma_get_omega": (i32, [vp, vp, i32]),
             "soma_set_external_field": (i32, [vp, vp, i32]),
             "soma_generate_state": (i32, [vp, u64, u64]),
+            "soma_init_from_density": (i32, [vp, vp, i32, u64, u64, u32, C.c_float]),
             "soma_validate_state": (i32, [vp, C.POINTER(soma_validation)]),
             "soma_get_step": (i32, [vp, C.POINTER(u64)]),
             "soma_destroy": (i32, [vp]),
@@ -208,6 +209,14 @@ def soma_set_external_field(h, ext):
 
 def soma_generate_state(h, gen_seed: int, step0: int = 0):
     _check(load_library().soma_generate_state(h, int(gen_seed), int(step0)), h)
+
+
+def soma_init_from_density(h, phi_target, gen_seed: int, step0: int = 0, n_equil_steps: int = 0, umbrella_k: float = 0.0):
+    """phi_target: [T][cells] fp32 numpy array or CUDA tensor."""
+    if isinstance(phi_target, np.ndarray):
+        phi_target = np.ascontiguousarray(phi_target, dtype=np.float32)
+    _check(load_library().soma_init_from_density(h, _ptr(phi_target), _is_device(phi_target), int(gen_seed), int(step0),
+                                                 int(n_equil_steps), float(umbrella_k)), h)
 
 
 def soma_validate_state(h) -> dict:
@@ -358,6 +367,9 @@ class Soma:
 
     def generate_state(self, gen_seed: int, step0: int = 0):
         soma_generate_state(self._h, gen_seed, step0)
+
+    def init_from_density(self, phi_target, gen_seed: int, step0: int = 0, n_equil_steps: int = 0, umbrella_k: float = 0.0):
+        soma_init_from_density(self._h, phi_target, gen_seed, step0, n_equil_steps, umbrella_k)
 
     def validate(self) -> dict:
         return soma_validate_state(self._h)

@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "soma_lean.cuh"
+#include "soma_init.cuh"
 
 using namespace soma;
 
@@ -26,6 +27,8 @@ struct Layout {            // byte offsets into the workspace
   uint64_t counts[2];      // [T][C] uint32, double-buffered
   uint64_t omega;          // [T][C] fp32
   uint64_t ext;            // [T][C] fp32 external field (used once soma_set_external_field has set one)
+  uint64_t phi_tgt;        // [T][C] fp32 target concentrations of soma_init_from_density (umbrella potential)
+  uint64_t cdf;            // [C] uint64 prefix sums of the cell weights, then [C / kScanChunk + 2] chunk sums
   uint64_t single[3];      // [S] fp32 each: positions of the single-bead molecules (never re-ordered)
   uint64_t slot_chain[2];  // [n] uint32: logical chain id of every slot (second copy: re-order target)
   uint64_t slot_pattern[2];// [n] uint8
@@ -49,7 +52,7 @@ uint64_t sort_bin_count(const uint32_t grid[3]) {
 }
 
 // n_bins: entries of the sort_bins array
-Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins, uint64_t S) {
+Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint64_t n_bins, uint64_t S, uint64_t cells) {
   Layout L{};
   uint64_t off = 0;
   for (int s = 0; s < 2; ++s)
@@ -57,6 +60,8 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   for (int s = 0; s < 2; ++s) { L.counts[s] = off; off += align_up(TC * 4); }
   L.omega = off; off += align_up(TC * 4);
   L.ext = off; off += align_up(TC * 4);
+  L.phi_tgt = off; off += align_up(TC * 4);
+  L.cdf = off; off += align_up((cells + cells / 2048 + 4) * 8);
   for (int d = 0; d < 3; ++d) { L.single[d] = off; off += align_up(S * 4); }
   for (int s = 0; s < 2; ++s) { L.slot_chain[s] = off; off += align_up(n * 4); }
   for (int s = 0; s < 2; ++s) { L.slot_pattern[s] = off; off += align_up(n); }
@@ -157,6 +162,10 @@ struct soma_handle {
   // state
   bool loaded;
   bool has_ext;          // an external field is set (soma_set_external_field)
+  bool umbrella;         // the umbrella potential toward phi_tgt is on (inside soma_init_from_density)
+  float umbrella_k;
+  std::vector<uint8_t>* host_patterns;     // [n_patterns][N] copy of the type patterns
+  std::vector<uint64_t>* pattern_chains;   // [n_patterns] chains of every pattern
   bool identity_order;   // slot_chain is the identity
   uint64_t step;
   int sm_count;
@@ -183,6 +192,8 @@ struct soma_handle {
   uint32_t* counts(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts[s]); }
   float* omega() const { return reinterpret_cast<float*>(ws + L.omega); }
   float* ext() const { return reinterpret_cast<float*>(ws + L.ext); }
+  float* phi_tgt() const { return reinterpret_cast<float*>(ws + L.phi_tgt); }
+  unsigned long long* cdf() const { return reinterpret_cast<unsigned long long*>(ws + L.cdf); }
   float* single(int d) const { return reinterpret_cast<float*>(ws + L.single[d]); }
   uint32_t* slot_chain(int s) const { return reinterpret_cast<uint32_t*>(ws + L.slot_chain[s]); }
   uint8_t* slot_pattern(int s) const { return reinterpret_cast<uint8_t*>(ws + L.slot_pattern[s]); }
@@ -204,6 +215,8 @@ void free_handle(soma_handle* h) {
     for (cudaEvent_t e : *h->ev) cudaEventDestroy(e);
     delete h->ev;
   }
+  delete h->host_patterns;
+  delete h->pattern_chains;
   delete h;
 }
 
@@ -304,6 +317,8 @@ int launch_omega(soma_handle* h) {
   A.counts_to_zero = h->counts(h->cur ^ 1);
   A.omega = h->omega();
   A.ext = h->has_ext ? h->ext() : nullptr;
+  A.phi_tgt = h->umbrella ? h->phi_tgt() : nullptr;
+  A.umbrella_k = h->umbrella_k;
   const unsigned g = blocks_for(h->cells, 256);
   switch (h->T) {
     case 1: omega_kernel<1><<<g, 256, 0, h->stream>>>(A); break;
@@ -528,7 +543,7 @@ uint64_t soma_workspace_bytes(const soma_params* p) {
   const uint64_t TC = (uint64_t)p->grid[0] * p->grid[1] * p->grid[2] * p->n_types;
   uint64_t S = 0;
   if (p->n_single) for (uint32_t t = 0; t < p->n_types; ++t) S += p->n_single[t];
-  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bin_count(p->grid) + 2, S).total;
+  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bin_count(p->grid) + 2, S, TC / p->n_types).total;
 }
 
 int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
@@ -540,7 +555,11 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   if (!h) return fail(nullptr, SOMA_ENOMEM, "host allocation failed");
   std::memset(static_cast<void*>(h), 0, sizeof *h);
   h->ev = new (std::nothrow) std::vector<cudaEvent_t>();
-  if (!h->ev) { free_handle(h); return fail(nullptr, SOMA_ENOMEM, "host allocation failed"); }
+  h->host_patterns = new (std::nothrow) std::vector<uint8_t>(p->type_patterns, p->type_patterns + (size_t)p->n_patterns * p->beads_per_chain);
+  h->pattern_chains = new (std::nothrow) std::vector<uint64_t>(p->n_patterns, 0);
+  if (!h->ev || !h->host_patterns || !h->pattern_chains) { free_handle(h); return fail(nullptr, SOMA_ENOMEM, "host allocation failed"); }
+  if (p->chain_pattern) for (uint64_t c = 0; c < p->n_chains; ++c) (*h->pattern_chains)[p->chain_pattern[c]]++;
+  else (*h->pattern_chains)[0] = p->n_chains;
   cudaError_t e = cudaGetDevice(&h->device);
   cudaDeviceProp prop{};
   if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, h->device);
@@ -585,7 +604,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   for (uint32_t k = 0; k < h->T * h->T; ++k) h->chiN[k] = p->chiN[k];
   h->seed = p->seed;
   h->n_bins = (uint32_t)sort_bin_count(p->grid);
-  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, sort_bin_count(p->grid) + 2, h->S);
+  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, sort_bin_count(p->grid) + 2, h->S, h->cells);
   if (p->workspace) {
     if (p->workspace_bytes < h->L.total || (reinterpret_cast<uintptr_t>(p->workspace) % kAlign)) {
       free_handle(h);
@@ -705,6 +724,95 @@ int soma_generate_state(soma_t* h, uint64_t gen_seed, uint64_t step0) {
     CU(h, cudaGetLastError());
   }
   return finish_load(h, step0);
+}
+
+namespace {
+// inclusive prefix sums of the [cells] weights in h->cdf(), in place; *total receives their sum (synchronises)
+int scan_weights(soma_handle* h, unsigned long long* total) {
+  const uint32_t n = h->cells, chunks = (n + kScanChunk - 1) / kScanChunk;
+  unsigned long long* chunk = h->cdf() + n;
+  scan_chunk_sums_kernel<<<chunks, 256, 0, h->stream>>>(n, h->cdf(), chunk);
+  scan_small_kernel<<<1, 1024, 0, h->stream>>>(chunks, chunk);
+  scan_apply_kernel<<<chunks, 256, 0, h->stream>>>(n, h->cdf(), chunk);
+  h->launches += 3;
+  CU(h, cudaGetLastError());
+  CU(h, cudaMemcpyAsync(total, chunk + chunks, 8, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  return SOMA_OK;
+}
+}  // namespace
+
+int soma_init_from_density(soma_t* h, const float* phi_target, int dev, uint64_t gen_seed, uint64_t step0,
+                           uint32_t n_equil_steps, float umbrella_k) {
+  int rc = check(h);
+  if (rc != SOMA_OK) return rc;
+  if (!phi_target) return fail(h, SOMA_EINVAL, "phi_target is NULL");
+  if (step0 + n_equil_steps >= (1ull << 48)) return fail(h, SOMA_EINVAL, "step index would reach 2^48");
+  if (!(umbrella_k == umbrella_k)) return fail(h, SOMA_EINVAL, "umbrella_k is NaN");
+  h->live = 0;
+  h->loaded = false;
+  h->umbrella = false;
+  const size_t TC = (size_t)h->cells * h->T;
+  CU(h, cudaMemcpyAsync(h->phi_tgt(), phi_target, TC * 4, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+  // Q_t(c) in the first count buffer (re-initialised by the binning below)
+  uint32_t* Q = h->counts(0);
+  CU(h, cudaMemsetAsync(h->range_flag(), 0, 4, h->stream));
+  quantise_target_kernel<<<blocks_for(TC, 256), 256, 0, h->stream>>>(TC, h->phi_tgt(), Q, h->range_flag());
+  h->launches++;
+  CU(h, cudaGetLastError());
+  uint32_t bad = 0;
+  CU(h, cudaMemcpyAsync(&bad, h->range_flag(), 4, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));                       // the caller's host array has been read
+  if (bad) return fail(h, SOMA_EINVAL, "phi_target holds a negative, NaN or >= 65536 value");
+  PlaceArgs P{};
+  P.n_chains = (uint32_t)h->n_chains; P.N = h->N;
+  P.cells = h->cells; P.ny = h->grid.ny; P.nz = h->grid.nz;
+  P.k0 = (uint32_t)gen_seed; P.k1 = (uint32_t)(gen_seed >> 32);
+  P.hx = (double)h->box[0] / (double)h->grid.nx; P.hy = (double)h->box[1] / (double)h->grid.ny; P.hz = (double)h->box[2] / (double)h->grid.nz;
+  P.sigma = (double)h->b / std::sqrt(3.0);
+  P.chain_pattern = h->pattern0();
+  P.prefix = h->cdf();
+  for (uint32_t pat = 0; pat < h->n_patterns; ++pat) {
+    if ((*h->pattern_chains)[pat] == 0) continue;
+    TypeCounts M{};
+    for (uint32_t i = 0; i < h->N; ++i) M.m[(*h->host_patterns)[(size_t)pat * h->N + i]]++;
+    cell_weight_kernel<<<blocks_for(h->cells, 256), 256, 0, h->stream>>>(h->cells, h->T, M, Q, h->cdf());
+    h->launches++;
+    unsigned long long total = 0;
+    if ((rc = scan_weights(h, &total)) != SOMA_OK) return rc;
+    if (total == 0) return fail(h, SOMA_EINVAL, "phi_target gives a chain pattern zero total weight");
+    P.pattern = pat;
+    P.x = h->pos(0, 0); P.y = h->pos(0, 1); P.z = h->pos(0, 2);
+    place_chains_kernel<<<blocks_for(h->n_chains, 128), 128, 0, h->stream>>>(P);
+    h->launches++;
+    CU(h, cudaGetLastError());
+  }
+  for (uint32_t t = 0; t < h->T && h->S; ++t) {
+    const uint32_t count = h->single_start[t + 1] - h->single_start[t];
+    if (count == 0) continue;
+    TypeCounts M{};
+    M.m[t] = 1;
+    cell_weight_kernel<<<blocks_for(h->cells, 256), 256, 0, h->stream>>>(h->cells, h->T, M, Q, h->cdf());
+    h->launches++;
+    unsigned long long total = 0;
+    if ((rc = scan_weights(h, &total)) != SOMA_OK) return rc;
+    if (total == 0) return fail(h, SOMA_EINVAL, "phi_target gives a single-bead species zero total weight");
+    P.x = h->single(0); P.y = h->single(1); P.z = h->single(2);
+    place_singles_kernel<<<blocks_for(count, 256), 256, 0, h->stream>>>(P, h->single_start[t], count, (uint32_t)h->n_chains);
+    h->launches++;
+    CU(h, cudaGetLastError());
+  }
+  if ((rc = finish_load(h, step0)) != SOMA_OK) return rc;
+  if (n_equil_steps) {                                           // equilibration under the umbrella potential, which is removed again
+    h->umbrella = true;
+    h->umbrella_k = umbrella_k;
+    if ((rc = launch_omega(h)) != SOMA_OK) return rc;
+    rc = soma_mc_steps(h, n_equil_steps, nullptr);
+    h->umbrella = false;
+    if (rc != SOMA_OK) return rc;
+    if ((rc = launch_omega(h)) != SOMA_OK) return rc;
+  }
+  return SOMA_OK;
 }
 
 int soma_mc_steps(soma_t* h, uint32_t n_steps, uint64_t* accepted) {

@@ -350,6 +350,8 @@ struct OmegaArgs {
   uint32_t* __restrict__ counts_to_zero;     // [T][C] buffer for the next step (may be null)
   float* __restrict__ omega;                 // [T][C]
   const float* __restrict__ ext;             // [T][C] external field added to omega (R21), or null
+  const float* __restrict__ phi_tgt;         // [T][C] target concentrations of the umbrella potential (R25), or null
+  float umbrella_k;
 };
 
 template <int T_>
@@ -376,8 +378,10 @@ omega_kernel(OmegaArgs A) {
 #pragma unroll
       for (uint32_t s = 0; s < (T_ > 0 ? T_ : kMaxTypes); ++s)
         if (s < T && s != t) acc = __fmaf_rn(A.chiN[t * T + s], phi[s], acc);
-      const float w = __fmul_rn(A.invN, acc);
-      A.omega[(size_t)t * A.cells + c] = A.ext ? __fadd_rn(w, A.ext[(size_t)t * A.cells + c]) : w;
+      float w = __fmul_rn(A.invN, acc);
+      if (A.ext) w = __fadd_rn(w, A.ext[(size_t)t * A.cells + c]);
+      if (A.phi_tgt) w = __fadd_rn(w, __fmul_rn(A.umbrella_k, __fsub_rn(phi[t], A.phi_tgt[(size_t)t * A.cells + c])));
+      A.omega[(size_t)t * A.cells + c] = w;
     }
   }
 }
