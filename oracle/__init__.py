@@ -80,6 +80,7 @@ def lib() -> C.CDLL:
             "oracle_init_from_density": (C.c_int, [vp, f32p, C.c_uint64, C.c_uint64]),
             "oracle_set_umbrella": (None, [vp, f32p, C.c_float]),
             "oracle_set_singles": (C.c_int, [vp, C.POINTER(C.c_uint64)]),
+            "oracle_set_species": (C.c_int, [vp, C.c_uint32, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), C.c_uint32]),
             "oracle_set_smc": (None, [vp, C.c_float]),
             "oracle_smc_margin": (C.c_float, [vp, C.c_uint64, C.c_float, C.c_float, C.c_float]),
             "oracle_smc_draws": (None, [vp, C.c_uint64, C.c_uint32, C.c_uint32, C.POINTER(C.c_double)]),
@@ -146,22 +147,33 @@ class Oracle:
     """One SCMF system held by the CPU oracle."""
 
     def __init__(self, n_chains, N, n_types, type_patterns, chain_pattern, b, chiN, kappaN,
-                 grid, box, move_halfwidth, seed, n_single=None):
+                 grid, box, move_halfwidth, seed, n_single=None, species=None):
+        """species: None, or [(n_chains_s, N_s), ...] -- polymer species of different chain lengths stored one
+        after the other (R26); N is then the reference chain length of 1/N and the pattern rows have
+        max N_s entries."""
         self.n_chains, self.N, self.T = int(n_chains), int(N), int(n_types)
-        self.B = self.n_chains * self.N
+        self.species = None if species is None else [(int(a), int(b_)) for a, b_ in species]
+        stride = self.N if species is None else max(ns for _, ns in self.species)
+        self.B = self.n_chains * self.N if species is None else sum(a * b_ for a, b_ in self.species)
         self.grid = tuple(int(g) for g in grid)
         self.Cells = self.grid[0] * self.grid[1] * self.grid[2]
-        pats = np.ascontiguousarray(type_patterns, dtype=np.uint8).reshape(-1, self.N)
+        pats = np.ascontiguousarray(type_patterns, dtype=np.uint8).reshape(-1, stride)
         cp = None if chain_pattern is None else np.ascontiguousarray(chain_pattern, dtype=np.uint8)
         chi = np.ascontiguousarray(chiN, dtype=np.float32).reshape(self.T, self.T)
         g = np.asarray(self.grid, dtype=np.uint32)
         bx = np.asarray(box, dtype=np.float32)
         self._h = lib().oracle_create(
-            self.n_chains, self.N, self.T, pats.shape[0], _p(pats, C.c_uint8),
+            self.n_chains, stride, self.T, pats.shape[0], _p(pats, C.c_uint8),
             None if cp is None else _p(cp, C.c_uint8), float(b), _p(chi, C.c_float),
             float(kappaN), _p(g, C.c_uint32), _p(bx, C.c_float), float(move_halfwidth), int(seed))
         if not self._h:
             raise ValueError("oracle_create rejected the parameters")
+        if species is not None:
+            assert sum(a for a, _ in self.species) == self.n_chains
+            cnt = np.array([a for a, _ in self.species], dtype=np.uint64)
+            lens = np.array([b_ for _, b_ in self.species], dtype=np.uint32)
+            if lib().oracle_set_species(self._h, len(self.species), _p(cnt, C.c_uint64), _p(lens, C.c_uint32), self.N) != 0:
+                raise ValueError("oracle_set_species rejected the species table")
         if n_single is not None:                     # single-bead molecules per type, stored after the chains (R23)
             ns = np.ascontiguousarray(n_single, dtype=np.uint64).reshape(self.T)
             if lib().oracle_set_singles(self._h, _p(ns, C.c_uint64)) != 0:
@@ -173,7 +185,8 @@ class Oracle:
         """`s` is a scmf_inputs.System (duck-typed; this package imports nothing of it)."""
         w = s.workload
         return cls(w.n_chains, w.N, w.n_types, s.type_patterns, s.chain_pattern, w.b, s.chiN,
-                   w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed, n_single=getattr(s, "n_single", None))
+                   w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed, n_single=getattr(s, "n_single", None),
+                   species=getattr(s, "species", None))
 
     def close(self):
         if getattr(self, "_h", None):

@@ -111,12 +111,36 @@ struct Oracle {
   float gA = 0.0f, sq2A = 0.0f, inv4A = 0.0f;   // fl(A * 2 kb), (float)sqrt(2 A), (float)(1 / (4 A))
   std::vector<uint64_t> n_single;       // [T] (empty = none)
   uint64_t S = 0;                       // their total
+  // polymer species of different chain lengths (R26): chains are stored species by species; N above is
+  // then only the reference chain length of 1/N (R3) and Nstride the row length of type_patterns
+  struct Species { uint64_t n, first_chain, bead_off; uint32_t N; };
+  std::vector<Species> species;         // at least one entry
+  uint32_t Nstride;
+  uint64_t NB;                          // beads in chains (the single-bead molecules follow them)
   uint64_t t;                           // absolute step index
   bool loaded;
 };
 
+inline const Oracle::Species& species_of_chain(const Oracle& o, uint64_t c) {
+  size_t k = 0;
+  while (k + 1 < o.species.size() && c >= o.species[k + 1].first_chain) ++k;
+  return o.species[k];
+}
+inline uint32_t chain_len(const Oracle& o, uint64_t c) { return species_of_chain(o, c).N; }
+inline uint64_t chain_bead0(const Oracle& o, uint64_t c) {
+  const Oracle::Species& sp = species_of_chain(o, c);
+  return sp.bead_off + (c - sp.first_chain) * sp.N;
+}
+inline void bead_to_chain(const Oracle& o, uint64_t j, uint64_t* c, uint32_t* i) {
+  size_t k = 0;
+  while (k + 1 < o.species.size() && j >= o.species[k + 1].bead_off) ++k;
+  const Oracle::Species& sp = o.species[k];
+  *c = sp.first_chain + (j - sp.bead_off) / sp.N;
+  *i = (uint32_t)((j - sp.bead_off) % sp.N);
+}
+
 inline uint8_t bead_type(const Oracle& o, uint64_t c, uint32_t i) {
-  return o.type_patterns[(size_t)o.chain_pattern[c] * o.N + i];
+  return o.type_patterns[(size_t)o.chain_pattern[c] * o.Nstride + i];
 }
 
 // DESIGN.md section 2 step 1 (R8): floorf, then a proper non-negative modulo per axis.
@@ -144,12 +168,12 @@ inline uint32_t single_type(const Oracle& o, uint64_t m) {
 void bin(Oracle& o) {
   std::fill(o.counts.begin(), o.counts.end(), 0u);
   for (uint64_t m = 0; m < o.S; ++m) {
-    const uint64_t j = o.n_chains * o.N + m;
+    const uint64_t j = o.NB + m;
     o.counts[(size_t)single_type(o, m) * o.C + cell_index(o, o.x[j], o.y[j], o.z[j])] += 1u;
   }
   for (uint64_t c = 0; c < o.n_chains; ++c)
-    for (uint32_t i = 0; i < o.N; ++i) {
-      const uint64_t j = c * o.N + i;
+    for (uint32_t i = 0; i < chain_len(o, c); ++i) {
+      const uint64_t j = chain_bead0(o, c) + i;
       const uint64_t cell = cell_index(o, o.x[j], o.y[j], o.z[j]);
       o.counts[(size_t)bead_type(o, c, i) * o.C + cell] += 1u;
     }
@@ -194,7 +218,7 @@ inline float bond_sq(float ax, float ay, float az, float bx, float by, float bz)
 // DESIGN.md section 2 steps 5.4-5.5 (NS: "harmonic bond energy plus the bead type's
 // quasi-instantaneous field omega at its grid cell").
 inline float delta_energy(const Oracle& o, uint64_t c, uint32_t i, float nx, float ny, float nz) {
-  const uint64_t j = c * o.N + i;
+  const uint64_t j = chain_bead0(o, c) + i;
   const float rx = o.x[j], ry = o.y[j], rz = o.z[j];
   float dq = 0.0f;
   bool have = false;
@@ -205,7 +229,7 @@ inline float delta_energy(const Oracle& o, uint64_t c, uint32_t i, float nx, flo
     dq = q_new - q_old;
     have = true;
   }
-  if (i + 1 < o.N) {                                    // then neighbour i+1
+  if (i + 1 < chain_len(o, c)) {                                    // then neighbour i+1
     const uint64_t k = j + 1;
     const float q_old = bond_sq(rx, ry, rz, o.x[k], o.y[k], o.z[k]);
     const float q_new = bond_sq(nx, ny, nz, o.x[k], o.y[k], o.z[k]);
@@ -220,12 +244,12 @@ inline float delta_energy(const Oracle& o, uint64_t c, uint32_t i, float nx, flo
 // The same Delta E in double from the same fp32 inputs: used only to classify near-threshold
 // moves for the GPU-vs-oracle mismatch rule (NS: "|dE + ln u| < 1e-4 kT").
 inline double delta_energy_f64(const Oracle& o, uint64_t c, uint32_t i, float nx, float ny, float nz) {
-  const uint64_t j = c * o.N + i;
+  const uint64_t j = chain_bead0(o, c) + i;
   const double r[3] = {o.x[j], o.y[j], o.z[j]}, n[3] = {nx, ny, nz};
   double dq = 0.0;
   for (int side = 0; side < 2; ++side) {
     if (side == 0 && i == 0) continue;
-    if (side == 1 && i + 1 >= o.N) continue;
+    if (side == 1 && i + 1 >= chain_len(o, c)) continue;
     const uint64_t k = side == 0 ? j - 1 : j + 1;
     const double nb[3] = {o.x[k], o.y[k], o.z[k]};
     double qo = 0.0, qn = 0.0;
@@ -302,13 +326,13 @@ inline int trial_move_smc(Oracle& o, uint64_t c, uint32_t i, uint32_t parity, do
   float xi[3];
   smc_deviates(w, v, xi);
   const float u = umap(w[3]);
-  const uint64_t j = c * o.N + i;
+  const uint64_t j = chain_bead0(o, c) + i;
   const float r[3] = {o.x[j], o.y[j], o.z[j]};
   float S[3] = {0.0f, 0.0f, 0.0f};
   bool have = false;
   for (int side = 0; side < 2; ++side) {
     if (side == 0 && i == 0) continue;
-    if (side == 1 && i + 1 >= o.N) continue;
+    if (side == 1 && i + 1 >= chain_len(o, c)) continue;
     const uint64_t k = side == 0 ? j - 1 : j + 1;
     const float s3[3] = {r[0] - o.x[k], r[1] - o.y[k], r[2] - o.z[k]};
     for (int d = 0; d < 3; ++d) S[d] = have ? S[d] + s3[d] : s3[d];
@@ -320,7 +344,7 @@ inline int trial_move_smc(Oracle& o, uint64_t c, uint32_t i, uint32_t parity, do
   have = false;
   for (int side = 0; side < 2; ++side) {
     if (side == 0 && i == 0) continue;
-    if (side == 1 && i + 1 >= o.N) continue;
+    if (side == 1 && i + 1 >= chain_len(o, c)) continue;
     const uint64_t k = side == 0 ? j - 1 : j + 1;
     const float s3[3] = {n[0] - o.x[k], n[1] - o.y[k], n[2] - o.z[k]};
     for (int d = 0; d < 3; ++d) S2[d] = have ? S2[d] + s3[d] : s3[d];
@@ -351,7 +375,7 @@ inline int trial_move(Oracle& o, uint64_t c, uint32_t i, uint32_t parity, double
   const float dy = o.a * tmap(w[1]);
   const float dz = o.a * tmap(w[2]);
   const float u = umap(w[3]);
-  const uint64_t j = c * o.N + i;
+  const uint64_t j = chain_bead0(o, c) + i;
   const float nx = o.x[j] + dx, ny = o.y[j] + dy, nz = o.z[j] + dz;
   const float dE = delta_energy(o, c, i, nx, ny, nz);
   const float m = dE + lnu32(u);
@@ -371,7 +395,7 @@ inline int trial_move_single(Oracle& o, uint64_t m, double* margin64) {
   const uint32_t key[2] = {(uint32_t)o.seed, (uint32_t)(o.seed >> 32)};
   uint32_t w[4];
   philox4x32_10(ctr, key, w);
-  const uint64_t j = o.n_chains * o.N + m;
+  const uint64_t j = o.NB + m;
   const float nx = o.x[j] + o.a * tmap(w[0]), ny = o.y[j] + o.a * tmap(w[1]), nz = o.z[j] + o.a * tmap(w[2]);
   const float u = umap(w[3]);
   const size_t tb = (size_t)single_type(o, m) * o.C;
@@ -392,15 +416,16 @@ uint64_t half_sweep(Oracle& o, uint32_t parity, int order, const uint64_t* perm,
   if (order == 2) {
     for (uint64_t k = 0; k < n_perm; ++k) {
       const uint64_t j = perm[k];
-      if (j >= o.n_chains * o.N) {                       // a single-bead molecule: half-sweep 0 only
+      if (j >= o.NB) {                       // a single-bead molecule: half-sweep 0 only
         if (parity != 0) continue;
-        const int acc = trial_move_single(o, j - o.n_chains * o.N, margins ? &margins[j] : nullptr);
+        const int acc = trial_move_single(o, j - o.NB, margins ? &margins[j] : nullptr);
         if (accept_mask) accept_mask[j] = (uint8_t)acc;
         accepted += (uint64_t)acc;
         continue;
       }
-      const uint64_t c = j / o.N;
-      const uint32_t i = (uint32_t)(j % o.N);
+      uint64_t c;
+      uint32_t i;
+      bead_to_chain(o, j, &c, &i);
       if ((i & 1u) != parity) continue;
       const int acc = trial_move(o, c, i, parity, margins ? &margins[j] : nullptr);
       if (accept_mask) accept_mask[j] = (uint8_t)acc;
@@ -410,11 +435,11 @@ uint64_t half_sweep(Oracle& o, uint32_t parity, int order, const uint64_t* perm,
   }
   for (uint64_t cc = 0; cc < o.n_chains; ++cc) {
     const uint64_t c = order == 0 ? cc : o.n_chains - 1 - cc;
-    const uint32_t n_par = (o.N + 1u - parity) / 2u;    // beads i = parity, parity+2, ... < N
+    const uint32_t n_par = (chain_len(o, c) + 1u - parity) / 2u;    // beads i = parity, parity+2, ... < N
     for (uint32_t kk = 0; kk < n_par; ++kk) {
       const uint32_t k = order == 0 ? kk : n_par - 1 - kk;
       const uint32_t i = parity + 2u * k;
-      const uint64_t j = c * o.N + i;
+      const uint64_t j = chain_bead0(o, c) + i;
       const int acc = trial_move(o, c, i, parity, margins ? &margins[j] : nullptr);
       if (accept_mask) accept_mask[j] = (uint8_t)acc;
       accepted += (uint64_t)acc;
@@ -423,7 +448,7 @@ uint64_t half_sweep(Oracle& o, uint32_t parity, int order, const uint64_t* perm,
   if (parity == 0)
     for (uint64_t mm = 0; mm < o.S; ++mm) {
       const uint64_t m = order == 0 ? mm : o.S - 1 - mm;
-      const uint64_t j = o.n_chains * o.N + m;
+      const uint64_t j = o.NB + m;
       const int acc = trial_move_single(o, m, margins ? &margins[j] : nullptr);
       if (accept_mask) accept_mask[j] = (uint8_t)acc;
       accepted += (uint64_t)acc;
@@ -463,6 +488,9 @@ void* oracle_create(uint64_t n_chains, uint32_t N, uint32_t T, uint32_t n_patter
   o->chiN.assign(chiN, chiN + (size_t)T * T);
   for (int d = 0; d < 3; ++d) { o->grid[d] = grid[d]; o->box[d] = box[d]; }
   o->B = n_chains * N;
+  o->NB = o->B;
+  o->Nstride = N;
+  o->species.assign(1, Oracle::Species{n_chains, 0, 0, N});
   o->C = (uint64_t)grid[0] * grid[1] * grid[2];
   o->kb = 1.5f / (b * b);
   for (int d = 0; d < 3; ++d) o->inv_h[d] = (float)grid[d] / box[d];
@@ -567,14 +595,16 @@ void oracle_smc_draws(void* h, uint64_t c, uint32_t i, uint32_t parity, double* 
 // fma(inv4A, qr - qf, dE) of moving bead `bead` to (nx, ny, nz): the bond-force-biased margin without ln u
 float oracle_smc_margin(void* h, uint64_t bead, float nx, float ny, float nz) {
   Oracle& o = *static_cast<Oracle*>(h);
-  const uint64_t c = bead / o.N, j = bead;
-  const uint32_t i = (uint32_t)(bead % o.N);
+  const uint64_t j = bead;
+  uint64_t c;
+  uint32_t i;
+  bead_to_chain(o, bead, &c, &i);
   const float r[3] = {o.x[j], o.y[j], o.z[j]}, n[3] = {nx, ny, nz};
   float S[3] = {0, 0, 0}, S2[3] = {0, 0, 0};
   bool have = false;
   for (int side = 0; side < 2; ++side) {
     if (side == 0 && i == 0) continue;
-    if (side == 1 && i + 1 >= o.N) continue;
+    if (side == 1 && i + 1 >= chain_len(o, c)) continue;
     const uint64_t k = side == 0 ? j - 1 : j + 1;
     const float nb[3] = {o.x[k], o.y[k], o.z[k]};
     for (int d = 0; d < 3; ++d) {
@@ -610,7 +640,35 @@ int oracle_set_singles(void* h, const uint64_t* n_single) {
   o.S = 0;
   for (uint32_t t = 0; t < o.T; ++t) o.S += o.n_single[t];
   if (o.n_chains + o.S >= (1ull << 32)) return -1;
-  o.B = o.n_chains * o.N + o.S;
+  o.B = o.NB + o.S;
+  o.dens_scale = (float)((double)o.C / (double)o.B);
+  o.x.assign(o.B, 0.0f); o.y.assign(o.B, 0.0f); o.z.assign(o.B, 0.0f);
+  o.loaded = false;
+  return 0;
+}
+
+// Polymer species of different chain lengths (SURVEY section 8(f) row f2 "mixed chain lengths"; PAPER.md:39, :133:
+// polymer, solvent and non-solvent in one system; R26): species s has n[s] chains of N[s] beads; the
+// chains are numbered and stored species by species (species 0 first), bead i of chain c at
+// bead_off(species) + (c - first_chain(species)) N[s] + i; a chain of N[s] beads takes the first N[s] entries of
+// its pattern row (rows have the length given at oracle_create, >= max N[s]); 1/N in omega and the N of chiN,
+// kappaN stay the reference length N_ref (R3).  Call right after oracle_create (before oracle_set_singles).
+int oracle_set_species(void* h, uint32_t n_species, const uint64_t* n, const uint32_t* N, uint32_t N_ref) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (!n_species || !N_ref) return -1;
+  o.species.clear();
+  uint64_t chains = 0, beads = 0;
+  for (uint32_t s = 0; s < n_species; ++s) {
+    if (!n[s] || !N[s] || N[s] > o.Nstride) return -1;
+    o.species.push_back(Oracle::Species{n[s], chains, beads, N[s]});
+    chains += n[s];
+    beads += n[s] * N[s];
+  }
+  if (chains != o.n_chains) return -1;
+  o.N = N_ref;
+  o.invN = 1.0f / (float)N_ref;
+  o.NB = beads;
+  o.B = beads + o.S;
   o.dens_scale = (float)((double)o.C / (double)o.B);
   o.x.assign(o.B, 0.0f); o.y.assign(o.B, 0.0f); o.z.assign(o.B, 0.0f);
   o.loaded = false;
@@ -638,7 +696,7 @@ int oracle_generate_state(void* h, uint64_t gen_seed, uint64_t step0) {
   auto U = [](uint32_t w) { return ((double)w + 0.5) * 0x1p-32; };
   for (uint64_t c = 0; c < o.n_chains; ++c) {
     double r[3] = {0.0, 0.0, 0.0};
-    for (uint32_t i = 0; i < o.N; ++i) {
+    for (uint32_t i = 0; i < chain_len(o, c); ++i) {
       const uint32_t ctr[4] = {i, (uint32_t)c, 0u, 1u << 8};
       uint32_t w[4];
       philox4x32_10(ctr, key, w);
@@ -650,7 +708,7 @@ int oracle_generate_state(void* h, uint64_t gen_seed, uint64_t step0) {
         r[1] += sigma * (ra * std::sin(two_pi * U(w[1])));
         r[2] += sigma * (rb * std::cos(two_pi * U(w[3])));
       }
-      const uint64_t j = c * o.N + i;
+      const uint64_t j = chain_bead0(o, c) + i;
       o.x[j] = (float)r[0]; o.y[j] = (float)r[1]; o.z[j] = (float)r[2];
     }
   }
@@ -658,7 +716,7 @@ int oracle_generate_state(void* h, uint64_t gen_seed, uint64_t step0) {
     const uint32_t ctr[4] = {0u, (uint32_t)(o.n_chains + m), 0u, 1u << 8};
     uint32_t w[4];
     philox4x32_10(ctr, key, w);
-    const uint64_t j = o.n_chains * o.N + m;
+    const uint64_t j = o.NB + m;
     o.x[j] = (float)((double)o.box[0] * U(w[0]));
     o.y[j] = (float)((double)o.box[1] * U(w[1]));
     o.z[j] = (float)((double)o.box[2] * U(w[2]));
@@ -722,25 +780,26 @@ int oracle_init_from_density(void* h, const float* phi_target, uint64_t gen_seed
     rstar[1] = ((double)iy + U(w[3])) * hcell[1];
     rstar[2] = ((double)iz + U(v[0])) * hcell[2];
   };
-  std::vector<double> sx(o.N), sy(o.N), sz(o.N);
+  std::vector<double> sx(o.Nstride), sy(o.Nstride), sz(o.Nstride);
+  for (const Oracle::Species& sp : o.species)            // a chain's cell weights depend on its pattern and its length
   for (uint32_t p = 0; p < o.n_patterns; ++p) {
     bool used = false;
-    for (uint64_t c = 0; c < o.n_chains && !used; ++c) used = o.chain_pattern[c] == p;
+    for (uint64_t c = sp.first_chain; c < sp.first_chain + sp.n && !used; ++c) used = o.chain_pattern[c] == p;
     if (!used) continue;
     uint64_t run = 0;
     for (uint64_t c = 0; c < o.C; ++c) {
       uint64_t wgt = 0;
-      for (uint32_t i = 0; i < o.N; ++i) wgt += Q[(size_t)o.type_patterns[(size_t)p * o.N + i] * o.C + c];
+      for (uint32_t i = 0; i < sp.N; ++i) wgt += Q[(size_t)o.type_patterns[(size_t)p * o.Nstride + i] * o.C + c];
       run += wgt;
       prefix[c] = run;
     }
     if (run == 0) return -2;
-    for (uint64_t c = 0; c < o.n_chains; ++c) {
+    for (uint64_t c = sp.first_chain; c < sp.first_chain + sp.n; ++c) {
       if (o.chain_pattern[c] != p) continue;
       double rstar[3];
       target_point(c, rstar);
       double r[3] = {0.0, 0.0, 0.0}, sum[3] = {0.0, 0.0, 0.0};
-      for (uint32_t i = 0; i < o.N; ++i) {
+      for (uint32_t i = 0; i < sp.N; ++i) {
         if (i > 0) {
           const uint32_t ctr[4] = {i, (uint32_t)c, 0u, 1u << 8};
           uint32_t w[4];
@@ -753,9 +812,9 @@ int oracle_init_from_density(void* h, const float* phi_target, uint64_t gen_seed
         sx[i] = r[0]; sy[i] = r[1]; sz[i] = r[2];
         sum[0] += r[0]; sum[1] += r[1]; sum[2] += r[2];
       }
-      const double base[3] = {rstar[0] - sum[0] / (double)o.N, rstar[1] - sum[1] / (double)o.N, rstar[2] - sum[2] / (double)o.N};
-      for (uint32_t i = 0; i < o.N; ++i) {
-        const uint64_t j = c * o.N + i;
+      const double base[3] = {rstar[0] - sum[0] / (double)sp.N, rstar[1] - sum[1] / (double)sp.N, rstar[2] - sum[2] / (double)sp.N};
+      for (uint32_t i = 0; i < sp.N; ++i) {
+        const uint64_t j = chain_bead0(o, c) + i;
         o.x[j] = (float)(base[0] + sx[i]); o.y[j] = (float)(base[1] + sy[i]); o.z[j] = (float)(base[2] + sz[i]);
       }
     }
@@ -769,7 +828,7 @@ int oracle_init_from_density(void* h, const float* phi_target, uint64_t gen_seed
     for (uint64_t m = m0; m < m0 + o.n_single[t]; ++m) {
       double rstar[3];
       target_point(o.n_chains + m, rstar);
-      const uint64_t j = o.n_chains * o.N + m;
+      const uint64_t j = o.NB + m;
       o.x[j] = (float)rstar[0]; o.y[j] = (float)rstar[1]; o.z[j] = (float)rstar[2];
     }
     m0 += o.n_single[t];
@@ -799,8 +858,8 @@ void oracle_validate(void* h, uint64_t* out, double* bond) {
   double qsum = 0.0;
   uint64_t nb = 0;
   for (uint64_t c = 0; c < o.n_chains; ++c)
-    for (uint32_t i = 0; i + 1 < o.N; ++i) {
-      const uint64_t j = c * o.N + i;
+    for (uint32_t i = 0; i + 1 < chain_len(o, c); ++i) {
+      const uint64_t j = chain_bead0(o, c) + i;
       const float q = bond_sq(o.x[j], o.y[j], o.z[j], o.x[j + 1], o.y[j + 1], o.z[j + 1]);
       if (q > qmax) qmax = q;
       qsum += (double)q;
@@ -817,13 +876,17 @@ uint64_t oracle_cell_index(void* h, float x, float y, float z) {
 }
 float oracle_delta_energy(void* h, uint64_t bead, float nx, float ny, float nz) {
   Oracle& o = *static_cast<Oracle*>(h);
-  return delta_energy(o, bead / o.N, (uint32_t)(bead % o.N), nx, ny, nz);
+  uint64_t c;
+  uint32_t i;
+  bead_to_chain(o, bead, &c, &i);
+  return delta_energy(o, c, i, nx, ny, nz);
 }
 // The trial position and u that the move stream gives bead `bead` at the current step (no move made).
 void oracle_trial(void* h, uint64_t bead, uint32_t parity, float* trial_xyz, float* u) {
   Oracle& o = *static_cast<Oracle*>(h);
-  const uint64_t c = bead / o.N;
-  const uint32_t i = (uint32_t)(bead % o.N);
+  uint64_t c;
+  uint32_t i;
+  bead_to_chain(o, bead, &c, &i);
   const uint32_t ctr[4] = {i, (uint32_t)c, (uint32_t)o.t,
                            parity | (RNG_DOMAIN_MOVE << 8) | ((uint32_t)(o.t >> 32) << 16)};
   const uint32_t key[2] = {(uint32_t)o.seed, (uint32_t)(o.seed >> 32)};

@@ -23,7 +23,7 @@ from typing import Optional, Tuple
 
 import numpy as np
 
-__all__ = ["Workload", "System", "CONFIGS", "config", "make_system", "scaled"]
+__all__ = ["Workload", "System", "CONFIGS", "config", "make_system", "scaled", "custom_system", "species_system"]
 
 
 @dataclass(frozen=True)
@@ -67,6 +67,8 @@ class System:
     z: np.ndarray
     extra: dict = field(default_factory=dict)
     n_single: Optional[np.ndarray] = None    # uint64 [T]: single-bead molecules per type, stored after the chains
+    species: Optional[list] = None           # [(n_chains_s, N_s), ...]: polymer species of different chain lengths, stored
+                                             # species by species; workload.N is then the reference length, pattern rows max N_s long
 
     @property
     def n_patterns(self) -> int:
@@ -75,7 +77,14 @@ class System:
     def bead_types(self) -> np.ndarray:
         """uint8 [n_chains*N] type of every bead (harness-side bookkeeping only)."""
         w = self.workload
-        if self.chain_pattern is None:
+        if self.species is not None:
+            cp = np.zeros(w.n_chains, dtype=np.int64) if self.chain_pattern is None else self.chain_pattern.astype(np.int64)
+            parts, c0 = [], 0
+            for n_s, N_s in self.species:
+                parts.append(self.type_patterns[cp[c0:c0 + n_s], :N_s].reshape(-1))
+                c0 += n_s
+            t = np.concatenate(parts)
+        elif self.chain_pattern is None:
             t = np.tile(self.type_patterns[0], w.n_chains)
         else:
             t = self.type_patterns[self.chain_pattern].reshape(-1)
@@ -178,3 +187,33 @@ def custom_system(n_chains: int, N: int, n_types: int, type_patterns, chain_patt
     cp = None if chain_pattern is None else np.ascontiguousarray(chain_pattern, dtype=np.uint8)
     chi = np.ascontiguousarray(np.asarray(chiN, dtype=np.float32).reshape(n_types, n_types))
     return System(w, pats, cp, chi, out[0], out[1], out[2], n_single=ns)
+
+
+def species_system(species, N_ref: int, n_types: int, type_patterns, chain_pattern, chiN, kappaN: float, grid, box,
+                   seed: int, b: float = 1.0, move_halfwidth: float = 0.5, name: str = "species", n_single=None) -> System:
+    """Several polymer species of different chain lengths in one box (the paper's polymer / solvent / non-solvent
+    systems): species = [(n_chains_s, N_s), ...], chains stored species by species; N_ref is the
+    reference chain length (the N of chiN, kappaN and of 1/N); type_patterns rows have max N_s entries, a chain
+    uses the first N_s of its row.  Gaussian random-walk start like the configs'."""
+    species = [(int(a), int(c)) for a, c in species]
+    n_chains = sum(a for a, _ in species)
+    n_max = max(c for _, c in species)
+    w = Workload(name, n_chains, int(N_ref), n_types, "custom", tuple(int(g) for g in grid), tuple(float(v) for v in box),
+                 0.0, float(kappaN), seed=seed, steps=1, b=b, move_halfwidth=move_halfwidth)
+    rng = np.random.Generator(np.random.Philox(key=[seed, 0x5C3F_1218]))
+    sigma = b / np.sqrt(3.0)
+    out = [[], [], []]
+    for n_s, N_s in species:
+        for d in range(3):
+            steps = rng.standard_normal((n_s, N_s)) * sigma
+            steps[:, 0] = rng.random(n_s) * box[d]
+            out[d].append(np.cumsum(steps, axis=1).reshape(-1).astype(np.float32))
+    ns = None
+    if n_single is not None:
+        ns = np.ascontiguousarray(n_single, dtype=np.uint64).reshape(n_types)
+        for d in range(3):
+            out[d].append((rng.random(int(ns.sum())) * box[d]).astype(np.float32))
+    pats = np.ascontiguousarray(np.asarray(type_patterns, dtype=np.uint8).reshape(-1, n_max))
+    cp = None if chain_pattern is None else np.ascontiguousarray(chain_pattern, dtype=np.uint8)
+    chi = np.ascontiguousarray(np.asarray(chiN, dtype=np.float32).reshape(n_types, n_types))
+    return System(w, pats, cp, chi, np.concatenate(out[0]), np.concatenate(out[1]), np.concatenate(out[2]), n_single=ns, species=species)
