@@ -49,14 +49,15 @@ extern "C" {
 typedef struct soma_handle soma_t;   /* opaque */
 
 /* Problem statement (`north_star`: "chains, bead types, bond length b, chiN, kappaN, grid, box").
- * All chains are linear and have the same number of beads.  Limits: n_chains < 2^32,
- * 1 <= n_types <= 8, n_types * cells < 2^32, beads_per_chain <= 65535. */
+ * All chains are linear.  They have the same number of beads unless n_species > 1 (below).  Limits:
+ * n_chains < 2^32, 1 <= n_types <= 8, n_types * cells < 2^32, beads_per_chain <= 65535. */
 typedef struct soma_params {
   uint64_t n_chains;            /* n                                                            */
   uint32_t beads_per_chain;     /* N >= 1                                                       */
   uint32_t n_types;             /* T                                                            */
   uint32_t n_patterns;          /* >= 1                                                         */
-  uint32_t reserved0;           /* must be 0                                                    */
+  uint32_t n_species;           /* 0 or 1: every chain has beads_per_chain beads.  >= 2 (at most 16): polymer species
+                                   of different chain lengths, see species_n_chains below                       */
   const uint8_t *type_patterns; /* host [n_patterns][N]: bead type at each position along a chain */
   const uint8_t *chain_pattern; /* host [n_chains]: pattern id of each chain, or NULL = all 0     */
   const float *chiN;            /* host [T][T]: chi*N, symmetric, zero diagonal                   */
@@ -84,6 +85,17 @@ typedef struct soma_params {
                                    (type 0 first), so B = n_chains*N + sum(n_single); molecule m is
                                    bead 0 of logical chain n_chains + m for the random stream, moves
                                    in half-sweep 0 and has no bonds.  n_chains + sum < 2^32.     */
+  const uint64_t *species_n_chains; /* host [n_species] (read only if n_species >= 2): chains of every species;   */
+  const uint32_t *species_beads;    /* host [n_species]: beads per chain of every species.  Mixed chain lengths
+                                   (the paper's systems hold polymer, solvent and
+                                   non-solvent; R26): chains are numbered and stored
+                                   species by species (species 0 first), bead i of chain c of species s at
+                                   bead_off(s) + (c - first_chain(s)) * species_beads[s] + i in every position
+                                   array; sum(species_n_chains) = n_chains; type_patterns rows are
+                                   max(species_beads) long and a chain uses the first species_beads[s] entries of
+                                   its row; beads_per_chain is then only the reference chain length N of chiN,
+                                   kappaN and of the 1/N in omega.  A species whose length is not 2P (P a power of
+                                   two <= 32) runs on the generic kernels, the others on the fused one.          */
 } soma_params;
 
 /* Device bytes a handle for `p` needs (positions x2, grids, chain tables).  0 on invalid `p`. */

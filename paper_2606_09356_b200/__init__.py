@@ -46,7 +46,7 @@ class soma_params(C.Structure):
         ("beads_per_chain", C.c_uint32),
         ("n_types", C.c_uint32),
         ("n_patterns", C.c_uint32),
-        ("reserved0", C.c_uint32),
+        ("n_species", C.c_uint32),
         ("type_patterns", C.c_void_p),
         ("chain_pattern", C.c_void_p),
         ("chiN", C.c_void_p),
@@ -62,6 +62,8 @@ class soma_params(C.Structure):
         ("workspace", C.c_void_p),
         ("workspace_bytes", C.c_uint64),
         ("n_single", C.c_void_p),
+        ("species_n_chains", C.c_void_p),
+        ("species_beads", C.c_void_p),
     ]
 
 
@@ -137,8 +139,9 @@ def _is_device(a) -> int:
 # ---- the C entry points, same names ------------------------------------------------------------
 
 def make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN, kappaN,
-                grid, box, move_halfwidth, seed, n_single=None, smc_mobility=0.0):
-    """Build a soma_params plus the numpy arrays it points to (keep the tuple alive until create)."""
+                grid, box, move_halfwidth, seed, n_single=None, smc_mobility=0.0, species=None):
+    """Build a soma_params plus the numpy arrays it points to (keep the tuple alive until create).
+    species: None or [(n_chains_s, beads_s), ...] (soma_params.n_species, species_n_chains, species_beads)."""
     pats = np.ascontiguousarray(type_patterns, dtype=np.uint8)
     n_patterns = 1 if pats.ndim < 2 else int(pats.shape[0])     # validation is the library's job
     cp = None if chain_pattern is None else np.ascontiguousarray(chain_pattern, dtype=np.uint8)
@@ -156,7 +159,12 @@ def make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern
     p.workspace, p.workspace_bytes = None, 0
     ns = None if n_single is None else np.ascontiguousarray(n_single, dtype=np.uint64)
     p.n_single = None if ns is None else ns.ctypes.data
-    return p, (pats, cp, chi, ns)
+    sn = sb = None
+    if species is not None:
+        sn = np.ascontiguousarray([a for a, _ in species], dtype=np.uint64)
+        sb = np.ascontiguousarray([c for _, c in species], dtype=np.uint32)
+        p.n_species, p.species_n_chains, p.species_beads = len(species), sn.ctypes.data, sb.ctypes.data
+    return p, (pats, cp, chi, ns, sn, sb)
 
 
 def soma_workspace_bytes(p: soma_params) -> int:
@@ -315,16 +323,18 @@ class Soma:
     """One SCMF system on the current CUDA device.  Device memory and stream come from PyTorch."""
 
     def __init__(self, n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN,
-                 kappaN, grid, box, move_halfwidth, seed, stream=None, lend_workspace: bool = True, n_single=None, smc_mobility=0.0):
+                 kappaN, grid, box, move_halfwidth, seed, stream=None, lend_workspace: bool = True, n_single=None, smc_mobility=0.0,
+                 species=None):
         import torch
         if not torch.cuda.is_available():
             raise SomaError(SOMA_ECUDA, "no CUDA device: this package has no CPU fallback")
         self.n_chains, self.N, self.T = int(n_chains), int(beads_per_chain), int(n_types)
-        self.B = self.n_chains * self.N + (0 if n_single is None else int(np.asarray(n_single, dtype=np.uint64).sum()))
+        chain_beads = self.n_chains * self.N if species is None else sum(int(a) * int(c) for a, c in species)
+        self.B = chain_beads + (0 if n_single is None else int(np.asarray(n_single, dtype=np.uint64).sum()))
         self.grid = tuple(int(g) for g in grid)
         self.cells = self.grid[0] * self.grid[1] * self.grid[2]
         p, keep = make_params(n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN,
-                              kappaN, grid, box, move_halfwidth, seed, n_single=n_single, smc_mobility=smc_mobility)
+                              kappaN, grid, box, move_halfwidth, seed, n_single=n_single, smc_mobility=smc_mobility, species=species)
         self._workspace = None
         if lend_workspace:
             nbytes = soma_workspace_bytes(p)
@@ -341,6 +351,7 @@ class Soma:
         """`s` is a scmf_inputs.System (duck-typed)."""
         w = s.workload
         kw.setdefault("n_single", getattr(s, "n_single", None))
+        kw.setdefault("species", getattr(s, "species", None))
         return cls(w.n_chains, w.N, w.n_types, s.type_patterns, s.chain_pattern, w.b, s.chiN,
                    w.kappaN, w.grid, w.box, w.move_halfwidth, w.seed, **kw)
 

@@ -20,6 +20,7 @@ namespace {
 thread_local char g_last_error[256] = "";
 
 constexpr uint64_t kAlign = 256;
+constexpr uint32_t kMaxSpecies = 16;
 inline uint64_t align_up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {            // byte offsets into the workspace
@@ -79,13 +80,38 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
 
 bool is_pow2(uint32_t v) { return v && !(v & (v - 1)); }
 
+// row length of type_patterns: the chain length, or the longest species' (R26)
+uint32_t pattern_stride(const soma_params* p) {
+  if (p->n_species <= 1) return p->beads_per_chain;
+  uint32_t m = 0;
+  for (uint32_t k = 0; k < p->n_species; ++k) m = p->species_beads[k] > m ? p->species_beads[k] : m;
+  return m;
+}
+uint64_t chain_beads(const soma_params* p) {
+  if (p->n_species <= 1) return p->n_chains * p->beads_per_chain;
+  uint64_t b = 0;
+  for (uint32_t k = 0; k < p->n_species; ++k) b += p->species_n_chains[k] * p->species_beads[k];
+  return b;
+}
+
 const char* validate(const soma_params* p) {
   if (!p) return "params is NULL";
   if (p->n_chains == 0 || p->n_chains >= (1ull << 32)) return "n_chains must be in [1, 2^32)";
   if (p->beads_per_chain == 0 || p->beads_per_chain > 65535) return "beads_per_chain must be in [1, 65535]";
   if (p->n_types == 0 || p->n_types > (uint32_t)kMaxTypes) return "n_types must be in [1, 8]";
   if (p->n_patterns == 0 || p->n_patterns > 256) return "n_patterns must be in [1, 256]";
-  if (p->reserved0 || p->reserved2 || p->reserved3 != 0.0f) return "reserved fields must be 0";
+  if (p->reserved2 || p->reserved3 != 0.0f) return "reserved fields must be 0";
+  if (p->n_species > 1) {
+    if (p->n_species > kMaxSpecies) return "n_species must be <= 16";
+    if (!p->species_n_chains || !p->species_beads) return "species_n_chains / species_beads is NULL but n_species > 1";
+    uint64_t tot = 0;
+    for (uint32_t k = 0; k < p->n_species; ++k) {
+      if (p->species_n_chains[k] == 0 || p->species_n_chains[k] >= (1ull << 32)) return "species_n_chains[s] must be in [1, 2^32)";
+      if (p->species_beads[k] == 0 || p->species_beads[k] > 65535) return "species_beads[s] must be in [1, 65535]";
+      tot += p->species_n_chains[k];
+    }
+    if (tot != p->n_chains) return "species_n_chains must sum to n_chains";
+  }
   if (!(p->smc_mobility >= 0.0f) || p->smc_mobility > 1e6f) return "smc_mobility must be in [0, 1e6]";
   if (!p->type_patterns) return "type_patterns is NULL";
   if (!p->chiN) return "chiN is NULL";
@@ -108,7 +134,7 @@ const char* validate(const soma_params* p) {
     }
     if (p->n_chains + S >= (1ull << 32)) return "n_chains + single-bead molecules must be < 2^32";
   }
-  const uint64_t npat = (uint64_t)p->n_patterns * p->beads_per_chain;
+  const uint64_t npat = (uint64_t)p->n_patterns * pattern_stride(p);
   for (uint64_t k = 0; k < npat; ++k)
     if (p->type_patterns[k] >= p->n_types) return "type_patterns holds a type >= n_types";
   if (p->chain_pattern)
@@ -136,7 +162,15 @@ int fused_lanes(uint32_t N) {   // P = N/2 if the fused kernel supports N, else 
 
 struct soma_handle {
   // problem
-  uint64_t n_chains, B;          // B = n_chains * N: beads in chains
+  uint64_t n_chains, B;          // all chains; B = beads in chains
+  // Polymer species of different chain lengths (R26): chains, slots and beads of species s are the
+  // ranges [first_chain, first_chain + n) and [bead_off, bead_off + B) of every per-chain / per-bead array.
+  // `v` is the species the per-species launchers below work on; N (below) is the reference chain length of 1/N.
+  struct View { uint64_t n, first_chain, bead_off, B; uint32_t N; };
+  View views[kMaxSpecies];
+  uint32_t n_views;
+  View v;
+  uint32_t Nstride;              // row length of the type patterns
   uint64_t S, Btot;              // single-bead molecules (R23) and all beads
   uint32_t single_start[kMaxTypes + 1];
   uint32_t N, T, n_patterns, cells;
@@ -189,6 +223,7 @@ struct soma_handle {
   char err[256];
 
   float* pos(int set, int d) const { return reinterpret_cast<float*>(ws + L.pos[set][d]); }
+  float* vpos(int set, int d) const { return pos(set, d) + v.bead_off; }                       // ... of the current species
   uint32_t* counts(int s) const { return reinterpret_cast<uint32_t*>(ws + L.counts[s]); }
   float* omega() const { return reinterpret_cast<float*>(ws + L.omega); }
   float* ext() const { return reinterpret_cast<float*>(ws + L.ext); }
@@ -199,6 +234,8 @@ struct soma_handle {
   uint8_t* slot_pattern(int s) const { return reinterpret_cast<uint8_t*>(ws + L.slot_pattern[s]); }
   uint32_t* slot_chain() const { return slot_chain(live); }
   uint8_t* slot_pattern() const { return slot_pattern(live); }
+  uint32_t* vslot_chain(int s) const { return slot_chain(s) + v.first_chain; }
+  uint8_t* vslot_pattern(int s) const { return slot_pattern(s) + v.first_chain; }
   uint32_t* range_flag() const { return reinterpret_cast<uint32_t*>(ws + L.range_flag); }
   uint32_t* sort_key() const { return reinterpret_cast<uint32_t*>(ws + L.sort_key); }
   uint32_t* sort_rank() const { return reinterpret_cast<uint32_t*>(ws + L.sort_rank); }
@@ -242,30 +279,31 @@ StepArgs step_args(const soma_handle* h) {
   StepArgs A{};
   A.grid = h->grid;
   A.cells = h->cells;
-  A.n_chains = (uint32_t)h->n_chains;
-  A.N = h->N;
+  A.n_chains = (uint32_t)h->v.n;
+  A.N = h->v.N;
+  A.pat_stride = h->Nstride;
   A.a = h->a;
   A.kb = h->kb;
   A.gA = h->gA; A.sq2A = h->sq2A; A.inv4A = h->inv4A;
   A.keys = h->keys;
   A.ctr2 = (uint32_t)h->step;
   A.ctr3_base = (0u << 8) | ((uint32_t)(h->step >> 32) << 16);   // domain 0 = MC move
-  A.x = h->pos(h->live, 0);
-  A.y = h->pos(h->live, 1);
-  A.z = h->pos(h->live, 2);
+  A.x = h->vpos(h->live, 0);
+  A.y = h->vpos(h->live, 1);
+  A.z = h->vpos(h->live, 2);
   A.omega = h->omega();
   A.counts_next = h->counts(h->cur ^ 1);
-  A.slot_chain = h->slot_chain();
-  A.slot_pattern = h->slot_pattern();
+  A.slot_chain = h->vslot_chain(h->live);
+  A.slot_pattern = h->vslot_pattern(h->live);
   A.patterns = h->patterns();
   A.accepted = h->accepted();
   return A;
 }
 
 int launch_half_sweep(soma_handle* h, uint32_t parity) {
-  const uint32_t n_par = (h->N + 1u - parity) / 2u;
+  const uint32_t n_par = (h->v.N + 1u - parity) / 2u;
   if (n_par == 0) return SOMA_OK;                               // N == 1 has no odd beads
-  const uint64_t total = h->n_chains * n_par;
+  const uint64_t total = h->v.n * n_par;
   const StepArgs A = step_args(h);
   if (h->pow2) half_sweep_kernel<true><<<blocks_for(total, 256), 256, 0, h->stream>>>(A, parity, n_par);
   else half_sweep_kernel<false><<<blocks_for(total, 256), 256, 0, h->stream>>>(A, parity, n_par);
@@ -279,6 +317,7 @@ int launch_singles(soma_handle* h, bool do_move, bool do_bin, uint32_t* counts, 
   if (h->S == 0) return SOMA_OK;
   SingleArgs A{};
   A.S = step_args(h);
+  A.S.n_chains = (uint32_t)h->n_chains;                          // first logical id of the molecules
   A.n_total = (uint32_t)h->S; A.T = h->T;
   for (int t = 0; t <= kMaxTypes; ++t) A.start[t] = h->single_start[t];
   A.x = h->single(0); A.y = h->single(1); A.z = h->single(2);
@@ -292,18 +331,29 @@ int launch_singles(soma_handle* h, bool do_move, bool do_bin, uint32_t* counts, 
   return SOMA_OK;
 }
 
+// bins the chains of the current species
+int launch_bin_chains(soma_handle* h, uint32_t* counts, uint32_t* flag) {
+  {
+    if (h->pow2)
+      bin_kernel<true><<<blocks_for(h->v.B, 256), 256, 0, h->stream>>>(
+          h->grid, h->cells, h->v.N, h->Nstride, h->v.B, h->vpos(h->live, 0), h->vpos(h->live, 1), h->vpos(h->live, 2),
+          h->vslot_pattern(h->live), h->patterns(), counts, flag);
+    else
+      bin_kernel<false><<<blocks_for(h->v.B, 256), 256, 0, h->stream>>>(
+          h->grid, h->cells, h->v.N, h->Nstride, h->v.B, h->vpos(h->live, 0), h->vpos(h->live, 1), h->vpos(h->live, 2),
+          h->vslot_pattern(h->live), h->patterns(), counts, flag);
+    h->launches++;
+    CU(h, cudaGetLastError());
+  }
+  return SOMA_OK;
+}
+// row a3 on its own: every species and the single-bead molecules
 int launch_bin(soma_handle* h, uint32_t* counts, bool check_range = false) {
-  uint32_t* flag = check_range ? h->range_flag() : nullptr;
-  if (h->pow2)
-    bin_kernel<true><<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
-        h->grid, h->cells, h->N, h->B, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2),
-        h->slot_pattern(), h->patterns(), counts, flag);
-  else
-    bin_kernel<false><<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
-        h->grid, h->cells, h->N, h->B, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2),
-        h->slot_pattern(), h->patterns(), counts, flag);
-  h->launches++;
-  CU(h, cudaGetLastError());
+  int rc;
+  for (uint32_t k = 0; k < h->n_views; ++k) {
+    h->v = h->views[k];
+    if ((rc = launch_bin_chains(h, counts, check_range ? h->range_flag() : nullptr)) != SOMA_OK) return rc;
+  }
   return launch_singles(h, false, true, counts, check_range);
 }
 
@@ -332,13 +382,13 @@ int launch_omega(soma_handle* h) {
 }
 
 bool lean_ok(const soma_handle* h) {
-  return h->fused_lean && h->fast_arith && h->pow2 && h->smcA == 0.0f && fused_lanes(h->N) != 0;
+  return h->fused_lean && h->fast_arith && h->pow2 && h->smcA == 0.0f && fused_lanes(h->v.N) != 0;
 }
 template <int P, bool MULTI, int NT>
 void launch_lean_k(soma_handle* h, LeanArgs& A) {
   constexpr int G = 32 / P;
   auto* k = lean_step_kernel<P, MULTI, NT>;
-  const uint64_t n_groups = (h->n_chains + G - 1) / G;
+  const uint64_t n_groups = (h->v.n + G - 1) / G;
   const uint64_t wpb = NT / 32;
   const uint64_t gpb = ((uint64_t)h->fused_chunk * (NT / 256) + wpb - 1) / wpb * wpb;   // fused_chunk is per 256 threads
   A.groups_per_block = (uint32_t)gpb;
@@ -360,7 +410,8 @@ int launch_lean_p(soma_handle* h) {
   A.mx = h->grid.nx - 1; A.my = h->grid.ny - 1; A.mz = h->grid.nz - 1;
   A.ny = h->grid.ny; A.nz = h->grid.nz;
   A.cells = h->cells;
-  A.n_chains = (uint32_t)h->n_chains;
+  A.n_chains = (uint32_t)h->v.n;
+  A.pat_stride = h->Nstride;
   A.a2 = 2.0f * h->a;
   A.ac = h->a * -0.99999988079071044921875f;       // a (2^-23 - 1), exact: a is a power of two
   A.kb = h->kb;
@@ -369,11 +420,11 @@ int launch_lean_p(soma_handle* h) {
   A.u0 = (uint32_t)(m1 >> 32) ^ h->keys.k0[0];
   A.u1 = (uint32_t)m1;
   A.ctr3_base = (0u << 8) | ((uint32_t)(h->step >> 32) << 16);   // domain 0 = MC move
-  A.x = h->pos(h->live, 0); A.y = h->pos(h->live, 1); A.z = h->pos(h->live, 2);
+  A.x = h->vpos(h->live, 0); A.y = h->vpos(h->live, 1); A.z = h->vpos(h->live, 2);
   A.omega = h->omega();
   A.counts_next = h->counts(h->cur ^ 1);
-  A.slot_chain = h->slot_chain();
-  A.slot_pattern = h->slot_pattern();
+  A.slot_chain = h->vslot_chain(h->live);
+  A.slot_pattern = h->vslot_pattern(h->live);
   A.patterns = h->patterns();
   A.accepted = h->accepted();
   switch (h->lean_threads) {
@@ -388,7 +439,7 @@ int launch_fused_p(soma_handle* h) {
   if (lean_ok(h)) return launch_lean_p<P>(h);
   const StepArgs A = step_args(h);
   constexpr int G = 32 / P;
-  const uint64_t n_groups = (h->n_chains + G - 1) / G;           // warps of work
+  const uint64_t n_groups = (h->v.n + G - 1) / G;                // warps of work
   const unsigned bs = 256, wpb = bs / 32;
   // chunks of fused_chunk warp groups (a multiple of the warps per block)
   uint64_t gpb = ((uint64_t)h->fused_chunk + wpb - 1) / wpb * wpb;
@@ -413,7 +464,7 @@ int launch_fused_p(soma_handle* h) {
 }
 
 int launch_fused(soma_handle* h) {
-  switch (fused_lanes(h->N)) {
+  switch (fused_lanes(h->v.N)) {
     case 1: return launch_fused_p<1>(h);
     case 2: return launch_fused_p<2>(h);
     case 4: return launch_fused_p<4>(h);
@@ -426,32 +477,38 @@ int launch_fused(soma_handle* h) {
 
 bool use_fused(const soma_handle* h) {
   if (h->path == 1) return false;
-  return fused_lanes(h->N) != 0;
+  if ((h->Nstride & 1u) && h->n_patterns > 1) return false;     // the fused kernels read a lane's two types as one aligned 16-bit word
+  return fused_lanes(h->v.N) != 0;
 }
 // Re-order the chains in memory by the coarse bin (cube of kSortBinEdge cells) of their centre of
 // mass: a counting sort on the device.
 int resort(soma_handle* h) {
   const int src = h->live, dst = h->live ^ 1;
-  SortArgs S{};
-  S.grid = h->grid; S.n_chains = (uint32_t)h->n_chains; S.N = h->N;
-  S.cbx = S.cby = S.cbz = kSortBinEdge;
-  S.ncy = (h->grid.ny + kSortBinEdge - 1) / kSortBinEdge;
-  S.ncz = (h->grid.nz + kSortBinEdge - 1) / kSortBinEdge;
-  const uint32_t n_bins = h->n_bins;
-  CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
-  if (h->pow2)
-    chain_key_kernel<true><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
-        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
-  else
-    chain_key_kernel<false><<<blocks_for(h->n_chains, 256), 256, 0, h->stream>>>(
-        S, h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->sort_bins(), h->sort_key(), h->sort_rank());
-  bin_scan_kernel<<<1, 1024, 0, h->stream>>>(n_bins + 1, h->sort_bins());      // entry n_bins becomes the total
-  chain_permute_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
-      h->B, h->N, h->sort_bins(), h->sort_key(), h->sort_rank(),
-      h->pos(src, 0), h->pos(src, 1), h->pos(src, 2), h->pos(dst, 0), h->pos(dst, 1), h->pos(dst, 2),
-      h->slot_chain(src), h->slot_pattern(src), h->slot_chain(dst), h->slot_pattern(dst));
-  h->launches += 3;
-  CU(h, cudaGetLastError());
+  for (uint32_t k = 0; k < h->n_views; ++k) {                     // every species inside its own range of slots
+    h->v = h->views[k];
+    SortArgs S{};
+    S.grid = h->grid; S.n_chains = (uint32_t)h->v.n; S.N = h->v.N;
+    S.cbx = S.cby = S.cbz = kSortBinEdge;
+    S.ncy = (h->grid.ny + kSortBinEdge - 1) / kSortBinEdge;
+    S.ncz = (h->grid.nz + kSortBinEdge - 1) / kSortBinEdge;
+    const uint32_t n_bins = h->n_bins;
+    uint32_t* key = h->sort_key() + h->v.first_chain;
+    uint32_t* rank = h->sort_rank() + h->v.first_chain;
+    CU(h, cudaMemsetAsync(h->sort_bins(), 0, ((size_t)n_bins + 1) * 4, h->stream));
+    if (h->pow2)
+      chain_key_kernel<true><<<blocks_for(h->v.n, 256), 256, 0, h->stream>>>(
+          S, h->vpos(src, 0), h->vpos(src, 1), h->vpos(src, 2), h->sort_bins(), key, rank);
+    else
+      chain_key_kernel<false><<<blocks_for(h->v.n, 256), 256, 0, h->stream>>>(
+          S, h->vpos(src, 0), h->vpos(src, 1), h->vpos(src, 2), h->sort_bins(), key, rank);
+    bin_scan_kernel<<<1, 1024, 0, h->stream>>>(n_bins + 1, h->sort_bins());      // entry n_bins becomes the total
+    chain_permute_kernel<<<blocks_for(h->v.B, 256), 256, 0, h->stream>>>(
+        h->v.B, h->v.N, h->sort_bins(), key, rank,
+        h->vpos(src, 0), h->vpos(src, 1), h->vpos(src, 2), h->vpos(dst, 0), h->vpos(dst, 1), h->vpos(dst, 2),
+        h->vslot_chain(src), h->vslot_pattern(src), h->vslot_chain(dst), h->vslot_pattern(dst));
+    h->launches += 3;
+    CU(h, cudaGetLastError());
+  }
   h->live = dst;
   h->identity_order = false;
   h->resorts++;
@@ -496,15 +553,19 @@ int one_step(soma_handle* h) {
     if ((rc = resort(h)) != SOMA_OK) return rc;
   const bool timed = h->timing && h->ev_used + 3 <= 3 * kMaxTimedSteps;
   if (timed) timing_mark(h);
-  if (use_fused(h)) {
-    if ((rc = launch_fused(h)) != SOMA_OK) return rc;            // a1 + a2 + a3 (+a5)
-    if ((rc = launch_singles(h, true, true, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;
-  } else {
-    if ((rc = launch_half_sweep(h, 0)) != SOMA_OK) return rc;    // a1
-    if ((rc = launch_singles(h, true, false, nullptr)) != SOMA_OK) return rc;   // a1, single-bead molecules
-    if ((rc = launch_half_sweep(h, 1)) != SOMA_OK) return rc;    // a2
-    if ((rc = launch_bin(h, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;   // a3 (chains and single-bead molecules)
+  // Chains interact only through omega, which is frozen during a step, so the species (and the single-bead
+  // molecules) can take their half-sweeps one after the other, each on the kernels its chain length allows.
+  for (uint32_t k = 0; k < h->n_views; ++k) {
+    h->v = h->views[k];
+    if (use_fused(h)) {
+      if ((rc = launch_fused(h)) != SOMA_OK) return rc;            // a1 + a2 + a3 (+a5)
+    } else {
+      if ((rc = launch_half_sweep(h, 0)) != SOMA_OK) return rc;    // a1
+      if ((rc = launch_half_sweep(h, 1)) != SOMA_OK) return rc;    // a2
+      if ((rc = launch_bin_chains(h, h->counts(h->cur ^ 1), nullptr)) != SOMA_OK) return rc;   // a3
+    }
   }
+  if ((rc = launch_singles(h, true, true, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;      // a1 + a3, single-bead molecules
   h->cur ^= 1;
   if (timed) timing_mark(h);
   if ((rc = launch_omega(h)) != SOMA_OK) return rc;              // a4
@@ -539,11 +600,11 @@ extern "C" {
 uint64_t soma_workspace_bytes(const soma_params* p) {
   const char* bad = validate(p);
   if (bad) { fail(nullptr, SOMA_EINVAL, bad); return 0; }
-  const uint64_t B = p->n_chains * p->beads_per_chain;
+  const uint64_t B = chain_beads(p);
   const uint64_t TC = (uint64_t)p->grid[0] * p->grid[1] * p->grid[2] * p->n_types;
   uint64_t S = 0;
   if (p->n_single) for (uint32_t t = 0; t < p->n_types; ++t) S += p->n_single[t];
-  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * p->beads_per_chain, sort_bin_count(p->grid) + 2, S, TC / p->n_types).total;
+  return make_layout(B, p->n_chains, TC, (uint64_t)p->n_patterns * pattern_stride(p), sort_bin_count(p->grid) + 2, S, TC / p->n_types).total;
 }
 
 int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
@@ -555,11 +616,24 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   if (!h) return fail(nullptr, SOMA_ENOMEM, "host allocation failed");
   std::memset(static_cast<void*>(h), 0, sizeof *h);
   h->ev = new (std::nothrow) std::vector<cudaEvent_t>();
-  h->host_patterns = new (std::nothrow) std::vector<uint8_t>(p->type_patterns, p->type_patterns + (size_t)p->n_patterns * p->beads_per_chain);
-  h->pattern_chains = new (std::nothrow) std::vector<uint64_t>(p->n_patterns, 0);
+  h->host_patterns = new (std::nothrow) std::vector<uint8_t>(p->type_patterns, p->type_patterns + (size_t)p->n_patterns * pattern_stride(p));
+  const uint32_t n_views = p->n_species > 1 ? p->n_species : 1u;
+  h->pattern_chains = new (std::nothrow) std::vector<uint64_t>((size_t)n_views * p->n_patterns, 0);      // [species][pattern]
   if (!h->ev || !h->host_patterns || !h->pattern_chains) { free_handle(h); return fail(nullptr, SOMA_ENOMEM, "host allocation failed"); }
-  if (p->chain_pattern) for (uint64_t c = 0; c < p->n_chains; ++c) (*h->pattern_chains)[p->chain_pattern[c]]++;
-  else (*h->pattern_chains)[0] = p->n_chains;
+  h->n_views = n_views;
+  h->Nstride = pattern_stride(p);
+  {
+    uint64_t c0 = 0, b0 = 0;
+    for (uint32_t k = 0; k < n_views; ++k) {
+      soma_handle::View& V = h->views[k];
+      V.n = n_views > 1 ? p->species_n_chains[k] : p->n_chains;
+      V.N = n_views > 1 ? p->species_beads[k] : p->beads_per_chain;
+      V.first_chain = c0; V.bead_off = b0; V.B = V.n * V.N;
+      for (uint64_t c = c0; c < c0 + V.n; ++c) (*h->pattern_chains)[(size_t)k * p->n_patterns + (p->chain_pattern ? p->chain_pattern[c] : 0)]++;
+      c0 += V.n; b0 += V.B;
+    }
+    h->v = h->views[0];
+  }
   cudaError_t e = cudaGetDevice(&h->device);
   cudaDeviceProp prop{};
   if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, h->device);
@@ -576,7 +650,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->sm_count = prop.multiProcessorCount;
   h->stream = static_cast<cudaStream_t>(cuda_stream);
   h->n_chains = p->n_chains; h->N = p->beads_per_chain; h->T = p->n_types; h->n_patterns = p->n_patterns;
-  h->B = h->n_chains * h->N;
+  h->B = chain_beads(p);
   h->S = 0;
   for (uint32_t t = 0; t < h->T; ++t) {
     h->single_start[t] = (uint32_t)h->S;
@@ -604,7 +678,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   for (uint32_t k = 0; k < h->T * h->T; ++k) h->chiN[k] = p->chiN[k];
   h->seed = p->seed;
   h->n_bins = (uint32_t)sort_bin_count(p->grid);
-  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->N, sort_bin_count(p->grid) + 2, h->S, h->cells);
+  h->L = make_layout(h->B, h->n_chains, (uint64_t)h->cells * h->T, (uint64_t)h->n_patterns * h->Nstride, sort_bin_count(p->grid) + 2, h->S, h->cells);
   if (p->workspace) {
     if (p->workspace_bytes < h->L.total || (reinterpret_cast<uintptr_t>(p->workspace) % kAlign)) {
       free_handle(h);
@@ -634,7 +708,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   if (p->chain_pattern) e = cudaMemcpyAsync(h->pattern0(), p->chain_pattern, h->n_chains, cudaMemcpyHostToDevice, h->stream);
   else e = cudaMemsetAsync(h->pattern0(), 0, h->n_chains, h->stream);
   if (e != cudaSuccess) return bail(e, "chain_pattern upload");
-  e = cudaMemcpyAsync(h->patterns(), p->type_patterns, (size_t)h->n_patterns * h->N, cudaMemcpyHostToDevice, h->stream);
+  e = cudaMemcpyAsync(h->patterns(), p->type_patterns, (size_t)h->n_patterns * h->Nstride, cudaMemcpyHostToDevice, h->stream);
   if (e != cudaSuccess) return bail(e, "type_patterns upload");
   if ((e = cudaStreamSynchronize(h->stream)) != cudaSuccess) return bail(e, "create sync");   // host buffers may go away
   for (int r = 0; r < 10; ++r) {
@@ -709,14 +783,17 @@ int soma_generate_state(soma_t* h, uint64_t gen_seed, uint64_t step0) {
   h->live = 0;
   h->loaded = false;
   GenArgs G{};
-  G.n_chains = (uint32_t)h->n_chains; G.N = h->N;
   G.k0 = (uint32_t)gen_seed; G.k1 = (uint32_t)(gen_seed >> 32);
   for (int d = 0; d < 3; ++d) G.box[d] = (double)h->box[d];
   G.sigma = (double)h->b / std::sqrt(3.0);
-  G.x = h->pos(0, 0); G.y = h->pos(0, 1); G.z = h->pos(0, 2);
-  generate_state_kernel<<<blocks_for(h->n_chains, 128), 128, 0, h->stream>>>(G);
-  h->launches++;
-  CU(h, cudaGetLastError());
+  for (uint32_t k = 0; k < h->n_views; ++k) {
+    h->v = h->views[k];
+    G.n_chains = (uint32_t)h->v.n; G.N = h->v.N; G.chain0 = (uint32_t)h->v.first_chain;
+    G.x = h->vpos(0, 0); G.y = h->vpos(0, 1); G.z = h->vpos(0, 2);
+    generate_state_kernel<<<blocks_for(h->v.n, 128), 128, 0, h->stream>>>(G);
+    h->launches++;
+    CU(h, cudaGetLastError());
+  }
   if (h->S) {
     generate_singles_kernel<<<blocks_for(h->S, 256), 256, 0, h->stream>>>(
         (uint32_t)h->S, (uint32_t)h->n_chains, G.k0, G.k1, G.box[0], G.box[1], G.box[2], h->single(0), h->single(1), h->single(2));
@@ -765,25 +842,27 @@ int soma_init_from_density(soma_t* h, const float* phi_target, int dev, uint64_t
   CU(h, cudaStreamSynchronize(h->stream));                       // the caller's host array has been read
   if (bad) return fail(h, SOMA_EINVAL, "phi_target holds a negative, NaN or >= 65536 value");
   PlaceArgs P{};
-  P.n_chains = (uint32_t)h->n_chains; P.N = h->N;
   P.cells = h->cells; P.ny = h->grid.ny; P.nz = h->grid.nz;
   P.k0 = (uint32_t)gen_seed; P.k1 = (uint32_t)(gen_seed >> 32);
   P.hx = (double)h->box[0] / (double)h->grid.nx; P.hy = (double)h->box[1] / (double)h->grid.ny; P.hz = (double)h->box[2] / (double)h->grid.nz;
   P.sigma = (double)h->b / std::sqrt(3.0);
-  P.chain_pattern = h->pattern0();
   P.prefix = h->cdf();
+  for (uint32_t k = 0; k < h->n_views; ++k)                      // a chain's cell weights depend on its pattern and its length
   for (uint32_t pat = 0; pat < h->n_patterns; ++pat) {
-    if ((*h->pattern_chains)[pat] == 0) continue;
+    if ((*h->pattern_chains)[(size_t)k * h->n_patterns + pat] == 0) continue;
+    h->v = h->views[k];
+    P.n_chains = (uint32_t)h->v.n; P.N = h->v.N; P.chain0 = (uint32_t)h->v.first_chain;
+    P.chain_pattern = h->pattern0() + h->v.first_chain;
     TypeCounts M{};
-    for (uint32_t i = 0; i < h->N; ++i) M.m[(*h->host_patterns)[(size_t)pat * h->N + i]]++;
+    for (uint32_t i = 0; i < h->v.N; ++i) M.m[(*h->host_patterns)[(size_t)pat * h->Nstride + i]]++;
     cell_weight_kernel<<<blocks_for(h->cells, 256), 256, 0, h->stream>>>(h->cells, h->T, M, Q, h->cdf());
     h->launches++;
     unsigned long long total = 0;
     if ((rc = scan_weights(h, &total)) != SOMA_OK) return rc;
     if (total == 0) return fail(h, SOMA_EINVAL, "phi_target gives a chain pattern zero total weight");
     P.pattern = pat;
-    P.x = h->pos(0, 0); P.y = h->pos(0, 1); P.z = h->pos(0, 2);
-    place_chains_kernel<<<blocks_for(h->n_chains, 128), 128, 0, h->stream>>>(P);
+    P.x = h->vpos(0, 0); P.y = h->vpos(0, 1); P.z = h->vpos(0, 2);
+    place_chains_kernel<<<blocks_for(h->v.n, 128), 128, 0, h->stream>>>(P);
     h->launches++;
     CU(h, cudaGetLastError());
   }
@@ -870,11 +949,14 @@ int soma_get_positions(soma_t* h, float* x, float* y, float* z, int dev) {
   int set = h->live;
   if (!h->identity_order) {      // back to the caller's chain order through the staging set
     set = h->live ^ 1;
-    unpermute_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
-        h->B, h->N, h->slot_chain(), h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2),
-        h->pos(set, 0), h->pos(set, 1), h->pos(set, 2));
-    h->launches++;
-    CU(h, cudaGetLastError());
+    for (uint32_t k = 0; k < h->n_views; ++k) {
+      h->v = h->views[k];
+      unpermute_kernel<<<blocks_for(h->v.B, 256), 256, 0, h->stream>>>(
+          h->v.B, h->v.N, (uint32_t)h->v.first_chain, h->vslot_chain(h->live), h->vpos(h->live, 0), h->vpos(h->live, 1), h->vpos(h->live, 2),
+          h->vpos(set, 0), h->vpos(set, 1), h->vpos(set, 2));
+      h->launches++;
+      CU(h, cudaGetLastError());
+    }
   }
   for (int d = 0; d < 3; ++d)
     CU(h, cudaMemcpyAsync(dst[d], h->pos(set, d), h->B * 4,
@@ -910,8 +992,14 @@ int soma_validate_state(soma_t* h, soma_validation* out) {
   unsigned long long* report = reinterpret_cast<unsigned long long*>(h->ws + h->L.validate);
   double* bond_sum = reinterpret_cast<double*>(report + 10);
   CU(h, cudaMemsetAsync(report, 0, 11 * 8, h->stream));
-  validate_positions_kernel<<<blocks_for(h->B, 256), 256, 0, h->stream>>>(
-      h->B, h->N, h->pos(h->live, 0), h->pos(h->live, 1), h->pos(h->live, 2), report, bond_sum);
+  uint64_t n_bonds = 0;
+  for (uint32_t k = 0; k < h->n_views; ++k) {
+    h->v = h->views[k];
+    validate_positions_kernel<<<blocks_for(h->v.B, 256), 256, 0, h->stream>>>(
+        h->v.B, h->v.N, h->vpos(h->live, 0), h->vpos(h->live, 1), h->vpos(h->live, 2), report, bond_sum);
+    n_bonds += h->v.n * (uint64_t)(h->v.N - 1);
+    if (k) h->launches++;
+  }
   if (h->S) {      // N = 1 in the kernel: no bonds, only the finiteness test
     validate_positions_kernel<<<blocks_for(h->S, 256), 256, 0, h->stream>>>(h->S, 1u, h->single(0), h->single(1), h->single(2), report, bond_sum);
     h->launches++;
@@ -930,7 +1018,6 @@ int soma_validate_state(soma_t* h, soma_validation* out) {
   std::memcpy(&out->max_bond_sq, &qbits, 4);
   double sum;
   std::memcpy(&sum, &host[10], 8);
-  const uint64_t n_bonds = h->n_chains * (uint64_t)(h->N - 1);
   out->mean_bond_sq = n_bonds ? sum / (double)n_bonds : 0.0;
   out->ok = (out->n_nonfinite == 0 && out->density_total == h->Btot) ? 1u : 0u;
   return SOMA_OK;
@@ -957,8 +1044,11 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
   if (!h || !name) return fail(h, SOMA_EINVAL, "NULL argument");
   if (!std::strcmp(name, "path")) {
     if (value < 0 || value > 2) return fail(h, SOMA_EINVAL, "path must be 0, 1 or 2");
-    if (value == 2 && !fused_lanes(h->N))
-      return fail(h, SOMA_EINVAL, "fused path needs beads_per_chain = 2P, P a power of two <= 32");
+    if (value == 2) {
+      bool any = false;
+      for (uint32_t k = 0; k < h->n_views; ++k) any = any || fused_lanes(h->views[k].N) != 0;
+      if (!any) return fail(h, SOMA_EINVAL, "fused path needs beads_per_chain = 2P, P a power of two <= 32");
+    }
     h->path = (int)value;
     return SOMA_OK;
   }
@@ -1005,7 +1095,10 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
 int soma_get_counters(const soma_t* h, uint64_t* out) {
   if (!h || !out) return SOMA_EINVAL;
   out[0] = h->launches; out[1] = h->steps_done; out[2] = h->resorts;
-  out[3] = use_fused(h) ? 2 : 1;
+  out[3] = 1;
+  if (h->path != 1)
+    for (uint32_t k = 0; k < h->n_views; ++k)
+      if (fused_lanes(h->views[k].N) && !((h->Nstride & 1u) && h->n_patterns > 1)) out[3] = 2;    // a species of another length takes the generic kernels
   return SOMA_OK;
 }
 
@@ -1035,7 +1128,10 @@ int soma_debug_half_sweep(soma_t* h, uint32_t parity, uint64_t* accepted) {
   if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
   if (parity > 1) return fail(h, SOMA_EINVAL, "parity must be 0 or 1");
   CU(h, cudaMemsetAsync(h->accepted(), 0, 8, h->stream));
-  if ((rc = launch_half_sweep(h, parity)) != SOMA_OK) return rc;
+  for (uint32_t k = 0; k < h->n_views; ++k) {
+    h->v = h->views[k];
+    if ((rc = launch_half_sweep(h, parity)) != SOMA_OK) return rc;
+  }
   if (parity == 0 && (rc = launch_singles(h, true, false, nullptr)) != SOMA_OK) return rc;
   if (accepted) {
     unsigned long long v = 0;

@@ -120,13 +120,14 @@ scan_apply_kernel(uint32_t n, unsigned long long* __restrict__ v, const unsigned
 }
 
 struct PlaceArgs {
-  uint32_t n_chains, N;             // chains in the system, beads per chain
+  uint32_t n_chains, N;             // chains of the species being placed, their length
+  uint32_t chain0;                  // logical id of its first chain
   uint32_t pattern;                 // place the chains of this pattern
   uint32_t cells, ny, nz;
   uint32_t k0, k1;                  // generator seed
   double hx, hy, hz;                // cell edges, (double)box / (double)grid
   double sigma;                     // b / sqrt 3
-  const uint8_t* __restrict__ chain_pattern;          // [n_chains]
+  const uint8_t* __restrict__ chain_pattern;          // [n_chains] of this species
   const unsigned long long* __restrict__ prefix;      // [cells] inclusive prefix sums of the cell weights
   float* __restrict__ x; float* __restrict__ y; float* __restrict__ z;
 };
@@ -149,7 +150,7 @@ __device__ __forceinline__ void target_point(const PlaceArgs& A, uint32_t id, do
 }
 
 // bond i -> i+1 of the random walk of DESIGN.md R22 (domain-1 draws of bead i)
-__device__ __forceinline__ void walk_step(const PlaceArgs& A, uint32_t c, uint32_t i, double& r0, double& r1, double& r2) {
+__device__ __forceinline__ void walk_step(const PlaceArgs& A, uint32_t c /* logical id */, uint32_t i, double& r0, double& r1, double& r2) {
   const double two_pi = 6.283185307179586;
   const Words4 w = philox4x32_10(i, c, 0u, 1u << 8, A.k0, A.k1);
   const double ra = sqrt(-2.0 * log(unit_open(w.w0))), rb = sqrt(-2.0 * log(unit_open(w.w2)));
@@ -163,12 +164,13 @@ __global__ void __launch_bounds__(128)
 place_chains_kernel(PlaceArgs A) {
   const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= A.n_chains || A.chain_pattern[c] != A.pattern) return;
+  const uint32_t id = A.chain0 + c;
   double tx, ty, tz;
-  target_point(A, c, tx, ty, tz);
+  target_point(A, id, tx, ty, tz);
   // first pass: centre of mass of the walk that starts at the origin (sums in bead order)
   double r0 = 0.0, r1 = 0.0, r2 = 0.0, s0 = 0.0, s1 = 0.0, s2 = 0.0;
   for (uint32_t i = 1; i < A.N; ++i) {
-    walk_step(A, c, i, r0, r1, r2);
+    walk_step(A, id, i, r0, r1, r2);
     s0 = __dadd_rn(s0, r0); s1 = __dadd_rn(s1, r1); s2 = __dadd_rn(s2, r2);
   }
   const double b0 = __dsub_rn(tx, __ddiv_rn(s0, (double)A.N)), b1 = __dsub_rn(ty, __ddiv_rn(s1, (double)A.N)),
@@ -177,7 +179,7 @@ place_chains_kernel(PlaceArgs A) {
   const uint64_t j0 = (uint64_t)c * A.N;
   r0 = r1 = r2 = 0.0;
   for (uint32_t i = 0; i < A.N; ++i) {
-    if (i) walk_step(A, c, i, r0, r1, r2);
+    if (i) walk_step(A, id, i, r0, r1, r2);
     A.x[j0 + i] = (float)__dadd_rn(b0, r0); A.y[j0 + i] = (float)__dadd_rn(b1, r1); A.z[j0 + i] = (float)__dadd_rn(b2, r2);
   }
 }

@@ -25,6 +25,7 @@ struct StepArgs {
   uint32_t cells;             // C
   uint32_t n_chains;          // n
   uint32_t N;                 // beads per chain
+  uint32_t pat_stride;        // row length of `patterns` (= N unless the system holds species of several lengths)
   float a;                    // trial half-width
   float kb;                   // 1.5f/(b*b)
   float gA, sq2A, inv4A;      // bond-force-biased moves (R24): fl(A * 2 kb), (float)sqrt(2A), (float)(1/(4A)); gA = 0: uniform moves
@@ -180,7 +181,7 @@ half_sweep_kernel(StepArgs A, uint32_t parity, uint32_t n_par /* beads of this p
     const uint32_t i = parity + 2u * (uint32_t)(k % n_par);
     const uint64_t j = (uint64_t)slot * A.N + i;
     const uint32_t chain = A.slot_chain[slot];
-    const uint32_t type = A.patterns[(uint32_t)A.slot_pattern[slot] * A.N + i];
+    const uint32_t type = A.patterns[(uint32_t)A.slot_pattern[slot] * A.pat_stride + i];
     float rx = A.x[j], ry = A.y[j], rz = A.z[j];
     const bool has_l = i > 0, has_r = i + 1 < A.N;
     float lx = 0, ly = 0, lz = 0, qx = 0, qy = 0, qz = 0;
@@ -201,14 +202,14 @@ half_sweep_kernel(StepArgs A, uint32_t parity, uint32_t n_par /* beads of this p
 // the range in which the conversion-free floor of soma_device.cuh is exact.
 template <bool POW2>
 __global__ void __launch_bounds__(256)
-bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint64_t B, const float* __restrict__ x,
+bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint32_t pat_stride, uint64_t B, const float* __restrict__ x,
            const float* __restrict__ y, const float* __restrict__ z,
            const uint8_t* __restrict__ slot_pattern, const uint8_t* __restrict__ patterns,
            uint32_t* __restrict__ counts, uint32_t* __restrict__ range_flag) {
   const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= B) return;
   const uint32_t slot = (uint32_t)(j / N), i = (uint32_t)(j % N);
-  const uint32_t type = patterns[(uint32_t)slot_pattern[slot] * N + i];
+  const uint32_t type = patterns[(uint32_t)slot_pattern[slot] * pat_stride + i];
   const float px = x[j], py = y[j], pz = z[j];
   if (range_flag) {
     const float m = fmaxf(fabsf(__fmul_rn(px, grid.inv_hx)), fmaxf(fabsf(__fmul_rn(py, grid.inv_hy)), fabsf(__fmul_rn(pz, grid.inv_hz))));
@@ -286,7 +287,7 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
     const uint32_t chain = chain_n;
     if (wg + wpb < g_end) fetch(wg + wpb);
     if (MULTI_PAT) {
-      const uint16_t tt = *reinterpret_cast<const uint16_t*>(A.patterns + (uint32_t)A.slot_pattern[slot] * A.N + 2u * l);
+      const uint16_t tt = *reinterpret_cast<const uint16_t*>(A.patterns + (uint32_t)A.slot_pattern[slot] * A.pat_stride + 2u * l);
       type0 = tt & 0xffu; type1 = tt >> 8;
     }
     const float* om0 = A.omega + (size_t)type0 * A.cells;
@@ -554,7 +555,8 @@ generate_singles_kernel(uint32_t n_total, uint32_t first_id, uint32_t k0, uint32
 // Philox domain 1; double-precision Box-Muller and accumulation, one rounding to fp32 per coordinate.
 // ---------------------------------------------------------------------------------------------
 struct GenArgs {
-  uint32_t n_chains, N;
+  uint32_t n_chains, N;            // chains of this species and their length
+  uint32_t chain0;                 // logical id of its first chain
   uint32_t k0, k1;                 // generator seed, low and high word
   double box[3];
   double sigma;                    // b / sqrt(3)
@@ -571,7 +573,7 @@ generate_state_kernel(GenArgs G) {
   double r0 = 0.0, r1 = 0.0, r2 = 0.0;
   const uint64_t j0 = (uint64_t)c * G.N;
   for (uint32_t i = 0; i < G.N; ++i) {
-    const Words4 w = philox4x32_10(i, c, 0u, 1u << 8, G.k0, G.k1);
+    const Words4 w = philox4x32_10(i, G.chain0 + c, 0u, 1u << 8, G.k0, G.k1);
     if (i == 0) {
       r0 = G.box[0] * unit_open(w.w0); r1 = G.box[1] * unit_open(w.w1); r2 = G.box[2] * unit_open(w.w2);
     } else {
@@ -630,13 +632,13 @@ validate_density_kernel(uint32_t cells, uint32_t T, const uint32_t* __restrict__
 // ---- data movement helpers ----
 // dst[slot_chain[s]*N + i] = src[s*N + i]  (slot order -> caller's chain order), one thread per bead
 __global__ void __launch_bounds__(256)
-unpermute_kernel(uint64_t B, uint32_t N, const uint32_t* __restrict__ slot_chain,
+unpermute_kernel(uint64_t B, uint32_t N, uint32_t first_chain, const uint32_t* __restrict__ slot_chain,
                  const float* __restrict__ sx, const float* __restrict__ sy, const float* __restrict__ sz,
                  float* __restrict__ dx, float* __restrict__ dy, float* __restrict__ dz) {
   const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= B) return;
   const uint32_t slot = (uint32_t)(j / N), i = (uint32_t)(j % N);
-  const uint64_t d = (uint64_t)slot_chain[slot] * N + i;
+  const uint64_t d = (uint64_t)(slot_chain[slot] - first_chain) * N + i;
   dx[d] = sx[j]; dy[d] = sy[j]; dz[d] = sz[j];
 }
 

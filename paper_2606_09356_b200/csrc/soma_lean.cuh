@@ -30,6 +30,7 @@ struct LeanArgs {
   uint32_t ny, nz;
   uint32_t cells;                    // C
   uint32_t n_chains;
+  uint32_t pat_stride;               // row length of `patterns`
   uint32_t groups_per_block;         // warp groups per block (a multiple of the warps per block)
   float a2, ac, kb;                  // 2a, a(2^-23 - 1), 1.5/b^2
   PhiloxKeys keys;
@@ -139,7 +140,7 @@ lean_step_kernel(const __grid_constant__ LeanArgs A) {
       chain_n = __ldg(A.slot_chain + slot + STEP);
     }
     if (MULTI_PAT) {
-      const uint16_t tt = __ldg(reinterpret_cast<const uint16_t*>(A.patterns + (uint32_t)__ldg(A.slot_pattern + slot) * N) + l);
+      const uint16_t tt = __ldg(reinterpret_cast<const uint16_t*>(A.patterns + (uint32_t)__ldg(A.slot_pattern + slot) * A.pat_stride) + l);
       t0 = tt & 0xffu; t1 = tt >> 8;
     }
     const uint32_t toff0 = t0 * A.cells, toff1 = t1 * A.cells;
