@@ -69,7 +69,9 @@ typedef struct soma_params {
                                    mc_polymer_iteration performs (SURVEY.md section 8(f) row
                                    f1; R24): r' = r + A F_bonded(r) + sqrt(2A) xi, xi standard normal,
                                    accepted with min(1, e^-dE T(r'->r)/T(r->r')); move_halfwidth is then
-                                   unused.  Runs on the general fused or the generic kernels.  Units: length^2/kT  */
+                                   used only by the single-bead molecules (n_single), which have no bonded force
+                                   and keep the uniform move.  Runs on the general fused or the generic kernels;
+                                   the position range is re-verified every 256 steps.  Units: length^2/kT  */
   uint32_t grid[3];             /* cells per axis                                               */
   uint32_t reserved2;           /* must be 0                                                    */
   float box[3];                 /* periodic box lengths; cell size = box/grid                   */
@@ -101,7 +103,10 @@ typedef struct soma_params {
 /* Device bytes a handle for `p` needs (positions x2, grids, chain tables).  0 on invalid `p`. */
 uint64_t soma_workspace_bytes(const soma_params *p);
 
-/* Create a handle on the current CUDA device.  `cuda_stream` is a cudaStream_t (e.g.
+/* The problem statement becomes a handle (`north_star`: "soma_create ... whose arguments follow the paper's
+ * problem statement: chains, bead types, bond length b, chiN, kappaN, grid, box"; the model itself is PAPER.md:41,
+ * section 2: "soft, coarse-grained polymer model", harmonic bonds, non-bonded interactions through the
+ * quasi-instantaneous field; readings R1-R3, R18).  Create a handle on the current CUDA device.  `cuda_stream` is a cudaStream_t (e.g.
  * torch.cuda.current_stream().cuda_stream), NULL = the default stream.  Copies all parameters.
  * Errors: SOMA_EINVAL (bad parameter, see limits), SOMA_ENOMEM, SOMA_ECUDA.  *out is NULL on error. */
 int soma_create(const soma_params *p, void *cuda_stream, soma_t **out);
@@ -172,10 +177,18 @@ int soma_validate_state(soma_t *h, soma_validation *out);
  * n_steps == 0 is a no-op.  Errors: SOMA_ESTATE (no state loaded), SOMA_ECUDA. */
 int soma_mc_steps(soma_t *h, uint32_t n_steps, uint64_t *accepted);
 
-/* Integer bead counts of the current configuration, [T][cells] uint32. */
+/* Integer bead counts of the current configuration, [T][cells] uint32, host or device: the per-type density
+ * grids of DESIGN.md section 2 step 2 (`north_star` part (2), "re-binning all beads into per-type density
+ * grids"; the paper's update_density_fields kernel; nearest-grid-point assignment, R9), as the last
+ * soma_load_state / soma_mc_steps left them.  Host destination: synchronises.  Errors: SOMA_EINVAL (NULL),
+ * SOMA_ESTATE (no state loaded), SOMA_ECUDA. */
 int soma_get_density(soma_t *h, uint32_t *counts, int ptr_is_device);
 
-/* Current positions in the caller's (chain, bead) order, unwrapped, [B] each. */
+/* Current positions in the caller's (chain, bead) order, unwrapped, [B] each, host or device: the state the
+ * half-sweeps of DESIGN.md section 2 step 5 (`north_star` part (1); the paper's mc_polymer_iteration kernel,
+ * PAPER.md:77) have produced.  The library keeps the chains in an order of its own in memory (sorted by
+ * position); this call undoes it.  Together with soma_get_step this is a complete checkpoint.  Host
+ * destination: synchronises.  Errors: SOMA_EINVAL (NULL), SOMA_ESTATE (no state loaded), SOMA_ECUDA. */
 int soma_get_positions(soma_t *h, float *x, float *y, float *z, int ptrs_are_device);
 
 /* Current field omega, [T][cells] fp32 (helper; not in north_star's list). */
@@ -192,7 +205,9 @@ int soma_set_external_field(soma_t *h, const float *ext, int ptr_is_device);
 /* Absolute step index (step0 + steps done). */
 int soma_get_step(soma_t *h, uint64_t *step);
 
-/* Free everything the library allocated.  soma_destroy(NULL) is a no-op returning SOMA_OK. */
+/* Free everything the library allocated (the last of `north_star`'s six calls): waits for the handle's
+ * stream, frees the workspace unless the caller lent it, and the handle.  soma_destroy(NULL) is a no-op
+ * returning SOMA_OK. */
 int soma_destroy(soma_t *h);
 
 /* Text of the last error on `h` ("" if none).  h == NULL: text of the last failed soma_create /
@@ -216,6 +231,8 @@ const char *soma_last_error(const soma_t *h);
  *   "resort_now"      re-order once, now (value ignored)
  *   "fused_chunk"     warp groups (32 bead pairs each) per block of the fused kernel (default 224; tuning)
  *   "lean_threads"    threads per block of the lean kernel: 256 (default), 512 or 1024 (tuning)
+ *   "omega_x4"        0 = the one-cell-per-thread omega kernel also where the four-cells-per-thread one applies
+ *                     (cells a multiple of 4, at most 3 types; default 1; same results)
  * Errors: SOMA_EINVAL (unknown name / unsupported value). */
 int soma_set_option(soma_t *h, const char *name, int64_t value);
 

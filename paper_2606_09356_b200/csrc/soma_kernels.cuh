@@ -387,6 +387,47 @@ omega_kernel(OmegaArgs A) {
   }
 }
 
+// The same pass, four consecutive cells per thread with 128-bit loads and stores (cells a multiple of 4;
+// every cell goes through omega_cell's arithmetic, so the results are those of omega_kernel bit for bit).
+template <int T_>
+__global__ void __launch_bounds__(256)
+omega_kernel_x4(OmegaArgs A) {
+  static_assert(T_ > 0, "fixed number of types");
+  const uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) * 4u;
+  if (c >= A.cells) return;
+  uint4 n[T_];
+#pragma unroll
+  for (int s = 0; s < T_; ++s) {
+    n[s] = *reinterpret_cast<const uint4*>(A.counts + (size_t)s * A.cells + c);
+    if (A.counts_to_zero) *reinterpret_cast<uint4*>(A.counts_to_zero + (size_t)s * A.cells + c) = make_uint4(0u, 0u, 0u, 0u);
+  }
+  float4 w[T_];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    float phi[T_], tot = 0.0f;
+#pragma unroll
+    for (int s = 0; s < T_; ++s) {
+      const uint32_t cnt = k == 0 ? n[s].x : k == 1 ? n[s].y : k == 2 ? n[s].z : n[s].w;
+      phi[s] = __fmul_rn((float)cnt, A.dens_scale);
+      tot = s == 0 ? phi[0] : __fadd_rn(tot, phi[s]);
+    }
+    const float p = __fmul_rn(A.kappaN, __fsub_rn(tot, 1.0f));
+#pragma unroll
+    for (int t = 0; t < T_; ++t) {
+      float acc = p;
+#pragma unroll
+      for (int s = 0; s < T_; ++s)
+        if (s != t) acc = __fmaf_rn(A.chiN[t * T_ + s], phi[s], acc);
+      float v = __fmul_rn(A.invN, acc);
+      if (A.ext) v = __fadd_rn(v, A.ext[(size_t)t * A.cells + c + k]);
+      if (A.phi_tgt) v = __fadd_rn(v, __fmul_rn(A.umbrella_k, __fsub_rn(phi[t], A.phi_tgt[(size_t)t * A.cells + c + k])));
+      (k == 0 ? w[t].x : k == 1 ? w[t].y : k == 2 ? w[t].z : w[t].w) = v;
+    }
+  }
+#pragma unroll
+  for (int t = 0; t < T_; ++t) *reinterpret_cast<float4*>(A.omega + (size_t)t * A.cells + c) = w[t];
+}
+
 // ---------------------------------------------------------------------------------------------
 // Chain re-ordering: a counting sort of the slots by the coarse bin (cb^3 cells, row-major) that
 // holds the chain's middle bead.  key -> per-bin count and rank (one atomic with return per chain),

@@ -367,3 +367,20 @@ def test_bond_force_biased_moves_parity(case, path):
             assert g.mc_steps(upto - done, want_accepted=True) == o.mc_steps(upto - done)
             done = upto
             assert_same_state(g, o, f"{case}, bond-force-biased moves, {upto} steps")
+
+
+@pytest.mark.parametrize("x4", [0, 1])
+def test_both_omega_kernels_give_the_oracle_field(x4):
+    """omega_kernel (one cell per thread) and omega_kernel_x4 (four cells per thread, 128-bit accesses) on a
+    system where both apply, with an external field: bit-identical omega after every step."""
+    s = _custom(2500, 16, 3, [[0] * 5 + [1] * 6 + [2] * 5], None, [[0, 12, 5], [12, 0, 21], [5, 21, 0]], 35.0, (8, 12, 4), (4.0, 6.0, 2.0), 51)
+    ext = np.random.default_rng(8).normal(0.0, 0.5, size=(3, 8 * 12 * 4)).astype(np.float32)
+    o = oracle.Oracle.from_system(s)
+    o.set_external_field(ext)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s, options=dict(omega_x4=x4)) as g:
+        g.set_external_field(ext)
+        g.load_state(s.x, s.y, s.z)
+        for _ in range(3):
+            assert g.mc_steps(1, want_accepted=True) == o.mc_steps(1)
+            assert_same_state(g, o, f"omega_x4={x4}")
