@@ -267,6 +267,12 @@ int soma_debug_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, u
 int soma_debug_maps(const uint32_t *words, float *tmap, float *u, float *lnu, float *lnu_fast, uint64_t n);
 int soma_debug_accept(const float *dE, const uint32_t *words, uint8_t *decision, uint64_t n);
 int soma_debug_accept_fma(const float *dE, const uint32_t *words, uint8_t *decision, uint64_t n);
+/* Throughput of the density increments on their own (`north_star`: "the atomic throughput of the histogram"):
+ * ceil(n_ops / 64) * 64 increments by threads of 64 each into n_counters uint32 counters of a scratch buffer.
+ * mode 0: red.global at uniformly random counters; 1: red.global with the locality of the sorted melt (the 32 lanes
+ * of a warp fall into a moving window of 2048 counters); 2: red.shared at random counters of a 32 KB window per
+ * block.  *ms (host) = best of three timed launches, CUDA events.  Errors: SOMA_EINVAL, SOMA_ECUDA. */
+int soma_debug_red_throughput(uint64_t n_counters, uint64_t n_ops, int mode, double *ms);
 /* Cell index of host positions under the handle's grid/box. */
 int soma_debug_cell_index(soma_t *h, const float *x, const float *y, const float *z, uint32_t *cell,
                           uint64_t n);

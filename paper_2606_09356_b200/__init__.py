@@ -29,7 +29,7 @@ EXPORTS = (
     "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_generate_state", "soma_init_from_density", "soma_validate_state", "soma_get_step", "soma_destroy", "soma_last_error",
     "soma_set_option", "soma_get_counters", "soma_get_kernel_times", "soma_debug_half_sweep", "soma_debug_finish_step",
     "soma_debug_set_omega", "soma_debug_philox", "soma_debug_maps", "soma_debug_accept",
-    "soma_debug_accept_fma", "soma_debug_cell_index",
+    "soma_debug_accept_fma", "soma_debug_cell_index", "soma_debug_red_throughput",
 )
 
 
@@ -112,6 +112,7 @@ def load_library() -> C.CDLL:
             "soma_debug_accept": (i32, [vp, vp, vp, u64]),
             "soma_debug_accept_fma": (i32, [vp, vp, vp, u64]),
             "soma_debug_cell_index": (i32, [vp, vp, vp, vp, vp, u64]),
+            "soma_debug_red_throughput": (i32, [u64, u64, i32, C.POINTER(C.c_double)]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(L, name)
@@ -315,6 +316,13 @@ def soma_debug_cell_index(h, x, y, z) -> np.ndarray:
     out = np.empty(x.size, dtype=np.uint32)
     _check(load_library().soma_debug_cell_index(h, x.ctypes.data, y.ctypes.data, z.ctypes.data, out.ctypes.data, x.size), h)
     return out
+
+
+def soma_debug_red_throughput(n_counters: int, n_ops: int, mode: int) -> float:
+    """milliseconds of the best of three launches; see include/soma.h"""
+    ms = C.c_double(0.0)
+    _check(load_library().soma_debug_red_throughput(int(n_counters), int(n_ops), int(mode), C.byref(ms)))
+    return float(ms.value)
 
 
 # ---- convenience wrapper -----------------------------------------------------------------------

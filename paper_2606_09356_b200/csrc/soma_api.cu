@@ -1255,6 +1255,31 @@ int soma_debug_accept_fma(const float* dE, const uint32_t* words, uint8_t* decis
   return SOMA_OK;
 }
 
+int soma_debug_red_throughput(uint64_t n_counters, uint64_t n_ops, int mode, double* ms) {
+  if (!ms || n_counters == 0 || n_counters >= (1ull << 32) || n_ops == 0 || mode < 0 || mode > 2) return fail(nullptr, SOMA_EINVAL, "bad argument");
+  DevBuf c;
+  CUG(c.alloc(n_counters * 4));
+  CUG(cudaMemset(c.p, 0, n_counters * 4));
+  const uint32_t per_thread = 64;
+  const uint64_t threads = (n_ops + per_thread - 1) / per_thread;
+  cudaEvent_t e0, e1;
+  CUG(cudaEventCreate(&e0)); CUG(cudaEventCreate(&e1));
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {                                 // first pass warms up; best of the rest
+    cudaEventRecord(e0);
+    debug_red_kernel<<<blocks_for(threads, 256), 256>>>((uint32_t*)c.p, (uint32_t)n_counters, per_thread, mode);
+    cudaEventRecord(e1);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float t = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&t, e0, e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); snprintf(g_last_error, 256, "%s", cudaGetErrorString(e)); return SOMA_ECUDA; }
+    if (rep > 0 && t < best) best = t;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *ms = (double)best;
+  return SOMA_OK;
+}
+
 int soma_debug_cell_index(soma_t* h, const float* x, const float* y, const float* z, uint32_t* cell, uint64_t n) {
   int rc = check(h);
   if (rc != SOMA_OK) return rc;

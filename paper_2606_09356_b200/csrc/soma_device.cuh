@@ -149,12 +149,15 @@ __device__ __forceinline__ Words4 philox_tail(const PhiloxKeys& K, const PhiloxL
 // includes dE <= 0: then the exact rule accepts, and either m < T - band or the slow path runs).
 constexpr float kLn2 = 0.693147182464599609375f;
 constexpr float kLnT = 16.6355323791503906250f;            // 24 ln 2
-__device__ __forceinline__ bool metropolis_accept_fma(float dE, uint32_t w3) {
-  const float m = __fmaf_rn(lg2_approx(umap_int(w3)), kLn2, dE);
+// u24 = u 2^24 as a float (umap_int); this is the routine both fused kernels call and soma_debug_accept_fma tests
+__device__ __forceinline__ bool accept_fma_u24(float dE, float u24) {
+  const float m = __fmaf_rn(lg2_approx(u24), kLn2, dE);
   bool acc = m < kLnT - kLnBand;
-  if (!acc && m <= kLnT + kLnBand) acc = __fadd_rn(dE, lnu_exact(umap(w3))) <= 0.0f;
+  if (!acc && m <= kLnT + kLnBand)                              // ~6e-5 of the moves: exact logarithm
+    acc = __fadd_rn(dE, lnu_exact(__fmul_rn(u24, 0x1p-24f))) <= 0.0f;
   return acc;
 }
+__device__ __forceinline__ bool metropolis_accept_fma(float dE, uint32_t w3) { return accept_fma_u24(dE, umap_int(w3)); }
 
 // ---- standard normal deviates for the bond-force-biased move (R24) -------------------
 // fp32 Box-Muller from U = ((w >> 9) + 0.5) 2^-23 with the logarithm and sine / cosine spelled out

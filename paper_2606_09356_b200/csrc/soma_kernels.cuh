@@ -721,4 +721,31 @@ __global__ void debug_cell_kernel(Grid g, uint64_t n, const float* x, const floa
   if (k < n) out[k] = cell_of<POW2>(g, x[k], y[k], z[k]);
 }
 
+// Throughput of the density increments on their own (soma_debug_red_throughput): every thread issues `per_thread`
+// increments.  mode 0: red.global at uniformly random counters; mode 1: red.global with the locality of the sorted
+// melt (a warp's 32 lanes fall into a window of 2048 counters that moves along with the warp index); mode 2:
+// red.shared at random counters of a 32 KB window.
+__global__ void __launch_bounds__(256)
+debug_red_kernel(uint32_t* __restrict__ counters, uint32_t n_counters, uint32_t per_thread, int mode) {
+  __shared__ uint32_t win[8192];
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  if (mode == 2) {
+    for (uint32_t k = threadIdx.x; k < 8192u; k += blockDim.x) win[k] = 0u;
+    __syncthreads();
+  }
+  uint32_t h = tid * 2654435761u + 12345u;
+  const uint32_t base = (uint32_t)(((uint64_t)(tid >> 5) * 613u) % n_counters);
+  for (uint32_t k = 0; k < per_thread; ++k) {
+    h = h * 1664525u + 1013904223u;
+    const uint32_t r = h >> 8;
+    if (mode == 0) atomicAdd(counters + r % n_counters, 1u);
+    else if (mode == 1) atomicAdd(counters + (base + (r & 2047u)) % n_counters, 1u);
+    else atomicAdd(win + (r & 8191u), 1u);
+  }
+  if (mode == 2) {
+    __syncthreads();
+    if (threadIdx.x == 0 && win[h & 8191u] == 0xffffffffu) counters[0] = 1u;     // keeps the window alive
+  }
+}
+
 }  // namespace soma

@@ -65,16 +65,9 @@ __device__ __forceinline__ float lean_trial(const LeanArgs& A, float r, uint32_t
   return __fadd_rn(r, __fmaf_rn(A.a2, h, A.ac));
 }
 
-// accept iff fl(dE + lnu) <= 0 (DESIGN.md section 2 step 5.6): the arithmetic of
-// metropolis_accept_fma with u 2^24 already converted.  `live` = false forces a rejection (lanes
-// beyond the end of the block's range).
-__device__ __forceinline__ bool lean_accept(float dE, float u24, bool live) {
-  const float m = __fmaf_rn(lg2_approx(u24), kLn2, dE);
-  bool acc = (m < kLnT - kLnBand) && live;
-  if (!(m < kLnT - kLnBand) && m <= kLnT + kLnBand)            // ~6e-5 of the moves: exact logarithm
-    acc = (__fadd_rn(dE, lnu_exact(__fmul_rn(u24, 0x1p-24f))) <= 0.0f) && live;
-  return acc;
-}
+// accept iff fl(dE + lnu) <= 0 (DESIGN.md section 2 step 5.6) by accept_fma_u24 (soma_device.cuh).  `live` = false
+// forces a rejection (lanes beyond the end of the block's range).
+__device__ __forceinline__ bool lean_accept(float dE, float u24, bool live) { return accept_fma_u24(dE, u24) && live; }
 // selects spelled as selp so that the accepted state is taken by predicated moves, not by a branch
 __device__ __forceinline__ float selp_f(bool p, float a, float b) {
   float r;

@@ -175,3 +175,17 @@ def test_cell_index_matches_oracle_including_edges(soma, grid, box):
         got = g.debug_cell_index(*pts)
     want = np.array([o.cell_index(pts[0][k], pts[1][k], pts[2][k]) for k in range(n)], dtype=np.uint32)
     assert np.array_equal(got, want)
+
+
+def test_red_throughput_hook_measures_the_three_increment_modes():
+    """soma_debug_red_throughput (north_star: "the atomic throughput of the histogram"): runs, rejects bad
+    arguments, and the rates are in a sane range for a B200 (10 G/s ... 10 T/s)."""
+    import paper_2606_09356_b200 as soma
+    n_ops = 1 << 26
+    for mode in (0, 1, 2):
+        ms = soma.soma_debug_red_throughput(1 << 24, n_ops, mode)
+        rate = n_ops / (ms * 1e-3)
+        assert 1e10 < rate < 1e13, (mode, rate)
+    for bad in ((0, 100, 0), (100, 0, 0), (100, 100, 3)):
+        with pytest.raises(soma.SomaError):
+            soma.soma_debug_red_throughput(*bad)
