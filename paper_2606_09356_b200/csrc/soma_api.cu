@@ -29,6 +29,7 @@ struct Layout {            // byte offsets into the workspace
   uint64_t omega;          // [T][C] fp32
   uint64_t ext;            // [T][C] fp32 external field (used once soma_set_external_field has set one)
   uint64_t phi_tgt;        // [T][C] fp32 target concentrations of soma_init_from_density (umbrella potential)
+  uint64_t stage;          // [T][C] uint32 staging area: unpacked counters on their way to the caller
   uint64_t cdf;            // [C] uint64 prefix sums of the cell weights, then [C / kScanChunk + 2] chunk sums
   uint64_t single[3];      // [S] fp32 each: positions of the single-bead molecules (never re-ordered)
   uint64_t slot_chain[2];  // [n] uint32: logical chain id of every slot (second copy: re-order target)
@@ -62,6 +63,7 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   L.omega = off; off += align_up(TC * 4);
   L.ext = off; off += align_up(TC * 4);
   L.phi_tgt = off; off += align_up(TC * 4);
+  L.stage = off; off += align_up(TC * 4);
   L.cdf = off; off += align_up((cells + cells / 2048 + 4) * 8);
   for (int d = 0; d < 3; ++d) { L.single[d] = off; off += align_up(S * 4); }
   for (int s = 0; s < 2; ++s) { L.slot_chain[s] = off; off += align_up(n * 4); }
@@ -69,7 +71,7 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   L.patterns = off; off += align_up(pat_bytes);
   L.pattern0 = off; off += align_up(n);
   L.accepted = off; off += align_up(8);
-  L.range_flag = off; off += align_up(4);
+  L.range_flag = off; off += align_up(8);      // [0] position out of range, [1] a 16-bit density counter at kCountGuard
   L.validate = off; off += align_up(88);
   L.sort_key = off; off += align_up(n * 4);
   L.sort_rank = off; off += align_up(n * 4);
@@ -196,6 +198,13 @@ struct soma_handle {
   // state
   bool loaded;
   bool has_ext;          // an external field is set (soma_set_external_field)
+  // density counters packed two types to a word (soma_device.cuh) and omega computed on the fly by the lean kernel
+  bool packed;           // layout of both count buffers for the state that is loaded
+  int packed_opt, otf_opt;      // options "packed_counts" (default 1), "omega_otf" (default -1 = by grid size)
+  bool omega_valid;      // the omega array holds the field of the current densities
+  bool guard_seen;       // the guard flag as verify_range last read it
+  bool omega_custom;     // soma_debug_set_omega has replaced the field: the next step reads the array
+  uint64_t steps_since_guard;   // MC steps since the 16-bit fields were last checked against kCountGuard
   bool umbrella;         // the umbrella potential toward phi_tgt is on (inside soma_init_from_density)
   float umbrella_k;
   std::vector<uint8_t>* host_patterns;     // [n_patterns][N] copy of the type patterns
@@ -283,6 +292,7 @@ StepArgs step_args(const soma_handle* h) {
   A.n_chains = (uint32_t)h->v.n;
   A.N = h->v.N;
   A.pat_stride = h->Nstride;
+  A.packed = h->packed ? 1u : 0u;
   A.a = h->a;
   A.kb = h->kb;
   A.gA = h->gA; A.sq2A = h->sq2A; A.inv4A = h->inv4A;
@@ -337,11 +347,11 @@ int launch_bin_chains(soma_handle* h, uint32_t* counts, uint32_t* flag) {
   {
     if (h->pow2)
       bin_kernel<true><<<blocks_for(h->v.B, 256), 256, 0, h->stream>>>(
-          h->grid, h->cells, h->v.N, h->Nstride, h->v.B, h->vpos(h->live, 0), h->vpos(h->live, 1), h->vpos(h->live, 2),
+          h->grid, h->cells, h->v.N, h->Nstride, h->packed ? 1u : 0u, h->v.B, h->vpos(h->live, 0), h->vpos(h->live, 1), h->vpos(h->live, 2),
           h->vslot_pattern(h->live), h->patterns(), counts, flag);
     else
       bin_kernel<false><<<blocks_for(h->v.B, 256), 256, 0, h->stream>>>(
-          h->grid, h->cells, h->v.N, h->Nstride, h->v.B, h->vpos(h->live, 0), h->vpos(h->live, 1), h->vpos(h->live, 2),
+          h->grid, h->cells, h->v.N, h->Nstride, h->packed ? 1u : 0u, h->v.B, h->vpos(h->live, 0), h->vpos(h->live, 1), h->vpos(h->live, 2),
           h->vslot_pattern(h->live), h->patterns(), counts, flag);
     h->launches++;
     CU(h, cudaGetLastError());
@@ -364,6 +374,8 @@ int launch_omega(soma_handle* h) {
   A.cells = h->cells; A.T = h->T;
   A.dens_scale = h->dens_scale; A.kappaN = h->kappaN; A.invN = h->invN;
   std::memcpy(A.chiN, h->chiN, sizeof A.chiN);
+  A.packed = h->packed ? 1u : 0u;
+  A.guard_flag = h->range_flag() + 1;
   A.counts = h->counts(h->cur);
   A.counts_to_zero = h->counts(h->cur ^ 1);
   A.omega = h->omega();
@@ -380,6 +392,9 @@ int launch_omega(soma_handle* h) {
     }
     h->launches++;
     CU(h, cudaGetLastError());
+    h->omega_valid = true;
+    h->omega_custom = false;
+    h->steps_since_guard = 0;
     return SOMA_OK;
   }
   switch (h->T) {
@@ -390,16 +405,55 @@ int launch_omega(soma_handle* h) {
   }
   h->launches++;
   CU(h, cudaGetLastError());
+  h->omega_valid = true;
+  h->omega_custom = false;
+  h->steps_since_guard = 0;
+  return SOMA_OK;
+}
+
+// Does the lean kernel compute omega from the packed counters itself (soma_lean.cuh, OTF)?
+// By default where the grids are too large to stay in the caches (>= 2^20 cells: cfg3 -3.6 %, cfg4 -8.9 % per
+// step; on cfg1 / cfg2, whose grids are L2-resident, the extra arithmetic costs 2-4 %).
+bool use_otf(const soma_handle* h) {
+  const bool want = h->otf_opt < 0 ? h->cells >= (1u << 20) : h->otf_opt != 0;
+  return h->packed && want && !h->has_ext && !h->umbrella && !h->omega_custom;
+}
+
+// The omega array is computed lazily while every mover computes the field itself: make it current.
+int ensure_omega(soma_handle* h) {
+  if (h->omega_valid) return SOMA_OK;
+  OmegaArgs A{};
+  A.cells = h->cells; A.T = h->T;
+  A.dens_scale = h->dens_scale; A.kappaN = h->kappaN; A.invN = h->invN;
+  std::memcpy(A.chiN, h->chiN, sizeof A.chiN);
+  A.packed = h->packed ? 1u : 0u;
+  A.guard_flag = h->range_flag() + 1;
+  A.counts = h->counts(h->cur);
+  A.counts_to_zero = nullptr;                                  // the next buffer was zeroed when the step ended
+  A.omega = h->omega();
+  A.ext = h->has_ext ? h->ext() : nullptr;
+  A.phi_tgt = h->umbrella ? h->phi_tgt() : nullptr;
+  A.umbrella_k = h->umbrella_k;
+  const unsigned g = blocks_for(h->cells, 256);
+  switch (h->T) {
+    case 1: omega_kernel<1><<<g, 256, 0, h->stream>>>(A); break;
+    case 2: omega_kernel<2><<<g, 256, 0, h->stream>>>(A); break;
+    case 3: omega_kernel<3><<<g, 256, 0, h->stream>>>(A); break;
+    default: omega_kernel<0><<<g, 256, 0, h->stream>>>(A); break;
+  }
+  h->launches++;
+  CU(h, cudaGetLastError());
+  h->omega_valid = true;
   return SOMA_OK;
 }
 
 bool lean_ok(const soma_handle* h) {
   return h->fused_lean && h->fast_arith && h->pow2 && h->smcA == 0.0f && fused_lanes(h->v.N) != 0;
 }
-template <int P, bool MULTI, int NT>
+template <int P, bool MULTI, bool OTF, int NT>
 void launch_lean_k(soma_handle* h, LeanArgs& A) {
   constexpr int G = 32 / P;
-  auto* k = lean_step_kernel<P, MULTI, NT>;
+  auto* k = lean_step_kernel<P, MULTI, OTF, NT>;
   const uint64_t n_groups = (h->v.n + G - 1) / G;
   const uint64_t wpb = NT / 32;
   const uint64_t gpb = ((uint64_t)h->fused_chunk * (NT / 256) + wpb - 1) / wpb * wpb;   // fused_chunk is per 256 threads
@@ -409,7 +463,8 @@ void launch_lean_k(soma_handle* h, LeanArgs& A) {
 }
 template <int P, int NT>
 int launch_lean_pn(soma_handle* h, LeanArgs& A) {
-  if (h->n_patterns > 1) launch_lean_k<P, true, NT>(h, A); else launch_lean_k<P, false, NT>(h, A);
+  if (use_otf(h)) { if (h->n_patterns > 1) launch_lean_k<P, true, true, NT>(h, A); else launch_lean_k<P, false, true, NT>(h, A); }
+  else            { if (h->n_patterns > 1) launch_lean_k<P, true, false, NT>(h, A); else launch_lean_k<P, false, false, NT>(h, A); }
   h->launches++;
   CU(h, cudaGetLastError());
   return SOMA_OK;
@@ -434,6 +489,10 @@ int launch_lean_p(soma_handle* h) {
   A.ctr3_base = (0u << 8) | ((uint32_t)(h->step >> 32) << 16);   // domain 0 = MC move
   A.x = h->vpos(h->live, 0); A.y = h->vpos(h->live, 1); A.z = h->vpos(h->live, 2);
   A.omega = h->omega();
+  A.counts_prev = h->counts(h->cur);
+  A.dens_scale = h->dens_scale; A.kappaN = h->kappaN; A.invN = h->invN;
+  A.chi01 = h->T > 1 ? h->chiN[1] : 0.0f;
+  A.packed = h->packed ? 1u : 0u;
   A.counts_next = h->counts(h->cur ^ 1);
   A.slot_chain = h->vslot_chain(h->live);
   A.slot_pattern = h->vslot_pattern(h->live);
@@ -533,14 +592,34 @@ int resort(soma_handle* h) {
 // bead drifts by at most a * inv_h cells per step and axis, so the check is repeated before 2^21
 // cells of drift could have accumulated.
 int verify_range(soma_handle* h) {
-  uint32_t flag = 0;
-  CU(h, cudaMemcpyAsync(&flag, h->range_flag(), 4, cudaMemcpyDeviceToHost, h->stream));
+  uint32_t flag[2] = {0, 0};
+  CU(h, cudaMemcpyAsync(flag, h->range_flag(), 8, cudaMemcpyDeviceToHost, h->stream));
   CU(h, cudaStreamSynchronize(h->stream));
-  if (flag) {
+  h->guard_seen = flag[1] != 0;
+  if (flag[0]) {
     h->loaded = false;
     return fail(h, SOMA_EINVAL, "a position is NaN or beyond 2^21 cells from the origin");
   }
+  if (flag[1] && h->packed && h->loaded) {                       // (at load time finish_load looks at the flag itself)
+    h->loaded = false;
+    return fail(h, SOMA_EINVAL, "a cell holds 32768 or more beads of one type: 16-bit density counters would overflow; "
+                                "set option packed_counts = 0 and load the state again");
+  }
   h->steps_since_check = 0;
+  return SOMA_OK;
+}
+
+// After a call that has synchronised anyway: has a 16-bit density counter reached kCountGuard?
+int guard_check(soma_handle* h) {
+  if (!h->packed) return SOMA_OK;
+  uint32_t flag = 0;
+  CU(h, cudaMemcpyAsync(&flag, h->range_flag() + 1, 4, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  if (flag) {
+    h->loaded = false;
+    return fail(h, SOMA_EINVAL, "a cell holds 32768 or more beads of one type: 16-bit density counters would overflow; "
+                                "set option packed_counts = 0 and load the state again");
+  }
   return SOMA_OK;
 }
 
@@ -563,6 +642,13 @@ int one_step(soma_handle* h) {
   int rc;
   if (h->resort_interval > 0 && (h->steps_since_sort >= (uint64_t)h->resort_interval || !h->sorted))
     if ((rc = resort(h)) != SOMA_OK) return rc;
+  // Does anything read the omega array in this step?  The lean kernel in OTF mode computes the field itself.
+  bool needs_omega = !use_otf(h) || h->S > 0;
+  for (uint32_t k = 0; k < h->n_views && !needs_omega; ++k) {
+    h->v = h->views[k];
+    needs_omega = !(use_fused(h) && lean_ok(h));
+  }
+  if (needs_omega && (rc = ensure_omega(h)) != SOMA_OK) return rc;
   const bool timed = h->timing && h->ev_used + 3 <= 3 * kMaxTimedSteps;
   if (timed) timing_mark(h);
   // Chains interact only through omega, which is frozen during a step, so the species (and the single-bead
@@ -580,7 +666,18 @@ int one_step(soma_handle* h) {
   if ((rc = launch_singles(h, true, true, h->counts(h->cur ^ 1))) != SOMA_OK) return rc;      // a1 + a3, single-bead molecules
   h->cur ^= 1;
   if (timed) timing_mark(h);
-  if ((rc = launch_omega(h)) != SOMA_OK) return rc;              // a4
+  if (needs_omega) {
+    if ((rc = launch_omega(h)) != SOMA_OK) return rc;            // a4 (also zeroes the next count buffer)
+  } else {                                                       // a4 happens inside the next step's moves
+    CU(h, cudaMemsetAsync(h->counts(h->cur ^ 1), 0, (size_t)h->cells * 4, h->stream));
+    h->omega_valid = false;
+    if (++h->steps_since_guard >= 64) {                          // nobody has looked at the 16-bit fields for 64 steps
+      count_guard_kernel<<<1184, 256, 0, h->stream>>>(h->cells, h->counts(h->cur), h->range_flag() + 1);
+      h->launches++;
+      CU(h, cudaGetLastError());
+      h->steps_since_guard = 0;
+    }
+  }
   if (timed) timing_mark(h);
   h->step += 1;
   h->steps_done += 1;
@@ -735,6 +832,8 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->fused_carveout = -1;
   h->fused_lean = 1;
   h->omega_x4 = 1;
+  h->packed_opt = 1;
+  h->otf_opt = -1;
   h->lean_threads = 256;
   {
     auto pow2f = [](float v) { int e; return v > 0.0f && std::frexp(v, &e) == 0.5f && e > -100 && e < 100; };
@@ -764,11 +863,16 @@ int finish_load(soma_handle* h, uint64_t step0) {
   h->identity_order = true;
   h->step = step0;
   h->cur = 0;
-  CU(h, cudaMemsetAsync(h->counts(0), 0, (size_t)h->cells * h->T * 4, h->stream));
-  CU(h, cudaMemsetAsync(h->range_flag(), 0, 4, h->stream));
-  if ((rc = launch_bin(h, h->counts(0), true)) != SOMA_OK) return rc;
-  if ((rc = launch_omega(h)) != SOMA_OK) return rc;     // also zeroes counts(1)
-  if ((rc = verify_range(h)) != SOMA_OK) return rc;     // synchronises: the caller may reuse its buffers
+  h->packed = h->packed_opt && h->T <= 2;               // 16-bit counters, two types to a word (soma_device.cuh) ...
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    CU(h, cudaMemsetAsync(h->counts(0), 0, (size_t)h->cells * h->T * 4, h->stream));
+    CU(h, cudaMemsetAsync(h->range_flag(), 0, 8, h->stream));
+    if ((rc = launch_bin(h, h->counts(0), true)) != SOMA_OK) return rc;
+    if ((rc = launch_omega(h)) != SOMA_OK) return rc;   // also zeroes counts(1) and raises the guard flag
+    if ((rc = verify_range(h)) != SOMA_OK) return rc;   // synchronises: the caller may reuse its buffers
+    if (!(h->packed && h->guard_seen)) break;
+    h->packed = false;                                  // ... unless this state is too dense for them: 32-bit counters
+  }
   h->steps_since_sort = 0;
   h->sorted = false;
   if (h->resort_interval > 0)
@@ -937,6 +1041,7 @@ int soma_mc_steps(soma_t* h, uint32_t n_steps, uint64_t* accepted) {
     CU(h, cudaMemcpyAsync(&v, h->accepted(), 8, cudaMemcpyDeviceToHost, h->stream));
     CU(h, cudaStreamSynchronize(h->stream));
     *accepted = v;
+    return guard_check(h);
   }
   return SOMA_OK;
 }
@@ -946,6 +1051,15 @@ int soma_get_density(soma_t* h, uint32_t* counts, int dev) {
   if (rc != SOMA_OK) return rc;
   if (!counts) return fail(h, SOMA_EINVAL, "counts is NULL");
   if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
+  if (h->packed) {                                       // unpack into the omega-sized staging area of the next count buffer's tail
+    uint32_t* stage = reinterpret_cast<uint32_t*>(h->ws + h->L.stage);
+    unpack_counts_kernel<<<blocks_for(h->cells, 256), 256, 0, h->stream>>>(h->cells, h->T, h->counts(h->cur), stage);
+    h->launches++;
+    CU(h, cudaGetLastError());
+    rc = copy_out(h, counts, stage, (uint64_t)h->cells * h->T, dev);
+    if (rc == SOMA_OK && !dev) rc = guard_check(h);
+    return rc;
+  }
   return copy_out(h, counts, h->counts(h->cur), (uint64_t)h->cells * h->T, dev);
 }
 
@@ -954,7 +1068,10 @@ int soma_get_omega(soma_t* h, float* omega, int dev) {
   if (rc != SOMA_OK) return rc;
   if (!omega) return fail(h, SOMA_EINVAL, "omega is NULL");
   if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
-  return copy_out(h, omega, h->omega(), (uint64_t)h->cells * h->T, dev);
+  if ((rc = ensure_omega(h)) != SOMA_OK) return rc;
+  rc = copy_out(h, omega, h->omega(), (uint64_t)h->cells * h->T, dev);
+  if (rc == SOMA_OK && !dev) rc = guard_check(h);
+  return rc;
 }
 
 int soma_get_positions(soma_t* h, float* x, float* y, float* z, int dev) {
@@ -1022,7 +1139,7 @@ int soma_validate_state(soma_t* h, soma_validation* out) {
     h->launches++;
   }
   const unsigned gx = blocks_for(h->cells, 256) < 1024u ? blocks_for(h->cells, 256) : 1024u;
-  validate_density_kernel<<<dim3(gx, h->T), 256, 0, h->stream>>>(h->cells, h->T, h->counts(h->cur), report);
+  validate_density_kernel<<<dim3(gx, h->T), 256, 0, h->stream>>>(h->cells, h->T, h->packed ? 1u : 0u, h->counts(h->cur), report);
   h->launches += 2;
   CU(h, cudaGetLastError());
   unsigned long long host[11];
@@ -1091,6 +1208,16 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     h->fused_lean = (int)value;
     return SOMA_OK;
   }
+  if (!std::strcmp(name, "packed_counts")) {           // takes effect at the next soma_load_state / generate / init
+    if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "packed_counts must be 0 or 1");
+    h->packed_opt = (int)value;
+    return SOMA_OK;
+  }
+  if (!std::strcmp(name, "omega_otf")) {
+    if (value < -1 || value > 1) return fail(h, SOMA_EINVAL, "omega_otf must be -1, 0 or 1");
+    h->otf_opt = (int)value;
+    return SOMA_OK;
+  }
   if (!std::strcmp(name, "omega_x4")) {                // 0: the one-cell-per-thread omega kernel everywhere
     if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "omega_x4 must be 0 or 1");
     h->omega_x4 = (int)value;
@@ -1149,6 +1276,7 @@ int soma_debug_half_sweep(soma_t* h, uint32_t parity, uint64_t* accepted) {
   if (rc != SOMA_OK) return rc;
   if (!h->loaded) return fail(h, SOMA_ESTATE, "no state loaded");
   if (parity > 1) return fail(h, SOMA_EINVAL, "parity must be 0 or 1");
+  if ((rc = ensure_omega(h)) != SOMA_OK) return rc;
   CU(h, cudaMemsetAsync(h->accepted(), 0, 8, h->stream));
   for (uint32_t k = 0; k < h->n_views; ++k) {
     h->v = h->views[k];
@@ -1181,6 +1309,8 @@ int soma_debug_set_omega(soma_t* h, const float* omega) {
   if (!omega) return fail(h, SOMA_EINVAL, "omega is NULL");
   CU(h, cudaMemcpyAsync(h->omega(), omega, (size_t)h->cells * h->T * 4, cudaMemcpyHostToDevice, h->stream));
   CU(h, cudaStreamSynchronize(h->stream));
+  h->omega_valid = true;                                       // ... in the sense that nobody may overwrite it before the next step has used it
+  h->omega_custom = true;
   return SOMA_OK;
 }
 

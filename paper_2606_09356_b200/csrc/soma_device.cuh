@@ -201,6 +201,19 @@ __device__ __forceinline__ void smc_deviates(const Words4& w, const Words4& v, f
   x0 = __fmul_rn(ra, cs); x1 = __fmul_rn(ra, sn); x2 = __fmul_rn(rb, cs2);
 }
 
+// ---- density counters ----------------------------------------------------
+// Either one uint32 per cell and type, [T][C], or -- "packed", systems of at most two types -- one uint32 per
+// cell that holds type 0 in its low and type 1 in its high 16 bits, [C].  An increment is one atomic add of
+// 1 or 65536; a field never carries into its neighbour as long as a cell holds fewer than 65536 beads of a type
+// (kCountGuard is the level at which the library raises an error, checked when a state is loaded and at
+// least every 64 steps).
+constexpr uint32_t kCountGuard = 0x8000u;
+__device__ __forceinline__ uint32_t count_word(uint32_t type, uint32_t cells, uint32_t packed) { return packed ? 0u : type * cells; }
+__device__ __forceinline__ uint32_t count_inc(uint32_t type, uint32_t packed) { return packed ? 1u << (type << 4) : 1u; }
+__device__ __forceinline__ uint32_t count_get(const uint32_t* __restrict__ counts, uint32_t type, uint32_t cells, uint32_t c, uint32_t packed) {
+  return packed ? (counts[c] >> (type << 4)) & 0xffffu : counts[(size_t)type * cells + c];
+}
+
 // ---- geometry ----
 struct Grid {
   uint32_t nx, ny, nz;          // cells per axis

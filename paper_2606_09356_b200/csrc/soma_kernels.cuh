@@ -26,6 +26,7 @@ struct StepArgs {
   uint32_t n_chains;          // n
   uint32_t N;                 // beads per chain
   uint32_t pat_stride;        // row length of `patterns` (= N unless the system holds species of several lengths)
+  uint32_t packed;            // layout of the density counters (soma_device.cuh)
   float a;                    // trial half-width
   float kb;                   // 1.5f/(b*b)
   float gA, sq2A, inv4A;      // bond-force-biased moves (R24): fl(A * 2 kb), (float)sqrt(2A), (float)(1/(4A)); gA = 0: uniform moves
@@ -202,7 +203,7 @@ half_sweep_kernel(StepArgs A, uint32_t parity, uint32_t n_par /* beads of this p
 // the range in which the conversion-free floor of soma_device.cuh is exact.
 template <bool POW2>
 __global__ void __launch_bounds__(256)
-bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint32_t pat_stride, uint64_t B, const float* __restrict__ x,
+bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint32_t pat_stride, uint32_t packed, uint64_t B, const float* __restrict__ x,
            const float* __restrict__ y, const float* __restrict__ z,
            const uint8_t* __restrict__ slot_pattern, const uint8_t* __restrict__ patterns,
            uint32_t* __restrict__ counts, uint32_t* __restrict__ range_flag) {
@@ -215,7 +216,7 @@ bin_kernel(Grid grid, uint32_t cells, uint32_t N, uint32_t pat_stride, uint64_t 
     const float m = fmaxf(fabsf(__fmul_rn(px, grid.inv_hx)), fmaxf(fabsf(__fmul_rn(py, grid.inv_hy)), fabsf(__fmul_rn(pz, grid.inv_hz))));
     if (!(m < kCellCoordLimit)) *range_flag = 1u;            // also catches NaN
   }
-  atomicAdd(counts + (size_t)type * cells + cell_of<POW2>(grid, px, py, pz), 1u);
+  atomicAdd(counts + count_word(type, cells, packed) + cell_of<POW2>(grid, px, py, pz), count_inc(type, packed));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -329,8 +330,8 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
       __stcs(reinterpret_cast<float2*>(A.x + j), make_float2(ex, ox));
       __stcs(reinterpret_cast<float2*>(A.y + j), make_float2(ey, oy));
       __stcs(reinterpret_cast<float2*>(A.z + j), make_float2(ez, oz));
-      atomicAdd(A.counts_next + (size_t)type0 * A.cells + cell_e, 1u);
-      atomicAdd(A.counts_next + (size_t)type1 * A.cells + cell_o, 1u);
+      atomicAdd(A.counts_next + count_word(type0, A.cells, A.packed) + cell_e, count_inc(type0, A.packed));
+      atomicAdd(A.counts_next + count_word(type1, A.cells, A.packed) + cell_o, count_inc(type1, A.packed));
     }
   }
   // accepted-move count: warp reduce, one atomic per warp
@@ -347,8 +348,10 @@ struct OmegaArgs {
   uint32_t cells, T;
   float dens_scale, kappaN, invN;
   float chiN[kMaxTypes * kMaxTypes];         // [T][T]
-  const uint32_t* __restrict__ counts;       // [T][C] fresh counts
-  uint32_t* __restrict__ counts_to_zero;     // [T][C] buffer for the next step (may be null)
+  uint32_t packed;                           // layout of the counters (soma_device.cuh)
+  uint32_t* __restrict__ guard_flag;         // packed: set to 1 if a 16-bit field has reached kCountGuard
+  const uint32_t* __restrict__ counts;       // fresh counts
+  uint32_t* __restrict__ counts_to_zero;     // buffer for the next step (may be null)
   float* __restrict__ omega;                 // [T][C]
   const float* __restrict__ ext;             // [T][C] external field added to omega (R21), or null
   const float* __restrict__ phi_tgt;         // [T][C] target concentrations of the umbrella potential (R25), or null
@@ -366,9 +369,11 @@ omega_kernel(OmegaArgs A) {
 #pragma unroll
   for (uint32_t s = 0; s < (T_ > 0 ? T_ : kMaxTypes); ++s) {
     if (s < T) {
-      phi[s] = __fmul_rn((float)A.counts[(size_t)s * A.cells + c], A.dens_scale);
+      const uint32_t cnt = count_get(A.counts, s, A.cells, c, A.packed);
+      if (A.packed && cnt >= kCountGuard) *A.guard_flag = 1u;
+      phi[s] = __fmul_rn((float)cnt, A.dens_scale);
       tot = s == 0 ? phi[0] : __fadd_rn(tot, phi[s]);
-      if (A.counts_to_zero) A.counts_to_zero[(size_t)s * A.cells + c] = 0u;
+      if (A.counts_to_zero && (!A.packed || s == 0)) A.counts_to_zero[(size_t)s * A.cells + c] = 0u;
     }
   }
   const float p = __fmul_rn(A.kappaN, __fsub_rn(tot, 1.0f));
@@ -396,10 +401,19 @@ omega_kernel_x4(OmegaArgs A) {
   const uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) * 4u;
   if (c >= A.cells) return;
   uint4 n[T_];
+  if (A.packed) {                                               // T_ <= 2: both types in one word
+    const uint4 p = *reinterpret_cast<const uint4*>(A.counts + c);
+    if (A.counts_to_zero) *reinterpret_cast<uint4*>(A.counts_to_zero + c) = make_uint4(0u, 0u, 0u, 0u);
+    n[0] = make_uint4(p.x & 0xffffu, p.y & 0xffffu, p.z & 0xffffu, p.w & 0xffffu);
+    if (T_ > 1) n[T_ > 1 ? 1 : 0] = make_uint4(p.x >> 16, p.y >> 16, p.z >> 16, p.w >> 16);
+    const uint32_t hi = (p.x | p.y | p.z | p.w);
+    if ((hi & 0x8000u) || (hi >> 31)) *A.guard_flag = 1u;
+  } else {
 #pragma unroll
-  for (int s = 0; s < T_; ++s) {
-    n[s] = *reinterpret_cast<const uint4*>(A.counts + (size_t)s * A.cells + c);
-    if (A.counts_to_zero) *reinterpret_cast<uint4*>(A.counts_to_zero + (size_t)s * A.cells + c) = make_uint4(0u, 0u, 0u, 0u);
+    for (int s = 0; s < T_; ++s) {
+      n[s] = *reinterpret_cast<const uint4*>(A.counts + (size_t)s * A.cells + c);
+      if (A.counts_to_zero) *reinterpret_cast<uint4*>(A.counts_to_zero + (size_t)s * A.cells + c) = make_uint4(0u, 0u, 0u, 0u);
+    }
   }
   float4 w[T_];
 #pragma unroll
@@ -572,7 +586,7 @@ singles_kernel(SingleArgs A) {
       acc = metropolis_accept(__fmaf_rn(A.S.kb, 0.0f, dw), w.w3);
       if (acc) { rx = t.x; ry = t.y; rz = t.z; A.x[m] = rx; A.y[m] = ry; A.z[m] = rz; }
     }
-    if (A.do_bin) atomicAdd(A.counts + (size_t)type * A.S.cells + cell_of<POW2>(G, rx, ry, rz), 1u);
+    if (A.do_bin) atomicAdd(A.counts + count_word(type, A.S.cells, A.S.packed) + cell_of<POW2>(G, rx, ry, rz), count_inc(type, A.S.packed));
   }
   const unsigned n_acc = __popc(__ballot_sync(0xffffffffu, acc));
   if ((threadIdx.x & 31u) == 0 && n_acc) atomicAdd(A.S.accepted, (unsigned long long)n_acc);
@@ -661,13 +675,30 @@ validate_positions_kernel(uint64_t B, uint32_t N, const float* __restrict__ x, c
 }
 
 __global__ void __launch_bounds__(256)
-validate_density_kernel(uint32_t cells, uint32_t T, const uint32_t* __restrict__ counts, unsigned long long* __restrict__ report) {
+validate_density_kernel(uint32_t cells, uint32_t T, uint32_t packed, const uint32_t* __restrict__ counts, unsigned long long* __restrict__ report) {
   const uint32_t t = blockIdx.y;
   unsigned long long sum = 0;
-  for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < cells; c += gridDim.x * blockDim.x) sum += counts[(size_t)t * cells + c];
+  for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < cells; c += gridDim.x * blockDim.x) sum += count_get(counts, t, cells, c, packed);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
   if ((threadIdx.x & 31u) == 0 && sum) atomicAdd(report + 1 + t, sum);
+}
+
+// packed counters -> [T][C] uint32 (soma_get_density)
+__global__ void __launch_bounds__(256)
+unpack_counts_kernel(uint32_t cells, uint32_t T, const uint32_t* __restrict__ packed_counts, uint32_t* __restrict__ out) {
+  const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= cells) return;
+  const uint32_t w = packed_counts[c];
+  out[c] = w & 0xffffu;
+  if (T > 1) out[(size_t)cells + c] = w >> 16;
+}
+// sets *guard_flag if a 16-bit field of the packed counters has reached kCountGuard
+__global__ void __launch_bounds__(256)
+count_guard_kernel(uint32_t cells, const uint32_t* __restrict__ packed_counts, uint32_t* __restrict__ guard_flag) {
+  uint32_t any = 0;
+  for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < cells; c += gridDim.x * blockDim.x) any |= packed_counts[c];
+  if ((any & 0x8000u) || (any >> 31)) *guard_flag = 1u;
 }
 
 // ---- data movement helpers ----

@@ -384,3 +384,49 @@ def test_both_omega_kernels_give_the_oracle_field(x4):
         for _ in range(3):
             assert g.mc_steps(1, want_accepted=True) == o.mc_steps(1)
             assert_same_state(g, o, f"omega_x4={x4}")
+
+
+@pytest.mark.parametrize("packed,otf", [(0, 0), (1, 0), (1, 1)])
+@pytest.mark.parametrize("case", ["cfg4_scaled_noncubic", "cfg1_scaled_T1_N64", "cfg3_scaled_blend_N64"])
+def test_counter_layouts_and_on_the_fly_omega_give_the_same_trajectory(case, packed, otf):
+    """32-bit counters, 16-bit counters two types to a word, and the lean kernel computing omega from the packed
+    counters itself: the oracle's state after 1 and 10 steps in every combination, with re-orderings, a path
+    switch in the middle (the generic kernels need the omega array: it is filled on demand) and a checkpoint."""
+    s = LEAN_CASES[case]()
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s, options=dict(packed_counts=packed, omega_otf=otf, resort_interval=4)) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert_same_state(g, o, "loaded")
+        assert g.mc_steps(1, want_accepted=True) == o.mc_steps(1)
+        assert_same_state(g, o, f"{case} packed={packed} otf={otf} after 1 step")
+        g.mc_steps(3)
+        g.set_option("path", GENERIC)
+        g.mc_steps(2)
+        g.set_option("path", 0)
+        g.mc_steps(4)
+        o.mc_steps(9)
+        assert_same_state(g, o, f"{case} packed={packed} otf={otf} after 10 steps")
+        x, y, z = g.positions()
+        with gpu_system(s, options=dict(packed_counts=1 - packed)) as g2:       # resume with the other counter layout
+            g2.load_state(x, y, z, g.step)
+            assert g2.mc_steps(3, want_accepted=True) == o.mc_steps(3)
+            assert_same_state(g2, o, "resumed")
+
+
+def test_a_state_too_dense_for_16_bit_counters_falls_back_to_32_bit_ones():
+    """40000 beads of one type in one cell: the load notices (guard at 32768) and keeps 32-bit counters; the
+    trajectory is the oracle's."""
+    n = 45000
+    s = _custom(n, 2, 2, [[0, 1]], None, [[0, 3], [3, 0]], 2.0, (4, 4, 4), (2.0, 2.0, 2.0), 61)
+    s.x[:] = 0.26 + 0.001 * (np.arange(2 * n) % 7)
+    s.y[:] = 0.3
+    s.z[:] = 1.1
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    assert int(o.density().max()) == n
+    with gpu_system(s) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert_same_state(g, o, "dense state loaded")
+        assert g.mc_steps(3, want_accepted=True) == o.mc_steps(3)
+        assert_same_state(g, o, "dense state after 3 steps")
