@@ -231,13 +231,14 @@ const char *soma_last_error(const soma_t *h);
  *   "resort_now"      re-order once, now (value ignored)
  *   "fused_chunk"     warp groups (32 bead pairs each) per block of the fused kernel (default 224; tuning)
  *   "lean_threads"    threads per block of the lean kernel: 256 (default), 512 or 1024 (tuning)
- *   "packed_counts"   1 (default) = in systems of one or two types the density counters are kept as 16-bit fields,
+ *   "packed_counts"   1 = in systems of one or two types the density counters are kept as 16-bit fields,
  *                     two types to a 32-bit word, whenever no cell of the loaded state holds 32768 or more beads of a
  *                     type (decided at soma_load_state / soma_generate_state / soma_init_from_density, which fall back
  *                     to 32-bit counters by themselves); should a field reach 32768 during a run -- a 2000-fold
  *                     density peak in the configs -- the next call that synchronises fails with SOMA_EINVAL and the
- *                     state has to be loaded again with this option 0.  0 = 32-bit counters.  soma_get_density
- *                     returns uint32 [T][cells] either way.  Takes effect at the next load
+ *                     state has to be loaded again with this option 0.  0 = 32-bit counters.  -1 (default) = 1 for
+ *                     grids of 2^20 cells or more, else 0.  soma_get_density returns uint32 [T][cells] either way.
+ *                     Takes effect at the next load
  *   "omega_otf"       1 = with packed counters and neither an external field nor an umbrella potential the lean
  *                     kernel computes omega from the previous step's counters itself (DESIGN.md section 2 step 3 in
  *                     its operation order) and the omega array is only filled when it is asked for (soma_get_omega,
@@ -249,8 +250,9 @@ const char *soma_last_error(const soma_t *h);
 int soma_set_option(soma_t *h, const char *name, int64_t value);
 
 /* Counters since soma_create: [0] kernels launched by this library, [1] MC steps done,
- * [2] chain re-orderings done; [3] the kernel path the next step will take (1 or 2).
- * `out` is a host pointer to 4 uint64. */
+ * [2] chain re-orderings done; [3] the kernel path the next step will take (1 or 2); [4] 1 if the density
+ * counters of the loaded state are packed 16-bit fields; [5] 1 if the next step computes omega on the fly
+ * (options "packed_counts", "omega_otf").  `out` is a host pointer to 6 uint64. */
 int soma_get_counters(const soma_t *h, uint64_t *out);
 
 /* Device time spent since the last call (or since "kernel_timing" was switched on), summed over the

@@ -251,9 +251,10 @@ def soma_set_option(h, name: str, value: int):
 
 
 def soma_get_counters(h) -> dict:
-    out = (C.c_uint64 * 4)()
+    out = (C.c_uint64 * 6)()
     _check(load_library().soma_get_counters(h, out), h)
-    return {"launches": int(out[0]), "steps": int(out[1]), "resorts": int(out[2]), "path": int(out[3])}
+    return {"launches": int(out[0]), "steps": int(out[1]), "resorts": int(out[2]), "path": int(out[3]),
+            "packed_counts": bool(out[4]), "omega_otf": bool(out[5])}
 
 
 def soma_get_kernel_times(h) -> dict:

@@ -200,7 +200,7 @@ struct soma_handle {
   bool has_ext;          // an external field is set (soma_set_external_field)
   // density counters packed two types to a word (soma_device.cuh) and omega computed on the fly by the lean kernel
   bool packed;           // layout of both count buffers for the state that is loaded
-  int packed_opt, otf_opt;      // options "packed_counts" (default 1), "omega_otf" (default -1 = by grid size)
+  int packed_opt, otf_opt;      // options "packed_counts", "omega_otf" (default -1 = by grid size)
   bool omega_valid;      // the omega array holds the field of the current densities
   bool guard_seen;       // the guard flag as verify_range last read it
   bool omega_custom;     // soma_debug_set_omega has replaced the field: the next step reads the array
@@ -832,7 +832,7 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
   h->fused_carveout = -1;
   h->fused_lean = 1;
   h->omega_x4 = 1;
-  h->packed_opt = 1;
+  h->packed_opt = -1;
   h->otf_opt = -1;
   h->lean_threads = 256;
   {
@@ -863,7 +863,9 @@ int finish_load(soma_handle* h, uint64_t step0) {
   h->identity_order = true;
   h->step = step0;
   h->cur = 0;
-  h->packed = h->packed_opt && h->T <= 2;               // 16-bit counters, two types to a word (soma_device.cuh) ...
+  // 16-bit counters, two types to a word (soma_device.cuh), by default where the lean kernel then computes omega
+  // from them (grids of >= 2^20 cells); on small dense grids two types in one word only add contention (cfg2: +5 %) ...
+  h->packed = (h->packed_opt < 0 ? h->cells >= (1u << 20) : h->packed_opt != 0) && h->T <= 2;
   for (int attempt = 0; attempt < 2; ++attempt) {
     CU(h, cudaMemsetAsync(h->counts(0), 0, (size_t)h->cells * h->T * 4, h->stream));
     CU(h, cudaMemsetAsync(h->range_flag(), 0, 8, h->stream));
@@ -911,7 +913,7 @@ int soma_generate_state(soma_t* h, uint64_t gen_seed, uint64_t step0) {
     h->v = h->views[k];
     G.n_chains = (uint32_t)h->v.n; G.N = h->v.N; G.chain0 = (uint32_t)h->v.first_chain;
     G.x = h->vpos(0, 0); G.y = h->vpos(0, 1); G.z = h->vpos(0, 2);
-    generate_state_kernel<<<blocks_for(h->v.n, 128), 128, 0, h->stream>>>(G);
+    generate_state_kernel<<<blocks_for(h->v.n, 64), 64, 0, h->stream>>>(G);
     h->launches++;
     CU(h, cudaGetLastError());
   }
@@ -1209,7 +1211,7 @@ int soma_set_option(soma_t* h, const char* name, int64_t value) {
     return SOMA_OK;
   }
   if (!std::strcmp(name, "packed_counts")) {           // takes effect at the next soma_load_state / generate / init
-    if (value != 0 && value != 1) return fail(h, SOMA_EINVAL, "packed_counts must be 0 or 1");
+    if (value < -1 || value > 1) return fail(h, SOMA_EINVAL, "packed_counts must be -1, 0 or 1");
     h->packed_opt = (int)value;
     return SOMA_OK;
   }
@@ -1248,6 +1250,8 @@ int soma_get_counters(const soma_t* h, uint64_t* out) {
   if (h->path != 1)
     for (uint32_t k = 0; k < h->n_views; ++k)
       if (fused_lanes(h->views[k].N) && !((h->Nstride & 1u) && h->n_patterns > 1)) out[3] = 2;    // a species of another length takes the generic kernels
+  out[4] = h->packed ? 1 : 0;
+  out[5] = (out[3] == 2 && use_otf(h)) ? 1 : 0;
   return SOMA_OK;
 }
 

@@ -620,25 +620,43 @@ struct GenArgs {
 
 __device__ __forceinline__ double unit_open(uint32_t w) { return ((double)w + 0.5) * 0x1p-32; }
 
-__global__ void __launch_bounds__(128)
+// One thread per chain (the walk is sequential along the chain); the coordinates go through a per-warp tile of
+// shared memory so that the stores are 128-byte rows of one chain instead of 32 rows strided by the chain length.
+__global__ void __launch_bounds__(64)
 generate_state_kernel(GenArgs G) {
-  const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= G.n_chains) return;
+  __shared__ float tile[2][3][32][33];
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  const uint32_t c0 = blockIdx.x * blockDim.x + warp * 32u;      // first chain of this warp
+  if (c0 >= G.n_chains) return;
+  const uint32_t c = c0 + lane;
+  const bool live = c < G.n_chains;
+  const uint32_t n_here = G.n_chains - c0 < 32u ? G.n_chains - c0 : 32u;
   const double two_pi = 6.283185307179586;
   double r0 = 0.0, r1 = 0.0, r2 = 0.0;
-  const uint64_t j0 = (uint64_t)c * G.N;
-  for (uint32_t i = 0; i < G.N; ++i) {
-    const Words4 w = philox4x32_10(i, G.chain0 + c, 0u, 1u << 8, G.k0, G.k1);
-    if (i == 0) {
-      r0 = G.box[0] * unit_open(w.w0); r1 = G.box[1] * unit_open(w.w1); r2 = G.box[2] * unit_open(w.w2);
-    } else {
-      const double ra = sqrt(-2.0 * log(unit_open(w.w0))), rb = sqrt(-2.0 * log(unit_open(w.w2)));
-      const double t1 = two_pi * unit_open(w.w1), t3 = two_pi * unit_open(w.w3);
-      r0 = __dadd_rn(r0, __dmul_rn(G.sigma, __dmul_rn(ra, cos(t1))));
-      r1 = __dadd_rn(r1, __dmul_rn(G.sigma, __dmul_rn(ra, sin(t1))));
-      r2 = __dadd_rn(r2, __dmul_rn(G.sigma, __dmul_rn(rb, cos(t3))));
+  for (uint32_t i0 = 0; i0 < G.N; i0 += 32u) {
+    const uint32_t cnt = G.N - i0 < 32u ? G.N - i0 : 32u;
+    for (uint32_t k = 0; k < cnt; ++k) {
+      const uint32_t i = i0 + k;
+      if (live) {
+        const Words4 w = philox4x32_10(i, G.chain0 + c, 0u, 1u << 8, G.k0, G.k1);
+        if (i == 0) {
+          r0 = G.box[0] * unit_open(w.w0); r1 = G.box[1] * unit_open(w.w1); r2 = G.box[2] * unit_open(w.w2);
+        } else {
+          const double ra = sqrt(-2.0 * log(unit_open(w.w0))), rb = sqrt(-2.0 * log(unit_open(w.w2)));
+          const double t1 = two_pi * unit_open(w.w1), t3 = two_pi * unit_open(w.w3);
+          r0 = __dadd_rn(r0, __dmul_rn(G.sigma, __dmul_rn(ra, cos(t1))));
+          r1 = __dadd_rn(r1, __dmul_rn(G.sigma, __dmul_rn(ra, sin(t1))));
+          r2 = __dadd_rn(r2, __dmul_rn(G.sigma, __dmul_rn(rb, cos(t3))));
+        }
+      }
+      tile[warp][0][lane][k] = (float)r0; tile[warp][1][lane][k] = (float)r1; tile[warp][2][lane][k] = (float)r2;
     }
-    G.x[j0 + i] = (float)r0; G.y[j0 + i] = (float)r1; G.z[j0 + i] = (float)r2;
+    __syncwarp();
+    for (uint32_t r = 0; r < n_here; ++r) {                      // row r of the tile = beads i0 .. i0 + cnt - 1 of chain c0 + r
+      const uint64_t j = (uint64_t)(c0 + r) * G.N + i0 + lane;
+      if (lane < cnt) { G.x[j] = tile[warp][0][r][lane]; G.y[j] = tile[warp][1][r][lane]; G.z[j] = tile[warp][2][r][lane]; }
+    }
+    __syncwarp();
   }
 }
 

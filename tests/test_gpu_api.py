@@ -164,11 +164,11 @@ def test_launch_counter_counts_kernels(small):
         after = g.counters()
         assert after["steps"] - before["steps"] == 5
         assert after["launches"] - before["launches"] == 5 * 2 + 3 * (after["resorts"] - before["resorts"])   # fused move+bin, omega
-    with gpu_system(s, path=2, options=dict(omega_otf=1)) as g:      # omega computed inside the move kernel: one launch per step
+    with gpu_system(s, path=2, options=dict(packed_counts=1, omega_otf=1)) as g:      # omega computed inside the move kernel: one launch per step
         g.load_state(s.x, s.y, s.z)
         before = g.counters()
         g.mc_steps(5)
-        assert g.counters()["launches"] - before["launches"] == 5
+        assert g.counters()["launches"] - before["launches"] == 5 and g.counters()["omega_otf"] and g.counters()["packed_counts"]
         g.omega()                                                   # the array is filled when it is asked for
         assert g.counters()["launches"] - before["launches"] == 6
     with gpu_system(s, path=1) as g:

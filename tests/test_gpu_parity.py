@@ -425,7 +425,7 @@ def test_a_state_too_dense_for_16_bit_counters_falls_back_to_32_bit_ones():
     o = oracle.Oracle.from_system(s)
     o.load_state(s.x, s.y, s.z)
     assert int(o.density().max()) == n
-    with gpu_system(s) as g:
+    with gpu_system(s, options=dict(packed_counts=1)) as g:
         g.load_state(s.x, s.y, s.z)
         assert_same_state(g, o, "dense state loaded")
         assert g.mc_steps(3, want_accepted=True) == o.mc_steps(3)
