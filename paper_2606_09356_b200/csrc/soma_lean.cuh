@@ -92,12 +92,15 @@ __device__ __forceinline__ uint32_t selp_u(bool p, uint32_t a, uint32_t b) {
 // omega of (type, cell) from the packed counters of the previous step: DESIGN.md section 2 step 3 for T <= 2,
 //   phi_s = (float)n_s * dens_scale; tot = phi_0 + phi_1; p = kappaN * (tot - 1); omega_t = invN * fma(chi01, phi_other, p)
 // (T = 1: the high half of the word is zero and chi01 = 0, so tot = phi_0 + 0 and the fma adds 0 * 0: the same bits
-// as the one-type formula).  `c` carries the type in the bit above the cell index, as for the omega array.
-__device__ __forceinline__ float lean_omega_otf(const LeanArgs& A, uint32_t c) {
-  const uint32_t word = __ldg(A.counts_prev + (c & (A.cells - 1u)));
-  const float p0 = __fmul_rn((float)(word & 0xffffu), A.dens_scale), p1 = __fmul_rn((float)(word >> 16), A.dens_scale);
-  const float p = __fmul_rn(A.kappaN, __fsub_rn(__fadd_rn(p0, p1), 1.0f));
-  return __fmul_rn(A.invN, __fmaf_rn(A.chi01, c >= A.cells ? p0 : p1, p));
+// as the one-type formula).  `c` is the plain cell index; sel_own / sel_other are the byte selectors (PRMT) of the
+// bead type's own half of the word and of the other one.  phi_own + phi_other = phi_0 + phi_1 bit for bit: an
+// IEEE addition does not depend on the order of its two operands.
+__device__ __forceinline__ float lean_omega_otf(const LeanArgs& A, uint32_t c, uint32_t sel_own, uint32_t sel_other) {
+  const uint32_t word = __ldg(A.counts_prev + c);
+  const float own = __fmul_rn((float)__byte_perm(word, 0u, sel_own), A.dens_scale);
+  const float other = __fmul_rn((float)__byte_perm(word, 0u, sel_other), A.dens_scale);
+  const float p = __fmul_rn(A.kappaN, __fsub_rn(__fadd_rn(own, other), 1.0f));
+  return __fmul_rn(A.invN, __fmaf_rn(A.chi01, other, p));
 }
 
 template <int P, bool MULTI_PAT, bool OTF, int NT>
@@ -156,25 +159,27 @@ lean_step_kernel(const __grid_constant__ LeanArgs A) {
       const uint16_t tt = __ldg(reinterpret_cast<const uint16_t*>(A.patterns + (uint32_t)__ldg(A.slot_pattern + slot) * A.pat_stride) + l);
       t0 = tt & 0xffu; t1 = tt >> 8;
     }
-    const uint32_t toff0 = t0 * A.cells, toff1 = t1 * A.cells;
+    const uint32_t toff0 = OTF ? 0u : t0 * A.cells, toff1 = OTF ? 0u : t1 * A.cells;   // OTF: one word per cell, the type picks its half
+    const uint32_t sel0 = t0 ? 0x4432u : 0x4410u, sel1 = t1 ? 0x4432u : 0x4410u;         // PRMT selectors: own half of the packed word
+    const uint32_t oth0 = sel0 ^ 0x0022u, oth1 = sel1 ^ 0x0022u;
     float ex = X.x, ey = Y.x, ez = Z.x;                         // even bead 2l
     float ox = X.y, oy = Y.y, oz = Z.y;                         // odd bead 2l+1
 
     // ---- everything that does not depend on a decision: old cells, both trial positions, four gathers ----
     uint32_t cell_e = lean_cell(A, ex, ey, ez, toff0);
     uint32_t cell_o = lean_cell(A, ox, oy, oz, toff1);
-#define GATHER(c) (OTF ? lean_omega_otf(A, (c)) : __ldg(A.omega + (c)))
-    const float w_old_e = GATHER(cell_e);
-    const float w_old_o = GATHER(cell_o);
+#define GATHER(c, own, oth) (OTF ? lean_omega_otf(A, (c), (own), (oth)) : __ldg(A.omega + (c)))
+    const float w_old_e = GATHER(cell_e, sel0, oth0);
+    const float w_old_o = GATHER(cell_o, sel1, oth1);
     const uint32_t c0_1 = A.u0 ^ chain;
     const Words4 We = philox_tail(A.keys, L0, c0_1);
     const float tex = lean_trial(A, ex, We.w0), tey = lean_trial(A, ey, We.w1), tez = lean_trial(A, ez, We.w2);
     const uint32_t cell_te = lean_cell(A, tex, tey, tez, toff0);
-    const float w_new_e = GATHER(cell_te);
+    const float w_new_e = GATHER(cell_te, sel0, oth0);
     const Words4 Wo = philox_tail(A.keys, L1, c0_1);
     const float tox = lean_trial(A, ox, Wo.w0), toy = lean_trial(A, oy, Wo.w1), toz = lean_trial(A, oz, Wo.w2);
     const uint32_t cell_to = lean_cell(A, tox, toy, toz, toff1);
-    const float w_new_o = GATHER(cell_to);
+    const float w_new_o = GATHER(cell_to, sel1, oth1);
     const float u24_e = umap_int(We.w3), u24_o = umap_int(Wo.w3);
 
     // ---- half-sweep 0: even bead; left neighbour = odd bead of lane l-1, right neighbour = own odd bead ----
