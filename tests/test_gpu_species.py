@@ -119,3 +119,33 @@ def test_species_parameters_are_validated():
         assert soma.soma_workspace_bytes(p) == 0, bad
     p, keep = soma.make_params(**base, species=[(2, 8), (3, 4)])
     assert soma.soma_workspace_bytes(p) > 0
+
+
+@pytest.mark.parametrize("packed,otf", [(1, 1), (1, 0), (0, 0)])
+def test_species_and_solvent_with_packed_counters_and_on_the_fly_omega(packed, otf):
+    """Two types, three species (N = 32 and 8 on the lean kernel with omega on the fly, N = 5 on the generic
+    kernels, which read the omega array) and single-bead solvent: all of them bin into the same packed counters,
+    the omega array is filled every step because somebody needs it.  Then an external field switches the
+    on-the-fly field off, and its removal on again."""
+    s = _mix([(1500, 32), (2000, 8), (900, 5)], [[0] * 16 + [1] * 16, [1] * 8, [0, 0, 1, 1, 0]], [[0, 13], [13, 0]], 30.0,
+             (16, 16, 8), (8.0, 8.0, 4.0), 7, n_single=[700, 1300])
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    with gpu_system(s, options=dict(packed_counts=packed, omega_otf=otf, resort_interval=2)) as g:
+        g.load_state(s.x, s.y, s.z)
+        c = g.counters()
+        assert c["packed_counts"] == bool(packed) and c["omega_otf"] == bool(otf)
+        assert g.mc_steps(4, want_accepted=True) == o.mc_steps(4)
+        assert_same_state(g, o, "species + solvent")
+        ext = np.random.default_rng(3).normal(0, 0.4, size=(2, 16 * 16 * 8)).astype(np.float32)
+        g.set_external_field(ext)
+        o.set_external_field(ext)
+        assert not g.counters()["omega_otf"]
+        assert g.mc_steps(3, want_accepted=True) == o.mc_steps(3)
+        assert_same_state(g, o, "with an external field")
+        g.set_external_field(None)
+        o.set_external_field(None)
+        assert g.counters()["omega_otf"] == bool(otf)
+        assert g.mc_steps(3, want_accepted=True) == o.mc_steps(3)
+        assert_same_state(g, o, "field removed")
+        assert g.validate()["ok"]
