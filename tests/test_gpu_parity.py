@@ -430,3 +430,40 @@ def test_a_state_too_dense_for_16_bit_counters_falls_back_to_32_bit_ones():
         assert_same_state(g, o, "dense state loaded")
         assert g.mc_steps(3, want_accepted=True) == o.mc_steps(3)
         assert_same_state(g, o, "dense state after 3 steps")
+
+
+def test_a_16_bit_counter_reaching_its_guard_during_a_run_is_an_error_not_a_wrong_result():
+    """32 760 beads in one cell at load (below the guard: packed counters are used), 400 more next door and a
+    field that pulls them in: as soon as the cell holds 32 768 beads the next synchronising call fails with
+    SOMA_EINVAL; with 32-bit counters the same run goes through and matches the oracle."""
+    import paper_2606_09356_b200 as soma
+    n0, n1 = 32760, 400
+    s = _custom(n0 + n1, 1, 1, [[0]], None, [[0]], 0.0, (4, 4, 4), (2.0, 2.0, 2.0), 71)
+    rng = np.random.default_rng(5)
+    s.x[:n0] = 0.05 + 0.4 * rng.random(n0).astype(np.float32)       # cell (0, 1, 1)
+    s.x[n0:] = 0.52 + 0.05 * rng.random(n1).astype(np.float32)      # cell (1, 1, 1), just across the face
+    s.y[:] = 0.75
+    s.z[:] = 0.75
+    ext = np.zeros((1, 64), dtype=np.float32)
+    ext[0, (0 * 4 + 1) * 4 + 1] = -25.0                             # the dense cell is a deep well: beads stay, neighbours come
+    o = oracle.Oracle.from_system(s)
+    o.set_external_field(ext)
+    o.load_state(s.x, s.y, s.z)
+    o.mc_steps(6)
+    assert int(o.density().max()) >= 32768
+    with gpu_system(s, options=dict(packed_counts=1)) as g:
+        g.set_external_field(ext)
+        g.load_state(s.x, s.y, s.z)
+        assert g.counters()["packed_counts"]
+        with pytest.raises(soma.SomaError) as e:
+            for _ in range(6):
+                g.mc_steps(1, want_accepted=True)
+        assert e.value.code == soma.SOMA_EINVAL and "16-bit density counters" in str(e.value)
+        with pytest.raises(soma.SomaError) as e2:
+            g.mc_steps(1)                                           # the state is gone: load again
+        assert e2.value.code == soma.SOMA_ESTATE
+        g.set_option("packed_counts", 0)
+        g.load_state(s.x, s.y, s.z)
+        assert not g.counters()["packed_counts"]
+        assert g.mc_steps(6, want_accepted=True) > 0
+        assert_same_state(g, o, "the same run on 32-bit counters")
