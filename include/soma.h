@@ -231,12 +231,15 @@ const char *soma_last_error(const soma_t *h);
  *   "resort_now"      re-order once, now (value ignored)
  *   "fused_chunk"     warp groups (32 bead pairs each) per block of the fused kernel (default 224; tuning)
  *   "lean_threads"    threads per block of the lean kernel: 256 (default), 512 or 1024 (tuning)
- *   "packed_counts"   1 = in systems of one or two types the density counters are kept as 16-bit fields,
- *                     two types to a 32-bit word, whenever no cell of the loaded state holds 32768 or more beads of a
- *                     type (decided at soma_load_state / soma_generate_state / soma_init_from_density, which fall back
- *                     to 32-bit counters by themselves); should a field reach 32768 during a run -- a 2000-fold
- *                     density peak in the configs -- the next call that synchronises fails with SOMA_EINVAL and the
- *                     state has to be loaded again with this option 0.  0 = 32-bit counters.  -1 (default) = 1 for
+ *   "packed_counts"   1 = in systems of one or two types (uniform moves) the density counters are kept as 16-bit fields,
+ *                     two types to a 32-bit word, whenever no cell of the loaded state holds G or more beads of a type,
+ *                     G = the guard level: the largest power of two with ((2r+1)^3 + 1) G <= 65536, r = the move reach
+ *                     in cells (r = 1: G = 2048, a hundred times the configs' densities).  Decided at soma_load_state /
+ *                     soma_generate_state / soma_init_from_density, which fall back to 32-bit counters by themselves.
+ *                     Every non-empty cell is looked at in every step; should a field reach G during a run, the next
+ *                     call that synchronises fails with SOMA_EINVAL (before any field can have wrapped: one step adds
+ *                     at most the beads of the (2r+1)^3 cells around) and the state has to be loaded again with this
+ *                     option 0.  0 = 32-bit counters.  -1 (default) = 1 for
  *                     grids of 2^20 cells or more, else 0.  soma_get_density returns uint32 [T][cells] either way.
  *                     Takes effect at the next load
  *   "omega_otf"       1 = with packed counters and neither an external field nor an umbrella potential the lean

@@ -71,7 +71,7 @@ Layout make_layout(uint64_t B, uint64_t n, uint64_t TC, uint64_t pat_bytes, uint
   L.patterns = off; off += align_up(pat_bytes);
   L.pattern0 = off; off += align_up(n);
   L.accepted = off; off += align_up(8);
-  L.range_flag = off; off += align_up(8);      // [0] position out of range, [1] a 16-bit density counter at kCountGuard
+  L.range_flag = off; off += align_up(8);      // [0] position out of range, [1] a 16-bit density counter at its guard level
   L.validate = off; off += align_up(88);
   L.sort_key = off; off += align_up(n * 4);
   L.sort_rank = off; off += align_up(n * 4);
@@ -204,7 +204,7 @@ struct soma_handle {
   bool omega_valid;      // the omega array holds the field of the current densities
   bool guard_seen;       // the guard flag as verify_range last read it
   bool omega_custom;     // soma_debug_set_omega has replaced the field: the next step reads the array
-  uint64_t steps_since_guard;   // MC steps since the 16-bit fields were last checked against kCountGuard
+  uint32_t guard_mask;   // bits of a packed word that are set once a 16-bit field has reached the guard level (soma_device.cuh); 0: never pack
   bool umbrella;         // the umbrella potential toward phi_tgt is on (inside soma_init_from_density)
   float umbrella_k;
   std::vector<uint8_t>* host_patterns;     // [n_patterns][N] copy of the type patterns
@@ -375,6 +375,7 @@ int launch_omega(soma_handle* h) {
   A.dens_scale = h->dens_scale; A.kappaN = h->kappaN; A.invN = h->invN;
   std::memcpy(A.chiN, h->chiN, sizeof A.chiN);
   A.packed = h->packed ? 1u : 0u;
+  A.guard_mask = h->guard_mask;
   A.guard_flag = h->range_flag() + 1;
   A.counts = h->counts(h->cur);
   A.counts_to_zero = h->counts(h->cur ^ 1);
@@ -394,7 +395,6 @@ int launch_omega(soma_handle* h) {
     CU(h, cudaGetLastError());
     h->omega_valid = true;
     h->omega_custom = false;
-    h->steps_since_guard = 0;
     return SOMA_OK;
   }
   switch (h->T) {
@@ -407,7 +407,6 @@ int launch_omega(soma_handle* h) {
   CU(h, cudaGetLastError());
   h->omega_valid = true;
   h->omega_custom = false;
-  h->steps_since_guard = 0;
   return SOMA_OK;
 }
 
@@ -427,6 +426,7 @@ int ensure_omega(soma_handle* h) {
   A.dens_scale = h->dens_scale; A.kappaN = h->kappaN; A.invN = h->invN;
   std::memcpy(A.chiN, h->chiN, sizeof A.chiN);
   A.packed = h->packed ? 1u : 0u;
+  A.guard_mask = h->guard_mask;
   A.guard_flag = h->range_flag() + 1;
   A.counts = h->counts(h->cur);
   A.counts_to_zero = nullptr;                                  // the next buffer was zeroed when the step ended
@@ -493,6 +493,8 @@ int launch_lean_p(soma_handle* h) {
   A.dens_scale = h->dens_scale; A.kappaN = h->kappaN; A.invN = h->invN;
   A.chi01 = h->T > 1 ? h->chiN[1] : 0.0f;
   A.packed = h->packed ? 1u : 0u;
+  A.guard_mask = h->guard_mask;
+  A.guard_flag = h->range_flag() + 1;
   A.counts_next = h->counts(h->cur ^ 1);
   A.slot_chain = h->vslot_chain(h->live);
   A.slot_pattern = h->vslot_pattern(h->live);
@@ -602,14 +604,14 @@ int verify_range(soma_handle* h) {
   }
   if (flag[1] && h->packed && h->loaded) {                       // (at load time finish_load looks at the flag itself)
     h->loaded = false;
-    return fail(h, SOMA_EINVAL, "a cell holds 32768 or more beads of one type: 16-bit density counters would overflow; "
-                                "set option packed_counts = 0 and load the state again");
+    return fail(h, SOMA_EINVAL, "a cell holds more beads of one type than the guard level of the 16-bit density counters "
+                                "allows (2048 for moves of at most one cell): set option packed_counts = 0 and load the state again");
   }
   h->steps_since_check = 0;
   return SOMA_OK;
 }
 
-// After a call that has synchronised anyway: has a 16-bit density counter reached kCountGuard?
+// After a call that has synchronised anyway: has a 16-bit density counter reached its guard level?
 int guard_check(soma_handle* h) {
   if (!h->packed) return SOMA_OK;
   uint32_t flag = 0;
@@ -617,8 +619,8 @@ int guard_check(soma_handle* h) {
   CU(h, cudaStreamSynchronize(h->stream));
   if (flag) {
     h->loaded = false;
-    return fail(h, SOMA_EINVAL, "a cell holds 32768 or more beads of one type: 16-bit density counters would overflow; "
-                                "set option packed_counts = 0 and load the state again");
+    return fail(h, SOMA_EINVAL, "a cell holds more beads of one type than the guard level of the 16-bit density counters "
+                                "allows (2048 for moves of at most one cell): set option packed_counts = 0 and load the state again");
   }
   return SOMA_OK;
 }
@@ -670,13 +672,7 @@ int one_step(soma_handle* h) {
     if ((rc = launch_omega(h)) != SOMA_OK) return rc;            // a4 (also zeroes the next count buffer)
   } else {                                                       // a4 happens inside the next step's moves
     CU(h, cudaMemsetAsync(h->counts(h->cur ^ 1), 0, (size_t)h->cells * 4, h->stream));
-    h->omega_valid = false;
-    if (++h->steps_since_guard >= 64) {                          // nobody has looked at the 16-bit fields for 64 steps
-      count_guard_kernel<<<1184, 256, 0, h->stream>>>(h->cells, h->counts(h->cur), h->range_flag() + 1);
-      h->launches++;
-      CU(h, cudaGetLastError());
-      h->steps_since_guard = 0;
-    }
+    h->omega_valid = false;                                      // (the lean kernel's old-cell gathers look at the 16-bit fields)
   }
   if (timed) timing_mark(h);
   h->step += 1;
@@ -841,6 +837,17 @@ int soma_create(const soma_params* p, void* cuda_stream, soma_t** out) {
                    h->grid.inv_hx >= 1.0f && h->grid.inv_hy >= 1.0f && h->grid.inv_hz >= 1.0f;
   }
   const double cells_per_step = (double)h->a * (double)fmaxf(h->grid.inv_hx, fmaxf(h->grid.inv_hy, h->grid.inv_hz));
+  {
+    // guard level of the packed 16-bit counters (soma_device.cuh): largest power of two G with ((2r+1)^3 + 1) G <= 65536
+    h->guard_mask = 0;
+    const double r = std::ceil(cells_per_step > 1.0 ? cells_per_step : 1.0);
+    const double span = (2.0 * r + 1.0) * (2.0 * r + 1.0) * (2.0 * r + 1.0) + 1.0;
+    if (h->smcA == 0.0f && span <= 1024.0) {                     // G >= 64
+      uint32_t G = 32768u;
+      while ((double)G * span > 65536.0) G >>= 1;
+      h->guard_mask = (~(G - 1u) & 0xffffu) * 0x00010001u;
+    }
+  }
   const double k = cells_per_step > 0.0 ? 2097152.0 / cells_per_step : 1e18;
   h->range_check_interval = k >= 1e18 ? (1ull << 60) : (k < 1.0 ? 1ull : (uint64_t)k);
   // Bond-force-biased moves are Gaussian, not bounded by a: a step beyond 8 standard deviations (sqrt(2A) per
@@ -865,8 +872,8 @@ int finish_load(soma_handle* h, uint64_t step0) {
   h->cur = 0;
   // 16-bit counters, two types to a word (soma_device.cuh), by default where the lean kernel then computes omega
   // from them (grids of >= 2^20 cells); on small dense grids two types in one word only add contention (cfg2: +5 %) ...
-  // (and not under bond-force-biased moves, which run on the general fused kernel and read the omega array: +4.6 %)
-  h->packed = (h->packed_opt < 0 ? (h->cells >= (1u << 20) && h->smcA == 0.0f) : h->packed_opt != 0) && h->T <= 2;
+  // (never under bond-force-biased moves: their reach per step is unbounded, and they read the omega array anyway)
+  h->packed = (h->packed_opt < 0 ? h->cells >= (1u << 20) : h->packed_opt != 0) && h->T <= 2 && h->guard_mask != 0;
   for (int attempt = 0; attempt < 2; ++attempt) {
     CU(h, cudaMemsetAsync(h->counts(0), 0, (size_t)h->cells * h->T * 4, h->stream));
     CU(h, cudaMemsetAsync(h->range_flag(), 0, 8, h->stream));

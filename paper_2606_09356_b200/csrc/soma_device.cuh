@@ -204,10 +204,15 @@ __device__ __forceinline__ void smc_deviates(const Words4& w, const Words4& v, f
 // ---- density counters ----------------------------------------------------
 // Either one uint32 per cell and type, [T][C], or -- "packed", systems of at most two types -- one uint32 per
 // cell that holds type 0 in its low and type 1 in its high 16 bits, [C].  An increment is one atomic add of
-// 1 or 65536; a field never carries into its neighbour as long as a cell holds fewer than 65536 beads of a type
-// (kCountGuard is the level at which the library raises an error, checked when a state is loaded and at
-// least every 64 steps).
-constexpr uint32_t kCountGuard = 0x8000u;
+// 1 or 65536; a field never carries into its neighbour as long as a cell holds fewer than 65536 beads of a type.
+// That is guaranteed, not assumed: with a move reach of r cells per step and axis a cell can receive, in one
+// step, at most the beads of the (2r+1)^3 cells around it.  The guard level G is the largest power of two with
+// ((2r+1)^3 + 1) G <= 65536 (r = 1: 2048 beads of one type in a cell -- two orders of magnitude above the
+// configs' densities); the word of every non-empty cell is inspected in every step (by the omega pass, or by the
+// old-cell gathers of the lean kernel when it computes omega itself), and a field that has reached G raises a
+// flag that fails the next synchronising call.  While no flag is up every field is < G, so after one more
+// step every field is < (2r+1)^3 G <= 65536 - G: it cannot have wrapped before it is seen.
+// guard_mask = ~(G - 1) on both halves of a word, e.g. 0xF800F800.
 __device__ __forceinline__ uint32_t count_word(uint32_t type, uint32_t cells, uint32_t packed) { return packed ? 0u : type * cells; }
 __device__ __forceinline__ uint32_t count_inc(uint32_t type, uint32_t packed) { return packed ? 1u << (type << 4) : 1u; }
 __device__ __forceinline__ uint32_t count_get(const uint32_t* __restrict__ counts, uint32_t type, uint32_t cells, uint32_t c, uint32_t packed) {

@@ -349,7 +349,8 @@ struct OmegaArgs {
   float dens_scale, kappaN, invN;
   float chiN[kMaxTypes * kMaxTypes];         // [T][T]
   uint32_t packed;                           // layout of the counters (soma_device.cuh)
-  uint32_t* __restrict__ guard_flag;         // packed: set to 1 if a 16-bit field has reached kCountGuard
+  uint32_t guard_mask;                       // packed: bits of a word that are set once a 16-bit field has reached the guard level
+  uint32_t* __restrict__ guard_flag;         // packed: set to 1 if that happened
   const uint32_t* __restrict__ counts;       // fresh counts
   uint32_t* __restrict__ counts_to_zero;     // buffer for the next step (may be null)
   float* __restrict__ omega;                 // [T][C]
@@ -370,7 +371,7 @@ omega_kernel(OmegaArgs A) {
   for (uint32_t s = 0; s < (T_ > 0 ? T_ : kMaxTypes); ++s) {
     if (s < T) {
       const uint32_t cnt = count_get(A.counts, s, A.cells, c, A.packed);
-      if (A.packed && cnt >= kCountGuard) *A.guard_flag = 1u;
+      if (A.packed && (cnt & A.guard_mask)) *A.guard_flag = 1u;
       phi[s] = __fmul_rn((float)cnt, A.dens_scale);
       tot = s == 0 ? phi[0] : __fadd_rn(tot, phi[s]);
       if (A.counts_to_zero && (!A.packed || s == 0)) A.counts_to_zero[(size_t)s * A.cells + c] = 0u;
@@ -406,8 +407,7 @@ omega_kernel_x4(OmegaArgs A) {
     if (A.counts_to_zero) *reinterpret_cast<uint4*>(A.counts_to_zero + c) = make_uint4(0u, 0u, 0u, 0u);
     n[0] = make_uint4(p.x & 0xffffu, p.y & 0xffffu, p.z & 0xffffu, p.w & 0xffffu);
     if (T_ > 1) n[T_ > 1 ? 1 : 0] = make_uint4(p.x >> 16, p.y >> 16, p.z >> 16, p.w >> 16);
-    const uint32_t hi = (p.x | p.y | p.z | p.w);
-    if ((hi & 0x8000u) || (hi >> 31)) *A.guard_flag = 1u;
+    if ((p.x | p.y | p.z | p.w) & A.guard_mask) *A.guard_flag = 1u;
   } else {
 #pragma unroll
     for (int s = 0; s < T_; ++s) {
@@ -710,13 +710,6 @@ unpack_counts_kernel(uint32_t cells, uint32_t T, const uint32_t* __restrict__ pa
   const uint32_t w = packed_counts[c];
   out[c] = w & 0xffffu;
   if (T > 1) out[(size_t)cells + c] = w >> 16;
-}
-// sets *guard_flag if a 16-bit field of the packed counters has reached kCountGuard
-__global__ void __launch_bounds__(256)
-count_guard_kernel(uint32_t cells, const uint32_t* __restrict__ packed_counts, uint32_t* __restrict__ guard_flag) {
-  uint32_t any = 0;
-  for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < cells; c += gridDim.x * blockDim.x) any |= packed_counts[c];
-  if ((any & 0x8000u) || (any >> 31)) *guard_flag = 1u;
 }
 
 // ---- data movement helpers ----

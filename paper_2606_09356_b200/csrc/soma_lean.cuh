@@ -49,6 +49,8 @@ struct LeanArgs {
   const uint32_t* __restrict__ counts_prev;  // OTF: packed counters of the previous step, [C]
   float dens_scale, kappaN, invN, chi01;     // OTF: the constants of DESIGN.md section 2 step 3 (chi01 = chiN[0][1])
   uint32_t packed;                           // layout of the density counters (soma_device.cuh)
+  uint32_t guard_mask;                       // OTF: see soma_device.cuh
+  uint32_t* __restrict__ guard_flag;
   uint32_t* __restrict__ counts_next;        // zeroed before the launch
   const uint32_t* __restrict__ slot_chain;
   const uint8_t* __restrict__ slot_pattern;
@@ -95,8 +97,13 @@ __device__ __forceinline__ uint32_t selp_u(bool p, uint32_t a, uint32_t b) {
 // as the one-type formula).  `c` is the plain cell index; sel_own / sel_other are the byte selectors (PRMT) of the
 // bead type's own half of the word and of the other one.  phi_own + phi_other = phi_0 + phi_1 bit for bit: an
 // IEEE addition does not depend on the order of its two operands.
-__device__ __forceinline__ float lean_omega_otf(const LeanArgs& A, uint32_t c, uint32_t sel_own, uint32_t sel_other) {
+// `seen` collects the words of the old cells: every non-empty cell is some bead's old cell, so or-ing them and testing
+// the guard bits once per thread inspects every counter in every step (soma_device.cuh).  (Measured on cfg4: this
+// form 0.951 ms per launch, a predicate instead 0.960, a predicated store per gather 0.973, no guard 0.942.)
+template <bool GUARD>
+__device__ __forceinline__ float lean_omega_otf(const LeanArgs& A, uint32_t c, uint32_t sel_own, uint32_t sel_other, uint32_t& seen) {
   const uint32_t word = __ldg(A.counts_prev + c);
+  if (GUARD) seen |= word;
   const float own = __fmul_rn((float)__byte_perm(word, 0u, sel_own), A.dens_scale);
   const float other = __fmul_rn((float)__byte_perm(word, 0u, sel_other), A.dens_scale);
   const float p = __fmul_rn(A.kappaN, __fsub_rn(__fadd_rn(own, other), 1.0f));
@@ -130,6 +137,7 @@ lean_step_kernel(const __grid_constant__ LeanArgs A) {
     t0 = tt & 0xffu; t1 = tt >> 8;
   }
   unsigned n_acc = 0;
+  uint32_t seen = 0;                                            // OTF: or of the old cells' counter words
   const float2* __restrict__ x2 = reinterpret_cast<const float2*>(A.x);
   const float2* __restrict__ y2 = reinterpret_cast<const float2*>(A.y);
   const float2* __restrict__ z2 = reinterpret_cast<const float2*>(A.z);
@@ -168,9 +176,9 @@ lean_step_kernel(const __grid_constant__ LeanArgs A) {
     // ---- everything that does not depend on a decision: old cells, both trial positions, four gathers ----
     uint32_t cell_e = lean_cell(A, ex, ey, ez, toff0);
     uint32_t cell_o = lean_cell(A, ox, oy, oz, toff1);
-#define GATHER(c, own, oth) (OTF ? lean_omega_otf(A, (c), (own), (oth)) : __ldg(A.omega + (c)))
-    const float w_old_e = GATHER(cell_e, sel0, oth0);
-    const float w_old_o = GATHER(cell_o, sel1, oth1);
+#define GATHER(c, own, oth) (OTF ? lean_omega_otf<false>(A, (c), (own), (oth), seen) : __ldg(A.omega + (c)))
+    const float w_old_e = OTF ? lean_omega_otf<true>(A, cell_e, sel0, oth0, seen) : __ldg(A.omega + cell_e);
+    const float w_old_o = OTF ? lean_omega_otf<true>(A, cell_o, sel1, oth1, seen) : __ldg(A.omega + cell_o);
     const uint32_t c0_1 = A.u0 ^ chain;
     const Words4 We = philox_tail(A.keys, L0, c0_1);
     const float tex = lean_trial(A, ex, We.w0), tey = lean_trial(A, ey, We.w1), tez = lean_trial(A, ez, We.w2);
@@ -230,6 +238,7 @@ lean_step_kernel(const __grid_constant__ LeanArgs A) {
     }
   }
 
+  if (OTF && (seen & A.guard_mask)) *A.guard_flag = 1u;
   // accepted-move count: warp reduce, one atomic per warp
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) n_acc += __shfl_xor_sync(0xffffffffu, n_acc, o);

@@ -415,7 +415,7 @@ def test_counter_layouts_and_on_the_fly_omega_give_the_same_trajectory(case, pac
 
 
 def test_a_state_too_dense_for_16_bit_counters_falls_back_to_32_bit_ones():
-    """40000 beads of one type in one cell: the load notices (guard at 32768) and keeps 32-bit counters; the
+    """45000 beads of each type in one cell: the load notices (guard level 2048) and keeps 32-bit counters; the
     trajectory is the oracle's."""
     n = 45000
     s = _custom(n, 2, 2, [[0, 1]], None, [[0, 3], [3, 0]], 2.0, (4, 4, 4), (2.0, 2.0, 2.0), 61)
@@ -433,11 +433,11 @@ def test_a_state_too_dense_for_16_bit_counters_falls_back_to_32_bit_ones():
 
 
 def test_a_16_bit_counter_reaching_its_guard_during_a_run_is_an_error_not_a_wrong_result():
-    """32 760 beads in one cell at load (below the guard: packed counters are used), 400 more next door and a
-    field that pulls them in: as soon as the cell holds 32 768 beads the next synchronising call fails with
-    SOMA_EINVAL; with 32-bit counters the same run goes through and matches the oracle."""
+    """2040 beads in one cell at load (below the guard level of 2048 for one-cell moves: packed counters are used),
+    400 more next door and a field that pulls them in: as soon as the cell holds 2048 beads the next synchronising
+    call fails with SOMA_EINVAL; with 32-bit counters the same run goes through and matches the oracle."""
     import paper_2606_09356_b200 as soma
-    n0, n1 = 32760, 400
+    n0, n1 = 2040, 400
     s = _custom(n0 + n1, 1, 1, [[0]], None, [[0]], 0.0, (4, 4, 4), (2.0, 2.0, 2.0), 71)
     rng = np.random.default_rng(5)
     s.x[:n0] = 0.05 + 0.4 * rng.random(n0).astype(np.float32)       # cell (0, 1, 1)
@@ -450,7 +450,7 @@ def test_a_16_bit_counter_reaching_its_guard_during_a_run_is_an_error_not_a_wron
     o.set_external_field(ext)
     o.load_state(s.x, s.y, s.z)
     o.mc_steps(6)
-    assert int(o.density().max()) >= 32768
+    assert int(o.density().max()) >= 2048
     with gpu_system(s, options=dict(packed_counts=1)) as g:
         g.set_external_field(ext)
         g.load_state(s.x, s.y, s.z)
