@@ -330,8 +330,11 @@ fused_step_kernel(StepArgs A, uint32_t groups_per_block) {
       __stcs(reinterpret_cast<float2*>(A.x + j), make_float2(ex, ox));
       __stcs(reinterpret_cast<float2*>(A.y + j), make_float2(ey, oy));
       __stcs(reinterpret_cast<float2*>(A.z + j), make_float2(ez, oz));
-      atomicAdd(A.counts_next + count_word(type0, A.cells, A.packed) + cell_e, count_inc(type0, A.packed));
-      atomicAdd(A.counts_next + count_word(type1, A.cells, A.packed) + cell_o, count_inc(type1, A.packed));
+      {
+        const uint32_t pk = SMC ? 0u : A.packed;                  // bond-force-biased moves never run on packed counters (soma_device.cuh)
+        atomicAdd(A.counts_next + count_word(type0, A.cells, pk) + cell_e, count_inc(type0, pk));
+        atomicAdd(A.counts_next + count_word(type1, A.cells, pk) + cell_o, count_inc(type1, pk));
+      }
     }
   }
   // accepted-move count: warp reduce, one atomic per warp
