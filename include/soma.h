@@ -97,7 +97,9 @@ typedef struct soma_params {
                                    max(species_beads) long and a chain uses the first species_beads[s] entries of
                                    its row; beads_per_chain is then only the reference chain length N of chiN,
                                    kappaN and of the 1/N in omega.  A species whose length is not 2P (P a power of
-                                   two <= 32) runs on the generic kernels, the others on the fused one.          */
+                                   two <= 32), or whose first bead lies at an odd offset in the position arrays
+                                   (an odd number of beads before it), runs on the generic kernels, the others
+                                   on the fused one.                                                             */
 } soma_params;
 
 /* Device bytes a handle for `p` needs (positions x2, grids, chain tables).  0 on invalid `p`. */

@@ -551,6 +551,7 @@ int launch_fused(soma_handle* h) {
 bool use_fused(const soma_handle* h) {
   if (h->path == 1) return false;
   if ((h->Nstride & 1u) && h->n_patterns > 1) return false;     // the fused kernels read a lane's two types as one aligned 16-bit word
+  if (h->v.bead_off & 1u) return false;                          // ... and a lane's two beads as one aligned 64-bit word
   return fused_lanes(h->v.N) != 0;
 }
 // Re-order the chains in memory by the coarse bin (cube of kSortBinEdge cells) of their centre of
@@ -1257,7 +1258,7 @@ int soma_get_counters(const soma_t* h, uint64_t* out) {
   out[3] = 1;
   if (h->path != 1)
     for (uint32_t k = 0; k < h->n_views; ++k)
-      if (fused_lanes(h->views[k].N) && !((h->Nstride & 1u) && h->n_patterns > 1)) out[3] = 2;    // a species of another length takes the generic kernels
+      if (fused_lanes(h->views[k].N) && !((h->Nstride & 1u) && h->n_patterns > 1) && !(h->views[k].bead_off & 1u)) out[3] = 2;    // a species of another length takes the generic kernels
   out[4] = h->packed ? 1 : 0;
   out[5] = (out[3] == 2 && use_otf(h)) ? 1 : 0;
   return SOMA_OK;

@@ -468,8 +468,8 @@ chain_key_kernel(SortArgs S, const float* __restrict__ x, const float* __restric
   if (s >= S.n_chains) return;
   const uint64_t j0 = (uint64_t)s * S.N;
   float sx = 0.f, sy = 0.f, sz = 0.f;
-  if ((S.N & 3u) == 0) {
-    for (uint32_t i = 0; i < S.N; i += 4) {
+  if ((S.N & 3u) == 0 && ((reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(y) | reinterpret_cast<uintptr_t>(z)) & 15u) == 0) {
+    for (uint32_t i = 0; i < S.N; i += 4) {    // (a species may start at any bead offset: 128-bit loads only where they are aligned)
       const float4 a = *reinterpret_cast<const float4*>(x + j0 + i);
       const float4 b = *reinterpret_cast<const float4*>(y + j0 + i);
       const float4 c = *reinterpret_cast<const float4*>(z + j0 + i);
