@@ -576,6 +576,13 @@ int resort(soma_handle* h) {
       chain_key_kernel<false><<<blocks_for(h->v.n, 256), 256, 0, h->stream>>>(
           S, h->vpos(src, 0), h->vpos(src, 1), h->vpos(src, 2), h->sort_bins(), key, rank);
     bin_scan_kernel<<<1, 1024, 0, h->stream>>>(n_bins + 1, h->sort_bins());      // entry n_bins becomes the total
+    if (h->v.N % 4u == 0 && h->v.bead_off % 4u == 0)               // whole 16-byte quads of a chain per thread
+      chain_permute4_kernel<<<blocks_for(h->v.B / 4, 256), 256, 0, h->stream>>>(
+          h->v.B / 4, h->v.N / 4, h->sort_bins(), key, rank,
+          reinterpret_cast<const float4*>(h->vpos(src, 0)), reinterpret_cast<const float4*>(h->vpos(src, 1)), reinterpret_cast<const float4*>(h->vpos(src, 2)),
+          reinterpret_cast<float4*>(h->vpos(dst, 0)), reinterpret_cast<float4*>(h->vpos(dst, 1)), reinterpret_cast<float4*>(h->vpos(dst, 2)),
+          h->vslot_chain(src), h->vslot_pattern(src), h->vslot_chain(dst), h->vslot_pattern(dst));
+    else
     chain_permute_kernel<<<blocks_for(h->v.B, 256), 256, 0, h->stream>>>(
         h->v.B, h->v.N, h->sort_bins(), key, rank,
         h->vpos(src, 0), h->vpos(src, 1), h->vpos(src, 2), h->vpos(dst, 0), h->vpos(dst, 1), h->vpos(dst, 2),

@@ -541,6 +541,24 @@ chain_permute_kernel(uint64_t B, uint32_t N, const uint32_t* __restrict__ bin_st
   if (i == 0) { d_chain[d] = s_chain[s]; d_pat[d] = s_pat[s]; }
 }
 
+// the same for chain lengths that are multiples of four (and 16-byte aligned arrays): one thread per four beads,
+// 128-bit loads and stores, no division by the chain length (quads per chain passed in)
+__global__ void __launch_bounds__(256)
+chain_permute4_kernel(uint64_t n_quads, uint32_t quads_per_chain, const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ key,
+                      const uint32_t* __restrict__ rank,
+                      const float4* __restrict__ sx, const float4* __restrict__ sy, const float4* __restrict__ sz,
+                      float4* __restrict__ dx, float4* __restrict__ dy, float4* __restrict__ dz,
+                      const uint32_t* __restrict__ s_chain, const uint8_t* __restrict__ s_pat,
+                      uint32_t* __restrict__ d_chain, uint8_t* __restrict__ d_pat) {
+  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n_quads) return;
+  const uint32_t s = (uint32_t)(j / quads_per_chain), q = (uint32_t)(j - (uint64_t)s * quads_per_chain);
+  const uint32_t d = __ldg(bin_start + __ldg(key + s)) + __ldg(rank + s);
+  const uint64_t k = (uint64_t)d * quads_per_chain + q;
+  dx[k] = __ldcs(sx + j); dy[k] = __ldcs(sy + j); dz[k] = __ldcs(sz + j);
+  if (q == 0) { d_chain[d] = s_chain[s]; d_pat[d] = s_pat[s]; }
+}
+
 // sets *range_flag if a bead's cell coordinate is NaN or beyond kCellCoordLimit (see floor_bits)
 __global__ void __launch_bounds__(256)
 range_check_kernel(Grid grid, uint64_t B, const float* __restrict__ x, const float* __restrict__ y,
