@@ -173,6 +173,41 @@ typedef struct soma_validation {
 } soma_validation;
 int soma_validate_state(soma_t *h, soma_validation *out);
 
+/* The same report for a state the CALLER holds in device memory, without a handle and without allocating
+ * anything: no cudaMalloc, no cudaFree, no library routine that allocates.  It is the one entry point of this
+ * library that can be used by
+ *   - a process whose device memory was handed out before it started and must not grow (the paper spawns the
+ *     particle simulation next to a running continuum solver; a PyTorch host has usually given
+ *     the free HBM to its caching allocator): there a late cudaMalloc can fail, or take what the neighbour needs;
+ *   - a time-critical loop, where the device-wide synchronisation inside cudaMalloc / cudaFree would stall
+ *     every other stream of the process;
+ *   - a check of a checkpoint or of a received state before any handle (and so any workspace) exists.
+ * What it computes is what soma_validate_state computes (the paper's "validation functions"):
+ *   x, y, z   device [B] fp32, B = n_chains * beads_per_chain, bead i of chain c at c*beads_per_chain + i (one
+ *             species per call: all chains of equal length; beads_per_chain = 1 for single-bead molecules);
+ *   counts    device [n_types][cells] uint32 as soma_get_density returns them, or NULL: then the density fields of
+ *             the report stay 0 and `ok` means only "no non-finite coordinate"; n_types <= 8, n_types*cells < 2^32;
+ *   out       host; n_nonfinite, density_*, max_bond_sq are equal to soma_validate_state's, mean_bond_sq agrees to
+ *             rounding (the sums run in another, fixed order: the same state gives the same bits on every call).
+ * Scratch: the partial results live in one fixed array of 1 589 376 bytes (about 1.6 MB) that is part of the
+ * library's device code, so every GPU that loads the library holds it until the process exits.  It has room for
+ * 65 536 partial results of 4096 beads each: a state of more than 268 435 456 beads (2^28; the largest config has
+ * 2^27) is refused with SOMA_EINVAL and a message that says so -- split it, or use soma_validate_state.
+ * Sharing: all calls on one device use that one array and it keeps the last call's contents.  Every slot a call
+ * reads it has written before, so nothing needs clearing and calls may follow each other freely on one stream;
+ * two calls that can run on the GPU at the same time (different streams, different threads) overwrite each
+ * other's partial results and both reports are then garbage.  Serialise them.
+ * First call: the first call on each device looks up the array's device address (which may load the library's
+ * device code).  Make that call with the device current and before any stream capture is begun; later calls on
+ * that device only launch three kernels on `cuda_stream` (a cudaStream_t, NULL = default stream), copy 88 bytes
+ * back and synchronise the stream.  The current device must be the one the pointers belong to.
+ * errbuf (may be NULL): receives the text of the error, at most errbuf_len bytes with the terminator.
+ * Errors: SOMA_EINVAL (NULL pointer, size 0, state too large for the scratch array, bad n_types / cells),
+ * SOMA_ECUDA. */
+int soma_validate_noalloc(const float *x, const float *y, const float *z, uint64_t n_chains, uint32_t beads_per_chain,
+                          const uint32_t *counts, uint32_t n_types, uint64_t cells, void *cuda_stream,
+                          soma_validation *out, char *errbuf, size_t errbuf_len);
+
 /* DESIGN.md section 2 step 6, `n_steps` times: half-sweep(even), half-sweep(odd), bin, omega,
  * step += 1.  `accepted` (host pointer, may be NULL) receives the number of accepted moves of this
  * call; passing it synchronises the stream, passing NULL keeps the call asynchronous.

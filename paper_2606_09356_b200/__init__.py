@@ -26,7 +26,7 @@ LIB_PATH: Path = _build.LIB_PATH
 # every symbol include/soma.h declares (tests check the library exports exactly these)
 EXPORTS = (
     "soma_workspace_bytes", "soma_create", "soma_load_state", "soma_mc_steps", "soma_get_density",
-    "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_generate_state", "soma_init_from_density", "soma_validate_state", "soma_get_step", "soma_destroy", "soma_last_error",
+    "soma_get_positions", "soma_get_omega", "soma_set_external_field", "soma_generate_state", "soma_init_from_density", "soma_validate_state", "soma_validate_noalloc", "soma_get_step", "soma_destroy", "soma_last_error",
     "soma_set_option", "soma_get_counters", "soma_get_kernel_times", "soma_debug_half_sweep", "soma_debug_finish_step",
     "soma_debug_set_omega", "soma_debug_philox", "soma_debug_maps", "soma_debug_accept",
     "soma_debug_accept_fma", "soma_debug_cell_index", "soma_debug_red_throughput",
@@ -98,6 +98,7 @@ def load_library() -> C.CDLL:
             "soma_generate_state": (i32, [vp, u64, u64]),
             "soma_init_from_density": (i32, [vp, vp, i32, u64, u64, u32, C.c_float]),
             "soma_validate_state": (i32, [vp, C.POINTER(soma_validation)]),
+            "soma_validate_noalloc": (i32, [vp, vp, vp, u64, u32, vp, u32, u64, vp, C.POINTER(soma_validation), C.c_char_p, C.c_size_t]),
             "soma_get_step": (i32, [vp, C.POINTER(u64)]),
             "soma_destroy": (i32, [vp]),
             "soma_last_error": (C.c_char_p, [vp]),
@@ -231,6 +232,26 @@ def soma_init_from_density(h, phi_target, gen_seed: int, step0: int = 0, n_equil
 def soma_validate_state(h) -> dict:
     v = soma_validation()
     _check(load_library().soma_validate_state(h, C.byref(v)), h)
+    return {"nonfinite": int(v.n_nonfinite), "density_total": int(v.density_total),
+            "density_per_type": [int(t) for t in v.density_per_type], "max_bond_sq": float(v.max_bond_sq),
+            "mean_bond_sq": float(v.mean_bond_sq), "ok": bool(v.ok)}
+
+
+def soma_validate_noalloc(x, y, z, n_chains: int, beads_per_chain: int, counts=None, n_types: int = 0, cells: int = 0,
+                          cuda_stream: int = 0) -> dict:
+    """Validation report of a state held in CUDA tensors, for callers that must not allocate device memory (a
+    process whose HBM is already spoken for, a loop that cannot afford cudaMalloc's device-wide stall, a check
+    made before any handle exists): the library keeps its partial results in a fixed 1.6 MB array of its own.
+    x, y, z: float32 CUDA tensors of n_chains * beads_per_chain elements; counts: uint32/int32 CUDA tensor
+    [n_types][cells] or None.  At most 2^28 beads per call; calls must not overlap on the GPU.  Same keys as
+    soma_validate_state.  This wrapper only marshals the arguments; it creates no tensor."""
+    v = soma_validation()
+    err = C.create_string_buffer(512)
+    rc = load_library().soma_validate_noalloc(_ptr(x), _ptr(y), _ptr(z), int(n_chains), int(beads_per_chain),
+                                              None if counts is None else _ptr(counts), int(n_types), int(cells),
+                                              C.c_void_p(cuda_stream), C.byref(v), err, len(err))
+    if rc != SOMA_OK:
+        raise SomaError(rc, err.value.decode())
     return {"nonfinite": int(v.n_nonfinite), "density_total": int(v.density_total),
             "density_per_type": [int(t) for t in v.density_per_type], "max_bond_sq": float(v.max_bond_sq),
             "mean_bond_sq": float(v.mean_bond_sq), "ok": bool(v.ok)}
