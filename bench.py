@@ -34,7 +34,9 @@ import numpy as np
 # from the committed table profiles/ncu_counters.csv, one row per (kernel path, config, source hash of the
 # kernels).  A row whose hash is not the hash of the sources this run was built from is stale and ignored.
 NCU_TABLE = os.path.join(ROOT, "profiles", "ncu_counters.csv")
-KERNEL_SOURCES = ("soma_device.cuh", "soma_kernels.cuh", "soma_lean.cuh")
+# soma_api.cu is in the key because the launch geometry of the captured kernel lives there (threads per block, chunk,
+# carve-out, the thresholds that pick packed counters and the on-the-fly field)
+KERNEL_SOURCES = ("soma_device.cuh", "soma_kernels.cuh", "soma_lean.cuh", "soma_api.cu")
 
 METRIC = "attempted bead moves/s"
 UNIT = "moves/s"
@@ -133,9 +135,10 @@ _REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_
 
 
 class ClockSampler:
-    def __init__(self, cuda_index: int, period_s: float = 0.004):
+    def __init__(self, cuda_index: int, period_s: float = 0.001):
         self.period, self.samples, self.mask, self.power = period_s, [], 0, []
         self.sm_max, self._stop, self._thread, self._h, self._nv = None, threading.Event(), None, None, None
+        self._running = threading.Event()
         try:
             import pynvml as nv
             import torch
@@ -152,6 +155,7 @@ class ClockSampler:
 
     def _run(self):
         nv = self._nv
+        self._running.set()
         while not self._stop.is_set():
             try:
                 self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
@@ -168,8 +172,10 @@ class ClockSampler:
         if self._nv is not None:
             self.samples, self.mask, self.power = [], 0, []
             self._stop.clear()
+            self._running.clear()
             self._thread = threading.Thread(target=self._run, daemon=True)
             self._thread.start()
+            self._running.wait(1.0)          # the sampling loop is up before the timed region begins: a 20 ms window gets >= 5 samples
 
     def stop(self) -> dict:
         if self._nv is None:
@@ -397,6 +403,29 @@ def run_ours(args):
     steady_local = (local_ms - resorts_in_window * resort_ms) / args.steps + (resort_ms / interval if interval else 0.0)
     steady_ms, _ = aggregate_over_ranks(steady_local, 0.0, dev)
 
+    # ---- one whole re-ordering cycle: the re-ordering and the interval_steps MC steps up to the next one, timed as one
+    # region.  Unlike the window above this holds everything a long run pays per step: the re-ordering itself, the decay of
+    # the memory locality between two re-orderings, and the clock the chip settles at under sustained load. ----
+    cycle_ms, cycle = None, None
+    if interval:
+        clocks_c = ClockSampler(local_rank)
+        q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        barrier()
+        cc0 = g.counters()
+        clocks_c.start()
+        q0.record(stream)
+        g.set_option("resort_now", 0)
+        g.mc_steps(interval)
+        q1.record(stream)
+        torch.cuda.synchronize()
+        clk_c = clocks_c.stop()
+        barrier()
+        cc1 = g.counters()
+        cycle_ms, _ = aggregate_over_ranks(q0.elapsed_time(q1) / interval, 0.0, dev)
+        cycle = {"steps": interval, "resorts": cc1["resorts"] - cc0["resorts"], "ms": cycle_ms * interval, "clocks": clk_c}
+    sustained_ms = cycle_ms if cycle_ms else steady_ms
+
     # ---- end to end: the config's own run through the C ABI, host buffers in and out -----------
     S = w.steps
     torch.cuda.synchronize()
@@ -434,9 +463,10 @@ def run_ours(args):
                 "row_a4": ("inside the move kernel: omega is computed from the previous step's packed counters where it is needed and never "
                            "stored; omega_kernel_ms is the memset of the next count buffer; `achieved` still counts SURVEY's algorithmic bytes "
                            "(omega written and read once), so the DRAM traffic is below them") if otf else "omega_kernel",
-                "step_frac": ab["step"] / (steady_ms * 1e-3) / 1e9 / peak,
-                "step_frac_of_8TBps": ab["step"] / (steady_ms * 1e-3) / 8e12,
-                "target_step_frac_of_8TBps": 0.60, "target_met": ab["step"] / (steady_ms * 1e-3) / 8e12 >= 0.60,
+                "step_frac": ab["step"] / (sustained_ms * 1e-3) / 1e9 / peak,
+                "step_frac_of_8TBps": ab["step"] / (sustained_ms * 1e-3) / 8e12,
+                "step_frac_basis": "resort.ms_per_step_cycle" if cycle_ms else "resort.ms_per_step_steady",
+                "target_step_frac_of_8TBps": 0.60, "target_met": ab["step"] / (sustained_ms * 1e-3) / 8e12 >= 0.60,
                 "bytes_per_move": ab["step"] / B}
     if ncu:
         roofline["ncu"] = {"source": f"profiles/ncu_counters.csv ({ncu['capture']})", "source_hash": ncu["source_hash"],
@@ -461,8 +491,12 @@ def run_ours(args):
         "resort": {"interval_steps": interval, "ms": resort_ms, "in_timed_window": int(resorts_in_window),
                    "ms_per_step_amortised": resort_ms / interval if interval else 0.0,
                    "ms_per_step_steady": steady_ms, "moves_per_s_steady": world * B / (steady_ms * 1e-3),
+                   "ms_per_step_cycle": cycle_ms, "moves_per_s_cycle": world * B / (cycle_ms * 1e-3) if cycle_ms else None,
+                   "cycle": cycle,
                    "what": "the chains are re-ordered in memory every interval_steps MC steps; ms_per_step_steady = the timed steps "
-                           "without the re-orderings that fell into the window + one re-ordering per interval_steps, so it does not depend on K"},
+                           "without the re-orderings that fell into the window + one re-ordering per interval_steps, so it does not depend on K; "
+                           "ms_per_step_cycle = one re-ordering + the interval_steps steps after it timed as one region (CUDA events), its own "
+                           "clock record in `cycle`: the sustained figure, and the one roofline.step_frac* and target_met are computed from"},
         "clocks": clk, "gpu_launches": int(launches),
         "e2e": {"value": e2e_moves / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 12 * B / S,
                 "d2h_bytes_per_step": (12 * B + 4 * w.n_types * w.n_cells) / S, "mc_steps": S, "ms": e2e_ms,

@@ -36,13 +36,26 @@ def _isa_flags():
         return []
 
 
+# SCMF_ORACLE_SANITIZE=1 (tests/test_oracle_sanitizers.py): the same source, instrumented with AddressSanitizer and
+# UndefinedBehaviorSanitizer, as a second library.  The process must then run with libasan preloaded.  Same flags
+# otherwise (-O2, no contraction), so the instrumented oracle computes the same bits.
+_SAN_LIB = _HERE / "libscmf_oracle_san.so"
+_SAN_FLAGS = ["-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined,float-cast-overflow,float-divide-by-zero",
+              "-fno-sanitize-recover=all"]
+
+
+def sanitized() -> bool:
+    return os.environ.get("SCMF_ORACLE_SANITIZE", "") == "1"
+
+
 def build(force: bool = False) -> Path:
     """Compile the oracle with g++ (no GPU involved).  Returns the path of the shared library."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
-        tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
-        subprocess.run(["g++", *_CXXFLAGS, *_isa_flags(), str(_SRC), "-o", str(tmp)], check=True)
-        os.replace(tmp, _LIB)
-    return _LIB
+    out, extra = (_SAN_LIB, _SAN_FLAGS) if sanitized() else (_LIB, [])
+    if force or not out.exists() or out.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = out.with_suffix(f".tmp{os.getpid()}.so")
+        subprocess.run(["g++", *_CXXFLAGS, *extra, *_isa_flags(), str(_SRC), "-o", str(tmp)], check=True)
+        os.replace(tmp, out)
+    return out
 
 
 _lib = None

@@ -354,7 +354,7 @@ class Soma:
 
     def __init__(self, n_chains, beads_per_chain, n_types, type_patterns, chain_pattern, b, chiN,
                  kappaN, grid, box, move_halfwidth, seed, stream=None, lend_workspace: bool = True, n_single=None, smc_mobility=0.0,
-                 species=None):
+                 species=None, workspace_fill: Optional[int] = None):
         import torch
         if not torch.cuda.is_available():
             raise SomaError(SOMA_ECUDA, "no CUDA device: this package has no CPU fallback")
@@ -371,6 +371,8 @@ class Soma:
             if nbytes == 0:
                 raise SomaError(SOMA_EINVAL, (load_library().soma_last_error(None) or b"").decode())
             self._workspace = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+            if workspace_fill is not None:      # tests: the library must not depend on what the lent memory holds
+                self._workspace.fill_(int(workspace_fill))
             p.workspace, p.workspace_bytes = self._workspace.data_ptr(), nbytes
         self._stream = stream if stream is not None else torch.cuda.current_stream()
         self._h = soma_create(p, self._stream.cuda_stream)

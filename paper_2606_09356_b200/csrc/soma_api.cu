@@ -1024,11 +1024,15 @@ int soma_init_from_density(soma_t* h, const float* phi_target, int dev, uint64_t
   if (n_equil_steps) {                                           // equilibration under the umbrella potential, which is removed again
     h->umbrella = true;
     h->umbrella_k = umbrella_k;
-    if ((rc = launch_omega(h)) != SOMA_OK) return rc;
-    rc = soma_mc_steps(h, n_equil_steps, nullptr);
-    h->umbrella = false;
-    if (rc != SOMA_OK) return rc;
-    if ((rc = launch_omega(h)) != SOMA_OK) return rc;
+    rc = launch_omega(h);
+    if (rc == SOMA_OK) rc = soma_mc_steps(h, n_equil_steps, nullptr);
+    h->umbrella = false;                                         // whatever happened: no later step may see the umbrella term
+    if (rc == SOMA_OK) rc = launch_omega(h);
+    if (rc == SOMA_OK) rc = guard_check(h);                      // the equilibration ran without a synchronising call of its own
+    if (rc != SOMA_OK) {                                         // the omega array may still hold the umbrella field: the state has to be loaded again
+      h->loaded = false;
+      return rc;
+    }
   }
   return SOMA_OK;
 }
@@ -1117,7 +1121,10 @@ int soma_get_positions(soma_t* h, float* x, float* y, float* z, int dev) {
     for (int d = 0; d < 3; ++d)
       CU(h, cudaMemcpyAsync(dst[d] + h->B, h->single(d), h->S * 4,
                             dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
-  if (!dev) CU(h, cudaStreamSynchronize(h->stream));
+  if (!dev) {
+    CU(h, cudaStreamSynchronize(h->stream));
+    return guard_check(h);                                       // positions + step index are a checkpoint: never hand one out past the guard
+  }
   return SOMA_OK;
 }
 
@@ -1172,7 +1179,7 @@ int soma_validate_state(soma_t* h, soma_validation* out) {
   std::memcpy(&sum, &host[10], 8);
   out->mean_bond_sq = n_bonds ? sum / (double)n_bonds : 0.0;
   out->ok = (out->n_nonfinite == 0 && out->density_total == h->Btot) ? 1u : 0u;
-  return SOMA_OK;
+  return guard_check(h);
 }
 
 int soma_get_step(soma_t* h, uint64_t* step) {

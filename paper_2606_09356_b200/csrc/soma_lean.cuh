@@ -164,7 +164,10 @@ lean_step_kernel(const __grid_constant__ LeanArgs A) {
       chain_n = __ldg(A.slot_chain + slot + STEP);
     }
     if (MULTI_PAT) {
-      const uint16_t tt = __ldg(reinterpret_cast<const uint16_t*>(A.patterns + (uint32_t)__ldg(A.slot_pattern + slot) * A.pat_stride) + l);
+      // a lane beyond the range (n_chains not a multiple of 32/P) looks up the block's first slot instead of reading
+      // slot_pattern past its end: whatever bytes lie there would otherwise pick the type, and through it the gather address
+      const uint32_t ps = live ? slot : s_begin;
+      const uint16_t tt = __ldg(reinterpret_cast<const uint16_t*>(A.patterns + (uint32_t)__ldg(A.slot_pattern + ps) * A.pat_stride) + l);
       t0 = tt & 0xffu; t1 = tt >> 8;
     }
     const uint32_t toff0 = OTF ? 0u : t0 * A.cells, toff1 = OTF ? 0u : t1 * A.cells;   // OTF: one word per cell, the type picks its half

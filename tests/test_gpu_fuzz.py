@@ -10,6 +10,9 @@ from helpers import assert_same_state, gpu_system
 
 pytestmark = pytest.mark.gpu
 
+STARTS = {}        # start kind -> cases run (second family)
+RESYNCED = []      # cases whose device-side start differed from the oracle's in a last bit
+
 
 def _random_system(rng):
     T = int(rng.integers(1, 4))
@@ -91,10 +94,14 @@ def test_random_system_with_fields_moves_and_device_side_starts(k):
             phi = rng.uniform(0.05, 1.5, size=(w.n_types, w.n_cells)).astype(np.float32)
             o.init_from_density(phi, 99 + k, n_equil_steps=2, umbrella_k=0.5)
             g.init_from_density(phi, 99 + k, n_equil_steps=2, umbrella_k=0.5)
+        STARTS[start] = STARTS.get(start, 0) + 1
         if not all(np.array_equal(a, b) for a, b in zip(g.positions(), o.positions())):
             for a, b in zip(g.positions(), o.positions()):
                 assert (a != b).mean() <= 1e-3 and np.all(np.abs(a.astype(np.float64) - b) <= 4 * np.spacing(np.abs(b)) + 1e-6), what
-            return
+            # a last-bit difference of the double log / sin / cos: the documented case.  The device takes over the oracle's
+            # start, so that the trajectory, the field switching and the move types of this seed are still compared
+            RESYNCED.append(what)
+            g.load_state(*o.positions(), step0=o.step)
         assert_same_state(g, o, what + " (start)")
         ext = rng.normal(0, 0.7, size=(w.n_types, w.n_cells)).astype(np.float32)
         for field in (None, ext, None):
@@ -102,3 +109,14 @@ def test_random_system_with_fields_moves_and_device_side_starts(k):
             o.set_external_field(field)
             assert g.mc_steps(2, want_accepted=True) == o.mc_steps(2), what
             assert_same_state(g, o, what)
+
+
+def test_how_many_device_side_starts_had_to_be_resynchronised():
+    """Runs after the cases above (same file, later in it): says how many of the generated / density-placed starts
+    differed from the oracle's in a last bit and were replaced by the oracle's start before the trajectory was compared.
+    More than a few would mean the start generators disagree beyond the documented libm / CUDA cases."""
+    n_device = STARTS.get("generate", 0) + STARTS.get("density", 0)
+    print(f"fuzz: starts {STARTS}; {len(RESYNCED)} of {n_device} device-side starts resynchronised to the oracle's")
+    for w in RESYNCED:
+        print("  resynchronised:", w)
+    assert len(RESYNCED) <= max(2, n_device // 10)

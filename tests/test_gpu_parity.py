@@ -467,3 +467,50 @@ def test_a_16_bit_counter_reaching_its_guard_during_a_run_is_an_error_not_a_wron
         assert not g.counters()["packed_counts"]
         assert g.mc_steps(6, want_accepted=True) > 0
         assert_same_state(g, o, "the same run on 32-bit counters")
+
+
+@pytest.mark.parametrize("reader", ["positions", "validate"])
+def test_a_guard_hit_during_an_asynchronous_run_stops_the_checkpoint_calls(reader):
+    """The same crowded cell, but run the way the wrapper runs by default: soma_mc_steps with accepted == NULL never
+    synchronises, so the first call that does is the reader of the checkpoint -- soma_get_positions to host memory, or
+    soma_validate_state.  It must fail with SOMA_EINVAL rather than hand out a state whose counters are past the guard."""
+    import paper_2606_09356_b200 as soma
+    n0, n1 = 2040, 400
+    s = _custom(n0 + n1, 1, 1, [[0]], None, [[0]], 0.0, (4, 4, 4), (2.0, 2.0, 2.0), 71)
+    rng = np.random.default_rng(5)
+    s.x[:n0] = 0.05 + 0.4 * rng.random(n0).astype(np.float32)
+    s.x[n0:] = 0.52 + 0.05 * rng.random(n1).astype(np.float32)
+    s.y[:] = 0.75
+    s.z[:] = 0.75
+    ext = np.zeros((1, 64), dtype=np.float32)
+    ext[0, (0 * 4 + 1) * 4 + 1] = -25.0
+    with gpu_system(s, options=dict(packed_counts=1)) as g:
+        g.set_external_field(ext)
+        g.load_state(s.x, s.y, s.z)
+        assert g.counters()["packed_counts"]
+        g.mc_steps(6)                                               # asynchronous: returns without looking at the flag
+        with pytest.raises(soma.SomaError) as e:
+            g.positions() if reader == "positions" else g.validate()
+        assert e.value.code == soma.SOMA_EINVAL and "16-bit density counters" in str(e.value)
+        with pytest.raises(soma.SomaError) as e2:
+            g.mc_steps(1)
+        assert e2.value.code == soma.SOMA_ESTATE
+
+
+@pytest.mark.parametrize("N,n", [(8, 517), (16, 259), (32, 131)])
+def test_lanes_beyond_the_last_chain_do_not_depend_on_what_the_workspace_holds(N, n):
+    """Chain counts that are not a multiple of 32/P leave lanes of the last warp of the lean kernel without a chain.  With
+    several chain patterns such a lane used to read a pattern id past the end of the slot table; the lent workspace is filled
+    with 0xFF here, so that id would be 255, the bead type 255 and the omega gather 255 grids past the array.  The lanes now
+    look up the block's first slot.  32-bit counters, omega array (the default of grids below 2^20 cells); the run must also
+    equal the oracle's."""
+    half = N // 2
+    pats = [[0] * half + [1] * half, [1] * half + [0] * half, [0] * N]
+    s = _custom(n, N, 2, pats, np.arange(n) % 3, [[0, 12], [12, 0]], 35.0, (8, 8, 8), (4, 4, 4), 31 + N)
+    o = oracle.Oracle.from_system(s)
+    o.load_state(s.x, s.y, s.z)
+    acc_o = o.mc_steps(3)
+    with gpu_system(s, path=2, options=dict(packed_counts=0), workspace_fill=0xFF) as g:
+        g.load_state(s.x, s.y, s.z)
+        assert g.mc_steps(3, want_accepted=True) == acc_o
+        assert_same_state(g, o, f"N={N}, {n} chains of three patterns, workspace of 0xFF")
