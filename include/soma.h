@@ -113,7 +113,11 @@ uint64_t soma_workspace_bytes(const soma_params *p);
  * Errors: SOMA_EINVAL (bad parameter, see limits), SOMA_ENOMEM, SOMA_ECUDA.  *out is NULL on error. */
 int soma_create(const soma_params *p, void *cuda_stream, soma_t **out);
 
-/* DESIGN.md section 2 step 4: copy the positions in, set the absolute step index to `step0`, bin
+/* The state enters the library (`north_star`: "soma_load_state"; parts (2) and (3) of its step run here once: "re-binning
+ * all beads into per-type integer density grids" -- the paper's update_density_fields kernel, section 2.2 --
+ * and "recomputing omega from the densities", the quasi-instantaneous field of PAPER.md:41, section 2; the paper's SOMA
+ * receives its start the same way, as positions reproducing a supplied image).  DESIGN.md section 2 step 4:
+ * copy the positions in, set the absolute step index to `step0`, bin
  * all beads and compute omega, so that the next step sees the field of the loaded state.
  * x, y, z: [B] fp32, host or device according to `ptrs_are_device`.  (positions, step index) is a
  * complete checkpoint: the random stream is a pure function of (seed, step, half-sweep, chain,
@@ -208,8 +212,15 @@ int soma_validate_noalloc(const float *x, const float *y, const float *z, uint64
                           const uint32_t *counts, uint32_t n_types, uint64_t cells, void *cuda_stream,
                           soma_validation *out, char *errbuf, size_t errbuf_len);
 
-/* DESIGN.md section 2 step 6, `n_steps` times: half-sweep(even), half-sweep(odd), bin, omega,
- * step += 1.  `accepted` (host pointer, may be NULL) receives the number of accepted moves of this
+/* The SCMF Monte-Carlo step itself, `n_steps` times (`north_star` parts (1)-(3): "Metropolis trial moves of every bead in two
+ * half-sweeps (even beads, then odd beads), scored by harmonic bond energy plus the bead type's field omega at its grid
+ * cell", "re-binning all beads into per-type integer density grids", "recomputing omega from the densities"; in the paper:
+ * mc_polymer_iteration "performs biased trial moves and energy evaluations" (65 % of SOMA's run time) and
+ * update_density_fields "updates particle density fields" (25 %), section 2.2, with the non-bonded interactions
+ * in the quasi-instantaneous-field approximation, section 2).  DESIGN.md section 2 step 6: half-sweep(even),
+ * half-sweep(odd), bin, omega, step += 1.  With packed 16-bit counters the guard flag is looked at whenever this call
+ * synchronises by itself (every range-check interval, and at the end if `accepted` is given), so a guard hit surfaces after a
+ * bounded number of steps and at the latest at the next synchronising call of any kind.  `accepted` (host pointer, may be NULL) receives the number of accepted moves of this
  * call; passing it synchronises the stream, passing NULL keeps the call asynchronous.
  * n_steps == 0 is a no-op.  Errors: SOMA_ESTATE (no state loaded), SOMA_ECUDA. */
 int soma_mc_steps(soma_t *h, uint32_t n_steps, uint64_t *accepted);

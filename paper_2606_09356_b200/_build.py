@@ -34,8 +34,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB_PATH.with_suffix(f".tmp{os.getpid()}.so")
-        extra = ["-DSOMA_MIN_BUILD"] if os.environ.get("SOMA_MIN_BUILD") else []    # development only: N = 32 tiles
-        cmd = [nvcc, *NVCC_FLAGS, *extra, *map(str, sources()), "-o", str(tmp)]
+        cmd = [nvcc, *NVCC_FLAGS, *map(str, sources()), "-o", str(tmp)]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode != 0:
             print(r.stdout + r.stderr)
