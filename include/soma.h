@@ -336,7 +336,10 @@ int soma_debug_accept_fma(const float *dE, const uint32_t *words, uint8_t *decis
  * ceil(n_ops / 64) * 64 increments by threads of 64 each into n_counters uint32 counters of a scratch buffer.
  * mode 0: red.global at uniformly random counters; 1: red.global with the locality of the sorted melt (the 32 lanes
  * of a warp fall into a moving window of 2048 counters); 2: red.shared at random counters of a 32 KB window per
- * block.  *ms (host) = best of three timed launches, CUDA events.  Errors: SOMA_EINVAL, SOMA_ECUDA. */
+ * block.  Modes 3-6 probe a window spread over the shared memories of a thread-block cluster (8192 words per CTA;
+ * n_counters is not used): 3 / 4: red.shared::cluster at uniformly random words of an 8- / 16-CTA cluster's window;
+ * 5 / 6: ld.shared::cluster gathers with the sorted-melt locality over an 8- / 16-CTA cluster.
+ * *ms (host) = best of three timed launches, CUDA events.  Errors: SOMA_EINVAL, SOMA_ECUDA. */
 int soma_debug_red_throughput(uint64_t n_counters, uint64_t n_ops, int mode, double *ms);
 /* Cell index of host positions under the handle's grid/box. */
 int soma_debug_cell_index(soma_t *h, const float *x, const float *y, const float *z, uint32_t *cell,

@@ -1413,7 +1413,10 @@ int soma_debug_accept_fma(const float* dE, const uint32_t* words, uint8_t* decis
 }
 
 int soma_debug_red_throughput(uint64_t n_counters, uint64_t n_ops, int mode, double* ms) {
-  if (!ms || n_counters == 0 || n_counters >= (1ull << 32) || n_ops == 0 || mode < 0 || mode > 2) return fail(nullptr, SOMA_EINVAL, "bad argument");
+  if (!ms || n_counters == 0 || n_counters >= (1ull << 32) || n_ops == 0 || mode < 0 || mode > 6) return fail(nullptr, SOMA_EINVAL, "bad argument");
+  const unsigned cluster = mode == 3 || mode == 5 ? 8u : 16u;         // modes 3-6: a window in distributed shared memory
+  if (mode >= 3 && cluster > 8)
+    CUG(cudaFuncSetAttribute(debug_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
   DevBuf c;
   CUG(c.alloc(n_counters * 4));
   CUG(cudaMemset(c.p, 0, n_counters * 4));
@@ -1424,7 +1427,19 @@ int soma_debug_red_throughput(uint64_t n_counters, uint64_t n_ops, int mode, dou
   float best = 1e30f;
   for (int rep = 0; rep < 4; ++rep) {                                 // first pass warms up; best of the rest
     cudaEventRecord(e0);
-    debug_red_kernel<<<blocks_for(threads, 256), 256>>>((uint32_t*)c.p, (uint32_t)n_counters, per_thread, mode);
+    if (mode <= 2) {
+      debug_red_kernel<<<blocks_for(threads, 256), 256>>>((uint32_t*)c.p, (uint32_t)n_counters, per_thread, mode);
+    } else {
+      cudaLaunchConfig_t cfg{};
+      cfg.gridDim = dim3((blocks_for(threads, 256) + cluster - 1) / cluster * cluster);
+      cfg.blockDim = dim3(256);
+      cudaLaunchAttribute attr{};
+      attr.id = cudaLaunchAttributeClusterDimension;
+      attr.val.clusterDim.x = cluster; attr.val.clusterDim.y = 1; attr.val.clusterDim.z = 1;
+      cfg.attrs = &attr; cfg.numAttrs = 1;
+      cudaError_t le = cudaLaunchKernelEx(&cfg, debug_cluster_kernel, (uint32_t*)c.p, per_thread, mode >= 5 ? 1 : 0);
+      if (le != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); snprintf(g_last_error, 256, "cluster launch: %s", cudaGetErrorString(le)); return SOMA_ECUDA; }
+    }
     cudaEventRecord(e1);
     cudaError_t e = cudaEventSynchronize(e1);
     float t = 0.f;

@@ -811,4 +811,42 @@ debug_red_kernel(uint32_t* __restrict__ counters, uint32_t n_counters, uint32_t 
   }
 }
 
+// The same probe for a window that is spread over the shared memories of a thread-block cluster (distributed shared
+// memory): every CTA of the cluster holds 8192 words (32 KB), the window is cluster-size x 8192 words, and a thread
+// reaches word w of CTA r through mapa + red.shared::cluster / ld.shared::cluster.  gather = 0: increments at uniformly
+// random words of the cluster's window ((size-1)/size of them land in another SM's memory); gather = 1: loads with the
+// locality of the sorted melt (the 32 lanes of a warp fall into 2048 consecutive words, i.e. into one or two CTAs'
+// memories).  This is the data flow a cluster-windowed step kernel would have; the probe says what it could cost at best.
+__global__ void __launch_bounds__(256)
+debug_cluster_kernel(uint32_t* __restrict__ sink, uint32_t per_thread, int gather) {
+  __shared__ uint32_t win[8192];
+  uint32_t csize;
+  asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(csize));
+  for (uint32_t k = threadIdx.x; k < 8192u; k += blockDim.x) win[k] = gather ? k : 0u;
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+  const uint32_t local = (uint32_t)__cvta_generic_to_shared(win);
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t total = csize * 8192u;                       // cluster sizes are powers of two
+  uint32_t h = tid * 2654435761u + 12345u;
+  const uint32_t base = ((tid >> 5) * 613u) & (total - 1u);
+  uint32_t acc = 0;
+  for (uint32_t k = 0; k < per_thread; ++k) {
+    h = h * 1664525u + 1013904223u;
+    const uint32_t r = h >> 8;
+    const uint32_t idx = gather ? (base + (r & 2047u)) & (total - 1u) : r & (total - 1u);
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local + ((idx & 8191u) << 2)), "r"(idx >> 13));
+    if (gather) {
+      uint32_t v;
+      asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(remote));
+      acc += v;
+    } else {
+      asm volatile("red.relaxed.cluster.shared::cluster.add.u32 [%0], %1;" ::"r"(remote), "r"(1u) : "memory");
+    }
+  }
+  // no CTA may leave while another one still reaches into its shared memory
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+  if (threadIdx.x == 0 && (acc == 0xdeadbeefu || win[h & 8191u] == 0xffffffffu)) sink[0] = 1u;   // keeps loads and window alive
+}
+
 }  // namespace soma

@@ -186,6 +186,10 @@ def test_red_throughput_hook_measures_the_three_increment_modes():
         ms = soma.soma_debug_red_throughput(1 << 24, n_ops, mode)
         rate = n_ops / (ms * 1e-3)
         assert 1e10 < rate < 1e13, (mode, rate)
-    for bad in ((0, 100, 0), (100, 0, 0), (100, 100, 3)):
+    for mode in (3, 4, 5, 6):                            # the window in distributed shared memory (clusters of 8 / 16 CTAs)
+        ms = soma.soma_debug_red_throughput(1 << 10, n_ops, mode)
+        rate = n_ops / (ms * 1e-3)
+        assert 1e10 < rate < 2e13, (mode, rate)
+    for bad in ((0, 100, 0), (100, 0, 0), (100, 100, 7)):
         with pytest.raises(soma.SomaError):
             soma.soma_debug_red_throughput(*bad)
