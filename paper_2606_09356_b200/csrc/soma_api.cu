@@ -575,7 +575,16 @@ int resort(soma_handle* h) {
     else
       chain_key_kernel<false><<<blocks_for(h->v.n, 256), 256, 0, h->stream>>>(
           S, h->vpos(src, 0), h->vpos(src, 1), h->vpos(src, 2), h->sort_bins(), key, rank);
-    bin_scan_kernel<<<1, 1024, 0, h->stream>>>(n_bins + 1, h->sort_bins());      // entry n_bins becomes the total
+    if (n_bins + 1 > 8u * kBinScanChunk) {                         // many bins: three short passes over many blocks
+      const uint32_t chunks = (n_bins + 1 + kBinScanChunk - 1) / kBinScanChunk;
+      uint32_t* chunk = reinterpret_cast<uint32_t*>(h->cdf());     // scratch of soma_init_from_density, idle here (same stream)
+      bin_chunk_sums_kernel<<<chunks, 256, 0, h->stream>>>(n_bins + 1, h->sort_bins(), chunk);
+      bin_scan_kernel<<<1, 1024, 0, h->stream>>>(chunks, chunk);
+      bin_scan_apply_kernel<<<chunks, 256, 0, h->stream>>>(n_bins + 1, h->sort_bins(), chunk);
+      h->launches += 2;
+    } else {
+      bin_scan_kernel<<<1, 1024, 0, h->stream>>>(n_bins + 1, h->sort_bins());    // entry n_bins becomes the total
+    }
     if (h->v.N % 4u == 0 && h->v.bead_off % 4u == 0)               // whole 16-byte quads of a chain per thread
       chain_permute4_kernel<<<blocks_for(h->v.B / 4, 256), 256, 0, h->stream>>>(
           h->v.B / 4, h->v.N / 4, h->sort_bins(), key, rank,
