@@ -126,3 +126,26 @@ def test_product_package_never_touches_the_oracle():
             assert not re.search(r"^\s*(import|from)\s+paper_2606_09356_b200\b", text, flags=re.M), f
             assert not re.search(r"#\s*include[^\n]*(soma|paper_2606)", text), f
             assert "libsoma_b200" not in text, f
+
+
+def test_noalloc_entry_point_refuses_oversized_and_malformed_calls_before_touching_a_device(soma):
+    """soma_validate_noalloc checks its sizes against the fixed scratch array before any CUDA call, so the refusal -- and
+    its message, which has to tell a caller who cannot allocate what the limit is -- can be checked without a GPU.  The
+    pointers are never dereferenced on this path."""
+    lib = soma.load_library()
+    dummy = np.zeros(8, dtype=np.float32)
+    ptr = dummy.ctypes.data
+    v = soma.soma_validation()
+    err = C.create_string_buffer(512)
+
+    def call(n_chains, N, counts=None, T=0, cells=0, x=ptr, out=C.byref(v)):
+        return lib.soma_validate_noalloc(x, ptr, ptr, n_chains, N, counts, T, cells, None, out, err, len(err))
+
+    assert call((1 << 28) // 32 + 1, 32) == soma.SOMA_EINVAL            # one chain more than 2^28 beads
+    assert b"268435456" in err.value and b"scratch" in err.value
+    assert call(1 << 40, 65535) == soma.SOMA_EINVAL                      # no overflow in the size check
+    assert call(0, 32) == soma.SOMA_EINVAL and call(4, 0) == soma.SOMA_EINVAL
+    assert call(4, 2, x=None) == soma.SOMA_EINVAL and call(4, 2, out=None) == soma.SOMA_EINVAL
+    assert call(4, 2, counts=ptr, T=9, cells=8) == soma.SOMA_EINVAL      # the report has eight per-type fields
+    assert call(4, 2, counts=ptr, T=2, cells=1 << 31) == soma.SOMA_EINVAL
+    assert lib.soma_validate_noalloc(ptr, ptr, ptr, 1 << 30, 32, None, 0, 0, None, C.byref(v), None, 0) == soma.SOMA_EINVAL   # errbuf is optional
